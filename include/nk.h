@@ -1,0 +1,130 @@
+/* nk.h -- C-ABI of libnk.so: the Nekbone conjugate-gradient hot path on one B200 (sm_100a), fp64.
+ *
+ * What it computes (citations: "P:n" = /root/reference/PAPER.md line n; "S" = SURVEY.md section;
+ * "BJ" = BASELINE.json north_star):
+ *   P:225-226, P:290  3-D Poisson problem on E hexahedral spectral elements with (N+1)^3 points
+ *                     each, solved by unpreconditioned conjugate gradients, fixed iteration count.
+ *   P:314             `ax`: action of the Poisson operator (matrix-free local Laplacian, S 8(c) O3).
+ *   P:183-187         `gs`: gather-scatter (direct-stiffness sum QQ^T) over copies of shared nodes.
+ *   P:312, Table V    "streaming" (axpy) and "reduction" (dot product) kernels of CG.
+ *   BJ                Dirichlet mask; fused axpy+dot; residual history.
+ *
+ * Layout.  n = N+1, P = n^3, L = E*P.  A "local vector" is L doubles, element-local layout:
+ * index l = e*P + i + n*j + n^2*k with i <-> r (fastest), j <-> s, k <-> t.  Copies of a node
+ * shared between elements are stored once per touching element.
+ *
+ * Pointers.  Each argument says HOST or DEVICE.  DEVICE pointers must be 16-byte aligned and are
+ * owned by the caller (PyTorch tensors' data_ptr()); nothing passed in is retained except the
+ * workspace, which must outlive the context.  `stream` is a cudaStream_t passed as void* (NULL =
+ * the legacy default stream).  All work is enqueued on `stream`; only nk_setup, the *_host calls
+ * and nk_get_scalars synchronise.  One in-flight call per context; calls on one context must be
+ * stream-ordered.
+ *
+ * Errors.  Every call returns 0 (NK_OK) or a negative NK_ERR_* code; it never throws, aborts or
+ * prints.  There is no CPU fallback anywhere: without a CUDA device every compute call returns
+ * NK_ERR_CUDA.
+ */
+#ifndef NK_H
+#define NK_H
+#include <stddef.h>
+#include <stdint.h>
+
+#ifdef __cplusplus
+extern "C" {
+#endif
+
+#define NK_OK              0
+#define NK_ERR_ARG        -1   /* null/misaligned pointer, E <= 0, N outside [1,15], niter < 0, L >= 2^31 */
+#define NK_ERR_WORKSPACE  -2   /* workspace too small or not 256-byte aligned */
+#define NK_ERR_ID         -3   /* negative glo_num */
+#define NK_ERR_MASK       -4   /* mask value not exactly 0.0/1.0, or copies of one node disagree */
+#define NK_ERR_GEOM       -5   /* Jacobian determinant <= 0 or non-finite at some point */
+#define NK_ERR_CUDA       -6   /* CUDA runtime error; nk_last_cuda_error() has the cudaError_t */
+#define NK_ERR_ALLOC      -7   /* host allocation failed */
+#define NK_ERR_MULT       -8   /* more than 127 distinct node multiplicities (unsupported) */
+
+#define NK_MAX_ORDER      15
+
+typedef struct nk_ctx nk_ctx;   /* opaque; one per mesh */
+
+/* Upper bound, from (E, N) only, on the DEVICE workspace nk_setup needs (S 8(b)). */
+int nk_workspace_bytes(int64_t E, int N, size_t *bytes);
+
+/* Set-up (S 8(a) row a0; "setup on CPU amortised", P:63 derivative matrices depend on N only).
+ * Computes the GLL basis for order N, the six geometric factors per point
+ *   G_ab = w_i w_j w_k * J * (grad a . grad b),  a,b in {r,s,t}   (S 8(c) O2)
+ * on the device, the gather-scatter plan (CSR of local indices grouped by global id), the
+ * multiplicity and the inverse-multiplicity weights c.  Synchronises `stream` before returning.
+ *   coords   HOST  3 planes x|y|z, each L doubles, local layout
+ *   glo_num  HOST  L int64, arbitrary ids >= 0 (need not be contiguous)
+ *   mask     HOST  L doubles, each exactly 0.0 (Dirichlet) or 1.0; equal on all copies of a node
+ *   workspace DEVICE, caller-owned, 256-byte aligned, >= nk_workspace_bytes(E,N)
+ * On error *ctx is NULL.  NK_ERR_GEOM for an inverted / left-handed element. */
+int nk_setup(nk_ctx **ctx, int64_t E, int N, const double *coords, const int64_t *glo_num,
+             const double *mask, void *workspace, size_t workspace_bytes, void *stream);
+void nk_free(nk_ctx *ctx);
+
+/* w = A_L u : element-local Laplacian, no gs, no mask (S 8(a) a1).  u, w DEVICE, L; u != w. */
+int nk_ax_e(nk_ctx *ctx, const double *u, double *w, void *stream);
+/* v = Q Q^T v in place, NO mask (S 8(a) a2).  v DEVICE, L. */
+int nk_gs(nk_ctx *ctx, double *v, void *stream);
+/* w = M Q Q^T A_L u : ax_e, then gs fused with the Dirichlet mask (S 8(a) a1-a3).  u != w. */
+int nk_ax(nk_ctx *ctx, const double *u, double *w, void *stream);
+/* out[0] = <a,b>_c = sum_l c_l a_l b_l, c = 1/multiplicity (S 8(a) a4).  a, b, out DEVICE.
+ * Deterministic: per-block partials, ordered finish; no floating-point atomics. */
+int nk_dot(nk_ctx *ctx, const double *a, const double *b, double *out, void *stream);
+
+/* Unpreconditioned CG (S 8(c) O8): x0 = 0 (incoming x ignored), r0 = mask o f, recursive
+ * residual.  res_hist[k] = sqrt(<r_k, r_k>_c), k = 0..niter (DEVICE, niter+1 doubles).
+ * f must be equal on all copies of a node (unchecked).  f, x DEVICE, L.  niter = 0 is legal.
+ * Guards: an iteration with rho = 0 or pap = 0 takes alpha = beta = 0 (f = 0 gives x = 0, no NaN).
+ * Never synchronises; alpha, beta, rho stay on the device. */
+int nk_cg(nk_ctx *ctx, const double *f, double *x, int niter, double *res_hist, void *stream);
+/* Same with HOST f, x, res_hist: copies f in, runs nk_cg on workspace buffers, copies x and the
+ * history out, synchronises.  Needs the extra 2*L doubles nk_workspace_bytes already counts. */
+int nk_cg_host(nk_ctx *ctx, const double *f_host, double *x_host, int niter,
+               double *res_hist_host, void *stream);
+
+/* Test entry points for lock-step parity (S 8(c) protocol 2): the CG state lives in the context.
+ *   nk_cg_init       r = mask o f, x = 0, p = r, rho = <r,r>_c  (x DEVICE L, caller-owned, kept)
+ *   nk_cg_load_state copies r, p (DEVICE, L) into the context and sets rho (x is the caller's)
+ *   nk_cg_step       one iteration on (x, ctx r, ctx p); leaves w = ax(p) in the context
+ *   nk_cg_get_state  copies ctx r, p, w out (DEVICE, L each; any may be NULL)
+ *   nk_get_scalars   HOST out[5] = rho (entering the last step), pap, alpha, rho', beta; synchronises */
+int nk_cg_init(nk_ctx *ctx, const double *f, double *x, void *stream);
+int nk_cg_load_state(nk_ctx *ctx, const double *r, const double *p, double rho, void *stream);
+int nk_cg_step(nk_ctx *ctx, double *x, void *stream);
+int nk_cg_get_state(nk_ctx *ctx, double *r, double *p, double *w, void *stream);
+int nk_get_scalars(nk_ctx *ctx, double *out5_host, void *stream);
+
+/* Options (all default 0 unless stated):
+ *   "ax_variant"   0 = auto, 1 = line kernel (thread per grid line, D as constant operands),
+ *                  2 = slab kernel (2-D slab, k loop, D rows in registers)
+ *   "fuse_pap"     1 (default) = pap accumulated inside ax_e through the dot-fusion identity
+ *                  <M QQ^T A_L p, p>_c = sum_l (A_L p)_l p_l; 0 = separate weighted dot after gs
+ *   "fuse_p"       1 (default) = p = r + beta p folded into the load of the next ax_e; 0 = own kernel
+ *   "graph"        1 = nk_cg records its launches into a CUDA graph and replays it
+ * Unknown name or bad value: NK_ERR_ARG. */
+int nk_set_option(nk_ctx *ctx, const char *name, int value);
+int nk_get_option(nk_ctx *ctx, const char *name, int *value);
+
+/* Introspection. */
+int nk_get_sizes(nk_ctx *ctx, int64_t *n_local, int64_t *n_unique, int64_t *n_shared_unique,
+                 int64_t *n_masked_unique);
+/* gs plan sizes: CSR rows, listed local copies, rows that are summed (shared, unmasked). */
+int nk_get_gs_sizes(nk_ctx *ctx, int64_t *n_rows, int64_t *n_listed, int64_t *n_sum_rows);
+int nk_get_mult(nk_ctx *ctx, double *mult, void *stream);   /* DEVICE out, L: multiplicity per point */
+int nk_get_geom(nk_ctx *ctx, double *G6, void *stream);     /* DEVICE out, planes rr|rs|rt|ss|st|tt, each L */
+/* HOST out: D[(N+1)^2] row-major D[i*(N+1)+m] = l_m'(xi_i); xi[N+1]; w[N+1].  Any may be NULL. */
+int nk_get_D(nk_ctx *ctx, double *D_host, double *xi_host, double *w_host);
+/* Kernel launches enqueued by this context so far (for bench.py's gpu_launches). */
+int nk_get_launch_count(nk_ctx *ctx, int64_t *count);
+
+const char *nk_strerror(int code);
+int nk_last_cuda_error(void);   /* cudaError_t of the last NK_ERR_CUDA on this thread, else 0 */
+const char *nk_version(void);
+
+#ifdef __cplusplus
+}
+#endif
+#endif

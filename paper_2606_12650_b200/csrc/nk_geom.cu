@@ -1,0 +1,94 @@
+// nk_geom.cu -- set-up kernel: geometric factors (S 8(a) a0, S 8(c) O2; BJ "the 6 symmetric
+// geometric factors G").  Per point: the 3x3 Jacobian d(x,y,z)/d(r,s,t) by applying D along
+// r, s, t to the coordinates; J = det > 0; G_ab = w_i w_j w_k * J * (grad a . grad b).
+//
+// Conditioning (reading R22): differentiating ABSOLUTE coordinates cancels
+// ~|D|max * |x| / (h/2) leading digits, so coordinates are first taken relative to the element's
+// first node (D annihilates constants; the subtraction of nearby numbers is exact or 1 ulp of the
+// small difference).  With inverse metrics = cofactors / J:
+//   G_ab = w3 * (cof_a . cof_b) / J,   cof_r = (x_s x x_t), cof_s = (x_t x x_r), cof_t = (x_r x x_s).
+// Output: three double2 planes (rr,rs) (rt,ss) (st,tt) -- always 16-byte aligned per point, also
+// for odd (N+1)^3 (S 7 hard part 5).  One block per element; run once, not on the timed path.
+#include "nk_internal.h"
+
+namespace {
+
+constexpr int GEOM_THREADS = 256;
+
+__global__ void __launch_bounds__(GEOM_THREADS)
+geom_kernel(const double *__restrict__ coords, const double *__restrict__ Dg, const double *__restrict__ wq,
+            int n, int64_t L, double2 *__restrict__ g01, double2 *__restrict__ g23,
+            double2 *__restrict__ g45, int *__restrict__ errflag)
+{
+    __shared__ double s_D[16 * 16];
+    __shared__ double s_w[16];
+    for (int t = threadIdx.x; t < n * n; t += GEOM_THREADS) s_D[t] = Dg[t];
+    if (threadIdx.x < n) s_w[threadIdx.x] = wq[threadIdx.x];
+    __syncthreads();
+    const int P = n * n * n;
+    const int64_t base = (int64_t)blockIdx.x * P;
+    const double *xe = coords + base, *ye = coords + L + base, *ze = coords + 2 * L + base;
+    const double x0 = xe[0], y0 = ye[0], z0 = ze[0];
+    int bad = 0;
+    for (int q = threadIdx.x; q < P; q += GEOM_THREADS) {
+        const int i = q % n, j = (q / n) % n, k = q / (n * n);
+        double xr = 0, xs = 0, xt = 0, yr = 0, ys = 0, yt = 0, zr = 0, zs = 0, zt = 0;
+        for (int m = 0; m < n; ++m) {
+            const double di = s_D[i * n + m], dj = s_D[j * n + m], dk = s_D[k * n + m];
+            const int qr = m + n * j + n * n * k, qs = i + n * m + n * n * k, qt = i + n * j + n * n * m;
+            xr = fma(di, xe[qr] - x0, xr); yr = fma(di, ye[qr] - y0, yr); zr = fma(di, ze[qr] - z0, zr);
+            xs = fma(dj, xe[qs] - x0, xs); ys = fma(dj, ye[qs] - y0, ys); zs = fma(dj, ze[qs] - z0, zs);
+            xt = fma(dk, xe[qt] - x0, xt); yt = fma(dk, ye[qt] - y0, yt); zt = fma(dk, ze[qt] - z0, zt);
+        }
+        // cofactor vectors (rows of J * inverse Jacobian)
+        const double rx = ys * zt - yt * zs, ry = zs * xt - zt * xs, rz = xs * yt - xt * ys;   // x_s x x_t
+        const double sx = yt * zr - yr * zt, sy = zt * xr - zr * xt, sz = xt * yr - xr * yt;   // x_t x x_r
+        const double tx = yr * zs - ys * zr, ty = zr * xs - zs * xr, tz = xr * ys - xs * yr;   // x_r x x_s
+        const double J = xr * rx + yr * ry + zr * rz;
+        if (!(J > 0.0) || !isfinite(J)) bad = 1;
+        const double sc = s_w[i] * s_w[j] * s_w[k] / J;
+        const double grr = sc * (rx * rx + ry * ry + rz * rz);
+        const double grs = sc * (rx * sx + ry * sy + rz * sz);
+        const double grt = sc * (rx * tx + ry * ty + rz * tz);
+        const double gss = sc * (sx * sx + sy * sy + sz * sz);
+        const double gst = sc * (sx * tx + sy * ty + sz * tz);
+        const double gtt = sc * (tx * tx + ty * ty + tz * tz);
+        g01[base + q] = make_double2(grr, grs);
+        g23[base + q] = make_double2(grt, gss);
+        g45[base + q] = make_double2(gst, gtt);
+    }
+    if (bad) atomicOr(errflag, 1);
+}
+
+// rr|rs|rt|ss|st|tt planes of L for nk_get_geom
+__global__ void __launch_bounds__(GEOM_THREADS)
+unpack_geom_kernel(const double2 *__restrict__ g01, const double2 *__restrict__ g23,
+                   const double2 *__restrict__ g45, double *__restrict__ G6, int64_t L)
+{
+    const int64_t stride = (int64_t)gridDim.x * blockDim.x;
+    for (int64_t l = (int64_t)blockIdx.x * blockDim.x + threadIdx.x; l < L; l += stride) {
+        const double2 a = g01[l], b = g23[l], c = g45[l];
+        G6[l] = a.x; G6[L + l] = a.y; G6[2 * L + l] = b.x;
+        G6[3 * L + l] = b.y; G6[4 * L + l] = c.x; G6[5 * L + l] = c.y;
+    }
+}
+
+}  // namespace
+
+cudaError_t nk_launch_geom(nk_ctx *c, const double *coords_dev, const double *D_dev, const double *wq_dev,
+                           cudaStream_t st)
+{
+    geom_kernel<<<(unsigned)c->E, GEOM_THREADS, 0, st>>>(coords_dev, D_dev, wq_dev, c->n, c->L, c->g01, c->g23,
+                                                         c->g45, c->errflag);
+    c->launches++;
+    return cudaGetLastError();
+}
+
+cudaError_t nk_launch_get_geom(nk_ctx *c, double *G6, cudaStream_t st)
+{
+    int64_t nb = (c->L + GEOM_THREADS - 1) / GEOM_THREADS;
+    if (nb > (int64_t)c->sm_count * 32) nb = (int64_t)c->sm_count * 32;
+    unpack_geom_kernel<<<(unsigned)nb, GEOM_THREADS, 0, st>>>(c->g01, c->g23, c->g45, G6, c->L);
+    c->launches++;
+    return cudaGetLastError();
+}

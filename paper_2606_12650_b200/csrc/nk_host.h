@@ -1,0 +1,55 @@
+// nk_host.h -- host-side helpers shared by nk_api.cu and nk_setup.cu (product code only).
+#pragma once
+#include <cstdint>
+#include <vector>
+
+#include "nk_internal.h"
+
+void nk_set_last_cuda(int e);
+
+inline int nk_cuda_fail(cudaError_t e)
+{
+    nk_set_last_cuda((int)e);
+    return NK_ERR_CUDA;
+}
+#define NK_CUDA(call)                                      \
+    do {                                                   \
+        cudaError_t e__ = (call);                          \
+        if (e__ != cudaSuccess) return nk_cuda_fail(e__);  \
+    } while (0)
+
+inline size_t nk_align_up(size_t x, size_t a) { return (x + a - 1) / a * a; }
+inline bool nk_aligned16(const void *p) { return (reinterpret_cast<uintptr_t>(p) & 15u) == 0; }
+
+struct nk_carve {
+    size_t g, vec, code, off, idx, tabs, partials, hist, scal, small, total;
+};
+
+// Worst case: every local point listed in the gs plan (n_listed <= L, n_rows <= L).
+inline nk_carve nk_carve_sizes(int64_t L)
+{
+    nk_carve c;
+    c.g = nk_align_up((size_t)L * sizeof(double2), 256);          // x3
+    c.vec = nk_align_up((size_t)L * sizeof(double), 256);         // x5 (r, p, w, hf, hx)
+    c.code = nk_align_up((size_t)L, 256);
+    c.off = nk_align_up(((size_t)L + 1) * sizeof(int32_t), 256);
+    c.idx = nk_align_up((size_t)L * sizeof(int32_t), 256);
+    c.tabs = nk_align_up(2 * NK_CTAB * sizeof(double) + (16 * 16 + 16) * sizeof(double), 256);
+    c.partials = nk_align_up(NK_MAX_PARTIALS * sizeof(double), 256);
+    c.hist = nk_align_up(NK_HIST_MAX * sizeof(double), 256);
+    c.scal = 256;
+    c.small = 256;                                                // counter, errflag, res_dummy
+    c.total = 3 * c.g + 5 * c.vec + c.code + c.off + c.idx + c.tabs + c.partials + c.hist + c.scal + c.small;
+    return c;
+}
+
+inline bool nk_valid_EN(int64_t E, int N, int64_t *L_out)
+{
+    if (E <= 0 || N < 1 || N > NK_MAX_ORDER) return false;
+    const int64_t n = N + 1, P = n * n * n;
+    if (E > ((int64_t)1 << 31) / P) return false;
+    const int64_t L = E * P;
+    if (L >= ((int64_t)1 << 31)) return false;
+    *L_out = L;
+    return true;
+}

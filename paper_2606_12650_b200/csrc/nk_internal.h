@@ -1,0 +1,86 @@
+// nk_internal.h -- shared declarations of libnk.so's translation units (product code only;
+// nothing here is used by, or taken from, oracle/).
+#pragma once
+#include <cuda_runtime.h>
+#include <stddef.h>
+#include <stdint.h>
+
+#include "../../include/nk.h"
+
+// Scalar block on the device (doubles).  Written only by reduction epilogues.
+enum { NK_S_RHO = 0, NK_S_PAP = 1, NK_S_ALPHA = 2, NK_S_RHO_NEW = 3, NK_S_BETA = 4, NK_S_RHO_OLD = 5,
+       NK_S_COUNT = 8 };
+
+// What the last block of a reduction does with the ordered total (S 8(a) a7).
+enum { NK_EPI_STORE = 0,   // out[0] = total
+       NK_EPI_RHO0 = 1,    // rho = total; hist[0] = sqrt(total); beta = 0
+       NK_EPI_PAP = 2,     // pap = total; alpha = rho/pap (guarded)
+       NK_EPI_RHO = 3 };   // rho' = total; hist[k] = sqrt; beta = rho'/rho (guarded); rho_old = rho; rho = rho'
+
+#define NK_MAX_PARTIALS 65536      // upper bound on blocks of any reducing kernel
+#define NK_VEC_THREADS 512         // P: Table V "local group size 512" for streaming kernels
+#define NK_CODE_MASKED 0x80u       // bit 7 of the per-point code: Dirichlet node
+#define NK_HIST_MAX 8192               // residual-history capacity of nk_cg_host
+#define NK_CTAB 128                // code & 0x7f indexes ctab[] = 1/multiplicity
+
+struct nk_reduce_ws {
+    double *partials;      // NK_MAX_PARTIALS doubles
+    unsigned *counter;     // one ticket counter, self-resetting (atomicInc wrap)
+    double *scal;          // NK_S_COUNT doubles
+};
+
+struct nk_ctx {
+    int64_t E, P, L;
+    int N, n;
+    int device;
+    int sm_count;
+    // host copies of the basis (long double evaluated, rounded once)
+    double D[16 * 16], xi[16], wq[16];
+    // workspace carve-up (all DEVICE)
+    void *ws;
+    size_t ws_bytes;
+    double2 *g01, *g23, *g45;    // geometric factors as three double2 planes: (rr,rs) (rt,ss) (st,tt)
+    double *r, *p, *w;           // CG state, L each (coords staging aliases these during set-up)
+    double *hf, *hx;             // staging for nk_cg_host, L each
+    uint8_t *code;               // L: multiplicity-table index | NK_CODE_MASKED
+    int32_t *row_off;            // n_rows + 1
+    int32_t *row_idx;            // n_listed local indices, rows in [0,n_sum_rows) are summed,
+                                 // rows in [n_sum_rows, n_rows) are masked nodes
+    double *ctab;                // NK_CTAB doubles: 1/multiplicity
+    double *mtab;                // NK_CTAB doubles: multiplicity
+    double *hist;                // NK_HIST_MAX doubles (nk_cg_host)
+    double *res_dummy;           // 1 double (history sink for nk_cg_step)
+    int *errflag;                // geometry error flag
+    nk_reduce_ws red;
+    // sizes
+    int64_t n_unique, n_shared_unique, n_masked_unique;
+    int64_t n_rows, n_listed, n_sum_rows, n_sum_listed;
+    // options / state
+    int opt_ax_variant, opt_fuse_pap, opt_fuse_p, opt_graph;
+    int p_pending;               // 1: p = r + beta p has not been applied yet (fuse_p)
+    int64_t launches;
+    // cached graph for nk_cg
+    cudaGraphExec_t graph_exec;
+    const double *graph_f; double *graph_x; double *graph_hist; int graph_niter; int graph_key;
+};
+
+// ---- kernels' host launchers (each returns a cudaError_t from the launch) -----------------------
+// nk_basis.cpp
+void nk_host_basis(int N, double *xi, double *w, double *D);
+// nk_ax.cu : w = A_L u.  If r_in != NULL: u := r_in + beta*u is applied first and written back to u.
+// If dot: sum_l u_l w_l is reduced with epilogue NK_EPI_PAP.
+cudaError_t nk_launch_ax_e(nk_ctx *c, double *u_rw, const double *u_ro, const double *r_in, double *w,
+                           int dot, int variant, cudaStream_t st);
+cudaError_t nk_upload_D_tables(void);
+// nk_geom.cu
+cudaError_t nk_launch_geom(nk_ctx *c, const double *coords_dev, const double *D_dev,
+                           const double *wq_dev, cudaStream_t st);
+cudaError_t nk_launch_get_geom(nk_ctx *c, double *G6, cudaStream_t st);
+// nk_gs.cu
+cudaError_t nk_launch_gs(nk_ctx *c, double *v, int with_mask, cudaStream_t st);
+// nk_vec.cu
+cudaError_t nk_launch_dot(nk_ctx *c, const double *a, const double *b, double *out, int epi, cudaStream_t st);
+cudaError_t nk_launch_cg_init(nk_ctx *c, const double *f, double *x, double *hist, cudaStream_t st);
+cudaError_t nk_launch_update_xr(nk_ctx *c, double *x, double *hist_k, cudaStream_t st);
+cudaError_t nk_launch_update_p(nk_ctx *c, cudaStream_t st);
+cudaError_t nk_launch_get_mult(nk_ctx *c, double *mult, cudaStream_t st);

@@ -1,0 +1,191 @@
+// nk_vec.cu -- CG "streaming" and "reduction" kernels (Table V; S 8(a) a4-a7).
+// Each kernel makes ONE pass over its vectors with 16-byte accesses, folds the dot product it
+// needs into that pass, and finishes the reduction on the device (nk_reduce.cuh).  The inverse
+// multiplicity c_l comes from a 1-byte code per point through a 128-entry table in shared memory
+// (multiplicities on a hex mesh are a handful of small integers), so <a,b>_c costs 1 B/pt, not 8.
+#include "nk_internal.h"
+#include "nk_reduce.cuh"
+
+namespace {
+
+// Fixed grid => fixed partial sums => run-to-run bitwise reproducible.
+inline int vec_blocks(const nk_ctx *c, int64_t pairs)
+{
+    int64_t want = (pairs + NK_VEC_THREADS - 1) / NK_VEC_THREADS;
+    int64_t cap = (int64_t)c->sm_count * 4 * 4;          // 4 resident blocks/SM x 4 waves
+    if (want > cap) want = cap;
+    if (want < 1) want = 1;
+    return (int)want;
+}
+
+__device__ __forceinline__ void load_ctab(double *s_c, const double *ctab)
+{
+    for (int t = threadIdx.x; t < NK_CTAB; t += blockDim.x) s_c[t] = ctab[t];
+    __syncthreads();
+}
+
+// out = <a,b>_c
+__global__ void __launch_bounds__(NK_VEC_THREADS)
+dot_kernel(const double *__restrict__ a, const double *__restrict__ b, const uint8_t *__restrict__ code,
+           const double *__restrict__ ctab, int64_t L, nk_reduce_ws ws, int epi, double *out)
+{
+    __shared__ double s_c[NK_CTAB];
+    __shared__ double s_red[33];
+    load_ctab(s_c, ctab);
+    const int64_t pairs = L >> 1;
+    const int64_t stride = (int64_t)gridDim.x * blockDim.x;
+    double acc = 0.0;
+    for (int64_t q = (int64_t)blockIdx.x * blockDim.x + threadIdx.x; q < pairs; q += stride) {
+        const double2 av = reinterpret_cast<const double2 *>(a)[q];
+        const double2 bv = reinterpret_cast<const double2 *>(b)[q];
+        const uchar2 cd = reinterpret_cast<const uchar2 *>(code)[q];
+        acc = fma(s_c[cd.x & 0x7f] * av.x, bv.x, acc);
+        acc = fma(s_c[cd.y & 0x7f] * av.y, bv.y, acc);
+    }
+    if ((L & 1) && blockIdx.x == 0 && threadIdx.x == 0) {
+        const int64_t l = L - 1;
+        acc = fma(s_c[code[l] & 0x7f] * a[l], b[l], acc);
+    }
+    nk_grid_reduce(acc, s_red, ws, epi, out);
+}
+
+// r = mask o f, x = 0, p = r, rho0 = <r,r>_c       (S 8(c) O8 initialisation)
+__global__ void __launch_bounds__(NK_VEC_THREADS)
+cg_init_kernel(const double *__restrict__ f, double *__restrict__ x, double *__restrict__ r,
+               double *__restrict__ p, const uint8_t *__restrict__ code, const double *__restrict__ ctab,
+               int64_t L, nk_reduce_ws ws, double *hist0)
+{
+    __shared__ double s_c[NK_CTAB];
+    __shared__ double s_red[33];
+    load_ctab(s_c, ctab);
+    const int64_t pairs = L >> 1;
+    const int64_t stride = (int64_t)gridDim.x * blockDim.x;
+    double acc = 0.0;
+    for (int64_t q = (int64_t)blockIdx.x * blockDim.x + threadIdx.x; q < pairs; q += stride) {
+        double2 fv = reinterpret_cast<const double2 *>(f)[q];
+        const uchar2 cd = reinterpret_cast<const uchar2 *>(code)[q];
+        if (cd.x & NK_CODE_MASKED) fv.x = 0.0;
+        if (cd.y & NK_CODE_MASKED) fv.y = 0.0;
+        reinterpret_cast<double2 *>(r)[q] = fv;
+        reinterpret_cast<double2 *>(p)[q] = fv;
+        reinterpret_cast<double2 *>(x)[q] = make_double2(0.0, 0.0);
+        acc = fma(s_c[cd.x & 0x7f] * fv.x, fv.x, acc);
+        acc = fma(s_c[cd.y & 0x7f] * fv.y, fv.y, acc);
+    }
+    if ((L & 1) && blockIdx.x == 0 && threadIdx.x == 0) {
+        const int64_t l = L - 1;
+        const uint8_t cd = code[l];
+        const double fv = (cd & NK_CODE_MASKED) ? 0.0 : f[l];
+        r[l] = fv; p[l] = fv; x[l] = 0.0;
+        acc = fma(s_c[cd & 0x7f] * fv, fv, acc);
+    }
+    nk_grid_reduce(acc, s_red, ws, NK_EPI_RHO0, hist0);
+}
+
+// x += alpha p; r -= alpha w; rho' = <r,r>_c          (S 8(a) a5: axpy, axpy and dot in one pass)
+__global__ void __launch_bounds__(NK_VEC_THREADS)
+update_xr_kernel(double *__restrict__ x, double *__restrict__ r, const double *__restrict__ p,
+                 const double *__restrict__ w, const uint8_t *__restrict__ code,
+                 const double *__restrict__ ctab, int64_t L, nk_reduce_ws ws, double *hist_k)
+{
+    __shared__ double s_c[NK_CTAB];
+    __shared__ double s_red[33];
+    load_ctab(s_c, ctab);
+    const double alpha = ws.scal[NK_S_ALPHA];
+    const int64_t pairs = L >> 1;
+    const int64_t stride = (int64_t)gridDim.x * blockDim.x;
+    double acc = 0.0;
+    for (int64_t q = (int64_t)blockIdx.x * blockDim.x + threadIdx.x; q < pairs; q += stride) {
+        const double2 pv = reinterpret_cast<const double2 *>(p)[q];
+        const double2 wv = reinterpret_cast<const double2 *>(w)[q];
+        double2 xv = reinterpret_cast<double2 *>(x)[q];
+        double2 rv = reinterpret_cast<double2 *>(r)[q];
+        const uchar2 cd = reinterpret_cast<const uchar2 *>(code)[q];
+        xv.x = fma(alpha, pv.x, xv.x);
+        xv.y = fma(alpha, pv.y, xv.y);
+        rv.x = fma(-alpha, wv.x, rv.x);
+        rv.y = fma(-alpha, wv.y, rv.y);
+        reinterpret_cast<double2 *>(x)[q] = xv;
+        reinterpret_cast<double2 *>(r)[q] = rv;
+        acc = fma(s_c[cd.x & 0x7f] * rv.x, rv.x, acc);
+        acc = fma(s_c[cd.y & 0x7f] * rv.y, rv.y, acc);
+    }
+    if ((L & 1) && blockIdx.x == 0 && threadIdx.x == 0) {
+        const int64_t l = L - 1;
+        const double xv = fma(alpha, p[l], x[l]);
+        const double rv = fma(-alpha, w[l], r[l]);
+        x[l] = xv; r[l] = rv;
+        acc = fma(s_c[code[l] & 0x7f] * rv, rv, acc);
+    }
+    nk_grid_reduce(acc, s_red, ws, NK_EPI_RHO, hist_k);
+}
+
+// p = r + beta p                                       (S 8(a) a6)
+__global__ void __launch_bounds__(NK_VEC_THREADS)
+update_p_kernel(double *__restrict__ p, const double *__restrict__ r, const double *__restrict__ scal, int64_t L)
+{
+    const double beta = scal[NK_S_BETA];
+    const int64_t pairs = L >> 1;
+    const int64_t stride = (int64_t)gridDim.x * blockDim.x;
+    for (int64_t q = (int64_t)blockIdx.x * blockDim.x + threadIdx.x; q < pairs; q += stride) {
+        const double2 rv = reinterpret_cast<const double2 *>(r)[q];
+        double2 pv = reinterpret_cast<double2 *>(p)[q];
+        pv.x = fma(beta, pv.x, rv.x);
+        pv.y = fma(beta, pv.y, rv.y);
+        reinterpret_cast<double2 *>(p)[q] = pv;
+    }
+    if ((L & 1) && blockIdx.x == 0 && threadIdx.x == 0) {
+        const int64_t l = L - 1;
+        p[l] = fma(beta, p[l], r[l]);
+    }
+}
+
+__global__ void __launch_bounds__(NK_VEC_THREADS)
+get_mult_kernel(double *__restrict__ mult, const uint8_t *__restrict__ code, const double *__restrict__ mtab, int64_t L)
+{
+    const int64_t stride = (int64_t)gridDim.x * blockDim.x;
+    for (int64_t l = (int64_t)blockIdx.x * blockDim.x + threadIdx.x; l < L; l += stride)
+        mult[l] = mtab[code[l] & 0x7f];
+}
+
+}  // namespace
+
+cudaError_t nk_launch_dot(nk_ctx *c, const double *a, const double *b, double *out, int epi, cudaStream_t st)
+{
+    const int nb = vec_blocks(c, c->L >> 1);
+    dot_kernel<<<nb, NK_VEC_THREADS, 0, st>>>(a, b, c->code, c->ctab, c->L, c->red, epi, out);
+    c->launches++;
+    return cudaGetLastError();
+}
+
+cudaError_t nk_launch_cg_init(nk_ctx *c, const double *f, double *x, double *hist, cudaStream_t st)
+{
+    const int nb = vec_blocks(c, c->L >> 1);
+    cg_init_kernel<<<nb, NK_VEC_THREADS, 0, st>>>(f, x, c->r, c->p, c->code, c->ctab, c->L, c->red, hist);
+    c->launches++;
+    return cudaGetLastError();
+}
+
+cudaError_t nk_launch_update_xr(nk_ctx *c, double *x, double *hist_k, cudaStream_t st)
+{
+    const int nb = vec_blocks(c, c->L >> 1);
+    update_xr_kernel<<<nb, NK_VEC_THREADS, 0, st>>>(x, c->r, c->p, c->w, c->code, c->ctab, c->L, c->red, hist_k);
+    c->launches++;
+    return cudaGetLastError();
+}
+
+cudaError_t nk_launch_update_p(nk_ctx *c, cudaStream_t st)
+{
+    const int nb = vec_blocks(c, c->L >> 1);
+    update_p_kernel<<<nb, NK_VEC_THREADS, 0, st>>>(c->p, c->r, c->red.scal, c->L);
+    c->launches++;
+    return cudaGetLastError();
+}
+
+cudaError_t nk_launch_get_mult(nk_ctx *c, double *mult, cudaStream_t st)
+{
+    const int nb = vec_blocks(c, c->L);
+    get_mult_kernel<<<nb, NK_VEC_THREADS, 0, st>>>(mult, c->code, c->mtab, c->L);
+    c->launches++;
+    return cudaGetLastError();
+}
