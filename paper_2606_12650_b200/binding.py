@@ -1,0 +1,250 @@
+"""Thin ctypes binding of libnk.so (include/nk.h): argument marshalling only.
+
+Every numerical step runs in the CUDA kernels behind the C-ABI; PyTorch supplies device memory
+(`torch.Tensor.data_ptr()`) and the current stream.  There is no CPU fallback: if libnk.so is
+missing, `load()` raises; on a box without a CUDA device every compute call returns NK_ERR_CUDA.
+This module never imports `oracle`.
+"""
+from __future__ import annotations
+
+import ctypes as C
+import os
+
+import numpy as np
+
+HERE = os.path.dirname(os.path.abspath(__file__))
+LIB_PATH = os.path.join(HERE, "libnk.so")
+
+NK_OK, NK_ERR_ARG, NK_ERR_WORKSPACE, NK_ERR_ID, NK_ERR_MASK = 0, -1, -2, -3, -4
+NK_ERR_GEOM, NK_ERR_CUDA, NK_ERR_ALLOC, NK_ERR_MULT = -5, -6, -7, -8
+
+# every symbol include/nk.h declares: name -> (restype, argtypes)
+_vp, _i, _i64, _sz, _d = C.c_void_p, C.c_int, C.c_int64, C.c_size_t, C.c_double
+SIGNATURES = {
+    "nk_workspace_bytes": (_i, [_i64, _i, C.POINTER(_sz)]),
+    "nk_setup": (_i, [C.POINTER(_vp), _i64, _i, _vp, _vp, _vp, _vp, _sz, _vp]),
+    "nk_free": (None, [_vp]),
+    "nk_ax_e": (_i, [_vp, _vp, _vp, _vp]),
+    "nk_gs": (_i, [_vp, _vp, _vp]),
+    "nk_ax": (_i, [_vp, _vp, _vp, _vp]),
+    "nk_dot": (_i, [_vp, _vp, _vp, _vp, _vp]),
+    "nk_cg": (_i, [_vp, _vp, _vp, _i, _vp, _vp]),
+    "nk_cg_host": (_i, [_vp, _vp, _vp, _i, _vp, _vp]),
+    "nk_cg_init": (_i, [_vp, _vp, _vp, _vp]),
+    "nk_cg_load_state": (_i, [_vp, _vp, _vp, _d, _vp]),
+    "nk_cg_step": (_i, [_vp, _vp, _vp]),
+    "nk_cg_get_state": (_i, [_vp, _vp, _vp, _vp, _vp]),
+    "nk_get_scalars": (_i, [_vp, _vp, _vp]),
+    "nk_set_option": (_i, [_vp, C.c_char_p, _i]),
+    "nk_get_option": (_i, [_vp, C.c_char_p, C.POINTER(_i)]),
+    "nk_get_sizes": (_i, [_vp, C.POINTER(_i64), C.POINTER(_i64), C.POINTER(_i64), C.POINTER(_i64)]),
+    "nk_get_gs_sizes": (_i, [_vp, C.POINTER(_i64), C.POINTER(_i64), C.POINTER(_i64)]),
+    "nk_get_mult": (_i, [_vp, _vp, _vp]),
+    "nk_get_geom": (_i, [_vp, _vp, _vp]),
+    "nk_get_D": (_i, [_vp, _vp, _vp, _vp]),
+    "nk_get_launch_count": (_i, [_vp, C.POINTER(_i64)]),
+    "nk_strerror": (C.c_char_p, [_i]),
+    "nk_last_cuda_error": (_i, []),
+    "nk_version": (C.c_char_p, []),
+}
+
+_lib = None
+
+
+class NkError(RuntimeError):
+    def __init__(self, code: int, msg: str):
+        super().__init__(f"nk error {code}: {msg}")
+        self.code = code
+
+
+def load():
+    """dlopen libnk.so (built in-tree by `python -m paper_2606_12650_b200.build`).  Fails loudly."""
+    global _lib
+    if _lib is not None:
+        return _lib
+    if not os.path.exists(LIB_PATH):
+        raise ImportError(f"{LIB_PATH} not found: run `python -m paper_2606_12650_b200.build` "
+                          "(there is no CPU fallback)")
+    lib = C.CDLL(LIB_PATH)
+    for name, (res, args) in SIGNATURES.items():
+        fn = getattr(lib, name)
+        fn.restype = res
+        fn.argtypes = args
+    _lib = lib
+    return lib
+
+
+def _check(rc: int):
+    if rc != NK_OK:
+        raise NkError(rc, load().nk_strerror(rc).decode())
+
+
+def workspace_bytes(E: int, N: int) -> int:
+    out = _sz()
+    _check(load().nk_workspace_bytes(int(E), int(N), C.byref(out)))
+    return int(out.value)
+
+
+def _np_ptr(a: np.ndarray):
+    return a.ctypes.data_as(_vp)
+
+
+def _stream():
+    import torch
+    return _vp(torch.cuda.current_stream().cuda_stream)
+
+
+class Nekbone:
+    """One mesh on the current CUDA device.  Vectors are float64 CUDA tensors of length L."""
+
+    def __init__(self, E: int, N: int, coords, glo_num, mask, device="cuda"):
+        import torch
+        self._lib = load()
+        self._ctx = _vp()
+        self.E, self.N, self.n = int(E), int(N), int(N) + 1
+        self.L = self.E * self.n ** 3
+        self.device = torch.device(device)
+        coords = np.ascontiguousarray(coords, dtype=np.float64).reshape(-1)
+        glo_num = np.ascontiguousarray(glo_num, dtype=np.int64).reshape(-1)
+        mask = np.ascontiguousarray(mask, dtype=np.float64).reshape(-1)
+        if coords.size != 3 * self.L or glo_num.size != self.L or mask.size != self.L:
+            raise ValueError("coords/glo_num/mask size does not match E*(N+1)^3")
+        nbytes = workspace_bytes(self.E, self.N)
+        # caller-owned workspace: one torch allocation (256-B aligned by the caching allocator)
+        self._ws = torch.empty(nbytes, dtype=torch.uint8, device=self.device)
+        with torch.cuda.device(self.device):
+            rc = self._lib.nk_setup(C.byref(self._ctx), self.E, self.N, _np_ptr(coords), _np_ptr(glo_num),
+                                    _np_ptr(mask), _vp(self._ws.data_ptr()), nbytes, _stream())
+        _check(rc)
+
+    @classmethod
+    def from_mesh(cls, mesh, device="cuda"):
+        return cls(mesh.E, mesh.N, mesh.coords, mesh.glo_num, mesh.mask, device=device)
+
+    def close(self):
+        if getattr(self, "_ctx", None) is not None and self._ctx:
+            self._lib.nk_free(self._ctx)
+            self._ctx = None
+            self._ws = None
+
+    def __del__(self):
+        try:
+            self.close()
+        except Exception:
+            pass
+
+    # -- helpers -------------------------------------------------------------------------
+    def _vec(self, t, name="vector"):
+        import torch
+        if not (isinstance(t, torch.Tensor) and t.is_cuda and t.dtype == torch.float64
+                and t.is_contiguous() and t.numel() == self.L):
+            raise ValueError(f"{name}: need a contiguous float64 CUDA tensor of length {self.L}")
+        return _vp(t.data_ptr())
+
+    def empty(self):
+        import torch
+        return torch.empty(self.L, dtype=torch.float64, device=self.device)
+
+    # -- operators -----------------------------------------------------------------------
+    def ax_e(self, u, w=None):
+        w = self.empty() if w is None else w
+        _check(self._lib.nk_ax_e(self._ctx, self._vec(u, "u"), self._vec(w, "w"), _stream()))
+        return w
+
+    def gs(self, v):
+        """In place."""
+        _check(self._lib.nk_gs(self._ctx, self._vec(v, "v"), _stream()))
+        return v
+
+    def ax(self, u, w=None):
+        w = self.empty() if w is None else w
+        _check(self._lib.nk_ax(self._ctx, self._vec(u, "u"), self._vec(w, "w"), _stream()))
+        return w
+
+    def dot(self, a, b, out=None):
+        import torch
+        out = torch.empty(1, dtype=torch.float64, device=self.device) if out is None else out
+        _check(self._lib.nk_dot(self._ctx, self._vec(a, "a"), self._vec(b, "b"), _vp(out.data_ptr()), _stream()))
+        return out
+
+    def cg(self, f, niter: int, x=None, res_hist=None):
+        """Device-resident CG: returns (x, res_hist) CUDA tensors; does not synchronise."""
+        import torch
+        x = self.empty() if x is None else x
+        if res_hist is None:
+            res_hist = torch.empty(int(niter) + 1, dtype=torch.float64, device=self.device)
+        _check(self._lib.nk_cg(self._ctx, self._vec(f, "f"), self._vec(x, "x"), int(niter),
+                               _vp(res_hist.data_ptr()), _stream()))
+        return x, res_hist
+
+    def cg_host(self, f_host: np.ndarray, niter: int, x_host=None, hist_host=None):
+        """End-to-end call with HOST buffers (numpy, ideally pinned): H2D f, CG, D2H x + history."""
+        if f_host.dtype != np.float64 or f_host.size != self.L or not f_host.flags.c_contiguous:
+            raise ValueError("f_host: contiguous float64 array of length L")
+        x_host = np.empty(self.L) if x_host is None else x_host
+        hist_host = np.empty(int(niter) + 1) if hist_host is None else hist_host
+        _check(self._lib.nk_cg_host(self._ctx, _np_ptr(f_host), _np_ptr(x_host), int(niter),
+                                    _np_ptr(hist_host), _stream()))
+        return x_host, hist_host
+
+    # -- lock-step test entry points -----------------------------------------------------
+    def cg_init(self, f, x):
+        _check(self._lib.nk_cg_init(self._ctx, self._vec(f, "f"), self._vec(x, "x"), _stream()))
+
+    def cg_load_state(self, r, p, rho: float):
+        _check(self._lib.nk_cg_load_state(self._ctx, self._vec(r, "r"), self._vec(p, "p"), float(rho), _stream()))
+
+    def cg_step(self, x):
+        _check(self._lib.nk_cg_step(self._ctx, self._vec(x, "x"), _stream()))
+
+    def cg_get_state(self):
+        r, p, w = self.empty(), self.empty(), self.empty()
+        _check(self._lib.nk_cg_get_state(self._ctx, self._vec(r), self._vec(p), self._vec(w), _stream()))
+        return r, p, w
+
+    def scalars(self) -> dict:
+        out = np.empty(5)
+        _check(self._lib.nk_get_scalars(self._ctx, _np_ptr(out), _stream()))
+        return dict(rho=out[0], pap=out[1], alpha=out[2], rho_new=out[3], beta=out[4])
+
+    # -- options / introspection ---------------------------------------------------------
+    def set_option(self, name: str, value: int):
+        _check(self._lib.nk_set_option(self._ctx, name.encode(), int(value)))
+
+    def get_option(self, name: str) -> int:
+        v = _i()
+        _check(self._lib.nk_get_option(self._ctx, name.encode(), C.byref(v)))
+        return int(v.value)
+
+    def sizes(self) -> dict:
+        v = [_i64() for _ in range(4)]
+        _check(self._lib.nk_get_sizes(self._ctx, *[C.byref(a) for a in v]))
+        return dict(n_local=v[0].value, n_unique=v[1].value, n_shared_unique=v[2].value,
+                    n_masked_unique=v[3].value)
+
+    def gs_sizes(self) -> dict:
+        v = [_i64() for _ in range(3)]
+        _check(self._lib.nk_get_gs_sizes(self._ctx, *[C.byref(a) for a in v]))
+        return dict(n_rows=v[0].value, n_listed=v[1].value, n_sum_rows=v[2].value)
+
+    def mult(self):
+        m = self.empty()
+        _check(self._lib.nk_get_mult(self._ctx, self._vec(m), _stream()))
+        return m
+
+    def geom(self):
+        import torch
+        G = torch.empty(6 * self.L, dtype=torch.float64, device=self.device)
+        _check(self._lib.nk_get_geom(self._ctx, _vp(G.data_ptr()), _stream()))
+        return G.view(6, self.L)
+
+    def basis(self):
+        n = self.n
+        D, xi, w = np.empty((n, n)), np.empty(n), np.empty(n)
+        _check(self._lib.nk_get_D(self._ctx, _np_ptr(D), _np_ptr(xi), _np_ptr(w)))
+        return xi, w, D
+
+    def launch_count(self) -> int:
+        v = _i64()
+        _check(self._lib.nk_get_launch_count(self._ctx, C.byref(v)))
+        return int(v.value)

@@ -1,0 +1,105 @@
+"""CPU tests of the boundary: libnk.so builds for sm_100a, loads without a GPU, and exports every
+symbol include/nk.h declares; host-only entry points behave as the header states.  No compute."""
+import ctypes as C
+import os
+import re
+
+import pytest
+
+ROOT = os.path.dirname(os.path.dirname(os.path.abspath(__file__)))
+
+
+@pytest.fixture(scope="module")
+def lib():
+    from paper_2606_12650_b200 import build, binding
+    build.build()
+    return binding.load()
+
+
+def _declared_symbols():
+    text = open(os.path.join(ROOT, "include", "nk.h")).read()
+    text = re.sub(r"/\*.*?\*/", "", text, flags=re.S)
+    return sorted(set(re.findall(r"\b(nk_[a-z_0-9A-Z]+)\s*\(", text)))
+
+
+def test_header_symbols_all_exported(lib):
+    names = _declared_symbols()
+    assert len(names) >= 20 and "nk_setup" in names and "nk_cg" in names
+    for name in names:
+        assert hasattr(lib, name), f"libnk.so does not export {name}"
+
+
+def test_binding_signature_table_matches_header():
+    from paper_2606_12650_b200 import binding
+    assert sorted(binding.SIGNATURES) == _declared_symbols()
+
+
+def test_no_torch_types_in_header():
+    text = open(os.path.join(ROOT, "include", "nk.h")).read()
+    assert "torch" not in re.sub(r"/\*.*?\*/", "", text, flags=re.S)
+    assert 'extern "C"' in text
+
+
+def test_workspace_bytes(lib):
+    from paper_2606_12650_b200 import workspace_bytes, NkError
+    L = 512 * 8 ** 3
+    b = workspace_bytes(512, 7)
+    # G (48 B/pt) + 5 vectors (40 B/pt) + code (1) + CSR worst case (8) and small tables
+    assert 97 * L <= b <= 97 * L + (1 << 20) + 4096
+    assert workspace_bytes(1, 1) > 0
+    for E, N in [(0, 3), (-1, 3), (8, 0), (8, 16), (1 << 31, 15)]:
+        with pytest.raises(NkError) as ei:
+            workspace_bytes(E, N)
+        assert ei.value.code == -1
+    assert lib.nk_workspace_bytes(8, 3, None) == -1
+
+
+def test_strerror_and_version(lib):
+    assert lib.nk_strerror(0) == b"ok"
+    seen = set()
+    for code in range(-8, 0):
+        s = lib.nk_strerror(code)
+        assert s and s != b"unknown error"
+        seen.add(s)
+    assert len(seen) == 8
+    assert lib.nk_strerror(-99) == b"unknown error"
+    assert b"sm_100a" in lib.nk_version()
+
+
+def test_null_context_is_an_argument_error(lib):
+    assert lib.nk_ax_e(None, None, None, None) == -1
+    assert lib.nk_gs(None, None, None) == -1
+    assert lib.nk_cg(None, None, None, 1, None, None) == -1
+    assert lib.nk_get_sizes(None, None, None, None, None) == -1
+    lib.nk_free(None)       # no-op
+
+
+def test_setup_argument_checks_need_no_gpu(lib):
+    ctx = C.c_void_p(123)
+    assert lib.nk_setup(C.byref(ctx), 8, 3, None, None, None, None, 0, None) == -1
+    assert ctx.value is None
+    import numpy as np
+    L = 8 * 64
+    co, gl, mk = np.zeros(3 * L), np.zeros(L, dtype=np.int64), np.ones(L)
+    p = lambda a: a.ctypes.data_as(C.c_void_p)
+    # null / misaligned / too-small workspace
+    assert lib.nk_setup(C.byref(ctx), 8, 3, p(co), p(gl), p(mk), None, 1 << 30, None) == -2
+    assert lib.nk_setup(C.byref(ctx), 8, 3, p(co), p(gl), p(mk), C.c_void_p(256 + 8), 1 << 30, None) == -2
+    assert lib.nk_setup(C.byref(ctx), 8, 3, p(co), p(gl), p(mk), C.c_void_p(4096), 16, None) == -2
+
+
+def test_product_does_not_import_oracle():
+    pkg = os.path.join(ROOT, "paper_2606_12650_b200")
+    for dirpath, _, files in os.walk(pkg):
+        for fn in files:
+            if fn.endswith((".py", ".cu", ".cuh", ".h", ".cpp")):
+                src = open(os.path.join(dirpath, fn)).read()
+                assert not re.search(r"^\s*(from|import)\s+oracle", src, flags=re.M), fn
+                assert "nko" not in src.replace("nekbone", ""), fn
+    for dirpath, _, files in os.walk(os.path.join(ROOT, "oracle")):
+        for fn in files:
+            if fn.endswith((".py", ".c", ".h")):
+                src = open(os.path.join(dirpath, fn)).read()
+                assert not re.search(r"^\s*(from|import)\s+paper_2606_12650_b200", src, flags=re.M), fn
+                assert not re.search(r'#include\s+"[^"]*nk(_\w+)?\.(h|cuh)"', src), fn
+                assert "CDLL" not in src or "libnk.so" not in src, fn

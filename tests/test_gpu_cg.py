@@ -1,0 +1,154 @@
+"""-m gpu parity of the CG iteration (SURVEY.md 8(c) protocol parts 2-4; R15):
+lock-step single iterations from oracle-provided state at 1e-12, free-running CG at 1e-10 where
+the oracle's own rounding band allows, every fusion option against the others, degenerate inputs."""
+import numpy as np
+import pytest
+
+from parity import elem_err, maxnorm_rel
+from gpu_common import pair_for_brick, pair_for_config, to_dev, to_np, TOL_OP, TOL_CG
+from workloads import CONFIGS, config_rhs, rhs_unique
+
+pytestmark = pytest.mark.gpu
+
+OPTION_SETS = [dict(fuse_pap=1, fuse_p=1, graph=0), dict(fuse_pap=0, fuse_p=0, graph=0),
+               dict(fuse_pap=1, fuse_p=0, graph=0), dict(fuse_pap=0, fuse_p=1, graph=0),
+               dict(fuse_pap=1, fuse_p=1, graph=1)]
+
+
+def _set(gpu, opts):
+    for k, v in opts.items():
+        gpu.set_option(k, v)
+        assert gpu.get_option(k) == v
+
+
+def _rel(a, b):
+    return abs(a - b) / abs(b) if b != 0 else abs(a)
+
+
+@pytest.mark.parametrize("name", ["config1", "config2"])
+@pytest.mark.parametrize("opts", OPTION_SETS[:4])
+def test_lockstep_iterations(name, opts):
+    """Load the ORACLE's state at iteration k into the GPU, run one GPU iteration, compare
+    (w, pap, alpha, x, r, rho', beta, p) -- every iteration-level formula, zero amplification."""
+    pr = pair_for_config(name)
+    _set(pr.gpu, opts)
+    niter = CONFIGS[name]["niter"]
+    f = config_rhs(name, pr.mesh)
+    x, r, p, rho = pr.orc.cg_init(f)
+    checks = {k for k in (1, 2, 5, 10, 25, 50, 75, 100) if k <= niter}
+    for k in range(1, niter + 1):
+        if k in checks:
+            xd = to_dev(x)
+            pr.gpu.cg_load_state(to_dev(r), to_dev(p), rho)
+            pr.gpu.cg_step(xd)
+            rg, pg, wg = (to_np(t) for t in pr.gpu.cg_get_state())
+            sg = pr.gpu.scalars()
+        w, so = pr.orc.cg_step(x, r, p, rho)          # advances x, r, p in place
+        if k in checks:
+            assert elem_err(wg, w, pr.P) <= TOL_OP, k
+            for key in ("pap", "alpha", "rho_new", "beta"):
+                assert _rel(sg[key], so[key]) <= TOL_OP, (k, key, sg[key], so[key])
+            assert elem_err(to_np(xd), x, pr.P) <= TOL_OP, k
+            assert elem_err(rg, r, pr.P) <= TOL_OP, k
+            assert elem_err(pg, p, pr.P) <= TOL_OP, k
+        rho = so["rho_new"]
+    _set(pr.gpu, OPTION_SETS[0])
+
+
+@pytest.mark.parametrize("name", ["config1", "config2"])
+@pytest.mark.parametrize("opts", OPTION_SETS)
+def test_free_running_cg(name, opts):
+    pr = pair_for_config(name)
+    _set(pr.gpu, opts)
+    niter = CONFIGS[name]["niter"]
+    f = config_rhs(name, pr.mesh)
+    xo, ho = pr.orc.cg(f, niter)
+    xg, hg = pr.gpu.cg(to_dev(f), niter)
+    xg, hg = to_np(xg), to_np(hg)
+    assert hg.shape == (niter + 1,)
+    assert np.all(np.abs(hg - ho) <= TOL_CG * ho), np.abs(hg / ho - 1).max()
+    assert elem_err(xg, xo, pr.P) <= TOL_CG
+    assert np.all(xg[pr.mesh.mask == 0.0] == 0.0)
+    _set(pr.gpu, OPTION_SETS[0])
+
+
+def test_golden_history_config1():
+    """tests/golden/config1_cg.txt was written by tests/golden/make_golden.py from the oracle only."""
+    import os
+    path = os.path.join(os.path.dirname(__file__), "golden", "config1_cg.txt")
+    gold = np.array([float(l.split()[-1]) for l in open(path) if l.strip() and not l.startswith("#")])
+    pr = pair_for_config("config1")
+    xg, hg = pr.gpu.cg(to_dev(config_rhs("config1", pr.mesh)), 20)
+    hg = to_np(hg)
+    assert gold.size == 22 and np.all(np.abs(hg - gold[:21]) <= TOL_CG * gold[:21])
+    assert abs(float(xg.abs().max()) - gold[21]) <= TOL_CG * gold[21]
+
+
+def test_cg_host_entry_equals_device_entry():
+    pr = pair_for_config("config2")
+    f = config_rhs("config2", pr.mesh)
+    xd, hd = pr.gpu.cg(to_dev(f), 30)
+    xh, hh = pr.gpu.cg_host(f, 30)
+    assert np.array_equal(to_np(xd), xh) and np.array_equal(to_np(hd), hh)
+
+
+def test_cg_reproducible_and_ignores_incoming_x():
+    pr = pair_for_config("config2")
+    f = to_dev(config_rhs("config2", pr.mesh))
+    x1, h1 = pr.gpu.cg(f, 40)
+    x2 = to_dev(np.full(pr.L, 123.0))
+    x2, h2 = pr.gpu.cg(f, 40, x=x2)
+    assert bool((x1 == x2).all()) and bool((h1 == h2).all())
+
+
+def test_degenerate_inputs():
+    import torch
+    pr = pair_for_config("config1")
+    f = config_rhs("config1", pr.mesh)
+    # niter = 0: hist[0] only, x = 0
+    xg, hg = pr.gpu.cg(to_dev(f), 0)
+    xo, ho = pr.orc.cg(f, 0)
+    assert hg.numel() == 1 and abs(float(hg[0]) - ho[0]) <= TOL_OP * ho[0] and not bool(xg.any())
+    # f = 0: x = 0, history identically 0, no NaN
+    xg, hg = pr.gpu.cg(torch.zeros(pr.L, dtype=torch.float64, device="cuda"), 5)
+    assert not bool(xg.any()) and not bool(hg.any())
+    # far past convergence rho underflows to 0: guards keep everything finite
+    xg, hg = pr.gpu.cg(to_dev(f), 400)
+    assert bool(torch.isfinite(xg).all()) and bool(torch.isfinite(hg).all())
+    xo, _ = pr.orc.cg(f, 400)
+    assert elem_err(to_np(xg), xo, pr.P) <= TOL_CG
+
+
+def test_mask_all_zero_and_single_element():
+    from oracle.nko import Oracle
+    from paper_2606_12650_b200 import Nekbone
+    from workloads import brick_mesh
+    m = brick_mesh(2, 2, 2, 3, 0.05)
+    gpu = Nekbone(m.E, m.N, m.coords, m.glo_num, np.zeros(m.L))
+    xg, hg = gpu.cg(to_dev(rhs_unique(m, 3)), 5)
+    assert not bool(xg.any()) and not bool(hg.any())
+    # E = 1 at N = 5: only the 4^3 interior nodes are free
+    m = brick_mesh(1, 1, 1, 5, 0.0)
+    f = rhs_unique(m, 4)
+    xo, ho = Oracle.from_mesh(m).cg(f, 30)
+    xg, hg = Nekbone.from_mesh(m).cg(to_dev(f), 30)
+    assert np.all(np.abs(to_np(hg) - ho) <= TOL_CG * ho + 1e-300)
+    assert elem_err(to_np(xg), xo, 216) <= TOL_CG
+
+
+def test_cg_argument_errors():
+    from paper_2606_12650_b200 import NkError
+    pr = pair_for_config("config1")
+    f = to_dev(config_rhs("config1", pr.mesh))
+    with pytest.raises(NkError):
+        pr.gpu.cg(f, -1)
+    with pytest.raises(NkError):
+        pr.gpu.cg(f, 3, x=f)                     # f == x
+    with pytest.raises(NkError):
+        pr.gpu.ax_e(f, f)                        # u == w
+    with pytest.raises(NkError):
+        pr.gpu.set_option("no_such_option", 1)
+    with pytest.raises(NkError):
+        pr.gpu.set_option("fuse_pap", 7)
+    with pytest.raises(ValueError):
+        pr.gpu.ax_e(f[:-1].contiguous())
