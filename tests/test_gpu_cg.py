@@ -131,8 +131,15 @@ def test_mask_all_zero_and_single_element():
     m = brick_mesh(1, 1, 1, 5, 0.0)
     f = rhs_unique(m, 4)
     xo, ho = Oracle.from_mesh(m).cg(f, 30)
+    _, hb = Oracle.from_mesh(m, fma=True).cg(f, 30)
     xg, hg = Nekbone.from_mesh(m).cg(to_dev(f), 30)
-    assert np.all(np.abs(to_np(hg) - ho) <= TOL_CG * ho + 1e-300)
+    # 64 free nodes: CG converges to rounding level well before iteration 30, after which the
+    # recursive residual is rounding noise.  R15 protocol: flat 1e-10 wherever the oracle's own
+    # band (contraction-on vs -off builds) is <= 1e-11, elsewhere max(1e-10, 10 x band).
+    band = np.maximum.accumulate(np.abs(hb - ho) / ho)      # rounding noise only grows
+    tol = np.where(band <= 1e-11, TOL_CG, np.maximum(TOL_CG, 10.0 * band))
+    assert band[:13].max() <= 1e-11
+    assert np.all(np.abs(to_np(hg) - ho) <= tol * ho)
     assert elem_err(to_np(xg), xo, 216) <= TOL_CG
 
 
