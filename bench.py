@@ -1,0 +1,384 @@
+#!/usr/bin/env python
+"""bench.py -- the Nekbone CG hot path on B200, one JSON line (contract: task prompt).
+
+    python bench.py [--gpus N] [--steps K] [--warmup W] [--workload config5] [--impl ours|reference]
+
+A "step" is one nk_cg call: cg_init + `niter` CG iterations (ax_e -> gs+mask -> update x,r + rtr,
+with pap and the direction update fused into ax_e) over one seeded synthetic RHS, i.e. one pass of
+every SURVEY 8(a) row.  Default workload = BASELINE.json configs[4] (E=32768, N=11, 100 iterations),
+the largest single-GPU configuration and the one the >= 70 % HBM target is quoted on.
+
+  value        CG fp64 GFLOP/s, model flops (12(N+1)+27 per local point + gs adds) / device time,
+               inputs resident in HBM, CUDA events on the launching stream, max over ranks
+  e2e          same metric through nk_cg_host: pinned HOST f in, HOST x + history out, inside the timer
+  roofline     the dominant kernel (ax_e as it runs inside CG) against the measured HBM copy peak;
+               per-launch time from CUDA events recorded between launches IN the timed region
+  cpu_baseline the oracle (oracle/, as it stands) on the host cores, on a bounded sample
+
+N > 1 (torchrun): the path is single-GPU; every rank solves an independent replica
+of the workload (no data-path collective), "scaling": "weak".
+`--impl reference` times the oracle (this tier's reference arm) on rank 0 only.
+"""
+from __future__ import annotations
+
+import argparse
+import json
+import os
+import subprocess
+import sys
+import threading
+import time
+
+ROOT = os.path.dirname(os.path.abspath(__file__))
+if ROOT not in sys.path:
+    sys.path.insert(0, ROOT)
+
+import numpy as np
+
+METRIC = "nekbone_cg_fp64_gflops"
+UNIT = "GFLOP/s"
+HBM_NOMINAL_GBS = 8000.0          # BASELINE.json: "fraction of ~8 TB/s"
+HBM_FALLBACK_GBS = 6650.0         # B200_PROFILING.md fallback if MEASURED_PEAKS.json is absent
+
+
+# ---- model -----------------------------------------------------------
+def flops_per_point_iter(N: int, gs_adds_per_pt: float) -> float:
+    """ax_e 12(N+1)+15, pap 3, update+rtr 7, p update 2 (= 12(N+1)+27) + gs adds."""
+    return 12.0 * (N + 1) + 27.0 + gs_adds_per_pt
+
+
+def gs_bytes(sizes: dict) -> float:
+    """20 B per listed local copy (8 read + 8 write + 4 index) + 4 B per CSR row."""
+    return 20.0 * sizes["n_listed"] + 4.0 * sizes["n_rows"]
+
+
+def iter_model_bytes(L: int, sizes: dict) -> float:
+    """Canonical unfused per-iteration model: 168 B/pt + gs."""
+    return 168.0 * L + gs_bytes(sizes)
+
+
+def measured_peaks():
+    path = os.path.join(ROOT, "MEASURED_PEAKS.json")
+    try:
+        with open(path) as fh:
+            return float(json.load(fh)["hbm_gbs"]), "measured"
+    except Exception:
+        return HBM_FALLBACK_GBS, "fallback"
+
+
+# ---- clocks during the timed region ---------------------------------------------------------------
+class ClockSampler:
+    Q = ("clocks.sm,clocks.max.sm,power.draw,clocks_event_reasons.hw_slowdown,"
+         "clocks_event_reasons.hw_thermal_slowdown,clocks_event_reasons.sw_thermal_slowdown,"
+         "clocks_event_reasons.sw_power_cap")
+    NAMES = ("hw_slowdown", "hw_thermal_slowdown", "sw_thermal_slowdown", "sw_power_cap")
+
+    def __init__(self, index: int):
+        self.rows, self.proc, self.thread, self.index = [], None, None, index
+
+    def start(self):
+        try:
+            self.proc = subprocess.Popen(
+                ["nvidia-smi", "-i", str(self.index), f"--query-gpu={self.Q}", "--format=csv,noheader,nounits",
+                 "-lms", "100"], stdout=subprocess.PIPE, stderr=subprocess.DEVNULL, text=True)
+        except OSError:
+            self.proc = None
+            return
+        self.thread = threading.Thread(target=self._pump, daemon=True)
+        self.thread.start()
+
+    def _pump(self):
+        for line in self.proc.stdout:
+            self.rows.append((time.time(), line.strip()))
+
+    def stop(self, t0: float, t1: float) -> dict:
+        if self.proc is None:
+            return {"sm_mhz": None, "sm_max_mhz": None, "reasons": ["nvidia-smi unavailable"]}
+        time.sleep(0.15)
+        self.proc.terminate()
+        try:
+            self.proc.wait(timeout=5)
+        except Exception:
+            self.proc.kill()
+        sm, smax, power, reasons = [], [], [], set()
+        for ts, line in self.rows:
+            if ts < t0 or ts > t1 + 0.1:
+                continue
+            f = [x.strip() for x in line.split(",")]
+            try:
+                sm.append(float(f[0])); smax.append(float(f[1])); power.append(float(f[2]))
+            except (ValueError, IndexError):
+                continue
+            for name, val in zip(self.NAMES, f[3:7]):
+                if val.lower().startswith("active"):
+                    reasons.add(name)
+        if not sm:   # region shorter than one sample: use whatever was seen
+            for ts, line in self.rows[-3:]:
+                f = [x.strip() for x in line.split(",")]
+                try:
+                    sm.append(float(f[0])); smax.append(float(f[1])); power.append(float(f[2]))
+                except (ValueError, IndexError):
+                    pass
+        return {"sm_mhz": float(np.median(sm)) if sm else None,
+                "sm_max_mhz": float(max(smax)) if smax else None,
+                "power_w_max": float(max(power)) if power else None,
+                "samples": len(sm), "reasons": sorted(reasons)}
+
+
+# ---- the oracle, timed (cpu_baseline and --impl reference) ------------------------------------------
+def sample_brick(cfg: dict):
+    """Bounded sample of a workload: same N and amplitude, a brick of at most 8x8x8 elements."""
+    return tuple(min(8, b) for b in cfg["brick"])
+
+
+class OracleSample:
+    """The oracle (test infrastructure, timed as it stands) set up on a bounded sample."""
+
+    def __init__(self, workload: str):
+        from oracle.nko import Oracle, num_threads
+        from workloads import CONFIGS, brick_mesh, rhs_unique
+        cfg = CONFIGS[workload]
+        self.cfg, self.brick = cfg, sample_brick(cfg)
+        self.mesh = brick_mesh(*self.brick, cfg["N"], cfg["amplitude"])
+        self.f = rhs_unique(self.mesh, cfg["seed"])
+        self.orc = Oracle.from_mesh(self.mesh)
+        self.cores = int(num_threads())
+        s = self.orc.sizes()
+        # gs adds per point, from the mesh alone: (copies - 1) per shared unique node
+        self.gs_adds = float(self.mesh.L - s["n_unique"]) / self.mesh.L
+        self.fpp = flops_per_point_iter(cfg["N"], self.gs_adds)
+
+    def time_iters(self, k: int) -> float:
+        t = time.perf_counter()
+        self.orc.cg(self.f, k)
+        return time.perf_counter() - t
+
+    def calibrate(self, budget_s: float) -> int:
+        self.time_iters(1)                                # first call: thread pool, page faults
+        t3 = self.time_iters(3)
+        return int(max(3, min(400, round(3 * budget_s / max(t3, 1e-6)))))
+
+    def gflops(self, k: int, seconds: float) -> float:
+        return self.fpp * self.mesh.L * k / seconds / 1e9
+
+    def describe(self, k: int) -> str:
+        m = self.mesh
+        return (f"oracle nko_cg, {k} CG iterations on E={m.E} ({'x'.join(map(str, self.brick))} brick), "
+                f"N={m.N}, amplitude {self.cfg['amplitude']}, L={m.L} (sample of the same workload)")
+
+
+def cpu_baseline(workload: str, budget_s: float = 12.0) -> dict:
+    s = OracleSample(workload)
+    k = s.calibrate(budget_s)
+    sec = s.time_iters(k)
+    return {"value": s.gflops(k, sec), "unit": UNIT, "cores": s.cores, "kind": "oracle",
+            "sample": s.describe(k), "seconds": sec}
+
+
+def run_reference(args) -> dict:
+    """This tier's reference arm: the oracle on the host cores, each step a bounded sample."""
+    from workloads import CONFIGS
+    s = OracleSample(args.workload)
+    total_budget = 150.0                                  # whole run within a few minutes
+    k = s.calibrate(total_budget / max(1, args.steps + args.warmup))
+    for _ in range(args.warmup):
+        s.time_iters(k)
+    t = 0.0
+    for _ in range(args.steps):
+        t += s.time_iters(k)
+    val = s.gflops(k * args.steps, t)
+    cfg = CONFIGS[args.workload]
+    return {"impl": "reference", "metric": METRIC, "value": val, "unit": UNIT, "n_gpus": args.gpus,
+            "steps": args.steps, "warmup": args.warmup, "ms_per_step": 1e3 * t / args.steps,
+            "higher_is_better": True, "scaling": "weak", "vs_baseline": None, "dtype": "f64",
+            "data": "synthetic", "gpu_launches": 0,
+            "config": workload_config(args.workload, cfg, args.gpus),
+            "cpu_baseline": {"value": val, "unit": UNIT, "cores": s.cores, "kind": "oracle",
+                             "sample": s.describe(k) + " per step"},
+            "e2e": {"value": val, "unit": UNIT, "h2d_bytes_per_step": 0, "d2h_bytes_per_step": 0}}
+
+
+def workload_config(name: str, cfg: dict, n_gpus: int) -> dict:
+    nx, ny, nz = cfg["brick"]
+    n = cfg["N"] + 1
+    return {"workload": f"{name}: E={nx * ny * nz} ({nx}x{ny}x{nz} brick), N={cfg['N']}, "
+                        f"amplitude {cfg['amplitude']}, boundary mask, f uniform[-1,1) seed {cfg['seed']}, "
+                        f"CG {cfg['niter']} iterations",
+            "E": nx * ny * nz, "N": cfg["N"], "n_local": nx * ny * nz * n ** 3, "niter": cfg["niter"],
+            "step": "one nk_cg call (cg_init + niter iterations)",
+            "parallelism": "single GPU" if n_gpus == 1 else f"{n_gpus} independent replicas (no collective)",
+            "l2": "inputs larger than L2" if nx * ny * nz * n ** 3 * 8 * 11 > 2 * 126e6 else "L2-resident: L2 flushed between steps"}
+
+
+# ---- our arm -----------------------------------------------------------------------------------------
+def run_ours(args) -> dict | None:
+    import torch
+    from paper_2606_12650_b200 import Nekbone          # raises if libnk.so is missing: no fallback
+    from workloads import CONFIGS, config_mesh, rhs_unique
+
+    rank = int(os.environ.get("RANK", "0"))
+    world = int(os.environ.get("WORLD_SIZE", "1"))
+    local = int(os.environ.get("LOCAL_RANK", "0"))
+    if not torch.cuda.is_available():
+        raise SystemExit("bench.py: no CUDA device (there is no CPU fallback; use --impl reference for the oracle)")
+    torch.cuda.set_device(local)
+    dist = None
+    if world > 1:
+        import torch.distributed as dist
+        dist.init_process_group("nccl", device_id=torch.device("cuda", local))
+
+    cfg = CONFIGS[args.workload]
+    niter, N = cfg["niter"], cfg["N"]
+    mesh = config_mesh(args.workload)
+    f_np = rhs_unique(mesh, cfg["seed"] + 7919 * rank)            # replica r: its own RHS
+    t0 = time.perf_counter()
+    nk = Nekbone.from_mesh(mesh)
+    setup_s = time.perf_counter() - t0
+    for k, v in (("fuse_pap", args.fuse_pap), ("fuse_p", args.fuse_p), ("graph", args.graph)):
+        nk.set_option(k, v)
+    sizes = {**nk.sizes(), **nk.gs_sizes()}
+    L = mesh.L
+    gs_adds = float(L - sizes["n_unique"]) / L
+    flops_step = flops_per_point_iter(N, gs_adds) * L * niter
+    stream = torch.cuda.current_stream()
+
+    f = torch.from_numpy(f_np).cuda()
+    x = nk.empty()
+    hist = torch.empty(niter + 1, dtype=torch.float64, device="cuda")
+    small = L * 8 * 11 <= 2 * 126e6                                # working set not >> L2: flush between steps
+    flush = torch.empty(256 << 20, dtype=torch.uint8, device="cuda") if small else None
+
+    def barrier():
+        if dist is not None:
+            dist.barrier()
+        torch.cuda.synchronize()
+
+    def step():
+        if flush is not None:
+            flush.fill_(1)
+        nk.cg(f, niter, x=x, res_hist=hist)
+
+    # ---- device-resident timed region, per-kernel events inside it ---------------------------------
+    for _ in range(args.warmup):
+        step()
+    barrier()
+    nk.set_option("profile", 1 if not args.graph else 0)
+    nk.kernel_times()
+    launches0 = nk.launch_count()
+    clocks = ClockSampler(local)
+    clocks.start()
+    time.sleep(0.25)
+    ev = [torch.cuda.Event(enable_timing=True) for _ in range(2 * args.steps)]
+    barrier()
+    w0 = time.time()
+    for s in range(args.steps):
+        if flush is not None:
+            flush.fill_(1)
+        ev[2 * s].record(stream)
+        nk.cg(f, niter, x=x, res_hist=hist)
+        ev[2 * s + 1].record(stream)
+    barrier()
+    w1 = time.time()
+    clk = clocks.stop(w0, w1)
+    ms = sum(ev[2 * s].elapsed_time(ev[2 * s + 1]) for s in range(args.steps))
+    launches = nk.launch_count() - launches0
+    ktimes = nk.kernel_times()
+    nk.set_option("profile", 0)
+    res_final = float(hist[-1])
+
+    # ---- end to end through nk_cg_host: pinned host buffers, copies inside the timer ---------------
+    f_pin = torch.from_numpy(f_np).pin_memory()
+    x_pin = torch.empty(L, dtype=torch.float64).pin_memory()
+    h_pin = torch.empty(niter + 1, dtype=torch.float64).pin_memory()
+    nk.cg_host(f_pin.numpy(), niter, x_pin.numpy(), h_pin.numpy())           # warm-up
+    barrier()
+    e0, e1 = torch.cuda.Event(enable_timing=True), torch.cuda.Event(enable_timing=True)
+    e0.record(stream)
+    for _ in range(args.steps):
+        if flush is not None:
+            flush.fill_(1)
+        nk.cg_host(f_pin.numpy(), niter, x_pin.numpy(), h_pin.numpy())
+    e1.record(stream)
+    barrier()
+    ms_e2e = e0.elapsed_time(e1)
+
+    if dist is not None:
+        t = torch.tensor([ms, ms_e2e], dtype=torch.float64, device="cuda")
+        dist.all_reduce(t, op=dist.ReduceOp.MAX)
+        ms, ms_e2e = float(t[0]), float(t[1])
+        dist.barrier()
+        dist.destroy_process_group()
+    if rank != 0:
+        return None
+
+    peak, peak_kind = measured_peaks()
+    value = world * flops_step * args.steps / (ms * 1e-3) / 1e9
+    e2e = world * flops_step * args.steps / (ms_e2e * 1e-3) / 1e9
+    out = {"metric": METRIC, "value": value, "unit": UNIT, "n_gpus": world, "steps": args.steps,
+           "warmup": args.warmup, "ms_per_step": ms / args.steps, "higher_is_better": True,
+           "scaling": "weak", "vs_baseline": None, "dtype": "f64", "data": "synthetic",
+           "config": workload_config(args.workload, cfg, world),
+           "e2e": {"value": e2e, "unit": UNIT, "h2d_bytes_per_step": 8 * L,
+                   "d2h_bytes_per_step": 8 * (L + niter + 1), "ms_per_step": ms_e2e / args.steps},
+           "gpu_launches": int(launches), "clocks": clk,
+           "options": {"fuse_pap": args.fuse_pap, "fuse_p": args.fuse_p, "graph": args.graph},
+           "setup_s": setup_s, "final_residual": res_final}
+
+    # ---- iteration-level and kernel-level bandwidth ---------------------------------------------------
+    it_bytes = iter_model_bytes(L, sizes)
+    it_gbs = it_bytes * niter * args.steps / (ms * 1e-3) / 1e9
+    out["iteration"] = {"model_bytes_per_point": it_bytes / L, "ms_per_iteration": ms / args.steps / niter,
+                        "gbs_model": it_gbs, "frac_of_measured_copy": it_gbs / peak,
+                        "frac_of_nominal_8TBs": it_gbs / HBM_NOMINAL_GBS,
+                        "gdofs_paper_eq1": mesh.E * N ** 3 * niter * args.steps / (ms * 1e-3) / 1e9}
+    ax_ms, ax_n = ktimes["ax_e"]
+    if ax_n > 0:
+        # bytes the ax_e launch moves by the S 8(d) model: u 8 + G 48 + w 8 = 64 B/pt, plus, when the
+        # direction update is folded in, r 8 read + p 8 written (the update's own 24 B/pt kernel is gone)
+        bpp = 64.0 + (16.0 if args.fuse_p else 0.0)
+        avg = ax_ms / ax_n
+        ach = bpp * L / (avg * 1e-3) / 1e9
+        out["roofline"] = {"kernel": "ax_line_kernel (ax_e" + (" + fused p=r+beta*p" if args.fuse_p else "")
+                                     + (" + fused pap" if args.fuse_pap else "") + ")",
+                           "bound": "hbm", "achieved": ach, "peak": peak, "unit": "GB/s", "frac": ach / peak,
+                           "peak_kind": peak_kind + " copy peak (burst)", "frac_of_nominal_8TBs": ach / HBM_NOMINAL_GBS,
+                           "bytes_per_point": bpp, "avg_launch_us": 1e3 * avg, "launches_timed": ax_n,
+                           "traffic": args.traffic, "share_of_step": ax_ms / ms}
+        kb = {"gs": gs_bytes(sizes) / L, "dot": 24.0, "update_xr": 56.0 + 1.0 - 8.0, "update_p": 24.0}
+        out["kernels"] = {k: {"avg_us": 1e3 * t / n, "launches": n, "share_of_step": t / ms,
+                              **({"gbs_model": kb[k] * L / (t / n * 1e-3) / 1e9} if k in kb else {})}
+                          for k, (t, n) in ktimes.items() if n > 0}
+    else:
+        out["roofline"] = None
+    if not args.no_cpu_baseline:
+        out["cpu_baseline"] = cpu_baseline(args.workload)
+    return out
+
+
+def main():
+    ap = argparse.ArgumentParser()
+    ap.add_argument("--gpus", type=int, default=1)
+    ap.add_argument("--steps", type=int, default=5)
+    ap.add_argument("--warmup", type=int, default=3)
+    ap.add_argument("--impl", default="ours", choices=["ours", "reference"])
+    ap.add_argument("--workload", default="config5", choices=["config1", "config2", "config3", "config5"])
+    ap.add_argument("--fuse-pap", type=int, default=1)
+    ap.add_argument("--fuse-p", type=int, default=1)
+    ap.add_argument("--graph", type=int, default=0)
+    ap.add_argument("--traffic", type=float, default=None,
+                    help="dram bytes per ax_e launch from the committed ncu --set full capture (profiles/)")
+    ap.add_argument("--no-cpu-baseline", action="store_true")
+    args = ap.parse_args()
+    args.warmup = max(args.warmup, 3) if args.impl == "ours" else args.warmup
+    rank = int(os.environ.get("RANK", "0"))
+    if args.impl == "reference":
+        if rank == 0:
+            print(json.dumps(run_reference(args)), flush=True)
+        return
+    out = run_ours(args)
+    if out is not None:
+        print(json.dumps(out), flush=True)
+
+
+if __name__ == "__main__":
+    main()

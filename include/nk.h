@@ -104,6 +104,9 @@ int nk_get_scalars(nk_ctx *ctx, double *out5_host, void *stream);
  *                  <M QQ^T A_L p, p>_c = sum_l (A_L p)_l p_l; 0 = separate weighted dot after gs
  *   "fuse_p"       1 (default) = p = r + beta p folded into the load of the next ax_e; 0 = own kernel
  *   "graph"        1 = nk_cg records its launches into a CUDA graph and replays it
+ *   "profile"      1 = record a CUDA event on `stream` between consecutive launches so that
+ *                  nk_get_kernel_times can report device time per kernel class (nk_cg then
+ *                  enqueues its launches directly even if "graph" is 1)
  * Unknown name or bad value: NK_ERR_ARG. */
 int nk_set_option(nk_ctx *ctx, const char *name, int value);
 int nk_get_option(nk_ctx *ctx, const char *name, int *value);
@@ -117,6 +120,12 @@ int nk_get_mult(nk_ctx *ctx, double *mult, void *stream);   /* DEVICE out, L: mu
 int nk_get_geom(nk_ctx *ctx, double *G6, void *stream);     /* DEVICE out, planes rr|rs|rt|ss|st|tt, each L */
 /* HOST out: D[(N+1)^2] row-major D[i*(N+1)+m] = l_m'(xi_i); xi[N+1]; w[N+1].  Any may be NULL. */
 int nk_get_D(nk_ctx *ctx, double *D_host, double *xi_host, double *w_host);
+/* Device time per kernel class since the last call, measured with CUDA events on the launching
+ * stream while the "profile" option is 1 (S 8(d): per-kernel time inside the timed region).
+ * HOST out: ms[6], count[6], classes NK_K_*: 0 ax_e (with whatever is fused into it), 1 gs(+mask),
+ * 2 dot, 3 update x,r + rtr, 4 update p, 5 cg init.  Synchronises `stream`; resets the record. */
+#define NK_K_CLASSES 6
+int nk_get_kernel_times(nk_ctx *ctx, double *ms_host, int64_t *count_host, void *stream);
 /* Kernel launches enqueued by this context so far (for bench.py's gpu_launches). */
 int nk_get_launch_count(nk_ctx *ctx, int64_t *count);
 

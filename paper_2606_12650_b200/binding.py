@@ -42,6 +42,7 @@ SIGNATURES = {
     "nk_get_mult": (_i, [_vp, _vp, _vp]),
     "nk_get_geom": (_i, [_vp, _vp, _vp]),
     "nk_get_D": (_i, [_vp, _vp, _vp, _vp]),
+    "nk_get_kernel_times": (_i, [_vp, _vp, _vp, _vp]),
     "nk_get_launch_count": (_i, [_vp, C.POINTER(_i64)]),
     "nk_strerror": (C.c_char_p, [_i]),
     "nk_last_cuda_error": (_i, []),
@@ -243,6 +244,14 @@ class Nekbone:
         D, xi, w = np.empty((n, n)), np.empty(n), np.empty(n)
         _check(self._lib.nk_get_D(self._ctx, _np_ptr(D), _np_ptr(xi), _np_ptr(w)))
         return xi, w, D
+
+    KERNEL_CLASSES = ("ax_e", "gs", "dot", "update_xr", "update_p", "cg_init")
+
+    def kernel_times(self) -> dict:
+        """{class: (total device ms, launches)} recorded since the last call (option "profile" = 1)."""
+        ms, cnt = np.zeros(6), np.zeros(6, dtype=np.int64)
+        _check(self._lib.nk_get_kernel_times(self._ctx, _np_ptr(ms), _np_ptr(cnt), _stream()))
+        return {k: (float(ms[i]), int(cnt[i])) for i, k in enumerate(self.KERNEL_CLASSES)}
 
     def launch_count(self) -> int:
         v = _i64()

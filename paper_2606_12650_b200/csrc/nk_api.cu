@@ -13,6 +13,38 @@ namespace {
 thread_local int t_last_cuda = 0;
 }  // namespace
 
+// "profile" option: one cudaEvent between consecutive launches on the caller's stream; the
+// interval ending at event i is the device time of the launch of class cls[i] (-1: not a kernel).
+struct nk_prof {
+    std::vector<cudaEvent_t> ev;
+    std::vector<int> cls;
+    size_t used = 0;
+    ~nk_prof() { for (cudaEvent_t e : ev) cudaEventDestroy(e); }
+};
+
+namespace {
+cudaError_t prof_mark(nk_ctx *c, int cls, cudaStream_t st)
+{
+    if (!c->opt_profile) return cudaSuccess;
+    if (!c->prof) c->prof = new nk_prof();
+    nk_prof *p = c->prof;
+    if (p->used == p->ev.size()) {
+        cudaEvent_t e;
+        cudaError_t rc = cudaEventCreate(&e);
+        if (rc != cudaSuccess) return rc;
+        p->ev.push_back(e);
+        p->cls.push_back(-1);
+    }
+    p->cls[p->used] = cls;
+    return cudaEventRecord(p->ev[p->used++], st);
+}
+#define NK_LAUNCH(cls, call)                                          \
+    do {                                                              \
+        if ((e = (call)) != cudaSuccess) return e;                    \
+        if ((e = prof_mark(c, (cls), st)) != cudaSuccess) return e;   \
+    } while (0)
+}  // namespace
+
 void nk_set_last_cuda(int e) { t_last_cuda = e; }
 
 extern "C" {
@@ -48,6 +80,7 @@ void nk_free(nk_ctx *c)
 {
     if (!c) return;
     if (c->graph_exec) cudaGraphExecDestroy(c->graph_exec);
+    delete c->prof;
     delete c;
 }
 
@@ -63,20 +96,18 @@ cudaError_t enqueue_iteration(nk_ctx *c, double *x, double *hist_k, cudaStream_t
     cudaError_t e;
     const int fuse_pap = c->opt_fuse_pap;
     if (c->p_pending) {          // p = r + beta p folded into this ax_e's load
-        e = nk_launch_ax_e(c, c->p, nullptr, c->r, c->w, fuse_pap, c->opt_ax_variant, st);
+        NK_LAUNCH(NK_K_AX, nk_launch_ax_e(c, c->p, nullptr, c->r, c->w, fuse_pap, c->opt_ax_variant, st));
         c->p_pending = 0;
     } else {
-        e = nk_launch_ax_e(c, nullptr, c->p, nullptr, c->w, fuse_pap, c->opt_ax_variant, st);
+        NK_LAUNCH(NK_K_AX, nk_launch_ax_e(c, nullptr, c->p, nullptr, c->w, fuse_pap, c->opt_ax_variant, st));
     }
-    if (e != cudaSuccess) return e;
-    if ((e = nk_launch_gs(c, c->w, 1, st)) != cudaSuccess) return e;
-    if (!fuse_pap)
-        if ((e = nk_launch_dot(c, c->w, c->p, nullptr, NK_EPI_PAP, st)) != cudaSuccess) return e;
-    if ((e = nk_launch_update_xr(c, x, hist_k, st)) != cudaSuccess) return e;
+    NK_LAUNCH(NK_K_GS, nk_launch_gs(c, c->w, 1, st));
+    if (!fuse_pap) NK_LAUNCH(NK_K_DOT, nk_launch_dot(c, c->w, c->p, nullptr, NK_EPI_PAP, st));
+    NK_LAUNCH(NK_K_UPDATE_XR, nk_launch_update_xr(c, x, hist_k, st));
     if (c->opt_fuse_p) {
         c->p_pending = 1;
     } else {
-        if ((e = nk_launch_update_p(c, st)) != cudaSuccess) return e;
+        NK_LAUNCH(NK_K_UPDATE_P, nk_launch_update_p(c, st));
     }
     return cudaSuccess;
 }
@@ -85,11 +116,12 @@ cudaError_t enqueue_cg(nk_ctx *c, const double *f, double *x, int niter, double 
 {
     cudaError_t e;
     c->p_pending = 0;
-    if ((e = nk_launch_cg_init(c, f, x, res_hist, st)) != cudaSuccess) return e;
+    if ((e = prof_mark(c, -1, st)) != cudaSuccess) return e;
+    NK_LAUNCH(NK_K_INIT, nk_launch_cg_init(c, f, x, res_hist, st));
     for (int k = 1; k <= niter; ++k)
         if ((e = enqueue_iteration(c, x, res_hist + k, st)) != cudaSuccess) return e;
     if (c->p_pending) {          // leave the context with p up to date
-        if ((e = nk_launch_update_p(c, st)) != cudaSuccess) return e;
+        NK_LAUNCH(NK_K_UPDATE_P, nk_launch_update_p(c, st));
         c->p_pending = 0;
     }
     return cudaSuccess;
@@ -102,22 +134,29 @@ extern "C" {
 int nk_ax_e(nk_ctx *c, const double *u, double *w, void *stream)
 {
     if (!c || !u || !w || u == w || !nk_aligned16(u) || !nk_aligned16(w)) return NK_ERR_ARG;
+    NK_CUDA(prof_mark(c, -1, S(stream)));
     NK_CUDA(nk_launch_ax_e(c, nullptr, u, nullptr, w, 0, c->opt_ax_variant, S(stream)));
+    NK_CUDA(prof_mark(c, NK_K_AX, S(stream)));
     return NK_OK;
 }
 
 int nk_gs(nk_ctx *c, double *v, void *stream)
 {
     if (!c || !v || !nk_aligned16(v)) return NK_ERR_ARG;
+    NK_CUDA(prof_mark(c, -1, S(stream)));
     NK_CUDA(nk_launch_gs(c, v, 0, S(stream)));
+    NK_CUDA(prof_mark(c, NK_K_GS, S(stream)));
     return NK_OK;
 }
 
 int nk_ax(nk_ctx *c, const double *u, double *w, void *stream)
 {
     if (!c || !u || !w || u == w || !nk_aligned16(u) || !nk_aligned16(w)) return NK_ERR_ARG;
+    NK_CUDA(prof_mark(c, -1, S(stream)));
     NK_CUDA(nk_launch_ax_e(c, nullptr, u, nullptr, w, 0, c->opt_ax_variant, S(stream)));
+    NK_CUDA(prof_mark(c, NK_K_AX, S(stream)));
     NK_CUDA(nk_launch_gs(c, w, 1, S(stream)));
+    NK_CUDA(prof_mark(c, NK_K_GS, S(stream)));
     return NK_OK;
 }
 
@@ -133,7 +172,7 @@ int nk_cg(nk_ctx *c, const double *f, double *x, int niter, double *res_hist, vo
     if (!c || !f || !x || !res_hist || niter < 0 || f == x || !nk_aligned16(f) || !nk_aligned16(x))
         return NK_ERR_ARG;
     cudaStream_t st = S(stream);
-    if (!c->opt_graph) {
+    if (!c->opt_graph || c->opt_profile) {
         NK_CUDA(enqueue_cg(c, f, x, niter, res_hist, st));
         return NK_OK;
     }
@@ -251,6 +290,7 @@ static int *option_slot(nk_ctx *c, const char *name, int *lo, int *hi)
     if (!std::strcmp(name, "fuse_pap")) { *lo = 0; *hi = 1; return &c->opt_fuse_pap; }
     if (!std::strcmp(name, "fuse_p")) { *lo = 0; *hi = 1; return &c->opt_fuse_p; }
     if (!std::strcmp(name, "graph")) { *lo = 0; *hi = 1; return &c->opt_graph; }
+    if (!std::strcmp(name, "profile")) { *lo = 0; *hi = 1; return &c->opt_profile; }
     return nullptr;
 }
 
@@ -313,6 +353,25 @@ int nk_get_D(nk_ctx *c, double *D_host, double *xi_host, double *w_host)
     if (D_host) std::memcpy(D_host, c->D, sizeof(double) * c->n * c->n);
     if (xi_host) std::memcpy(xi_host, c->xi, sizeof(double) * c->n);
     if (w_host) std::memcpy(w_host, c->wq, sizeof(double) * c->n);
+    return NK_OK;
+}
+
+int nk_get_kernel_times(nk_ctx *c, double *ms_host, int64_t *count_host, void *stream)
+{
+    if (!c || !ms_host || !count_host) return NK_ERR_ARG;
+    for (int k = 0; k < NK_K_COUNT; ++k) { ms_host[k] = 0.0; count_host[k] = 0; }
+    NK_CUDA(cudaStreamSynchronize(S(stream)));
+    nk_prof *p = c->prof;
+    if (!p) return NK_OK;
+    for (size_t i = 1; i < p->used; ++i) {
+        const int k = p->cls[i];
+        if (k < 0) continue;
+        float ms = 0.f;
+        NK_CUDA(cudaEventElapsedTime(&ms, p->ev[i - 1], p->ev[i]));
+        ms_host[k] += (double)ms;
+        count_host[k] += 1;
+    }
+    p->used = 0;
     return NK_OK;
 }
 

@@ -23,6 +23,10 @@ enum { NK_EPI_STORE = 0,   // out[0] = total
 #define NK_HIST_MAX 8192               // residual-history capacity of nk_cg_host
 #define NK_CTAB 128                // code & 0x7f indexes ctab[] = 1/multiplicity
 
+// kernel classes of nk_get_kernel_times
+enum { NK_K_AX = 0, NK_K_GS = 1, NK_K_DOT = 2, NK_K_UPDATE_XR = 3, NK_K_UPDATE_P = 4, NK_K_INIT = 5, NK_K_COUNT = 6 };
+struct nk_prof;     // nk_api.cu
+
 struct nk_reduce_ws {
     double *partials;      // NK_MAX_PARTIALS doubles
     unsigned *counter;     // one ticket counter, self-resetting (atomicInc wrap)
@@ -56,9 +60,11 @@ struct nk_ctx {
     int64_t n_unique, n_shared_unique, n_masked_unique;
     int64_t n_rows, n_listed, n_sum_rows, n_sum_listed;
     // options / state
-    int opt_ax_variant, opt_fuse_pap, opt_fuse_p, opt_graph;
+    int opt_ax_variant, opt_fuse_pap, opt_fuse_p, opt_graph, opt_profile;
     int p_pending;               // 1: p = r + beta p has not been applied yet (fuse_p)
     int64_t launches;
+    // per-kernel-class device timing ("profile" option): chained events, interval i = kernel class cls[i]
+    nk_prof *prof;
     // cached graph for nk_cg
     cudaGraphExec_t graph_exec;
     const double *graph_f; double *graph_x; double *graph_hist; int graph_niter; int graph_key;
