@@ -62,8 +62,7 @@ struct LineCfg {
 template <int N>
 __global__ void __launch_bounds__(LineCfg<N>::THREADS)
 ax_line_kernel(double *__restrict__ u_rw, const double *__restrict__ u_ro, const double *__restrict__ r_in,
-               double *__restrict__ w, const double2 *__restrict__ g01, const double2 *__restrict__ g23,
-               const double2 *__restrict__ g45, int64_t E, int dot, nk_reduce_ws red)
+               double *__restrict__ w, const double2 *__restrict__ g, int64_t E, int dot, nk_reduce_ws red)
 {
     using C = LineCfg<N>;
     constexpr int n = C::n, n2 = C::n2, S1 = C::S1, S2 = C::S2, SE = C::SE, EPB = C::EPB;
@@ -137,7 +136,8 @@ ax_line_kernel(double *__restrict__ u_rw, const double *__restrict__ u_ro, const
         }
 #pragma unroll
         for (int k = 0; k < n; ++k) {
-            const double2 ga = g01[gbase + k * n2], gb = g23[gbase + k * n2], gc = g45[gbase + k * n2];
+            const double2 *gk = g + nk_g_index(e, k, 0, t2, n);
+            const double2 ga = gk[0], gb = gk[n2], gc = gk[2 * n2];
             const double ur = sa[pbase + k * S2], us = sb[pbase + k * S2], ut = wt[k];
             sa[pbase + k * S2] = fma(ga.x, ur, fma(ga.y, us, gb.x * ut));   // w_r = rr ur + rs us + rt ut
             sb[pbase + k * S2] = fma(ga.y, ur, fma(gb.y, us, gc.x * ut));   // w_s = rs ur + ss us + st ut
@@ -193,8 +193,7 @@ cudaError_t launch_line(nk_ctx *c, double *u_rw, const double *u_ro, const doubl
     using C = LineCfg<N>;
     const int64_t nb = (c->E + C::EPB - 1) / C::EPB;
     if (dot && nb > NK_MAX_PARTIALS) return cudaErrorInvalidConfiguration;
-    ax_line_kernel<N><<<(unsigned)nb, C::THREADS, C::SMEM, st>>>(u_rw, u_ro, r_in, w, c->g01, c->g23, c->g45,
-                                                                 c->E, dot, c->red);
+    ax_line_kernel<N><<<(unsigned)nb, C::THREADS, C::SMEM, st>>>(u_rw, u_ro, r_in, w, c->g, c->E, dot, c->red);
     c->launches++;
     return cudaGetLastError();
 }
@@ -226,7 +225,7 @@ cudaError_t nk_upload_D_tables(void)
 cudaError_t nk_launch_ax_e(nk_ctx *c, double *u_rw, const double *u_ro, const double *r_in, double *w, int dot,
                            int variant, cudaStream_t st)
 {
-    (void)variant;
+    if (variant != 1) return nk_launch_ax_tma(c, u_rw, u_ro, r_in, w, dot, st);
     switch (c->N) {
 #define NK_CASE(NN) case NN: return launch_line<NN>(c, u_rw, u_ro, r_in, w, dot, st);
         NK_CASE(1) NK_CASE(2) NK_CASE(3) NK_CASE(4) NK_CASE(5) NK_CASE(6) NK_CASE(7) NK_CASE(8)

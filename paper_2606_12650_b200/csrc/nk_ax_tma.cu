@@ -1,0 +1,398 @@
+// nk_ax_tma.cu -- ax_e: w = A_L u, TMA-pipelined persistent kernel for sm_100a (the default variant).
+// ("the action of the Poisson operator", the most expensive kernel; S 8(a) a1, S 8(c) O3;
+// BJ north_star (1).)
+//
+// Why this shape: ax_e moves 64 B per point (u 8, G 48, w 8) for 12(N+1)+15 flops and
+// must run at HBM speed.  The first kernel of this round (nk_ax.cu, one CTA per element batch, load
+// -> compute -> store, one CTA resident per SM) reached 39 % of the copy peak with the fp64 pipe
+// 17 % busy: nothing was in flight while a CTA computed.  Here one persistent CTA per SM splits
+// into
+//   * a producer warp: one lane streams the geometric factors -- 75 % of the bytes -- into a
+//     shared-memory ring with cp.async.bulk (TMA bulk copies, SASS UBLKCP) completing on mbarriers,
+//     k-plane by k-plane, running up to a whole element batch ahead of the arithmetic;
+//   * compute warps: the "line" scheme (every thread owns a whole grid line in each of the three
+//     directions, D entries are compile-time-indexed __constant__ operands of the DFMAs, 16
+//     shared-memory accesses per point) on the batch whose G has landed, while the next batch's
+//     u pencil is already on its way into registers.
+// G never touches registers before it is used and u is read exactly once, so DRAM traffic equals
+// the algorithmic bytes, and the bytes in flight per SM (ring of ~110-170 KB) exceed the ~30 KB
+// that 5.6 TB/s x ~0.8 us of latency asks for.
+//
+//   u_r = D u along r, u_s = D u along s, u_t = D u along t            (3 x (N+1) fma per point)
+//   (w_r, w_s, w_t) = G (u_r, u_s, u_t),  G symmetric 3x3 per point    (15 flops per point)
+//   w = D^T w_r along r + D^T w_s along s + D^T w_t along t            (3 x (N+1) fma per point)
+//
+// Fusions on the CG path (S 8(f) f-1), as in nk_ax.cu:
+//   dot   : sum_l u_l w_l reduced in the same pass (dot-fusion identity), epilogue alpha = rho/pap;
+//   r_in  : p = r + beta p applied while loading (p written back).
+#include "nk_internal.h"
+#include "nk_reduce.cuh"
+
+namespace {
+
+__host__ __device__ constexpr int doff(int n) { int s = 0; for (int q = 2; q < n; ++q) s += q * q; return s; }
+constexpr int D_TOTAL = 2 * doff(17);
+// per order: D (row-major, D[i][m] = l_m'(xi_i)) followed by its transpose, so that both D and D^T
+// lines read their matrix row-wise (16-byte uniform constant loads)
+__constant__ double c_Dt[D_TOTAL];
+
+constexpr int SMEM_CAP = 232448 - 1024;     // 227 KB opt-in limit minus this kernel's static shared memory
+constexpr int BAR_BYTES = 1024;             // 2 x 64 mbarriers
+
+// elements per batch: ~256 compute threads, fewer where shared memory is the limit
+__host__ __device__ constexpr int tma_epb(int n)
+{
+#ifdef NK_TMA_EPB
+    return NK_TMA_EPB;
+#else
+    return n <= 2 ? 32 : n == 3 ? 28 : n == 4 ? 16 : n == 5 ? 10 : n == 6 ? 7 : n == 7 ? 5 : n == 8 ? 4
+         : n == 9 ? 3 : n <= 12 ? 2 : 1;
+#endif
+}
+
+template <int N>
+struct TmaCfg {
+    static constexpr int n = N + 1, n2 = n * n, P = n2 * n;
+    static constexpr int EPB = tma_epb(n);
+    static constexpr int CT = EPB * n2;                       // compute threads in use
+    static constexpr int CW = (CT + 31) / 32;                 // compute warps
+    static constexpr int THREADS = CW * 32 + 32;              // + producer warp
+    static constexpr int S1 = (n & 1) ? n : n + 1;            // odd row stride: conflict-free lines
+    static constexpr int S2 = n * S1, SE = n * S2;            // padded plane / cube (doubles)
+    // a ring stage holds KP k-planes of every element of the batch: whole elements for small n
+    // (one bulk copy per batch), single k-planes otherwise (one bulk copy per element and plane)
+    static constexpr int KP = (n <= 6) ? n : 1;
+    static constexpr int STAGE_D2 = EPB * KP * 3 * n2;        // double2 per stage
+    static constexpr int STAGE_BYTES = STAGE_D2 * 16;
+    static constexpr int SPB = n / KP;                        // stages per batch
+    static constexpr int work_bytes(int nw) { return nw * EPB * SE * 8; }
+    static constexpr int ring_for(int nw) { return (SMEM_CAP - BAR_BYTES - work_bytes(nw)) / STAGE_BYTES; }
+    // three work arrays (4 barriers per batch) if the ring then still holds 1.5 batches, else two
+    static constexpr int NW = (ring_for(3) >= (3 * SPB + 1) / 2) ? 3 : 2;
+    static constexpr int RMAX = ring_for(NW) < 3 * SPB ? ring_for(NW) : 3 * SPB;
+    static constexpr int R = RMAX > 64 ? 64 : RMAX;
+    static constexpr int WORK_BYTES = work_bytes(NW);
+    static constexpr int SMEM = R * STAGE_BYTES + WORK_BYTES + BAR_BYTES;
+    static_assert(R >= 2, "ring too small");
+};
+
+// ---- mbarrier / bulk-copy PTX ---------------------------------------------------------------------
+__device__ __forceinline__ uint32_t smem_u32(const void *p) { return (uint32_t)__cvta_generic_to_shared(p); }
+__device__ __forceinline__ void mbar_init(uint32_t bar, uint32_t count)
+{
+    asm volatile("mbarrier.init.shared::cta.b64 [%0], %1;" ::"r"(bar), "r"(count) : "memory");
+}
+__device__ __forceinline__ void mbar_expect_tx(uint32_t bar, uint32_t bytes)
+{
+    asm volatile("mbarrier.arrive.expect_tx.shared::cta.b64 _, [%0], %1;" ::"r"(bar), "r"(bytes) : "memory");
+}
+__device__ __forceinline__ void mbar_arrive(uint32_t bar)
+{
+    asm volatile("mbarrier.arrive.shared::cta.b64 _, [%0];" ::"r"(bar) : "memory");
+}
+__device__ __forceinline__ void mbar_wait(uint32_t bar, uint32_t parity)
+{
+    asm volatile(
+        "{\n"
+        ".reg .pred P1;\n"
+        "NK_WAIT:\n"
+        "mbarrier.try_wait.parity.shared::cta.b64 P1, [%0], %1;\n"
+        "@P1 bra NK_DONE;\n"
+        "bra NK_WAIT;\n"
+        "NK_DONE:\n"
+        "}\n" ::"r"(bar), "r"(parity) : "memory");
+}
+// global -> shared bulk copy (TMA, 1-D), completes `bytes` on the mbarrier; 16-byte aligned, size % 16 == 0
+__device__ __forceinline__ void bulk_g2s(uint32_t dst, const void *src, uint32_t bytes, uint32_t bar)
+{
+    asm volatile("cp.async.bulk.shared::cluster.global.mbarrier::complete_tx::bytes [%0], [%1], %2, [%3];"
+                 ::"r"(dst), "l"(src), "r"(bytes), "r"(bar) : "memory");
+}
+template <int COUNT>
+__device__ __forceinline__ void compute_sync()     // named barrier 1: the compute warps only
+{
+    asm volatile("bar.sync 1, %0;" ::"n"(COUNT) : "memory");
+}
+
+// One grid line through the n x n matrix M stored row-major at c_Dt[MOFF]: out_i = sum_m M[i][m] ln[m].
+// D is centro-antisymmetric (D[i][m] = -D[n-1-i][n-1-m], GLL nodes are symmetric), and so is D^T, so
+// one constant operand M[i][m] feeds two DFMAs: out_i += M[i][m] ln[m] and out_{n-1-i} += M[i][m] (-ln[n-1-m]).
+// IB rows advance together: 2 IB independent DFMA chains per thread, every M entry a compile-time-
+// indexed __constant__ operand (uniform datapath: no vector registers, no shared-memory traffic).
+template <int n, int MOFF, class Store>
+__device__ __forceinline__ void line_apply(const double (&ln)[n], Store store)
+{
+    constexpr int IB = 2, H = (n + 1) / 2;
+#pragma unroll
+    for (int i0 = 0; i0 < H; i0 += IB) {
+        double accA[IB], accB[IB];
+#pragma unroll
+        for (int j = 0; j < IB; ++j)
+            if (i0 + j < H) {
+                const double d = c_Dt[MOFF + (i0 + j) * n];
+                accA[j] = d * ln[0];
+                accB[j] = d * -ln[n - 1];
+            }
+#pragma unroll
+        for (int m = 1; m < n; ++m) {
+#pragma unroll
+            for (int j = 0; j < IB; ++j)
+                if (i0 + j < H) {
+                    const double d = c_Dt[MOFF + (i0 + j) * n + m];
+                    accA[j] = fma(d, ln[m], accA[j]);
+                    accB[j] = fma(d, -ln[n - 1 - m], accB[j]);
+                }
+        }
+#pragma unroll
+        for (int j = 0; j < IB; ++j)
+            if (i0 + j < H) {
+                store(i0 + j, accA[j]);
+                if (n - 1 - (i0 + j) != i0 + j) store(n - 1 - (i0 + j), accB[j]);
+            }
+    }
+}
+
+template <int N, bool FUSEP>
+__global__ void __launch_bounds__(TmaCfg<N>::THREADS, 1)
+ax_tma_kernel(double *__restrict__ u_rw, const double *__restrict__ u_ro, const double *__restrict__ r_in,
+              double *__restrict__ w, const double2 *__restrict__ g, int64_t E, int dot, nk_reduce_ws red)
+{
+    using C = TmaCfg<N>;
+    constexpr int n = C::n, n2 = C::n2, P = C::P, S1 = C::S1, S2 = C::S2, SE = C::SE, EPB = C::EPB;
+    constexpr int R = C::R, KP = C::KP, NW = C::NW, CW = C::CW, CTHREADS = C::CW * 32;
+    constexpr int DOFF = 2 * doff(n), TOFF = DOFF + n * n;     // D and D^T in c_Dt
+    extern __shared__ __align__(128) unsigned char smem_raw[];
+    __shared__ double s_red[33];
+    const double2 *ring = reinterpret_cast<const double2 *>(smem_raw);
+    double *work = reinterpret_cast<double *>(smem_raw + (size_t)R * C::STAGE_BYTES);
+    const uint32_t ring0 = smem_u32(smem_raw);
+    const uint32_t full0 = ring0 + R * C::STAGE_BYTES + C::WORK_BYTES, empty0 = full0 + 8 * R;
+
+    const int tid = threadIdx.x;
+    if (tid == 0) {
+        for (int s = 0; s < R; ++s) { mbar_init(full0 + 8 * s, 1); mbar_init(empty0 + 8 * s, CW); }
+        asm volatile("fence.mbarrier_init.release.cluster;" ::: "memory");
+    }
+    __syncthreads();
+
+    const int64_t nb = (E + EPB - 1) / EPB;
+    const int nit = (nb > (int64_t)blockIdx.x) ? (int)((nb - blockIdx.x + gridDim.x - 1) / gridDim.x) : 0;
+    double dsum = 0.0;
+
+    if (tid >= CTHREADS) {
+        // ---- producer warp: one lane streams G into the ring ----------------------------------------
+        if (tid == CTHREADS) {
+            int stage = 0;
+            uint32_t phase = 0;
+            for (int it = 0; it < nit; ++it) {
+                const int64_t e0 = ((int64_t)blockIdx.x + (int64_t)it * gridDim.x) * EPB;
+                const int ne = (int)((E - e0 < EPB) ? (E - e0) : EPB);
+#pragma unroll 1
+                for (int ks = 0; ks < C::SPB; ++ks) {
+                    mbar_wait(empty0 + 8 * stage, phase ^ 1u);
+                    const uint32_t fb = full0 + 8 * stage, dst = ring0 + stage * C::STAGE_BYTES;
+                    if (KP == n) {       // whole elements: the batch is one contiguous chunk
+                        mbar_expect_tx(fb, (uint32_t)ne * P * 48);
+                        bulk_g2s(dst, g + nk_g_index(e0, 0, 0, 0, n), (uint32_t)ne * P * 48, fb);
+                    } else {             // one k-plane of every element of the batch
+                        mbar_expect_tx(fb, (uint32_t)ne * n2 * 48);
+                        for (int q = 0; q < ne; ++q)
+                            bulk_g2s(dst + q * n2 * 48, g + nk_g_index(e0 + q, ks, 0, 0, n), n2 * 48, fb);
+                    }
+                    if (++stage == R) { stage = 0; phase ^= 1u; }
+                }
+            }
+        }
+    } else {
+        // ---- compute warps ----------------------------------------------------------------------------
+        // No arithmetic below sits under a thread-dependent branch: D reaches the DFMAs through the
+        // uniform datapath (LDCU -> UR operand), which ptxas only uses in warp-uniform code.  Threads
+        // without an element (ragged last warp, tail batch) compute on stale shared memory and only
+        // their stores are predicated off.
+        const int lane = tid & 31;
+        const int slot = tid / n2;
+        const int t2 = tid - slot * n2;
+        const int a = t2 % n, b = t2 / n;
+        const bool mapped = slot < EPB;
+        double *sA = work + (size_t)(mapped ? slot : 0) * NW * SE;     // u, then (NW = 2) the s direction
+        double *sB = sA + SE;                                          // r direction
+        double *sC = (NW == 3) ? sB + SE : sA;                         // s direction
+        const int pbase = a + b * S1;                   // pencil (i,j) = (a,b): + k*S2
+        const int rbase = (a + n * b) * S1;             // row (j,k) = (a,b): + i
+        const int cbase = a + b * S2;                   // column (i,k) = (a,b): + j*S1
+        const double2 *gslot = ring + (mapped ? slot : 0) * KP * 3 * n2 + t2;
+        const double beta = FUSEP ? red.scal[NK_S_BETA] : 0.0;
+        int stage = 0;
+        uint32_t phase = 0;
+
+        double nu[n], nr[FUSEP ? n : 1];               // next batch's pencil, in flight
+        {
+            const int64_t e = (int64_t)blockIdx.x * EPB + slot;
+            const bool act = mapped && nit > 0 && e < E;
+            const int64_t gb = act ? e * P + t2 : 0;
+#pragma unroll
+            for (int k = 0; k < n; ++k) {
+                nu[k] = act ? (FUSEP ? u_rw[gb + k * n2] : u_ro[gb + k * n2]) : 0.0;
+                if (FUSEP) nr[k] = act ? r_in[gb + k * n2] : 0.0;
+            }
+        }
+        for (int it = 0; it < nit; ++it) {
+            const int64_t e = ((int64_t)blockIdx.x + (int64_t)it * gridDim.x) * EPB + slot;
+            const bool active = mapped && e < E;
+            const int64_t gbase = e * P + t2;
+            double ru[n];
+            // P1: pencil -> padded cube (and p = r + beta p written back)
+#pragma unroll
+            for (int k = 0; k < n; ++k) ru[k] = FUSEP ? fma(beta, nu[k], nr[k]) : nu[k];
+            if (mapped) {
+#pragma unroll
+                for (int k = 0; k < n; ++k) sA[pbase + k * S2] = ru[k];
+            }
+            if (FUSEP && active) {
+#pragma unroll
+                for (int k = 0; k < n; ++k) u_rw[gbase + k * n2] = ru[k];
+            }
+            compute_sync<CTHREADS>();
+            // P2: r derivative along rows (A -> B), s derivative along columns (A -> C)
+            {
+                double ln[n];
+#pragma unroll
+                for (int m = 0; m < n; ++m) ln[m] = sA[rbase + m];
+                line_apply<n, DOFF>(ln, [&](int i, double v) { if (mapped) sB[rbase + i] = v; });
+            }
+            if (NW == 2) {
+                double ln[n];                           // columns overwrite A in place: read, barrier, write
+#pragma unroll
+                for (int m = 0; m < n; ++m) ln[m] = sA[cbase + m * S1];
+                compute_sync<CTHREADS>();
+                line_apply<n, DOFF>(ln, [&](int j, double v) { if (mapped) sC[cbase + j * S1] = v; });
+            } else {
+                double ln[n];
+#pragma unroll
+                for (int m = 0; m < n; ++m) ln[m] = sA[cbase + m * S1];
+                line_apply<n, DOFF>(ln, [&](int j, double v) { if (mapped) sC[cbase + j * S1] = v; });
+            }
+            compute_sync<CTHREADS>();
+            // P3: t derivative in registers; G from the ring; t transpose in registers
+            double rw[n];
+            {
+                double wt[n];
+                line_apply<n, DOFF>(ru, [&](int k, double v) { wt[k] = v; });
+#pragma unroll
+                for (int k = 0; k < n; ++k) {
+                    if (k % KP == 0) mbar_wait(full0 + 8 * stage, phase);
+                    const double2 *gs = gslot + (size_t)stage * C::STAGE_D2 + (k % KP) * 3 * n2;
+                    const double2 ga = gs[0], gb = gs[n2], gc = gs[2 * n2];
+                    const double ur = sB[pbase + k * S2], us = sC[pbase + k * S2], ut = wt[k];
+                    const double wr = fma(ga.x, ur, fma(ga.y, us, gb.x * ut));          // w_r = rr ur + rs us + rt ut
+                    const double ws = fma(ga.y, ur, fma(gb.y, us, gc.x * ut));          // w_s = rs ur + ss us + st ut
+                    const double wk = fma(gb.x, ur, fma(gc.x, us, gc.y * ut));          // w_t = rt ur + st us + tt ut
+                    if (mapped) {
+                        sB[pbase + k * S2] = wr;
+                        sC[pbase + k * S2] = ws;
+                    }
+                    wt[k] = wk;
+                    // <u, A_L u> = sum over points of grad(u)^T G grad(u): the fused pap needs no u later on
+                    dsum += active ? fma(ur, wr, fma(us, ws, ut * wk)) : 0.0;
+                    if (k % KP == KP - 1) {          // this warp is done with the stage: hand it back
+                        __syncwarp();
+                        if (lane == 0) mbar_arrive(empty0 + 8 * stage);
+                        if (++stage == R) { stage = 0; phase ^= 1u; }
+                    }
+                }
+                line_apply<n, TOFF>(wt, [&](int m, double v) { rw[m] = v; });
+            }
+            compute_sync<CTHREADS>();
+            {   // prefetch the next batch's pencil: issued after P3, where register pressure peaks (the
+                // register file is split four ways, so > 8 warps means <= 168 registers per thread);
+                // in flight through P4 and P5
+                const int64_t e1 = e + (int64_t)gridDim.x * EPB;
+                const bool act = mapped && it + 1 < nit && e1 < E;
+                const int64_t gb = act ? e1 * P + t2 : 0;
+#pragma unroll
+                for (int k = 0; k < n; ++k) {
+                    nu[k] = act ? (FUSEP ? u_rw[gb + k * n2] : u_ro[gb + k * n2]) : 0.0;
+                    if (FUSEP) nr[k] = act ? r_in[gb + k * n2] : 0.0;
+                }
+            }
+            // P4: D^T along rows (B in place) and columns (C in place)
+            {
+                double ln[n];
+#pragma unroll
+                for (int m = 0; m < n; ++m) ln[m] = sB[rbase + m];
+                line_apply<n, TOFF>(ln, [&](int i, double v) { if (mapped) sB[rbase + i] = v; });
+#pragma unroll
+                for (int m = 0; m < n; ++m) ln[m] = sC[cbase + m * S1];
+                line_apply<n, TOFF>(ln, [&](int j, double v) { if (mapped) sC[cbase + j * S1] = v; });
+            }
+            compute_sync<CTHREADS>();
+            // P5: sum the three directions, store
+#pragma unroll
+            for (int k = 0; k < n; ++k) {
+                const double wv = rw[k] + (sB[pbase + k * S2] + sC[pbase + k * S2]);
+                if (active) w[gbase + k * n2] = wv;
+            }
+            if (NW == 2) compute_sync<CTHREADS>();      // next P1 writes A, which P5 still reads as C
+        }
+    }
+    if (dot) nk_grid_reduce(dsum, s_red, red, NK_EPI_PAP, nullptr);
+}
+
+template <int N>
+cudaError_t launch_tma(nk_ctx *c, double *u_rw, const double *u_ro, const double *r_in, double *w, int dot,
+                       cudaStream_t st)
+{
+    using C = TmaCfg<N>;
+    const int64_t nb = (c->E + C::EPB - 1) / C::EPB;
+    const unsigned grid = (unsigned)(nb < (int64_t)c->sm_count ? nb : (int64_t)c->sm_count);   // one CTA per SM
+    if (r_in != nullptr)
+        ax_tma_kernel<N, true><<<grid, C::THREADS, C::SMEM, st>>>(u_rw, nullptr, r_in, w, c->g, c->E, dot, c->red);
+    else
+        ax_tma_kernel<N, false><<<grid, C::THREADS, C::SMEM, st>>>(nullptr, u_ro, nullptr, w, c->g, c->E, dot, c->red);
+    c->launches++;
+    return cudaGetLastError();
+}
+
+template <int N>
+cudaError_t prepare_tma()
+{
+    cudaError_t e = cudaFuncSetAttribute(ax_tma_kernel<N, true>, cudaFuncAttributeMaxDynamicSharedMemorySize,
+                                         TmaCfg<N>::SMEM);
+    if (e != cudaSuccess) return e;
+    return cudaFuncSetAttribute(ax_tma_kernel<N, false>, cudaFuncAttributeMaxDynamicSharedMemorySize,
+                                TmaCfg<N>::SMEM);
+}
+
+}  // namespace
+
+cudaError_t nk_upload_D_tables_tma(void)
+{
+    static double h[D_TOTAL];
+    double xi[16], wq[16];
+    for (int N = 1; N <= NK_MAX_ORDER; ++N) {
+        const int n = N + 1;
+        double *D = h + 2 * doff(n), *T = D + n * n;
+        nk_host_basis(N, xi, wq, D);
+        for (int i = 0; i < n; ++i)
+            for (int m = 0; m < n; ++m) T[i * n + m] = D[m * n + i];
+    }
+    cudaError_t e = cudaMemcpyToSymbol(c_Dt, h, sizeof(h));
+    if (e != cudaSuccess) return e;
+#define NK_CASE(NN) if ((e = prepare_tma<NN>()) != cudaSuccess) return e;
+    NK_CASE(1) NK_CASE(2) NK_CASE(3) NK_CASE(4) NK_CASE(5) NK_CASE(6) NK_CASE(7) NK_CASE(8)
+    NK_CASE(9) NK_CASE(10) NK_CASE(11) NK_CASE(12) NK_CASE(13) NK_CASE(14) NK_CASE(15)
+#undef NK_CASE
+    return cudaSuccess;
+}
+
+cudaError_t nk_launch_ax_tma(nk_ctx *c, double *u_rw, const double *u_ro, const double *r_in, double *w, int dot,
+                             cudaStream_t st)
+{
+    switch (c->N) {
+#define NK_CASE(NN) case NN: return launch_tma<NN>(c, u_rw, u_ro, r_in, w, dot, st);
+        NK_CASE(1) NK_CASE(2) NK_CASE(3) NK_CASE(4) NK_CASE(5) NK_CASE(6) NK_CASE(7) NK_CASE(8)
+        NK_CASE(9) NK_CASE(10) NK_CASE(11) NK_CASE(12) NK_CASE(13) NK_CASE(14) NK_CASE(15)
+#undef NK_CASE
+    }
+    return cudaErrorInvalidValue;
+}

@@ -7,8 +7,8 @@
 // first node (D annihilates constants; the subtraction of nearby numbers is exact or 1 ulp of the
 // small difference).  With inverse metrics = cofactors / J:
 //   G_ab = w3 * (cof_a . cof_b) / J,   cof_r = (x_s x x_t), cof_s = (x_t x x_r), cof_t = (x_r x x_s).
-// Output: three double2 planes (rr,rs) (rt,ss) (st,tt) -- always 16-byte aligned per point, also
-// for odd (N+1)^3 (S 7 hard part 5).  One block per element; run once, not on the timed path.
+// Output: double2 pairs (rr,rs) (rt,ss) (st,tt) in the layout of nk_g_index() -- always 16-byte
+// aligned per point, also for odd (N+1)^3 (S 7 hard part 5).  One block per element; run once, not on the timed path.
 #include "nk_internal.h"
 
 namespace {
@@ -17,8 +17,7 @@ constexpr int GEOM_THREADS = 256;
 
 __global__ void __launch_bounds__(GEOM_THREADS)
 geom_kernel(const double *__restrict__ coords, const double *__restrict__ Dg, const double *__restrict__ wq,
-            int n, int64_t L, double2 *__restrict__ g01, double2 *__restrict__ g23,
-            double2 *__restrict__ g45, int *__restrict__ errflag)
+            int n, int64_t L, double2 *__restrict__ g, int *__restrict__ errflag)
 {
     __shared__ double s_D[16 * 16];
     __shared__ double s_w[16];
@@ -53,21 +52,25 @@ geom_kernel(const double *__restrict__ coords, const double *__restrict__ Dg, co
         const double gss = sc * (sx * sx + sy * sy + sz * sz);
         const double gst = sc * (sx * tx + sy * ty + sz * tz);
         const double gtt = sc * (tx * tx + ty * ty + tz * tz);
-        g01[base + q] = make_double2(grr, grs);
-        g23[base + q] = make_double2(grt, gss);
-        g45[base + q] = make_double2(gst, gtt);
+        const int t2 = i + n * j;
+        g[nk_g_index(blockIdx.x, k, 0, t2, n)] = make_double2(grr, grs);
+        g[nk_g_index(blockIdx.x, k, 1, t2, n)] = make_double2(grt, gss);
+        g[nk_g_index(blockIdx.x, k, 2, t2, n)] = make_double2(gst, gtt);
     }
     if (bad) atomicOr(errflag, 1);
 }
 
 // rr|rs|rt|ss|st|tt planes of L for nk_get_geom
 __global__ void __launch_bounds__(GEOM_THREADS)
-unpack_geom_kernel(const double2 *__restrict__ g01, const double2 *__restrict__ g23,
-                   const double2 *__restrict__ g45, double *__restrict__ G6, int64_t L)
+unpack_geom_kernel(const double2 *__restrict__ g, double *__restrict__ G6, int64_t L, int n)
 {
     const int64_t stride = (int64_t)gridDim.x * blockDim.x;
+    const int n2 = n * n, P = n2 * n;
     for (int64_t l = (int64_t)blockIdx.x * blockDim.x + threadIdx.x; l < L; l += stride) {
-        const double2 a = g01[l], b = g23[l], c = g45[l];
+        const int64_t e = l / P;
+        const int q = (int)(l - e * P), k = q / n2, t2 = q - k * n2;
+        const double2 a = g[nk_g_index(e, k, 0, t2, n)], b = g[nk_g_index(e, k, 1, t2, n)],
+                      c = g[nk_g_index(e, k, 2, t2, n)];
         G6[l] = a.x; G6[L + l] = a.y; G6[2 * L + l] = b.x;
         G6[3 * L + l] = b.y; G6[4 * L + l] = c.x; G6[5 * L + l] = c.y;
     }
@@ -78,8 +81,7 @@ unpack_geom_kernel(const double2 *__restrict__ g01, const double2 *__restrict__ 
 cudaError_t nk_launch_geom(nk_ctx *c, const double *coords_dev, const double *D_dev, const double *wq_dev,
                            cudaStream_t st)
 {
-    geom_kernel<<<(unsigned)c->E, GEOM_THREADS, 0, st>>>(coords_dev, D_dev, wq_dev, c->n, c->L, c->g01, c->g23,
-                                                         c->g45, c->errflag);
+    geom_kernel<<<(unsigned)c->E, GEOM_THREADS, 0, st>>>(coords_dev, D_dev, wq_dev, c->n, c->L, c->g, c->errflag);
     c->launches++;
     return cudaGetLastError();
 }
@@ -88,7 +90,7 @@ cudaError_t nk_launch_get_geom(nk_ctx *c, double *G6, cudaStream_t st)
 {
     int64_t nb = (c->L + GEOM_THREADS - 1) / GEOM_THREADS;
     if (nb > (int64_t)c->sm_count * 32) nb = (int64_t)c->sm_count * 32;
-    unpack_geom_kernel<<<(unsigned)nb, GEOM_THREADS, 0, st>>>(c->g01, c->g23, c->g45, G6, c->L);
+    unpack_geom_kernel<<<(unsigned)nb, GEOM_THREADS, 0, st>>>(c->g, G6, c->L, c->n);
     c->launches++;
     return cudaGetLastError();
 }

@@ -27,6 +27,14 @@ enum { NK_EPI_STORE = 0,   // out[0] = total
 enum { NK_K_AX = 0, NK_K_GS = 1, NK_K_DOT = 2, NK_K_UPDATE_XR = 3, NK_K_UPDATE_P = 4, NK_K_INIT = 5, NK_K_COUNT = 6 };
 struct nk_prof;     // nk_api.cu
 
+// Layout of the geometric factors in HBM: G[e][k][c2][t2] as double2, c2 = 0 (rr,rs),
+// 1 (rt,ss), 2 (st,tt), t2 = i + n j.  One element is one contiguous 48 P-byte chunk and one k-plane
+// of it a contiguous 48 n^2-byte chunk, always 16-byte aligned: the unit a TMA bulk copy moves.
+__host__ __device__ __forceinline__ int64_t nk_g_index(int64_t e, int k, int c2, int t2, int n)
+{
+    return ((e * n + k) * 3 + c2) * (int64_t)(n * n) + t2;
+}
+
 struct nk_reduce_ws {
     double *partials;      // NK_MAX_PARTIALS doubles
     unsigned *counter;     // one ticket counter, self-resetting (atomicInc wrap)
@@ -43,7 +51,8 @@ struct nk_ctx {
     // workspace carve-up (all DEVICE)
     void *ws;
     size_t ws_bytes;
-    double2 *g01, *g23, *g45;    // geometric factors as three double2 planes: (rr,rs) (rt,ss) (st,tt)
+    double2 *g;                  // geometric factors, 3 L double2, layout nk_g_index(): per element and
+                                 // k-plane one contiguous chunk [c2][i + n j] of (rr,rs) (rt,ss) (st,tt)
     double *r, *p, *w;           // CG state, L each (coords staging aliases these during set-up)
     double *hf, *hx;             // staging for nk_cg_host, L each
     uint8_t *code;               // L: multiplicity-table index | NK_CODE_MASKED
@@ -78,6 +87,10 @@ void nk_host_basis(int N, double *xi, double *w, double *D);
 cudaError_t nk_launch_ax_e(nk_ctx *c, double *u_rw, const double *u_ro, const double *r_in, double *w,
                            int dot, int variant, cudaStream_t st);
 cudaError_t nk_upload_D_tables(void);
+// nk_ax_tma.cu : same contract, TMA-pipelined persistent kernel (the default variant)
+cudaError_t nk_launch_ax_tma(nk_ctx *c, double *u_rw, const double *u_ro, const double *r_in, double *w,
+                             int dot, cudaStream_t st);
+cudaError_t nk_upload_D_tables_tma(void);
 // nk_geom.cu
 cudaError_t nk_launch_geom(nk_ctx *c, const double *coords_dev, const double *D_dev,
                            const double *wq_dev, cudaStream_t st);

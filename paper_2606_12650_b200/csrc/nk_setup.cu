@@ -134,6 +134,7 @@ int setup_impl(nk_ctx *c, const double *coords, const int64_t *glo_num, const do
     double *coords_dev = c->r;
     NK_CUDA(cudaMemcpyAsync(coords_dev, coords, 3 * (size_t)L * sizeof(double), cudaMemcpyHostToDevice, st));
     NK_CUDA(nk_upload_D_tables());
+    NK_CUDA(nk_upload_D_tables_tma());
     NK_CUDA(nk_launch_geom(c, coords_dev, D_dev, wq_dev, st));
     int err = 0;
     NK_CUDA(cudaMemcpyAsync(&err, c->errflag, sizeof(int), cudaMemcpyDeviceToHost, st));
@@ -166,9 +167,7 @@ extern "C" int nk_setup(nk_ctx **ctx, int64_t E, int N, const double *coords, co
     c->opt_fuse_pap = 1; c->opt_fuse_p = 1;
     nk_host_basis(N, c->xi, c->wq, c->D);
     char *q = static_cast<char *>(workspace);
-    c->g01 = reinterpret_cast<double2 *>(q); q += cv.g;
-    c->g23 = reinterpret_cast<double2 *>(q); q += cv.g;
-    c->g45 = reinterpret_cast<double2 *>(q); q += cv.g;
+    c->g = reinterpret_cast<double2 *>(q); q += cv.g;
     c->r = reinterpret_cast<double *>(q); q += cv.vec;
     c->p = reinterpret_cast<double *>(q); q += cv.vec;
     c->w = reinterpret_cast<double *>(q); q += cv.vec;
