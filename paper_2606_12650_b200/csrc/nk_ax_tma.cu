@@ -90,17 +90,28 @@ __device__ __forceinline__ void mbar_arrive(uint32_t bar)
 {
     asm volatile("mbarrier.arrive.shared::cta.b64 _, [%0];" ::"r"(bar) : "memory");
 }
-__device__ __forceinline__ void mbar_wait(uint32_t bar, uint32_t parity)
+__device__ __forceinline__ uint32_t mbar_try_wait(uint32_t bar, uint32_t parity)
 {
+    uint32_t done;
     asm volatile(
         "{\n"
         ".reg .pred P1;\n"
-        "NK_WAIT:\n"
-        "mbarrier.try_wait.parity.shared::cta.b64 P1, [%0], %1;\n"
-        "@P1 bra NK_DONE;\n"
-        "bra NK_WAIT;\n"
-        "NK_DONE:\n"
-        "}\n" ::"r"(bar), "r"(parity) : "memory");
+        "mbarrier.try_wait.parity.shared::cta.b64 P1, [%1], %2;\n"
+        "selp.u32 %0, 1, 0, P1;\n"
+        "}\n" : "=r"(done) : "r"(bar), "r"(parity) : "memory");
+    return done;
+}
+// Producer lane: plain spin.
+__device__ __forceinline__ void mbar_wait(uint32_t bar, uint32_t parity)
+{
+    while (!mbar_try_wait(bar, parity)) {}
+}
+// Compute warps: every lane probes (each needs the acquire), the loop branch is a warp vote.  A
+// per-thread spin would leave ptxas unable to prove the warp converged afterwards, and all D
+// operands behind it would fall off the uniform datapath (LDC into vector registers, not LDCU).
+__device__ __forceinline__ void mbar_wait_warp(uint32_t bar, uint32_t parity)
+{
+    while (!__all_sync(0xffffffffu, mbar_try_wait(bar, parity))) {}
 }
 // global -> shared bulk copy (TMA, 1-D), completes `bytes` on the mbarrier; 16-byte aligned, size % 16 == 0
 __device__ __forceinline__ void bulk_g2s(uint32_t dst, const void *src, uint32_t bytes, uint32_t bar)
@@ -280,7 +291,7 @@ ax_tma_kernel(double *__restrict__ u_rw, const double *__restrict__ u_ro, const 
                 line_apply<n, DOFF>(ru, [&](int k, double v) { wt[k] = v; });
 #pragma unroll
                 for (int k = 0; k < n; ++k) {
-                    if (k % KP == 0) mbar_wait(full0 + 8 * stage, phase);
+                    if (k % KP == 0) mbar_wait_warp(full0 + 8 * stage, phase);
                     const double2 *gs = gslot + (size_t)stage * C::STAGE_D2 + (k % KP) * 3 * n2;
                     const double2 ga = gs[0], gb = gs[n2], gc = gs[2 * n2];
                     const double ur = sB[pbase + k * S2], us = sC[pbase + k * S2], ut = wt[k];
