@@ -363,7 +363,7 @@ def main():
     ap.add_argument("--impl", default="ours", choices=["ours", "reference"])
     ap.add_argument("--workload", default="config5", choices=["config1", "config2", "config3", "config5"])
     ap.add_argument("--fuse-pap", type=int, default=1)
-    ap.add_argument("--fuse-p", type=int, default=1)
+    ap.add_argument("--fuse-p", type=int, default=0)
     ap.add_argument("--graph", type=int, default=0)
     ap.add_argument("--traffic", type=float, default=None,
                     help="dram bytes per ax_e launch from the committed ncu --set full capture (profiles/)")

@@ -102,7 +102,7 @@ int nk_get_scalars(nk_ctx *ctx, double *out5_host, void *stream);
  *                  2 = slab kernel (2-D slab, k loop, D rows in registers)
  *   "fuse_pap"     1 (default) = pap accumulated inside ax_e through the dot-fusion identity
  *                  <M QQ^T A_L p, p>_c = sum_l (A_L p)_l p_l; 0 = separate weighted dot after gs
- *   "fuse_p"       1 (default) = p = r + beta p folded into the load of the next ax_e; 0 = own kernel
+ *   "fuse_p"       1 = p = r + beta p folded into the load of the next ax_e; 0 (default) = own kernel
  *   "graph"        1 = nk_cg records its launches into a CUDA graph and replays it
  *   "profile"      1 = record a CUDA event on `stream` between consecutive launches so that
  *                  nk_get_kernel_times can report device time per kernel class (nk_cg then
