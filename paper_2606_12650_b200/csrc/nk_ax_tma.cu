@@ -30,12 +30,22 @@
 
 namespace {
 
-__host__ __device__ constexpr int doff(int n) { int s = 0; for (int q = 2; q < n; ++q) s += q * q; return s; }
-constexpr int D_TOTAL = 2 * doff(17);
-// per order: D (row-major, D[i][m] = l_m'(xi_i)) followed by its transpose, so that both D and D^T
-// lines read their matrix row-wise (16-byte uniform constant loads)
+// Even-odd tables.  D and D^T are centro-antisymmetric (M[n-1-i][n-1-m] = -M[i][m]: the GLL
+// nodes are symmetric), so with e_m = v_m + v_{n-1-m}, o_m = v_m - v_{n-1-m}, h = floor(n/2), H = ceil(n/2):
+//   S_i = sum_{m<h} Me[i][m] e_m (+ M[i][mid] v_mid, n odd),   Me[i][m] = (M[i][m] + M[i][n-1-m]) / 2
+//   A_i = sum_{m<h} Mo[i][m] o_m,                               Mo[i][m] = (M[i][m] - M[i][n-1-m]) / 2
+//   (M v)_i = A_i + S_i,   (M v)_{n-1-i} = A_i - S_i            for i < H
+// -- n^2/2 DFMAs and 2n DADDs per grid line instead of n^2 DFMAs.  Per order n and per matrix (D, then
+// D^T) the table holds H rows of [Mo[i][0..h) | Me[i][0..h) (, M[i][mid])].
+__host__ __device__ constexpr int eo_row(int n) { return n / 2 + (n + 1) / 2; }
+__host__ __device__ constexpr int eo_mat(int n) { return (n + 1) / 2 * eo_row(n); }
+__host__ __device__ constexpr int eo_off(int n) { int s = 0; for (int q = 2; q < n; ++q) s += 2 * eo_mat(q); return s; }
+constexpr int D_TOTAL = eo_off(17);
 __constant__ double c_Dt[D_TOTAL];
 
+#ifndef NK_TMA_KG
+#define NK_TMA_KG 1
+#endif
 constexpr int SMEM_CAP = 232448 - 1024;     // 227 KB opt-in limit minus this kernel's static shared memory
 constexpr int BAR_BYTES = 1024;             // 2 x 64 mbarriers
 
@@ -54,9 +64,17 @@ template <int N>
 struct TmaCfg {
     static constexpr int n = N + 1, n2 = n * n, P = n2 * n;
     static constexpr int EPB = tma_epb(n);
-    static constexpr int CT = EPB * n2;                       // compute threads in use
-    static constexpr int CW = (CT + 31) / 32;                 // compute warps
-    static constexpr int THREADS = CW * 32 + 32;              // + producer warp
+    // Sync groups: the element slots of a batch that share one named barrier.  From n^2 >= 64 on every
+    // slot is its own group of whole warps, so the elements of a batch drift apart and the
+    // shared-memory-bound phases of one overlap the DFMA-bound phases of the other.
+    static constexpr int SG = (n == 8 || n == 10 || n == 11 || n == 16) ? 1 : EPB;   // slots per group
+    // (only where a slot fills whole warps well; elsewhere per-slot groups cost a warp and registers)
+    static constexpr int NG = EPB / SG;                       // groups
+    static constexpr int GTH = (SG * n2 + 31) / 32 * 32;      // threads per group
+    static constexpr int CT = NG * GTH;                       // compute threads
+    static constexpr int CW = CT / 32;                        // compute warps
+    static constexpr int THREADS = CT + 32;                   // + producer warp
+    static_assert(EPB % SG == 0 && NG <= 15, "sync groups");
     static constexpr int S1 = (n & 1) ? n : n + 1;            // odd row stride: conflict-free lines
     static constexpr int S2 = n * S1, SE = n * S2;            // padded plane / cube (doubles)
     // a ring stage holds KP k-planes of every element of the batch: whole elements for small n
@@ -120,45 +138,55 @@ __device__ __forceinline__ void bulk_g2s(uint32_t dst, const void *src, uint32_t
                  ::"r"(dst), "l"(src), "r"(bytes), "r"(bar) : "memory");
 }
 template <int COUNT>
-__device__ __forceinline__ void compute_sync()     // named barrier 1: the compute warps only
+__device__ __forceinline__ void group_sync(int grp)     // named barrier 1 + grp: one sync group's warps
 {
-    asm volatile("bar.sync 1, %0;" ::"n"(COUNT) : "memory");
+    asm volatile("bar.sync %0, %1;" ::"r"(grp + 1), "n"(COUNT) : "memory");
 }
 
-// One grid line through the n x n matrix M stored row-major at c_Dt[MOFF]: out_i = sum_m M[i][m] ln[m].
-// D is centro-antisymmetric (D[i][m] = -D[n-1-i][n-1-m], GLL nodes are symmetric), and so is D^T, so
-// one constant operand M[i][m] feeds two DFMAs: out_i += M[i][m] ln[m] and out_{n-1-i} += M[i][m] (-ln[n-1-m]).
-// IB rows advance together: 2 IB independent DFMA chains per thread, every M entry a compile-time-
-// indexed __constant__ operand (uniform datapath: no vector registers, no shared-memory traffic).
+// One grid line through M = D (MOFF = DOFF) or D^T (MOFF = TOFF): out_i = sum_m M[i][m] ln[m], by the
+// even-odd splitting above.  IB rows advance together (2 IB independent DFMA chains per thread); every
+// table entry is a compile-time-indexed __constant__ operand (uniform datapath: LDCU -> UR).
 template <int n, int MOFF, class Store>
 __device__ __forceinline__ void line_apply(const double (&ln)[n], Store store)
 {
-    constexpr int IB = 2, H = (n + 1) / 2;
+    constexpr int IB = 2, h = n / 2, H = (n + 1) / 2, ROW = eo_row(n);
+    double ev[H], od[h > 0 ? h : 1];
+#pragma unroll
+    for (int m = 0; m < h; ++m) {
+        ev[m] = ln[m] + ln[n - 1 - m];
+        od[m] = ln[m] - ln[n - 1 - m];
+    }
+    if (n & 1) ev[H - 1] = ln[H - 1];
 #pragma unroll
     for (int i0 = 0; i0 < H; i0 += IB) {
-        double accA[IB], accB[IB];
+        double S[IB], A[IB];
 #pragma unroll
         for (int j = 0; j < IB; ++j)
             if (i0 + j < H) {
-                const double d = c_Dt[MOFF + (i0 + j) * n];
-                accA[j] = d * ln[0];
-                accB[j] = d * -ln[n - 1];
+                const double *row = c_Dt + MOFF + (i0 + j) * ROW;
+                A[j] = row[0] * od[0];
+                S[j] = row[h] * ev[0];
             }
 #pragma unroll
-        for (int m = 1; m < n; ++m) {
+        for (int m = 1; m < H; ++m) {
 #pragma unroll
             for (int j = 0; j < IB; ++j)
                 if (i0 + j < H) {
-                    const double d = c_Dt[MOFF + (i0 + j) * n + m];
-                    accA[j] = fma(d, ln[m], accA[j]);
-                    accB[j] = fma(d, -ln[n - 1 - m], accB[j]);
+                    const double *row = c_Dt + MOFF + (i0 + j) * ROW;
+                    if (m < h) A[j] = fma(row[m], od[m], A[j]);
+                    S[j] = fma(row[h + m], ev[m], S[j]);
                 }
         }
 #pragma unroll
         for (int j = 0; j < IB; ++j)
             if (i0 + j < H) {
-                store(i0 + j, accA[j]);
-                if (n - 1 - (i0 + j) != i0 + j) store(n - 1 - (i0 + j), accB[j]);
+                const int i = i0 + j;
+                if (n - 1 - i != i) {
+                    store(i, A[j] + S[j]);
+                    store(n - 1 - i, A[j] - S[j]);
+                } else {
+                    store(i, A[j]);          // middle row of an odd n: its even part vanishes
+                }
             }
     }
 }
@@ -170,8 +198,8 @@ ax_tma_kernel(double *__restrict__ u_rw, const double *__restrict__ u_ro, const 
 {
     using C = TmaCfg<N>;
     constexpr int n = C::n, n2 = C::n2, P = C::P, S1 = C::S1, S2 = C::S2, SE = C::SE, EPB = C::EPB;
-    constexpr int R = C::R, KP = C::KP, NW = C::NW, CW = C::CW, CTHREADS = C::CW * 32;
-    constexpr int DOFF = 2 * doff(n), TOFF = DOFF + n * n;     // D and D^T in c_Dt
+    constexpr int R = C::R, KP = C::KP, NW = C::NW, CW = C::CW, CTHREADS = C::CT, GTH = C::GTH, SG = C::SG;
+    constexpr int DOFF = eo_off(n), TOFF = DOFF + eo_mat(n);     // even-odd tables of D and D^T in c_Dt
     extern __shared__ __align__(128) unsigned char smem_raw[];
     __shared__ double s_red[33];
     const double2 *ring = reinterpret_cast<const double2 *>(smem_raw);
@@ -221,17 +249,18 @@ ax_tma_kernel(double *__restrict__ u_rw, const double *__restrict__ u_ro, const 
         // without an element (ragged last warp, tail batch) compute on stale shared memory and only
         // their stores are predicated off.
         const int lane = tid & 31;
-        const int slot = tid / n2;
-        const int t2 = tid - slot * n2;
+        const int grp = tid / GTH, lt = tid - grp * GTH;
+        const int sl = lt / n2, t2 = lt - sl * n2;
         const int a = t2 % n, b = t2 / n;
-        const bool mapped = slot < EPB;
-        double *sA = work + (size_t)(mapped ? slot : 0) * NW * SE;     // u, then (NW = 2) the s direction
+        const bool mapped = sl < SG;
+        const int slot = grp * SG + (mapped ? sl : 0);
+        double *sA = work + (size_t)slot * NW * SE;     // u, then (NW = 2) the s direction
         double *sB = sA + SE;                                          // r direction
         double *sC = (NW == 3) ? sB + SE : sA;                         // s direction
         const int pbase = a + b * S1;                   // pencil (i,j) = (a,b): + k*S2
         const int rbase = (a + n * b) * S1;             // row (j,k) = (a,b): + i
         const int cbase = a + b * S2;                   // column (i,k) = (a,b): + j*S1
-        const double2 *gslot = ring + (mapped ? slot : 0) * KP * 3 * n2 + t2;
+        const double2 *gslot = ring + slot * KP * 3 * n2 + t2;
         const double beta = FUSEP ? red.scal[NK_S_BETA] : 0.0;
         int stage = 0;
         uint32_t phase = 0;
@@ -263,7 +292,7 @@ ax_tma_kernel(double *__restrict__ u_rw, const double *__restrict__ u_ro, const 
 #pragma unroll
                 for (int k = 0; k < n; ++k) u_rw[gbase + k * n2] = ru[k];
             }
-            compute_sync<CTHREADS>();
+            group_sync<GTH>(grp);
             // P2: r derivative along rows (A -> B), s derivative along columns (A -> C)
             {
                 double ln[n];
@@ -275,7 +304,7 @@ ax_tma_kernel(double *__restrict__ u_rw, const double *__restrict__ u_ro, const 
                 double ln[n];                           // columns overwrite A in place: read, barrier, write
 #pragma unroll
                 for (int m = 0; m < n; ++m) ln[m] = sA[cbase + m * S1];
-                compute_sync<CTHREADS>();
+                group_sync<GTH>(grp);
                 line_apply<n, DOFF>(ln, [&](int j, double v) { if (mapped) sC[cbase + j * S1] = v; });
             } else {
                 double ln[n];
@@ -283,37 +312,58 @@ ax_tma_kernel(double *__restrict__ u_rw, const double *__restrict__ u_ro, const 
                 for (int m = 0; m < n; ++m) ln[m] = sA[cbase + m * S1];
                 line_apply<n, DOFF>(ln, [&](int j, double v) { if (mapped) sC[cbase + j * S1] = v; });
             }
-            compute_sync<CTHREADS>();
+            group_sync<GTH>(grp);
             // P3: t derivative in registers; G from the ring; t transpose in registers
             double rw[n];
             {
                 double wt[n];
                 line_apply<n, DOFF>(ru, [&](int k, double v) { wt[k] = v; });
+                // planes are waited for, used and handed back KG at a time, so that the loads and
+                // the 15 flops of several planes interleave (the waits are compiler barriers)
+                constexpr int KG = (KP == 1) ? NK_TMA_KG : n;
 #pragma unroll
-                for (int k = 0; k < n; ++k) {
-                    if (k % KP == 0) mbar_wait_warp(full0 + 8 * stage, phase);
-                    const double2 *gs = gslot + (size_t)stage * C::STAGE_D2 + (k % KP) * 3 * n2;
-                    const double2 ga = gs[0], gb = gs[n2], gc = gs[2 * n2];
-                    const double ur = sB[pbase + k * S2], us = sC[pbase + k * S2], ut = wt[k];
-                    const double wr = fma(ga.x, ur, fma(ga.y, us, gb.x * ut));          // w_r = rr ur + rs us + rt ut
-                    const double ws = fma(ga.y, ur, fma(gb.y, us, gc.x * ut));          // w_s = rs ur + ss us + st ut
-                    const double wk = fma(gb.x, ur, fma(gc.x, us, gc.y * ut));          // w_t = rt ur + st us + tt ut
-                    if (mapped) {
-                        sB[pbase + k * S2] = wr;
-                        sC[pbase + k * S2] = ws;
+                for (int k0 = 0; k0 < n; k0 += KG) {
+                    int st[KG];
+#pragma unroll
+                    for (int j = 0; j < KG; ++j) {
+                        if (k0 + j < n && (KP == 1 || j == 0)) {
+                            mbar_wait_warp(full0 + 8 * stage, phase);
+                            st[j] = stage;
+                            if (KP == 1) { if (++stage == R) { stage = 0; phase ^= 1u; } }
+                        } else {
+                            st[j] = st[0];
+                        }
                     }
-                    wt[k] = wk;
-                    // <u, A_L u> = sum over points of grad(u)^T G grad(u): the fused pap needs no u later on
-                    dsum += active ? fma(ur, wr, fma(us, ws, ut * wk)) : 0.0;
-                    if (k % KP == KP - 1) {          // this warp is done with the stage: hand it back
-                        __syncwarp();
-                        if (lane == 0) mbar_arrive(empty0 + 8 * stage);
-                        if (++stage == R) { stage = 0; phase ^= 1u; }
+#pragma unroll
+                    for (int j = 0; j < KG; ++j) {
+                        const int k = k0 + j;
+                        if (k < n) {
+                            const double2 *gs = gslot + (size_t)st[j] * C::STAGE_D2 + (k % KP) * 3 * n2;
+                            const double2 ga = gs[0], gb = gs[n2], gc = gs[2 * n2];
+                            const double ur = sB[pbase + k * S2], us = sC[pbase + k * S2], ut = wt[k];
+                            const double wr = fma(ga.x, ur, fma(ga.y, us, gb.x * ut));  // w_r = rr ur + rs us + rt ut
+                            const double ws = fma(ga.y, ur, fma(gb.y, us, gc.x * ut));  // w_s = rs ur + ss us + st ut
+                            const double wk = fma(gb.x, ur, fma(gc.x, us, gc.y * ut));  // w_t = rt ur + st us + tt ut
+                            if (mapped) {
+                                sB[pbase + k * S2] = wr;
+                                sC[pbase + k * S2] = ws;
+                            }
+                            wt[k] = wk;
+                            // <u, A_L u> = sum over points of grad(u)^T G grad(u): the fused pap needs no u later on
+                            dsum += active ? fma(ur, wr, fma(us, ws, ut * wk)) : 0.0;
+                        }
                     }
+                    __syncwarp();                    // this warp is done with these stages: hand them back
+                    if (lane == 0) {
+#pragma unroll
+                        for (int j = 0; j < KG; ++j)
+                            if (k0 + j < n && (KP == 1 || j == 0)) mbar_arrive(empty0 + 8 * st[j]);
+                    }
+                    if (KP != 1) { if (++stage == R) { stage = 0; phase ^= 1u; } }
                 }
                 line_apply<n, TOFF>(wt, [&](int m, double v) { rw[m] = v; });
             }
-            compute_sync<CTHREADS>();
+            group_sync<GTH>(grp);
             {   // prefetch the next batch's pencil: issued after P3, where register pressure peaks (the
                 // register file is split four ways, so > 8 warps means <= 168 registers per thread);
                 // in flight through P4 and P5
@@ -336,14 +386,14 @@ ax_tma_kernel(double *__restrict__ u_rw, const double *__restrict__ u_ro, const 
                 for (int m = 0; m < n; ++m) ln[m] = sC[cbase + m * S1];
                 line_apply<n, TOFF>(ln, [&](int j, double v) { if (mapped) sC[cbase + j * S1] = v; });
             }
-            compute_sync<CTHREADS>();
+            group_sync<GTH>(grp);
             // P5: sum the three directions, store
 #pragma unroll
             for (int k = 0; k < n; ++k) {
                 const double wv = rw[k] + (sB[pbase + k * S2] + sC[pbase + k * S2]);
                 if (active) w[gbase + k * n2] = wv;
             }
-            if (NW == 2) compute_sync<CTHREADS>();      // next P1 writes A, which P5 still reads as C
+            if (NW == 2) group_sync<GTH>(grp);      // next P1 writes A, which P5 still reads as C
         }
     }
     if (dot) nk_grid_reduce(dsum, s_red, red, NK_EPI_PAP, nullptr);
@@ -381,11 +431,23 @@ cudaError_t nk_upload_D_tables_tma(void)
     static double h[D_TOTAL];
     double xi[16], wq[16];
     for (int N = 1; N <= NK_MAX_ORDER; ++N) {
-        const int n = N + 1;
-        double *D = h + 2 * doff(n), *T = D + n * n;
+        const int n = N + 1, hh = n / 2, H = (n + 1) / 2, ROW = eo_row(n);
+        double D[16 * 16];
         nk_host_basis(N, xi, wq, D);
-        for (int i = 0; i < n; ++i)
-            for (int m = 0; m < n; ++m) T[i * n + m] = D[m * n + i];
+        for (int t = 0; t < 2; ++t) {                  // t = 0: M = D, t = 1: M = D^T
+            double *tab = h + eo_off(n) + t * eo_mat(n);
+            for (int i = 0; i < H; ++i)
+                for (int m = 0; m < H; ++m) {
+                    const double a = t ? D[m * n + i] : D[i * n + m];
+                    const double b = t ? D[(n - 1 - m) * n + i] : D[i * n + (n - 1 - m)];
+                    if (m < hh) {
+                        tab[i * ROW + m] = 0.5 * (a - b);
+                        tab[i * ROW + hh + m] = 0.5 * (a + b);
+                    } else {
+                        tab[i * ROW + hh + m] = a;     // middle column of an odd n
+                    }
+                }
+        }
     }
     cudaError_t e = cudaMemcpyToSymbol(c_Dt, h, sizeof(h));
     if (e != cudaSuccess) return e;
