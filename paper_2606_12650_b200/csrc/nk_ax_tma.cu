@@ -67,7 +67,7 @@ struct TmaCfg {
     // Sync groups: the element slots of a batch that share one named barrier.  From n^2 >= 64 on every
     // slot is its own group of whole warps, so the elements of a batch drift apart and the
     // shared-memory-bound phases of one overlap the DFMA-bound phases of the other.
-    static constexpr int SG = (n == 8 || n == 10 || n == 11 || n == 16) ? 1 : EPB;   // slots per group
+    static constexpr int SG = (n == 8 || n == 10 || n == 11 || n == 12 || n == 16) ? 1 : EPB;   // slots per group
     // (only where a slot fills whole warps well; elsewhere per-slot groups cost a warp and registers)
     static constexpr int NG = EPB / SG;                       // groups
     static constexpr int GTH = (SG * n2 + 31) / 32 * 32;      // threads per group
