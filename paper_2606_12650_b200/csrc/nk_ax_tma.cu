@@ -92,6 +92,8 @@ struct TmaCfg {
     static constexpr int WORK_BYTES = work_bytes(NW);
     static constexpr int SMEM = R * STAGE_BYTES + WORK_BYTES + BAR_BYTES;
     static_assert(R >= 2, "ring too small");
+    // where the next batch's u pencil is requested: 1 = after P3, 2 = after P4 (measured per order)
+    static constexpr int PF = (n == 12) ? 2 : 1;
 };
 
 // ---- mbarrier / bulk-copy PTX ---------------------------------------------------------------------
@@ -364,9 +366,9 @@ ax_tma_kernel(double *__restrict__ u_rw, const double *__restrict__ u_ro, const 
                 line_apply<n, TOFF>(wt, [&](int m, double v) { rw[m] = v; });
             }
             group_sync<GTH>(grp);
-            {   // prefetch the next batch's pencil: issued after P3, where register pressure peaks (the
-                // register file is split four ways, so > 8 warps means <= 168 registers per thread);
-                // in flight through P4 and P5
+            auto prefetch = [&]() {
+                // the next batch's pencil, in flight while this batch finishes (the register file is
+                // split four ways, so > 8 warps means <= 168 registers: not before P3, where pressure peaks)
                 const int64_t e1 = e + (int64_t)gridDim.x * EPB;
                 const bool act = mapped && it + 1 < nit && e1 < E;
                 const int64_t gb = act ? e1 * P + t2 : 0;
@@ -375,7 +377,8 @@ ax_tma_kernel(double *__restrict__ u_rw, const double *__restrict__ u_ro, const 
                     nu[k] = act ? (FUSEP ? u_rw[gb + k * n2] : u_ro[gb + k * n2]) : 0.0;
                     if (FUSEP) nr[k] = act ? r_in[gb + k * n2] : 0.0;
                 }
-            }
+            };
+            if (C::PF == 1) prefetch();
             // P4: D^T along rows (B in place) and columns (C in place)
             {
                 double ln[n];
@@ -387,6 +390,7 @@ ax_tma_kernel(double *__restrict__ u_rw, const double *__restrict__ u_ro, const 
                 line_apply<n, TOFF>(ln, [&](int j, double v) { if (mapped) sC[cbase + j * S1] = v; });
             }
             group_sync<GTH>(grp);
+            if (C::PF == 2) prefetch();
             // P5: sum the three directions, store
 #pragma unroll
             for (int k = 0; k < n; ++k) {
@@ -394,6 +398,7 @@ ax_tma_kernel(double *__restrict__ u_rw, const double *__restrict__ u_ro, const 
                 if (active) w[gbase + k * n2] = wv;
             }
             if (NW == 2) group_sync<GTH>(grp);      // next P1 writes A, which P5 still reads as C
+            if (C::PF == 0) prefetch();
         }
     }
     if (dot) nk_grid_reduce(dsum, s_red, red, NK_EPI_PAP, nullptr);
