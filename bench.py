@@ -338,12 +338,19 @@ def run_ours(args) -> dict | None:
         bpp = 64.0 + (16.0 if args.fuse_p else 0.0)
         avg = ax_ms / ax_n
         ach = bpp * L / (avg * 1e-3) / 1e9
-        out["roofline"] = {"kernel": "ax_line_kernel (ax_e" + (" + fused p=r+beta*p" if args.fuse_p else "")
+        traffic = args.traffic
+        if traffic is None:
+            try:
+                with open(os.path.join(ROOT, "profiles", "traffic.json.txt")) as fh:
+                    traffic = float(json.load(fh)[args.workload]["dram_bytes_per_launch"])
+            except Exception:
+                traffic = None
+        out["roofline"] = {"kernel": "ax_tma_kernel (ax_e" + (" + fused p=r+beta*p" if args.fuse_p else "")
                                      + (" + fused pap" if args.fuse_pap else "") + ")",
                            "bound": "hbm", "achieved": ach, "peak": peak, "unit": "GB/s", "frac": ach / peak,
                            "peak_kind": peak_kind + " copy peak (burst)", "frac_of_nominal_8TBs": ach / HBM_NOMINAL_GBS,
                            "bytes_per_point": bpp, "avg_launch_us": 1e3 * avg, "launches_timed": ax_n,
-                           "traffic": args.traffic, "share_of_step": ax_ms / ms}
+                           "traffic": traffic, "algorithmic_bytes_per_launch": bpp * L, "share_of_step": ax_ms / ms}
         kb = {"gs": gs_bytes(sizes) / L, "dot": 24.0, "update_xr": 56.0 + 1.0 - 8.0, "update_p": 24.0}
         out["kernels"] = {k: {"avg_us": 1e3 * t / n, "launches": n, "share_of_step": t / ms,
                               **({"gbs_model": kb[k] * L / (t / n * 1e-3) / 1e9} if k in kb else {})}
