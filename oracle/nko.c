@@ -31,6 +31,7 @@ struct nko_ctx {
     int64_t *order;
     int64_t n_shared_unique, n_masked_unique;
     int dot_mode;
+    long double Dl[65 * 65];      /* D before rounding to double (geometry only) */
 };
 
 /* ------------------------------------------------------------------------------------------
@@ -50,7 +51,8 @@ static void legendre(int N, long double x, long double *PN, long double *PNm1)
     *PNm1 = p0;
 }
 
-int nko_basis(int N, double *xi, double *w, double *D)
+/* Dl (may be NULL): the derivative matrix before its rounding to double, for O2 (R22). */
+static int basis_ld(int N, double *xi, double *w, double *D, long double *Dl)
 {
     if (N < 1 || N > 64 || !xi || !w || !D) return NKO_ERR_ARG;
     const int n = N + 1;
@@ -100,11 +102,14 @@ int nko_basis(int N, double *xi, double *w, double *D)
             else if (i == N) d = (long double)N * (N + 1) / 4.0L;
             else d = 0.0L;
             D[i * n + m] = (double)d;
+            if (Dl) Dl[i * n + m] = d;
         }
     free(x);
     free(P);
     return NKO_OK;
 }
+
+int nko_basis(int N, double *xi, double *w, double *D) { return basis_ld(N, xi, w, D, NULL); }
 
 /* ------------------------------------------------------------------------------------------
  * O2. Geometry: x_r = sum_m D[i][m] x(m,j,k), x_s = sum_m D[j][m] x(i,m,k),
@@ -115,7 +120,9 @@ static int geometry(nko_ctx *c, const double *coords)
 {
     const int n = c->n;
     const int64_t P = (int64_t)n * n * n, L = c->L;
-    const double *D = c->D, *wq = c->wq;
+    const long double *D = c->Dl;      /* unrounded: a rounded D has row sums ~1e-16 |D|, which
+                                        * times |x| / (h/2) would cost G three digits (R22) */
+    const double *wq = c->wq;
     const double *X = coords, *Y = coords + L, *Z = coords + 2 * L;
     int bad = 0;
 #pragma omp parallel for schedule(static) reduction(| : bad)
@@ -132,15 +139,15 @@ static int geometry(nko_ctx *c, const double *coords)
                         const int64_t lr = m + n * j + n * n * k;
                         const int64_t ls = i + n * m + n * n * k;
                         const int64_t lt = i + n * j + n * n * m;
-                        xr += (long double)D[i * n + m] * x[lr];
-                        yr += (long double)D[i * n + m] * y[lr];
-                        zr += (long double)D[i * n + m] * z[lr];
-                        xs += (long double)D[j * n + m] * x[ls];
-                        ys += (long double)D[j * n + m] * y[ls];
-                        zs += (long double)D[j * n + m] * z[ls];
-                        xt += (long double)D[k * n + m] * x[lt];
-                        yt += (long double)D[k * n + m] * y[lt];
-                        zt += (long double)D[k * n + m] * z[lt];
+                        xr += D[i * n + m] * x[lr];
+                        yr += D[i * n + m] * y[lr];
+                        zr += D[i * n + m] * z[lr];
+                        xs += D[j * n + m] * x[ls];
+                        ys += D[j * n + m] * y[ls];
+                        zs += D[j * n + m] * z[ls];
+                        xt += D[k * n + m] * x[lt];
+                        yt += D[k * n + m] * y[lt];
+                        zt += D[k * n + m] * z[lt];
                     }
                     const long double J = xr * (ys * zt - yt * zs) - xs * (yr * zt - yt * zr)
                                         + xt * (yr * zs - ys * zr);
@@ -246,7 +253,7 @@ int nko_setup(nko_ctx **out, int64_t E, int N, const double *coords,
     int ok = c->xi && c->wq && c->D && c->J && c->mask && c->c && c->mult;
     for (int a = 0; a < 6; ++a) ok = ok && c->G[a];
     if (!ok) { nko_free(c); return NKO_ERR_ALLOC; }
-    int rc = nko_basis(N, c->xi, c->wq, c->D);
+    int rc = basis_ld(N, c->xi, c->wq, c->D, c->Dl);
     if (rc == NKO_OK) rc = build_groups(c, glo_num, mask);
     if (rc == NKO_OK) rc = geometry(c, coords);
     if (rc != NKO_OK) { nko_free(c); return rc; }

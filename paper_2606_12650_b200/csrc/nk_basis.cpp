@@ -26,7 +26,7 @@ void legendre3(int deg, long double x, long double *pm, long double *p0, long do
 
 }  // namespace
 
-void nk_host_basis(int N, double *xi, double *w, double *D)
+void nk_host_basis_dd(int N, double *xi, double *w, double *D, double *Dlo)
 {
     const int n = N + 1;
     long double x[16], pn[16];
@@ -65,5 +65,8 @@ void nk_host_basis(int N, double *xi, double *w, double *D)
             else if (i == N) d = (long double)N * (N + 1) / 4.0L;
             else d = 0.0L;
             D[i * n + m] = (double)d;
+            if (Dlo) Dlo[i * n + m] = (double)(d - (long double)(double)d);   // D = hi + lo to ~2^-64
         }
 }
+
+void nk_host_basis(int N, double *xi, double *w, double *D) { nk_host_basis_dd(N, xi, w, D, nullptr); }

@@ -15,13 +15,32 @@ namespace {
 
 constexpr int GEOM_THREADS = 256;
 
+// Double-double accumulation of one derivative sum: acc += (dh + dl) * v, products by FMA (exact
+// two-product), sums by two-sum.  The nine coordinate derivatives cancel ~|D|max |x| / (h/2)
+// leading digits even after the shift to the element's first node, and D rounded to double is
+// itself only good to 2^-53: with D = hi + lo (from the host's long double) and a double-double
+// accumulator the derivatives come out correctly rounded, and G to a few ulp (R22).
+struct dd { double hi, lo; };
+__device__ __forceinline__ void dd_fma(dd &acc, double dh, double dl, double v)
+{
+    const double p = dh * v;
+    const double e = fma(dh, v, -p) + dl * v;        // exact product error + low part
+    const double s = acc.hi + p;
+    const double bb = s - acc.hi;
+    const double err = (acc.hi - (s - bb)) + (p - bb);
+    acc.hi = s;
+    acc.lo += err + e;
+}
+__device__ __forceinline__ double dd_val(const dd &a) { return a.hi + a.lo; }
+
 __global__ void __launch_bounds__(GEOM_THREADS)
-geom_kernel(const double *__restrict__ coords, const double *__restrict__ Dg, const double *__restrict__ wq,
+geom_kernel(const double *__restrict__ coords, const double *__restrict__ Dg, const double *__restrict__ Dlg,
+            const double *__restrict__ wq,
             int n, int64_t L, double2 *__restrict__ g, int *__restrict__ errflag)
 {
-    __shared__ double s_D[16 * 16];
+    __shared__ double s_D[16 * 16], s_Dl[16 * 16];
     __shared__ double s_w[16];
-    for (int t = threadIdx.x; t < n * n; t += GEOM_THREADS) s_D[t] = Dg[t];
+    for (int t = threadIdx.x; t < n * n; t += GEOM_THREADS) { s_D[t] = Dg[t]; s_Dl[t] = Dlg[t]; }
     if (threadIdx.x < n) s_w[threadIdx.x] = wq[threadIdx.x];
     __syncthreads();
     const int P = n * n * n;
@@ -31,14 +50,18 @@ geom_kernel(const double *__restrict__ coords, const double *__restrict__ Dg, co
     int bad = 0;
     for (int q = threadIdx.x; q < P; q += GEOM_THREADS) {
         const int i = q % n, j = (q / n) % n, k = q / (n * n);
-        double xr = 0, xs = 0, xt = 0, yr = 0, ys = 0, yt = 0, zr = 0, zs = 0, zt = 0;
+        dd axr{0, 0}, axs{0, 0}, axt{0, 0}, ayr{0, 0}, ays{0, 0}, ayt{0, 0}, azr{0, 0}, azs{0, 0}, azt{0, 0};
         for (int m = 0; m < n; ++m) {
             const double di = s_D[i * n + m], dj = s_D[j * n + m], dk = s_D[k * n + m];
+            const double li = s_Dl[i * n + m], lj = s_Dl[j * n + m], lk = s_Dl[k * n + m];
             const int qr = m + n * j + n * n * k, qs = i + n * m + n * n * k, qt = i + n * j + n * n * m;
-            xr = fma(di, xe[qr] - x0, xr); yr = fma(di, ye[qr] - y0, yr); zr = fma(di, ze[qr] - z0, zr);
-            xs = fma(dj, xe[qs] - x0, xs); ys = fma(dj, ye[qs] - y0, ys); zs = fma(dj, ze[qs] - z0, zs);
-            xt = fma(dk, xe[qt] - x0, xt); yt = fma(dk, ye[qt] - y0, yt); zt = fma(dk, ze[qt] - z0, zt);
+            dd_fma(axr, di, li, xe[qr] - x0); dd_fma(ayr, di, li, ye[qr] - y0); dd_fma(azr, di, li, ze[qr] - z0);
+            dd_fma(axs, dj, lj, xe[qs] - x0); dd_fma(ays, dj, lj, ye[qs] - y0); dd_fma(azs, dj, lj, ze[qs] - z0);
+            dd_fma(axt, dk, lk, xe[qt] - x0); dd_fma(ayt, dk, lk, ye[qt] - y0); dd_fma(azt, dk, lk, ze[qt] - z0);
         }
+        const double xr = dd_val(axr), xs = dd_val(axs), xt = dd_val(axt);
+        const double yr = dd_val(ayr), ys = dd_val(ays), yt = dd_val(ayt);
+        const double zr = dd_val(azr), zs = dd_val(azs), zt = dd_val(azt);
         // cofactor vectors (rows of J * inverse Jacobian)
         const double rx = ys * zt - yt * zs, ry = zs * xt - zt * xs, rz = xs * yt - xt * ys;   // x_s x x_t
         const double sx = yt * zr - yr * zt, sy = zt * xr - zr * xt, sz = xt * yr - xr * yt;   // x_t x x_r
@@ -78,10 +101,11 @@ unpack_geom_kernel(const double2 *__restrict__ g, double *__restrict__ G6, int64
 
 }  // namespace
 
-cudaError_t nk_launch_geom(nk_ctx *c, const double *coords_dev, const double *D_dev, const double *wq_dev,
+cudaError_t nk_launch_geom(nk_ctx *c, const double *coords_dev, const double *D_dev, const double *Dlo_dev,
+                           const double *wq_dev,
                            cudaStream_t st)
 {
-    geom_kernel<<<(unsigned)c->E, GEOM_THREADS, 0, st>>>(coords_dev, D_dev, wq_dev, c->n, c->L, c->g, c->errflag);
+    geom_kernel<<<(unsigned)c->E, GEOM_THREADS, 0, st>>>(coords_dev, D_dev, Dlo_dev, wq_dev, c->n, c->L, c->g, c->errflag);
     c->launches++;
     return cudaGetLastError();
 }

@@ -82,6 +82,7 @@ struct nk_ctx {
 // ---- kernels' host launchers (each returns a cudaError_t from the launch) -----------------------
 // nk_basis.cpp
 void nk_host_basis(int N, double *xi, double *w, double *D);
+void nk_host_basis_dd(int N, double *xi, double *w, double *D, double *Dlo);   // D = D + Dlo (long double split)
 // nk_ax.cu : w = A_L u.  If r_in != NULL: u := r_in + beta*u is applied first and written back to u.
 // If dot: sum_l u_l w_l is reduced with epilogue NK_EPI_PAP.
 cudaError_t nk_launch_ax_e(nk_ctx *c, double *u_rw, const double *u_ro, const double *r_in, double *w,
@@ -92,7 +93,7 @@ cudaError_t nk_launch_ax_tma(nk_ctx *c, double *u_rw, const double *u_ro, const 
                              int dot, cudaStream_t st);
 cudaError_t nk_upload_D_tables_tma(void);
 // nk_geom.cu
-cudaError_t nk_launch_geom(nk_ctx *c, const double *coords_dev, const double *D_dev,
+cudaError_t nk_launch_geom(nk_ctx *c, const double *coords_dev, const double *D_dev, const double *Dlo_dev,
                            const double *wq_dev, cudaStream_t st);
 cudaError_t nk_launch_get_geom(nk_ctx *c, double *G6, cudaStream_t st);
 // nk_gs.cu

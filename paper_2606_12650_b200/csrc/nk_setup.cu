@@ -128,6 +128,11 @@ int setup_impl(nk_ctx *c, const double *coords, const int64_t *glo_num, const do
     NK_CUDA(cudaMemcpyAsync(c->mtab, mtab, sizeof(mtab), cudaMemcpyHostToDevice, st));
     NK_CUDA(cudaMemcpyAsync(D_dev, c->D, sizeof(double) * c->n * c->n, cudaMemcpyHostToDevice, st));
     NK_CUDA(cudaMemcpyAsync(wq_dev, c->wq, sizeof(double) * c->n, cudaMemcpyHostToDevice, st));
+    // low parts of D (set-up only): staged in the residual-history scratch
+    double Dhi[16 * 16], Dlo[16 * 16], xi_t[16], wq_t[16];
+    nk_host_basis_dd(c->N, xi_t, wq_t, Dhi, Dlo);
+    double *Dlo_dev = c->hist;
+    NK_CUDA(cudaMemcpyAsync(Dlo_dev, Dlo, sizeof(double) * c->n * c->n, cudaMemcpyHostToDevice, st));
     NK_CUDA(cudaMemsetAsync(c->red.scal, 0, 256, st));
     NK_CUDA(cudaMemsetAsync(c->red.counter, 0, 256, st));       // counter, errflag, res_dummy
     // coordinates (x|y|z planes at stride L) are staged in the r|p|w block, which is >= 3L doubles
@@ -135,7 +140,7 @@ int setup_impl(nk_ctx *c, const double *coords, const int64_t *glo_num, const do
     NK_CUDA(cudaMemcpyAsync(coords_dev, coords, 3 * (size_t)L * sizeof(double), cudaMemcpyHostToDevice, st));
     NK_CUDA(nk_upload_D_tables());
     NK_CUDA(nk_upload_D_tables_tma());
-    NK_CUDA(nk_launch_geom(c, coords_dev, D_dev, wq_dev, st));
+    NK_CUDA(nk_launch_geom(c, coords_dev, D_dev, Dlo_dev, wq_dev, st));
     int err = 0;
     NK_CUDA(cudaMemcpyAsync(&err, c->errflag, sizeof(int), cudaMemcpyDeviceToHost, st));
     NK_CUDA(cudaStreamSynchronize(st));

@@ -1,0 +1,118 @@
+"""-m gpu parity at BASELINE.json's full sizes, in the launch configuration bench.py times
+(default options, device-resident vectors): config 3 (E=4096, N=9) and config 5 (E=32768, N=11).
+
+* ax_e on sampled elements: ax_e is element-local, so the oracle is set up on the sampled elements
+  alone (their coordinates, private ids) and compared entry by entry with the GPU's output there.
+* properties that hold at any size: symmetry of gs o ax_e, null space, analytic multiplicity counts.
+* CG: residual history and x against the oracle; config 3 by the R15 protocol (flat 1e-10 up to K*,
+  the last iteration with oracle band <= 1e-11; max(1e-10, 10 x band) beyond), config 5 flat 1e-10.
+"""
+import numpy as np
+import pytest
+
+from parity import elem_err
+from gpu_common import to_dev, to_np, TOL_OP, TOL_CG
+from workloads import CONFIGS, config_mesh, config_rhs, brick_counts
+
+pytestmark = pytest.mark.gpu
+
+_cache = {}
+
+
+def _gpu(name):
+    from paper_2606_12650_b200 import Nekbone
+    if name not in _cache:
+        _cache.clear()                       # one full-size context at a time
+        mesh = config_mesh(name)
+        _cache[name] = (mesh, Nekbone.from_mesh(mesh))
+    return _cache[name]
+
+
+def _sample_elements(E, count, seed):
+    rng = np.random.Generator(np.random.PCG64(seed))
+    pick = set(rng.choice(E, size=count, replace=False).tolist()) | {0, 1, E - 2, E - 1}
+    return np.array(sorted(pick))
+
+
+@pytest.mark.parametrize("name", ["config3", "config5"])
+def test_ax_e_sampled_elements(name):
+    from oracle.nko import Oracle
+    mesh, gpu = _gpu(name)
+    P = mesh.n ** 3
+    u = np.random.Generator(np.random.PCG64(77)).uniform(-1, 1, mesh.L)
+    wg = to_np(gpu.ax_e(to_dev(u))).reshape(mesh.E, P)
+    els = _sample_elements(mesh.E, 96, 5)
+    coords = mesh.coords.reshape(3, mesh.E, P)[:, els, :].reshape(3, -1)
+    glo = np.arange(els.size * P, dtype=np.int64)                 # private ids: no sharing
+    orc = Oracle(els.size, mesh.N, coords, glo, np.ones(els.size * P))
+    wo = orc.ax_e(u.reshape(mesh.E, P)[els].reshape(-1))
+    assert elem_err(wg[els].reshape(-1), wo, P) <= TOL_OP
+    # geometric factors on the same elements
+    Gg = to_np(gpu.geom()).reshape(6, mesh.E, P)[:, els, :]
+    Go = orc.geom()[0].reshape(6, els.size, P)
+    sc = np.abs(Go).max(axis=(0, 2))[None, :, None]       # per element, over all six factors (R14):
+    assert (np.abs(Gg - Go) <= TOL_OP * np.maximum(np.abs(Go), sc)).all()   # off-diagonals vanish on the boundary
+
+
+@pytest.mark.parametrize("name", ["config3", "config5"])
+def test_properties_full_size(name):
+    import torch
+    mesh, gpu = _gpu(name)
+    c = CONFIGS[name]
+    counts = brick_counts(*c["brick"], c["N"])
+    s = gpu.sizes()
+    assert s["n_local"] == counts["L"] and s["n_unique"] == counts["U"]
+    assert s["n_shared_unique"] == counts["shared_unique"]
+    assert s["n_masked_unique"] == counts["masked_unique"]
+    mult = gpu.mult()
+    assert set(torch.unique(mult).tolist()) <= {1.0, 2.0, 4.0, 8.0}
+    assert float((1.0 / mult).sum()) == pytest.approx(counts["U"], rel=1e-12)
+    # null space before masking: gs(ax_e(1)) = 0 relative to the size of the addends
+    one = torch.ones(mesh.L, dtype=torch.float64, device="cuda")
+    w = gpu.ax_e(one)
+    scale = float(gpu.geom().abs().max()) * 6 * mesh.n
+    gpu.gs(w)
+    assert float(w.abs().max()) <= 1e-12 * scale
+    # symmetry of the assembled, masked operator on consistent fields
+    rng = np.random.Generator(np.random.PCG64(9))
+    inv = _unique_index(mesh)                        # consistent AND masked: M A M is the symmetric operator
+    uu = to_dev(rng.uniform(-1, 1, counts["U"])[inv] * mesh.mask)
+    vv = to_dev(rng.uniform(-1, 1, counts["U"])[inv] * mesh.mask)
+    a = float(gpu.dot(uu, gpu.ax(vv))[0])
+    b = float(gpu.dot(vv, gpu.ax(uu))[0])
+    assert abs(a - b) <= 1e-11 * max(abs(a), abs(b))
+
+
+def _unique_index(mesh):
+    _, inv = np.unique(mesh.glo_num, return_inverse=True)
+    return inv
+
+
+@pytest.mark.parametrize("name", ["config3", "config5"])
+def test_free_running_cg_full_size(name):
+    from oracle.nko import Oracle
+    mesh, gpu = _gpu(name)
+    niter = CONFIGS[name]["niter"]
+    f = config_rhs(name, mesh)
+    xg, hg = gpu.cg(to_dev(f), niter)
+    xg, hg = to_np(xg), to_np(hg)
+    orc = Oracle.from_mesh(mesh)
+    xo, ho = orc.cg(f, niter)
+    orc.close()
+    P = mesh.n ** 3
+    if name == "config3":
+        # the oracle's own rounding band decides how far the flat 1e-10 applies (R15)
+        ofm = Oracle.from_mesh(mesh, fma=True)
+        xb, hb = ofm.cg(f, niter)
+        ofm.close()
+        band = np.maximum.accumulate(np.abs(hb - ho) / ho)
+        tol = np.where(band <= 1e-11, TOL_CG, np.maximum(TOL_CG, 10.0 * band))
+        kstar = int(np.nonzero(band <= 1e-11)[0].max())
+        assert kstar >= 50, kstar
+        assert np.all(np.abs(hg - ho) <= tol * ho), (kstar, float(np.abs(hg / ho - 1).max()))
+        xband = elem_err(xb, xo, P)
+        assert elem_err(xg, xo, P) <= max(TOL_CG, 10.0 * xband)
+    else:
+        assert np.all(np.abs(hg - ho) <= TOL_CG * ho), float(np.abs(hg / ho - 1).max())
+        assert elem_err(xg, xo, P) <= TOL_CG
+    assert np.all(xg[mesh.mask == 0.0] == 0.0)
