@@ -175,3 +175,59 @@ def test_cyclic_axis_relabelling_permutes_G():
     # the off-diagonal planes are distinct, so a swapped pair would be caught
     assert np.max(np.abs(G[RS] - G[RT])) > 1e-4 * scale
     assert np.max(np.abs(G[RS] - G[ST])) > 1e-4 * scale
+
+
+def test_fine_mesh_element_against_40_digit_arithmetic():
+    """Conditioning pin (R22): on a fine, deformed mesh the derivative sums of absolute
+    coordinates cancel ~10^3 leading digits, and a derivative matrix rounded to double (row sums
+    ~1e-16 |D| instead of 0) alone costs G three digits.  O2 re-evaluated with mpmath at 40 digits
+    (GLL nodes by Newton on P_N', D and weights from their closed forms, S 8(c) O1-O2) must agree
+    with the oracle's G to a few ulp of the element scale."""
+    mp = pytest.importorskip("mpmath")
+    mp.mp.dps = 40
+    N = 9
+    m = brick_mesh(32, 2, 2, N, 0.1)
+    n, P = m.n, m.n ** 3
+    G, _ = nko.Oracle.from_mesh(m).geom()
+    G = G.reshape(6, m.E, P)
+
+    def leg(x):                      # P_N(x), P_{N-1}(x) by the three-term recurrence
+        a, b = mp.mpf(1), x
+        for k in range(1, N):
+            a, b = b, ((2 * k + 1) * x * b - k * a) / (k + 1)
+        return b, a
+
+    xi, _, _ = nko.basis(N)
+    xs = [mp.mpf(-1)] + [None] * (N - 1) + [mp.mpf(1)]
+    for i in range(1, N):
+        t = mp.mpf(float(xi[i]))
+        for _ in range(60):          # Newton on q = P_{N+1} - P_{N-1}, q' = (2N+1) P_N
+            pn, pm = leg(t)
+            pp = ((2 * N + 1) * t * pn - N * pm) / (N + 1)
+            t -= (pp - pm) / ((2 * N + 1) * pn)
+        xs[i] = t
+    pn = [leg(x)[0] for x in xs]
+    D = [[(pn[i] / (pn[q] * (xs[i] - xs[q])) if i != q else
+           (-mp.mpf(N * (N + 1)) / 4 if i == 0 else (mp.mpf(N * (N + 1)) / 4 if i == N else mp.mpf(0))))
+          for q in range(n)] for i in range(n)]
+    w = [2 / (N * (N + 1) * p * p) for p in pn]
+
+    e = 31 + 32 * 3                  # last element along x: coordinates near 1, spacing 1/32
+    X = [[mp.mpf(float(v)) for v in m.coords[c].reshape(m.E, P)[e]] for c in range(3)]
+    idx = lambda i, j, k: i + n * j + n * n * k
+    worst = 0.0
+    scale = float(np.abs(G[:, e, :]).max())
+    for (i, j, k) in [(0, 0, 0), (n - 1, n - 1, n - 1), (3, 5, 7), (n - 1, 0, 4), (4, 4, 4), (1, 8, 2)]:
+        d = [[sum(D[i][q] * X[c][idx(q, j, k)] for q in range(n)),
+              sum(D[j][q] * X[c][idx(i, q, k)] for q in range(n)),
+              sum(D[k][q] * X[c][idx(i, j, q)] for q in range(n))] for c in range(3)]
+        (xr, xs_, xt), (yr, ys, yt), (zr, zs, zt) = d
+        r = (ys * zt - yt * zs, zs * xt - zt * xs_, xs_ * yt - xt * ys)
+        s = (yt * zr - yr * zt, zt * xr - zr * xt, xt * yr - xr * yt)
+        t = (yr * zs - ys * zr, zr * xs_ - zs * xr, xr * ys - xs_ * yr)
+        J = xr * r[0] + yr * r[1] + zr * r[2]
+        sc = w[i] * w[j] * w[k] / J
+        dot = lambda a, b: a[0] * b[0] + a[1] * b[1] + a[2] * b[2]
+        for c, (a, b) in enumerate([(r, r), (r, s), (r, t), (s, s), (s, t), (t, t)]):
+            worst = max(worst, abs(float(sc * dot(a, b)) - G[c, e, idx(i, j, k)]) / scale)
+    assert worst <= 4e-16, worst
