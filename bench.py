@@ -210,6 +210,27 @@ def workload_config(name: str, cfg: dict, n_gpus: int) -> dict:
             "l2": "inputs larger than L2" if nx * ny * nz * n ** 3 * 8 * 11 > 2 * 126e6 else "L2-resident: L2 flushed between steps"}
 
 
+# ---- rank plumbing (no data-path collective: the path is single-GPU, N ranks = N replicas) ------------
+def replica_seed(seed: int, rank: int) -> int:
+    """Replica `rank` solves the same mesh with its own RHS."""
+    return int(seed) + 7919 * int(rank)
+
+
+def max_over_ranks(dist, values, device):
+    """Element-wise MAX over ranks of a short list of timings (ms); identity without a process group."""
+    import torch
+    if dist is None:
+        return [float(v) for v in values]
+    t = torch.tensor([float(v) for v in values], dtype=torch.float64, device=device)
+    dist.all_reduce(t, op=dist.ReduceOp.MAX)
+    return [float(v) for v in t]
+
+
+def whole_job_value(flops_per_step_per_rank: float, steps: int, world: int, ms_max: float) -> float:
+    """Aggregate GFLOP/s over all replicas: every rank did `steps` steps within the slowest rank's time."""
+    return world * flops_per_step_per_rank * steps / (ms_max * 1e-3) / 1e9
+
+
 # ---- our arm -----------------------------------------------------------------------------------------
 def run_ours(args) -> dict | None:
     import torch
@@ -230,7 +251,7 @@ def run_ours(args) -> dict | None:
     cfg = CONFIGS[args.workload]
     niter, N = cfg["niter"], cfg["N"]
     mesh = config_mesh(args.workload)
-    f_np = rhs_unique(mesh, cfg["seed"] + 7919 * rank)            # replica r: its own RHS
+    f_np = rhs_unique(mesh, replica_seed(cfg["seed"], rank))
     t0 = time.perf_counter()
     nk = Nekbone.from_mesh(mesh)
     setup_s = time.perf_counter() - t0
@@ -302,18 +323,16 @@ def run_ours(args) -> dict | None:
     barrier()
     ms_e2e = e0.elapsed_time(e1)
 
+    ms, ms_e2e = max_over_ranks(dist, [ms, ms_e2e], "cuda")
     if dist is not None:
-        t = torch.tensor([ms, ms_e2e], dtype=torch.float64, device="cuda")
-        dist.all_reduce(t, op=dist.ReduceOp.MAX)
-        ms, ms_e2e = float(t[0]), float(t[1])
         dist.barrier()
         dist.destroy_process_group()
     if rank != 0:
         return None
 
     peak, peak_kind = measured_peaks()
-    value = world * flops_step * args.steps / (ms * 1e-3) / 1e9
-    e2e = world * flops_step * args.steps / (ms_e2e * 1e-3) / 1e9
+    value = whole_job_value(flops_step, args.steps, world, ms)
+    e2e = whole_job_value(flops_step, args.steps, world, ms_e2e)
     out = {"metric": METRIC, "value": value, "unit": UNIT, "n_gpus": world, "steps": args.steps,
            "warmup": args.warmup, "ms_per_step": ms / args.steps, "higher_is_better": True,
            "scaling": "weak", "vs_baseline": None, "dtype": "f64", "data": "synthetic",
