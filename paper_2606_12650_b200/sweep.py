@@ -1,0 +1,110 @@
+"""Roofline sweep of ax_e, gs and ax (BASELINE.json configs[3]).
+
+    python -m paper_2606_12650_b200.sweep [--which e|n|both] [--reps 50] [--out sweep.csv]
+
+4a: brick meshes with E = 2^10 .. 2^17 at N = 7;  4b: N = 3 .. 15 at E = 4096 (16^3); perturbed
+geometry (amplitude 0.05), u uniform[-1,1) per LOCAL point (seed 1004), `reps` back-to-back
+applications timed with CUDA events after 3 untimed ones, best and median of 5 repeats.
+Reported per point: us per application, model GB/s (ax_e 64 B/pt; gs 20 B per listed copy + 4 B per
+row; ax = both), model GFLOP/s (12(N+1)+15 per point), fraction of the measured copy peak
+(MEASURED_PEAKS.json, else the guide's fallback) and of the nominal 8 TB/s, and whether the working
+set fits in L2 ("L2-resident": effective GB/s can then exceed the HBM peak; the >= 70 % claim is made
+on the other points only).  No oracle here: parity is the tests' job.
+"""
+from __future__ import annotations
+
+import argparse
+import json
+import os
+import sys
+
+import numpy as np
+
+ROOT = os.path.dirname(os.path.dirname(os.path.abspath(__file__)))
+if ROOT not in sys.path:
+    sys.path.insert(0, ROOT)
+
+L2_BYTES = 126e6
+
+
+def _peak():
+    try:
+        with open(os.path.join(ROOT, "MEASURED_PEAKS.json")) as fh:
+            return float(json.load(fh)["hbm_gbs"]), "measured"
+    except Exception:
+        return 6650.0, "fallback"
+
+
+def _time(fn, reps, repeats=5):
+    import torch
+    for _ in range(3):
+        fn()
+    torch.cuda.synchronize()
+    out = []
+    for _ in range(repeats):
+        e0, e1 = torch.cuda.Event(enable_timing=True), torch.cuda.Event(enable_timing=True)
+        e0.record()
+        for _ in range(reps):
+            fn()
+        e1.record()
+        torch.cuda.synchronize()
+        out.append(e0.elapsed_time(e1) / reps * 1e3)          # us per application
+    return min(out), float(np.median(out))
+
+
+def run_point(point, reps):
+    import torch
+    from paper_2606_12650_b200 import Nekbone
+    from workloads import sweep_mesh, sweep_field
+    mesh = sweep_mesh(point)
+    nk = Nekbone.from_mesh(mesh)
+    u = torch.from_numpy(sweep_field(mesh)).cuda()
+    w = nk.empty()
+    v = u.clone()
+    s = nk.gs_sizes()
+    L, N = mesh.L, mesh.N
+    b_ax_e = 64.0 * L
+    b_gs = 20.0 * s["n_listed"] + 4.0 * s["n_rows"]
+    fl = (12.0 * (N + 1) + 15.0) * L
+    rows = []
+    for name, fn, nbytes, flops in (("ax_e", lambda: nk.ax_e(u, w), b_ax_e, fl),
+                                    ("gs", lambda: nk.gs(v), b_gs, 0.0),
+                                    ("ax", lambda: nk.ax(u, w), b_ax_e + b_gs, fl)):
+        if name == "gs":
+            v.copy_(u)                                         # 50 in-place gs scale shared entries by <= 8^50: finite
+        best, med = _time(fn, reps)
+        rows.append(dict(kernel=name, E=mesh.E, N=N, L=L, us_best=best, us_median=med,
+                         gbs=nbytes / best / 1e3, gflops=flops / best / 1e3,
+                         working_set_mb=(72.0 * L) / 1e6, l2_resident=bool(72.0 * L <= L2_BYTES)))
+    nk.close()
+    del u, w, v
+    torch.cuda.empty_cache()
+    return rows
+
+
+def main():
+    ap = argparse.ArgumentParser()
+    ap.add_argument("--which", default="both", choices=["e", "n", "both"])
+    ap.add_argument("--reps", type=int, default=None)
+    ap.add_argument("--out", default=None)
+    args = ap.parse_args()
+    from workloads import E_SWEEP, N_SWEEP, SWEEP_REPEATS
+    reps = args.reps or SWEEP_REPEATS
+    peak, kind = _peak()
+    points = (E_SWEEP if args.which in ("e", "both") else []) + (N_SWEEP if args.which in ("n", "both") else [])
+    lines = ["sweep,kernel,E,N,L,us_best,us_median,model_GBs,frac_of_%s_copy_peak,frac_of_8TBs,model_GFLOPs,"
+             "working_set_MB,l2_resident" % kind]
+    for p in points:
+        tag = "4a" if p in E_SWEEP else "4b"
+        for r in run_point(p, reps):
+            lines.append(f"{tag},{r['kernel']},{r['E']},{r['N']},{r['L']},{r['us_best']:.2f},{r['us_median']:.2f},"
+                         f"{r['gbs']:.1f},{r['gbs'] / peak:.4f},{r['gbs'] / 8000.0:.4f},{r['gflops']:.1f},"
+                         f"{r['working_set_mb']:.1f},{int(r['l2_resident'])}")
+            print(lines[-1], flush=True)
+    if args.out:
+        with open(args.out, "w") as fh:
+            fh.write("\n".join(lines) + "\n")
+
+
+if __name__ == "__main__":
+    main()
