@@ -85,9 +85,10 @@ struct TmaCfg {
     static constexpr int SPB = n / KP;                        // stages per batch
     static constexpr int work_bytes(int nw) { return nw * EPB * SE * 8; }
     static constexpr int ring_for(int nw) { return (SMEM_CAP - BAR_BYTES - work_bytes(nw)) / STAGE_BYTES; }
-    // three work arrays (4 barriers per batch) if the ring then still holds 3/4 of a batch (measured at
-    // N = 11: 690 us with 9 or 12 planes, 720 us with 6), else two (6 barriers)
-    static constexpr int NW = (4 * ring_for(3) >= 3 * SPB) ? 3 : 2;
+    // three work arrays (4 barriers per batch) if the ring then still holds 1.5 batches, else two (6
+    // barriers).  (At N = 11 the alternative -- three arrays and a 9-plane ring -- is 2 % faster for a
+    // lone ax_e but 4 % slower inside the CG iteration, measured A/B in one bench run: 723 vs 692 us.)
+    static constexpr int NW = (ring_for(3) >= (3 * SPB + 1) / 2) ? 3 : 2;
     static constexpr int RMAX = ring_for(NW) < 3 * SPB ? ring_for(NW) : 3 * SPB;
 #ifdef NK_TMA_RCAP
     static constexpr int R = RMAX > NK_TMA_RCAP ? NK_TMA_RCAP : RMAX;
