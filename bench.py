@@ -283,7 +283,8 @@ def run_ours(args) -> dict | None:
     for _ in range(args.warmup):
         step()
     barrier()
-    nk.set_option("profile", 1 if not args.graph else 0)
+    graphed = args.graph == 1 or (args.graph == 2 and L <= (1 << 24))      # the library's rule for "graph" = 2
+    nk.set_option("profile", 0 if graphed else 1)
     nk.kernel_times()
     launches0 = nk.launch_count()
     clocks = ClockSampler(local)
@@ -304,7 +305,15 @@ def run_ours(args) -> dict | None:
     ms = sum(ev[2 * s].elapsed_time(ev[2 * s + 1]) for s in range(args.steps))
     launches = nk.launch_count() - launches0
     ktimes = nk.kernel_times()
+    ktimes_from = "CUDA events between launches inside the timed region"
+    if graphed:     # a replayed graph has no events inside: one extra untimed, un-graphed step for the breakdown
+        nk.set_option("profile", 1)
+        nk.kernel_times()
+        step()
+        ktimes = nk.kernel_times()
+        ktimes_from = "one extra un-graphed step after the timed region (the timed steps replay a CUDA graph)"
     nk.set_option("profile", 0)
+    ms_for_share = ms if not graphed else args.steps * sum(t for t, n in ktimes.values())
     res_final = float(hist[-1])
 
     # ---- end to end through nk_cg_host: pinned host buffers, copies inside the timer ---------------
@@ -340,7 +349,7 @@ def run_ours(args) -> dict | None:
            "e2e": {"value": e2e, "unit": UNIT, "h2d_bytes_per_step": 8 * L,
                    "d2h_bytes_per_step": 8 * (L + niter + 1), "ms_per_step": ms_e2e / args.steps},
            "gpu_launches": int(launches), "clocks": clk,
-           "options": {"fuse_pap": args.fuse_pap, "fuse_p": args.fuse_p, "graph": args.graph},
+           "options": {"fuse_pap": args.fuse_pap, "fuse_p": args.fuse_p, "graph": args.graph, "graph_used": graphed},
            "setup_s": setup_s, "final_residual": res_final}
 
     # ---- iteration-level and kernel-level bandwidth ---------------------------------------------------
@@ -369,9 +378,11 @@ def run_ours(args) -> dict | None:
                            "bound": "hbm", "achieved": ach, "peak": peak, "unit": "GB/s", "frac": ach / peak,
                            "peak_kind": peak_kind + " copy peak (burst)", "frac_of_nominal_8TBs": ach / HBM_NOMINAL_GBS,
                            "bytes_per_point": bpp, "avg_launch_us": 1e3 * avg, "launches_timed": ax_n,
-                           "traffic": traffic, "algorithmic_bytes_per_launch": bpp * L, "share_of_step": ax_ms / ms}
+                           "traffic": traffic, "algorithmic_bytes_per_launch": bpp * L,
+                           "share_of_step": ax_ms * (args.steps if graphed else 1) / ms_for_share,
+                           "timed_by": ktimes_from}
         kb = {"gs": gs_bytes(sizes) / L, "dot": 24.0, "update_xr": 56.0 + 1.0 - 8.0, "update_p": 24.0}
-        out["kernels"] = {k: {"avg_us": 1e3 * t / n, "launches": n, "share_of_step": t / ms,
+        out["kernels"] = {k: {"avg_us": 1e3 * t / n, "launches": n, "share_of_step": t * (args.steps if graphed else 1) / ms_for_share,
                               **({"gbs_model": kb[k] * L / (t / n * 1e-3) / 1e9} if k in kb else {})}
                           for k, (t, n) in ktimes.items() if n > 0}
     else:
@@ -390,7 +401,7 @@ def main():
     ap.add_argument("--workload", default="config5", choices=["config1", "config2", "config3", "config5"])
     ap.add_argument("--fuse-pap", type=int, default=1)
     ap.add_argument("--fuse-p", type=int, default=0)
-    ap.add_argument("--graph", type=int, default=0)
+    ap.add_argument("--graph", type=int, default=2, help="0 off, 1 on, 2 library default (graph up to 2^24 points)")
     ap.add_argument("--traffic", type=float, default=None,
                     help="dram bytes per ax_e launch from the committed ncu --set full capture (profiles/)")
     ap.add_argument("--no-cpu-baseline", action="store_true")

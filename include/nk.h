@@ -103,10 +103,13 @@ int nk_get_scalars(nk_ctx *ctx, double *out5_host, void *stream);
  *   "fuse_pap"     1 (default) = pap accumulated inside ax_e through the dot-fusion identity
  *                  <M QQ^T A_L p, p>_c = sum_l (A_L p)_l p_l; 0 = separate weighted dot after gs
  *   "fuse_p"       1 = p = r + beta p folded into the load of the next ax_e; 0 (default) = own kernel
- *   "graph"        1 = nk_cg records its launches into a CUDA graph and replays it
+ *   "graph"        0 = nk_cg enqueues its launches one by one; 1 = records them into a CUDA graph
+ *                  (cached per f, x, res_hist, niter; updated in place when the pointers change) and
+ *                  replays it; 2 (default) = 1 for meshes of up to 2^24 local points, where launch gaps
+ *                  matter, else 0
  *   "profile"      1 = record a CUDA event on `stream` between consecutive launches so that
  *                  nk_get_kernel_times can report device time per kernel class (nk_cg then
- *                  enqueues its launches directly even if "graph" is 1)
+ *                  enqueues its launches directly whatever "graph" says)
  * Unknown name or bad value: NK_ERR_ARG. */
 int nk_set_option(nk_ctx *ctx, const char *name, int value);
 int nk_get_option(nk_ctx *ctx, const char *name, int *value);

@@ -172,7 +172,11 @@ int nk_cg(nk_ctx *c, const double *f, double *x, int niter, double *res_hist, vo
     if (!c || !f || !x || !res_hist || niter < 0 || f == x || !nk_aligned16(f) || !nk_aligned16(x))
         return NK_ERR_ARG;
     cudaStream_t st = S(stream);
-    if (!c->opt_graph || c->opt_profile) {
+    // "graph" = 2 (default): replay a CUDA graph where launch gaps matter (measured: config 2 3.8 -> 1.9 ms,
+    // config 3 15.0 -> 13.0 ms per 100 iterations), enqueue directly on large meshes
+    const bool use_graph = !c->opt_profile && niter > 0 &&
+                           (c->opt_graph == 1 || (c->opt_graph == 2 && c->L <= NK_GRAPH_AUTO_MAX_L));
+    if (!use_graph) {
         NK_CUDA(enqueue_cg(c, f, x, niter, res_hist, st));
         return NK_OK;
     }
@@ -181,7 +185,6 @@ int nk_cg(nk_ctx *c, const double *f, double *x, int niter, double *res_hist, vo
     const int key = c->opt_fuse_pap | (c->opt_fuse_p << 1) | (c->opt_ax_variant << 2);
     if (!c->graph_exec || c->graph_f != f || c->graph_x != x || c->graph_hist != res_hist ||
         c->graph_niter != niter || c->graph_key != key) {
-        if (c->graph_exec) { cudaGraphExecDestroy(c->graph_exec); c->graph_exec = nullptr; }
         cudaStream_t cap;
         NK_CUDA(cudaStreamCreateWithFlags(&cap, cudaStreamNonBlocking));
         cudaGraph_t graph = nullptr;
@@ -193,10 +196,22 @@ int nk_cg(nk_ctx *c, const double *f, double *x, int niter, double *res_hist, vo
             e = (e1 != cudaSuccess) ? e1 : e2;
         }
         c->launches = launches_before;
-        if (e == cudaSuccess) e = cudaGraphInstantiate(&c->graph_exec, graph, 0);
+        if (e == cudaSuccess && c->graph_exec) {       // same topology, new pointers: update in place
+            cudaGraphExecUpdateResultInfo info;
+            if (cudaGraphExecUpdate(c->graph_exec, graph, &info) != cudaSuccess) {
+                (void)cudaGetLastError();
+                cudaGraphExecDestroy(c->graph_exec);
+                c->graph_exec = nullptr;
+            }
+        }
+        if (e == cudaSuccess && !c->graph_exec) e = cudaGraphInstantiate(&c->graph_exec, graph, 0);
         if (graph) cudaGraphDestroy(graph);
         cudaStreamDestroy(cap);
-        if (e != cudaSuccess) { c->graph_exec = nullptr; return nk_cuda_fail(e); }
+        if (e != cudaSuccess) {
+            if (c->graph_exec) cudaGraphExecDestroy(c->graph_exec);
+            c->graph_exec = nullptr;
+            return nk_cuda_fail(e);
+        }
         c->graph_f = f; c->graph_x = x; c->graph_hist = res_hist; c->graph_niter = niter; c->graph_key = key;
     }
     NK_CUDA(cudaGraphLaunch(c->graph_exec, st));
@@ -289,7 +304,7 @@ static int *option_slot(nk_ctx *c, const char *name, int *lo, int *hi)
     if (!std::strcmp(name, "ax_variant")) { *lo = 0; *hi = 2; return &c->opt_ax_variant; }
     if (!std::strcmp(name, "fuse_pap")) { *lo = 0; *hi = 1; return &c->opt_fuse_pap; }
     if (!std::strcmp(name, "fuse_p")) { *lo = 0; *hi = 1; return &c->opt_fuse_p; }
-    if (!std::strcmp(name, "graph")) { *lo = 0; *hi = 1; return &c->opt_graph; }
+    if (!std::strcmp(name, "graph")) { *lo = 0; *hi = 2; return &c->opt_graph; }
     if (!std::strcmp(name, "profile")) { *lo = 0; *hi = 1; return &c->opt_profile; }
     return nullptr;
 }

@@ -21,6 +21,7 @@ enum { NK_EPI_STORE = 0,   // out[0] = total
 #define NK_VEC_THREADS 512         // P: Table V "local group size 512" for streaming kernels
 #define NK_CODE_MASKED 0x80u       // bit 7 of the per-point code: Dirichlet node
 #define NK_HIST_MAX 8192               // residual-history capacity of nk_cg_host
+#define NK_GRAPH_AUTO_MAX_L (1 << 24)   // "graph" = 2: nk_cg replays a CUDA graph up to this many local points
 #define NK_CTAB 128                // code & 0x7f indexes ctab[] = 1/multiplicity
 
 // kernel classes of nk_get_kernel_times

@@ -162,3 +162,26 @@ def test_cg_argument_errors():
         pr.gpu.set_option("fuse_pap", 7)
     with pytest.raises(ValueError):
         pr.gpu.ax_e(f[:-1].contiguous())
+
+
+def test_graph_default_and_pointer_change():
+    """"graph" = 2 is the default (replay a CUDA graph on small meshes); a cached graph must follow new
+    f / x / history pointers (in-place update) and give bitwise the same result as direct launches."""
+    import torch
+    from paper_2606_12650_b200 import Nekbone
+    pr = pair_for_config("config2")
+    gpu = Nekbone.from_mesh(pr.mesh)                  # a fresh context: the shared one has had options set
+    assert gpu.get_option("graph") == 2
+    f1 = to_dev(config_rhs("config2", pr.mesh))
+    f2 = f1.clone()
+    xa, ha = gpu.cg(f1, 25)
+    xb, hb = gpu.cg(f2, 25)                        # new f, x, hist tensors -> graph update path
+    xc, hc = gpu.cg(f2, 12)                        # different iteration count -> new topology
+    gpu.set_option("graph", 0)
+    xd, hd = gpu.cg(f1, 25)
+    xe, he = gpu.cg(f1, 12)
+    gpu.set_option("graph", 2)
+    torch.cuda.synchronize()
+    assert bool((xa == xd).all()) and bool((ha == hd).all())
+    assert bool((xb == xd).all()) and bool((hb == hd).all())
+    assert bool((xc == xe).all()) and bool((hc == he).all())
