@@ -99,7 +99,11 @@ struct TmaCfg {
     static constexpr int SMEM = R * STAGE_BYTES + WORK_BYTES + BAR_BYTES;
     static_assert(R >= 2, "ring too small");
     // where the next batch's u pencil is requested: 1 = after P3, 2 = after P4 (measured per order)
+#ifdef NK_TMA_PF12
+    static constexpr int PF = (n == 12) ? NK_TMA_PF12 : 1;
+#else
     static constexpr int PF = (n == 12) ? 2 : 1;
+#endif
 };
 
 // ---- mbarrier / bulk-copy PTX ---------------------------------------------------------------------
