@@ -1,6 +1,6 @@
 """Roofline sweep of ax_e, gs and ax (BASELINE.json configs[3]).
 
-    python -m paper_2606_12650_b200.sweep [--which e|n|both] [--reps 50] [--out sweep.csv]
+    python -m paper_2606_12650_b200.sweep [--which e|n|both|paper] [--reps 50] [--out sweep.csv]
 
 4a: brick meshes with E = 2^10 .. 2^17 at N = 7;  4b: N = 3 .. 15 at E = 4096 (16^3); perturbed
 geometry (amplitude 0.05), u uniform[-1,1) per LOCAL point (seed 1004), `reps` back-to-back
@@ -82,12 +82,52 @@ def run_point(point, reps):
     return rows
 
 
+def run_paper_sweep(out):
+    """The paper's own sweep (S 8(f) f-2, Figs 7-12): N in {4, 6, 8}, E = 2^1 .. 2^14,
+    100 warm-up + 100 timed CG iterations, mean of 5 runs, GDOFS = E N^3 100 / (t 1e9) (Eq. 1) and the
+    final residual.  Meshes and RHS are this repo's seeded bricks (amplitude 0.05, seed 1004): the
+    paper's own generator is not available, so only the SHAPE of its curves is comparable."""
+    import torch
+    from paper_2606_12650_b200 import Nekbone
+    from workloads import brick_mesh, rhs_unique, sweep_brick
+    from workloads.configs import SWEEP_AMPLITUDE, SWEEP_SEED
+    lines = ["N,E,n_local,dofs_E_N3,ms_per_100_iterations_mean_of_5,GDOFS,final_residual,graph"]
+    for N in (4, 6, 8):
+        for k in range(1, 15):
+            mesh = brick_mesh(*sweep_brick(k), N, SWEEP_AMPLITUDE)
+            nk = Nekbone.from_mesh(mesh)
+            f = torch.from_numpy(rhs_unique(mesh, SWEEP_SEED)).cuda()
+            x = nk.empty()
+            hist = torch.empty(101, dtype=torch.float64, device="cuda")
+            nk.cg(f, 100, x=x, res_hist=hist)                       # 100 warm-up iterations
+            torch.cuda.synchronize()
+            ts = []
+            for _ in range(5):
+                e0, e1 = torch.cuda.Event(enable_timing=True), torch.cuda.Event(enable_timing=True)
+                e0.record()
+                nk.cg(f, 100, x=x, res_hist=hist)
+                e1.record()
+                torch.cuda.synchronize()
+                ts.append(e0.elapsed_time(e1))
+            t = float(np.mean(ts))
+            dofs = mesh.E * N ** 3
+            lines.append(f"{N},{mesh.E},{mesh.L},{dofs},{t:.4f},{dofs * 100 / (t * 1e-3) / 1e9:.4f},"
+                         f"{float(hist[-1]):.6e},{int(mesh.L <= (1 << 24))}")
+            print(lines[-1], flush=True)
+            nk.close()
+    if out:
+        with open(out, "w") as fh:
+            fh.write("\n".join(lines) + "\n")
+
+
 def main():
     ap = argparse.ArgumentParser()
-    ap.add_argument("--which", default="both", choices=["e", "n", "both"])
+    ap.add_argument("--which", default="both", choices=["e", "n", "both", "paper"])
     ap.add_argument("--reps", type=int, default=None)
     ap.add_argument("--out", default=None)
     args = ap.parse_args()
+    if args.which == "paper":
+        return run_paper_sweep(args.out)
     from workloads import E_SWEEP, N_SWEEP, SWEEP_REPEATS
     reps = args.reps or SWEEP_REPEATS
     peak, kind = _peak()
