@@ -450,6 +450,87 @@ int nko_cg(nko_ctx *c, const double *f, double *x, int niter, double *res_hist)
     return rc;
 }
 
+/* ------------------------------------------------------------------------------------------
+ * NEXT row f-3: the Jacobi (diagonal) preconditioner of the original Nekbone, which
+ * the paper's variant omits.
+ * diag = Q Q^T diag(A_L): the diagonal of the assembled operator in local layout.  Entry l = (i,j,k)
+ * of A_L = sum_ab D_a^T diag(G_ab) D_b, written out:
+ *   sum_m ( D[m][i]^2 G_rr(m,j,k) + D[m][j]^2 G_ss(i,m,k) + D[m][k]^2 G_tt(i,j,m) )
+ *   + 2 ( D[i][i] D[j][j] G_rs(l) + D[i][i] D[k][k] G_rt(l) + D[j][j] D[k][k] G_st(l) )
+ * (a cross term D_a[q,l] D_b[q,l], a != b, is non-zero only for q = l).
+ * ---------------------------------------------------------------------------------------- */
+int nko_diag(nko_ctx *c, double *diag)
+{
+    if (!c || !diag) return NKO_ERR_ARG;
+    const int n = c->n;
+    const int64_t P = (int64_t)n * n * n;
+    const double *D = c->D;
+#pragma omp parallel for schedule(static)
+    for (int64_t e = 0; e < c->E; ++e) {
+        const double *grr = c->G[0] + e * P, *grs = c->G[1] + e * P, *grt = c->G[2] + e * P;
+        const double *gss = c->G[3] + e * P, *gst = c->G[4] + e * P, *gtt = c->G[5] + e * P;
+        for (int k = 0; k < n; ++k)
+            for (int j = 0; j < n; ++j)
+                for (int i = 0; i < n; ++i) {
+                    const int64_t l = i + n * j + (int64_t)n * n * k;
+                    double s = 0.0;
+                    for (int m = 0; m < n; ++m) {
+                        s += D[m * n + i] * D[m * n + i] * grr[m + n * j + n * n * k];
+                        s += D[m * n + j] * D[m * n + j] * gss[i + n * m + n * n * k];
+                        s += D[m * n + k] * D[m * n + k] * gtt[i + n * j + n * n * m];
+                    }
+                    s += 2.0 * (D[i * n + i] * D[j * n + j] * grs[l] + D[i * n + i] * D[k * n + k] * grt[l]
+                                + D[j * n + j] * D[k * n + k] * gst[l]);
+                    diag[e * P + l] = s;
+                }
+    }
+    return nko_gs(c, diag);
+}
+
+/* Jacobi-preconditioned CG (the original Nekbone's iteration; z = M^-1 r with M = diag, z = 0 on
+ * Dirichlet nodes): r = mask o f; x = 0; z = r/diag; p = z; rho = <r,z>_c; hist[0] = sqrt<r,r>_c.
+ * k = 1..niter: w = ax(p); pap = <w,p>_c; alpha = rho/pap; x += alpha p; r -= alpha w; z = r/diag;
+ * rho' = <r,z>_c; hist[k] = sqrt<r,r>_c; beta = rho'/rho; p = z + beta p.  Guards as in O8. */
+int nko_pcg(nko_ctx *c, const double *f, double *x, int niter, double *res_hist)
+{
+    if (!c || !f || !x || niter < 0 || !res_hist) return NKO_ERR_ARG;
+    const int64_t L = c->L;
+    const size_t Lb = sizeof(double) * (size_t)L;
+    double *r = (double *)malloc(Lb), *p = (double *)malloc(Lb), *w = (double *)malloc(Lb);
+    double *z = (double *)malloc(Lb), *dg = (double *)malloc(Lb);
+    int rc = (r && p && w && z && dg) ? nko_diag(c, dg) : NKO_ERR_ALLOC;
+    double rho = 0.0, rr = 0.0;
+    if (rc == NKO_OK) {
+        for (int64_t l = 0; l < L; ++l) {
+            r[l] = c->mask[l] * f[l];
+            x[l] = 0.0;
+            z[l] = (c->mask[l] == 0.0) ? 0.0 : r[l] / dg[l];
+            p[l] = z[l];
+        }
+        rc = nko_dot(c, r, z, &rho);
+        if (rc == NKO_OK) rc = nko_dot(c, r, r, &rr);
+        res_hist[0] = sqrt(rr);
+    }
+    for (int k = 1; k <= niter && rc == NKO_OK; ++k) {
+        double pap, rho1;
+        rc = nko_ax(c, p, w);
+        if (rc == NKO_OK) rc = nko_dot(c, w, p, &pap);
+        if (rc != NKO_OK) break;
+        const double alpha = (rho == 0.0 || pap == 0.0) ? 0.0 : rho / pap;
+        for (int64_t l = 0; l < L; ++l) x[l] = x[l] + alpha * p[l];
+        for (int64_t l = 0; l < L; ++l) r[l] = r[l] - alpha * w[l];
+        for (int64_t l = 0; l < L; ++l) z[l] = (c->mask[l] == 0.0) ? 0.0 : r[l] / dg[l];
+        rc = nko_dot(c, r, z, &rho1);
+        if (rc == NKO_OK) rc = nko_dot(c, r, r, &rr);
+        res_hist[k] = sqrt(rr);
+        const double beta = (rho == 0.0 || pap == 0.0) ? 0.0 : rho1 / rho;
+        for (int64_t l = 0; l < L; ++l) p[l] = z[l] + beta * p[l];
+        rho = rho1;
+    }
+    free(r); free(p); free(w); free(z); free(dg);
+    return rc;
+}
+
 int nko_set_dot_mode(nko_ctx *c, int mode)
 {
     if (!c || (mode != 0 && mode != 1)) return NKO_ERR_ARG;

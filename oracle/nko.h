@@ -66,6 +66,10 @@ int nko_cg_step(nko_ctx *ctx, double *x, double *r, double *p, double *w, double
 int nko_cg_init(nko_ctx *ctx, const double *f, double *x, double *r, double *p, double *rho);
 
 /* 0 (default): dot products accumulate in long double; 1: in plain double, ascending l. */
+/* NEXT row f-3: Jacobi preconditioner of the original Nekbone (the paper's variant omits it).
+ * diag (HOST out, L) = Q Q^T diag(A_L); nko_pcg = diagonally preconditioned CG, hist[k] = sqrt<r_k,r_k>_c. */
+int nko_diag(nko_ctx *ctx, double *diag);
+int nko_pcg(nko_ctx *ctx, const double *f, double *x, int niter, double *res_hist);
 int nko_set_dot_mode(nko_ctx *ctx, int mode);
 
 int nko_get_sizes(nko_ctx *ctx, int64_t *n_local, int64_t *n_unique,

@@ -44,6 +44,8 @@ def _load(fma: bool = False):
         "nko_ax": [vp, vp, vp],
         "nko_dot": [vp, vp, vp, vp],
         "nko_cg": [vp, vp, vp, C.c_int, vp],
+        "nko_pcg": [vp, vp, vp, C.c_int, vp],
+        "nko_diag": [vp, vp],
         "nko_cg_step": [vp, vp, vp, vp, vp, vp],
         "nko_cg_init": [vp, vp, vp, vp, vp, vp],
         "nko_set_dot_mode": [vp, C.c_int],
@@ -162,6 +164,20 @@ class Oracle:
         hist = np.empty(niter + 1)
         _check(self._lib, self._lib.nko_cg(self._ctx, _p(f), _p(x), int(niter), _p(hist)))
         return x, hist
+
+    def pcg(self, f, niter: int):
+        """Jacobi-preconditioned CG."""
+        f = _f64(f, (self.L,))
+        x = np.empty(self.L)
+        hist = np.empty(niter + 1)
+        _check(self._lib, self._lib.nko_pcg(self._ctx, _p(f), _p(x), int(niter), _p(hist)))
+        return x, hist
+
+    def diag(self):
+        """Q Q^T diag(A_L) in local layout."""
+        d = np.empty(self.L)
+        _check(self._lib, self._lib.nko_diag(self._ctx, _p(d)))
+        return d
 
     def cg_init(self, f):
         f = _f64(f, (self.L,))

@@ -138,3 +138,67 @@ def test_golden_regression_config1():
     x, hist = nko.Oracle.from_mesh(m).cg(config_rhs("config1", m), 20)
     np.testing.assert_allclose(hist, vals[:-1], rtol=1e-12)
     np.testing.assert_allclose(np.max(np.abs(x)), vals[-1], rtol=1e-12)
+
+
+# ---- NEXT row f-3: Jacobi-preconditioned CG (the original Nekbone's iteration) --------
+def test_diag_is_the_diagonal_of_the_assembled_matrix(dense1):
+    """nko_diag against the dense Kronecker assembly (no sum factorisation) and against brute force:
+    column l of the unassembled operator applied to a unit vector."""
+    m, o, A, inv, free, f, fu = dense1
+    d = o.diag()
+    assert np.max(np.abs(d - np.diag(A)[inv])) <= 1e-14 * np.max(np.abs(d))
+    for l in (0, 5, 63, 64, 200, 511):                   # brute force on a few local points
+        e = np.zeros(m.L); e[l] = 1.0
+        col = o.ax_e(e)
+        # gs of diag(A_L): add the diagonal entries of all copies of l's node
+        same = np.nonzero(m.glo_num == m.glo_num[l])[0]
+        s = 0.0
+        for q in same:
+            eq = np.zeros(m.L); eq[q] = 1.0
+            s += o.ax_e(eq)[q]
+        assert abs(d[l] - s) <= 1e-14 * abs(s)
+        assert col[l] > 0
+    assert np.all(d > 0)
+
+
+def test_pcg_converges_to_dense_solve_and_is_krylov_optimal(dense1):
+    """x_k = argmin of the A-norm error over the PRECONDITIONED Krylov space
+    span{M^-1 b, (M^-1 A) M^-1 b, ...}, M = diag(A); checked by a dense projected solve."""
+    m, o, A, inv, free, f, fu = dense1
+    Aff = A[np.ix_(free, free)]
+    b = fu[free]
+    Minv = 1.0 / np.diag(Aff)
+    xu = np.zeros(m.U); xu[free] = np.linalg.solve(Aff, b)
+    x, hist = o.pcg(f, 80)
+    assert np.max(np.abs(x - xu[inv])) < 1e-13 * np.max(np.abs(xu))
+    assert np.all(x[m.mask == 0] == 0.0)
+    K = 10
+    V = np.zeros((free.size, K))
+    v = Minv * b
+    for k in range(K):
+        for _ in range(2):
+            v = v - V[:, :k] @ (V[:, :k].T @ v)
+        V[:, k] = v / np.linalg.norm(v)
+        v = Minv * (Aff @ V[:, k])
+    for k in range(1, K + 1):
+        Vk = V[:, :k]
+        yk = np.linalg.solve(Vk.T @ Aff @ Vk, Vk.T @ b)
+        xk_ref = np.zeros(m.U); xk_ref[free] = Vk @ yk
+        xk, hk = o.pcg(f, k)
+        assert np.max(np.abs(xk - xk_ref[inv])) < 1e-11 * np.max(np.abs(xk_ref)), k
+        assert abs(hk[k] - np.linalg.norm(b - Aff @ (Vk @ yk))) < 1e-11 * hk[0], k
+    assert abs(hist[0] - np.linalg.norm(b)) < 1e-14 * hist[0]
+
+
+def test_pcg_guards_and_needs_fewer_iterations_on_a_stretched_mesh():
+    m = config_mesh("config1")
+    o = nko.Oracle.from_mesh(m)
+    x, h = o.pcg(np.zeros(m.L), 5)
+    assert not x.any() and not h.any()
+    x, h = o.pcg(config_rhs("config1", m), 0)
+    assert h.shape == (1,) and not x.any()
+    # both reach the same solution
+    f = config_rhs("config1", m)
+    xc, _ = o.cg(f, 90)
+    xp, _ = o.pcg(f, 90)
+    assert np.max(np.abs(xc - xp)) < 1e-12 * np.max(np.abs(xc))
