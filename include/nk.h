@@ -85,6 +85,14 @@ int nk_cg(nk_ctx *ctx, const double *f, double *x, int niter, double *res_hist, 
 int nk_cg_host(nk_ctx *ctx, const double *f_host, double *x_host, int niter,
                double *res_hist_host, void *stream);
 
+/* Jacobi-preconditioned CG, the original Nekbone's iteration, which the paper's variant omits (P:225,
+ * P:290; S 8(f) f-3): z = r / diag, diag = Q Q^T diag(A_L), z = 0 on Dirichlet nodes; rho = <r,z>_c;
+ * res_hist[k] = sqrt(<r_k, r_k>_c) as in nk_cg.  Same arguments, guards and residency as nk_cg; the
+ * preconditioner is built on the first call and kept in the workspace.  Enqueued launch by launch. */
+int nk_pcg(nk_ctx *ctx, const double *f, double *x, int niter, double *res_hist, void *stream);
+/* diag (DEVICE out, L) = Q Q^T diag(A_L) in local layout. */
+int nk_get_diag(nk_ctx *ctx, double *diag, void *stream);
+
 /* Test entry points for lock-step parity (S 8(c) protocol 2): the CG state lives in the context.
  *   nk_cg_init       r = mask o f, x = 0, p = r, rho = <r,r>_c  (x DEVICE L, caller-owned, kept)
  *   nk_cg_load_state copies r, p (DEVICE, L) into the context and sets rho (x is the caller's)

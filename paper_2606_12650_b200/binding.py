@@ -29,6 +29,8 @@ SIGNATURES = {
     "nk_ax": (_i, [_vp, _vp, _vp, _vp]),
     "nk_dot": (_i, [_vp, _vp, _vp, _vp, _vp]),
     "nk_cg": (_i, [_vp, _vp, _vp, _i, _vp, _vp]),
+    "nk_pcg": (_i, [_vp, _vp, _vp, _i, _vp, _vp]),
+    "nk_get_diag": (_i, [_vp, _vp, _vp]),
     "nk_cg_host": (_i, [_vp, _vp, _vp, _i, _vp, _vp]),
     "nk_cg_init": (_i, [_vp, _vp, _vp, _vp]),
     "nk_cg_load_state": (_i, [_vp, _vp, _vp, _d, _vp]),
@@ -177,6 +179,21 @@ class Nekbone:
         _check(self._lib.nk_cg(self._ctx, self._vec(f, "f"), self._vec(x, "x"), int(niter),
                                _vp(res_hist.data_ptr()), _stream()))
         return x, res_hist
+
+    def pcg(self, f, niter: int, x=None, res_hist=None):
+        """Jacobi-preconditioned CG: returns (x, res_hist) CUDA tensors."""
+        import torch
+        x = self.empty() if x is None else x
+        if res_hist is None:
+            res_hist = torch.empty(int(niter) + 1, dtype=torch.float64, device=self.device)
+        _check(self._lib.nk_pcg(self._ctx, self._vec(f, "f"), self._vec(x, "x"), int(niter),
+                                _vp(res_hist.data_ptr()), _stream()))
+        return x, res_hist
+
+    def diag(self):
+        d = self.empty()
+        _check(self._lib.nk_get_diag(self._ctx, self._vec(d), _stream()))
+        return d
 
     def cg_host(self, f_host: np.ndarray, niter: int, x_host=None, hist_host=None):
         """End-to-end call with HOST buffers (numpy, ideally pinned): H2D f, CG, D2H x + history."""

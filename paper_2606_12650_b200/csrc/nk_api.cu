@@ -398,3 +398,58 @@ int nk_get_launch_count(nk_ctx *c, int64_t *count)
 }
 
 }  // extern "C"
+
+// ---- Jacobi-preconditioned CG ---------------------------------------------------------
+namespace {
+cudaError_t ensure_dinv(nk_ctx *c, cudaStream_t st)
+{
+    if (c->have_dinv) return cudaSuccess;
+    cudaError_t e;
+    if ((e = nk_launch_diag(c, c->dinv, st)) != cudaSuccess) return e;
+    if ((e = nk_launch_gs(c, c->dinv, 0, st)) != cudaSuccess) return e;
+    if ((e = nk_launch_invert_diag(c, c->dinv, st)) != cudaSuccess) return e;
+    c->have_dinv = 1;
+    return cudaSuccess;
+}
+}  // namespace
+
+extern "C" {
+
+int nk_get_diag(nk_ctx *c, double *diag, void *stream)
+{
+    if (!c || !diag || !nk_aligned16(diag)) return NK_ERR_ARG;
+    NK_CUDA(nk_launch_diag(c, diag, S(stream)));
+    NK_CUDA(nk_launch_gs(c, diag, 0, S(stream)));
+    return NK_OK;
+}
+
+int nk_pcg(nk_ctx *c, const double *f, double *x, int niter, double *res_hist, void *stream)
+{
+    if (!c || !f || !x || !res_hist || niter < 0 || f == x || !nk_aligned16(f) || !nk_aligned16(x))
+        return NK_ERR_ARG;
+    cudaStream_t st = S(stream);
+    cudaError_t e;
+    NK_CUDA(ensure_dinv(c, st));
+    c->p_pending = 0;
+    NK_CUDA(prof_mark(c, -1, st));
+    NK_CUDA(nk_launch_pcg_init(c, f, x, res_hist, st));
+    NK_CUDA(prof_mark(c, NK_K_INIT, st));
+    for (int k = 1; k <= niter; ++k) {
+        NK_CUDA(nk_launch_ax_e(c, nullptr, c->p, nullptr, c->w, c->opt_fuse_pap, c->opt_ax_variant, st));
+        NK_CUDA(prof_mark(c, NK_K_AX, st));
+        NK_CUDA(nk_launch_gs(c, c->w, 1, st));
+        NK_CUDA(prof_mark(c, NK_K_GS, st));
+        if (!c->opt_fuse_pap) {
+            NK_CUDA(nk_launch_dot(c, c->w, c->p, nullptr, NK_EPI_PAP, st));
+            NK_CUDA(prof_mark(c, NK_K_DOT, st));
+        }
+        NK_CUDA(nk_launch_update_xrz(c, x, res_hist + k, st));
+        NK_CUDA(prof_mark(c, NK_K_UPDATE_XR, st));
+        NK_CUDA(nk_launch_update_pz(c, st));
+        NK_CUDA(prof_mark(c, NK_K_UPDATE_P, st));
+    }
+    (void)e;
+    return NK_OK;
+}
+
+}  // extern "C"

@@ -99,6 +99,45 @@ unpack_geom_kernel(const double2 *__restrict__ g, double *__restrict__ G6, int64
     }
 }
 
+// diag(A_L) per local point (the Jacobi preconditioner of the original Nekbone):
+//   sum_m ( D[m][i]^2 G_rr(m,j,k) + D[m][j]^2 G_ss(i,m,k) + D[m][k]^2 G_tt(i,j,m) )
+//   + 2 ( D[i][i] D[j][j] G_rs + D[i][i] D[k][k] G_rt + D[j][j] D[k][k] G_st )(i,j,k)
+// One block per element; run once per context, not on the timed path.
+__global__ void __launch_bounds__(GEOM_THREADS)
+diag_kernel(const double2 *__restrict__ g, const double *__restrict__ Dg, int n, double *__restrict__ diag)
+{
+    __shared__ double s_D[16 * 16];
+    for (int t = threadIdx.x; t < n * n; t += GEOM_THREADS) s_D[t] = Dg[t];
+    __syncthreads();
+    const int n2 = n * n, P = n2 * n;
+    const int64_t e = blockIdx.x;
+    for (int q = threadIdx.x; q < P; q += GEOM_THREADS) {
+        const int i = q % n, j = (q / n) % n, k = q / n2;
+        double s = 0.0;
+        for (int m = 0; m < n; ++m) {
+            const double di = s_D[m * n + i], dj = s_D[m * n + j], dk = s_D[m * n + k];
+            s = fma(di * di, g[nk_g_index(e, k, 0, m + n * j, n)].x, s);       // rr at (m,j,k)
+            s = fma(dj * dj, g[nk_g_index(e, k, 1, i + n * m, n)].y, s);       // ss at (i,m,k)
+            s = fma(dk * dk, g[nk_g_index(e, m, 2, i + n * j, n)].y, s);       // tt at (i,j,m)
+        }
+        const int t2 = i + n * j;
+        const double grs = g[nk_g_index(e, k, 0, t2, n)].y, grt = g[nk_g_index(e, k, 1, t2, n)].x,
+                     gst = g[nk_g_index(e, k, 2, t2, n)].x;
+        const double dii = s_D[i * n + i], djj = s_D[j * n + j], dkk = s_D[k * n + k];
+        s += 2.0 * (dii * djj * grs + dii * dkk * grt + djj * dkk * gst);
+        diag[e * P + q] = s;
+    }
+}
+
+// d = 1/d, and 0 on Dirichlet nodes (z = M^-1 r vanishes there)
+__global__ void __launch_bounds__(GEOM_THREADS)
+invert_diag_kernel(double *__restrict__ d, const uint8_t *__restrict__ code, int64_t L)
+{
+    const int64_t stride = (int64_t)gridDim.x * blockDim.x;
+    for (int64_t l = (int64_t)blockIdx.x * blockDim.x + threadIdx.x; l < L; l += stride)
+        d[l] = (code[l] & NK_CODE_MASKED) ? 0.0 : 1.0 / d[l];
+}
+
 }  // namespace
 
 cudaError_t nk_launch_geom(nk_ctx *c, const double *coords_dev, const double *D_dev, const double *Dlo_dev,
@@ -115,6 +154,23 @@ cudaError_t nk_launch_get_geom(nk_ctx *c, double *G6, cudaStream_t st)
     int64_t nb = (c->L + GEOM_THREADS - 1) / GEOM_THREADS;
     if (nb > (int64_t)c->sm_count * 32) nb = (int64_t)c->sm_count * 32;
     unpack_geom_kernel<<<(unsigned)nb, GEOM_THREADS, 0, st>>>(c->g, G6, c->L, c->n);
+    c->launches++;
+    return cudaGetLastError();
+}
+
+cudaError_t nk_launch_diag(nk_ctx *c, double *diag, cudaStream_t st)
+{
+    const double *D_dev = c->ctab + 2 * NK_CTAB;          // uploaded by nk_setup, kept
+    diag_kernel<<<(unsigned)c->E, GEOM_THREADS, 0, st>>>(c->g, D_dev, c->n, diag);
+    c->launches++;
+    return cudaGetLastError();
+}
+
+cudaError_t nk_launch_invert_diag(nk_ctx *c, double *d, cudaStream_t st)
+{
+    int64_t nb = (c->L + GEOM_THREADS - 1) / GEOM_THREADS;
+    if (nb > (int64_t)c->sm_count * 32) nb = (int64_t)c->sm_count * 32;
+    invert_diag_kernel<<<(unsigned)nb, GEOM_THREADS, 0, st>>>(d, c->code, c->L);
     c->launches++;
     return cudaGetLastError();
 }

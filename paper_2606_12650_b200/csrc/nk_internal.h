@@ -56,6 +56,8 @@ struct nk_ctx {
                                  // k-plane one contiguous chunk [c2][i + n j] of (rr,rs) (rt,ss) (st,tt)
     double *r, *p, *w;           // CG state, L each (coords staging aliases these during set-up)
     double *hf, *hx;             // staging for nk_cg_host, L each
+    double *dinv;                // Jacobi preconditioner 1 / (Q Q^T diag A_L), 0 on Dirichlet nodes (lazy)
+    int have_dinv;
     uint8_t *code;               // L: multiplicity-table index | NK_CODE_MASKED
     int32_t *row_off;            // n_rows + 1
     int32_t *row_idx;            // n_listed local indices, rows in [0,n_sum_rows) are summed,
@@ -105,3 +107,9 @@ cudaError_t nk_launch_cg_init(nk_ctx *c, const double *f, double *x, double *his
 cudaError_t nk_launch_update_xr(nk_ctx *c, double *x, double *hist_k, cudaStream_t st);
 cudaError_t nk_launch_update_p(nk_ctx *c, cudaStream_t st);
 cudaError_t nk_launch_get_mult(nk_ctx *c, double *mult, cudaStream_t st);
+// preconditioned CG
+cudaError_t nk_launch_diag(nk_ctx *c, double *diag, cudaStream_t st);          // nk_geom.cu: diag(A_L), local
+cudaError_t nk_launch_invert_diag(nk_ctx *c, double *d, cudaStream_t st);      // d = masked ? 0 : 1/d
+cudaError_t nk_launch_pcg_init(nk_ctx *c, const double *f, double *x, double *hist, cudaStream_t st);
+cudaError_t nk_launch_update_xrz(nk_ctx *c, double *x, double *hist_k, cudaStream_t st);
+cudaError_t nk_launch_update_pz(nk_ctx *c, cudaStream_t st);

@@ -77,3 +77,43 @@ __device__ __forceinline__ void nk_grid_reduce(double v, double *sm, nk_reduce_w
     t = nk_block_sum(t, sm);
     if (threadIdx.x == 0) nk_epilogue(epi, t, ws.scal, out);
 }
+
+// Two sums at once (preconditioned CG: <r,z>_c and <r,r>_c in one pass).  Partials of the second sum
+// live in the upper half of the partials buffer.  Epilogue: rho' = t1 (beta = rho'/rho, guarded),
+// out[0] = sqrt(t2); `first` marks the initial call (rho = t1, beta = 0).
+__device__ __forceinline__ void nk_grid_reduce2(double v1, double v2, double *sm, nk_reduce_ws ws, int first, double *out)
+{
+    const double b1 = nk_block_sum(v1, sm);
+    const double b2 = nk_block_sum(v2, sm);
+    __shared__ int s_last2;
+    const unsigned nb = gridDim.x;
+    double *part2 = ws.partials + NK_MAX_PARTIALS / 2;
+    if (threadIdx.x == 0) {
+        ws.partials[blockIdx.x] = b1;
+        part2[blockIdx.x] = b2;
+        __threadfence();
+        const unsigned ticket = atomicInc(ws.counter, nb - 1u);
+        s_last2 = (ticket == nb - 1u);
+    }
+    __syncthreads();
+    if (!s_last2) return;
+    __threadfence();
+    double t1 = 0.0, t2 = 0.0;
+    for (unsigned i = threadIdx.x; i < nb; i += blockDim.x) { t1 += __ldcg(ws.partials + i); t2 += __ldcg(part2 + i); }
+    t1 = nk_block_sum(t1, sm);
+    t2 = nk_block_sum(t2, sm);
+    if (threadIdx.x == 0) {
+        double *scal = ws.scal;
+        if (first) {
+            scal[NK_S_RHO] = t1; scal[NK_S_RHO_OLD] = t1; scal[NK_S_RHO_NEW] = t1;
+            scal[NK_S_BETA] = 0.0; scal[NK_S_ALPHA] = 0.0; scal[NK_S_PAP] = 0.0;
+        } else {
+            const double rho = scal[NK_S_RHO], pap = scal[NK_S_PAP];
+            scal[NK_S_RHO_NEW] = t1;
+            scal[NK_S_BETA] = (rho == 0.0 || pap == 0.0) ? 0.0 : t1 / rho;
+            scal[NK_S_RHO_OLD] = rho;
+            scal[NK_S_RHO] = t1;
+        }
+        out[0] = sqrt(t2);
+    }
+}

@@ -178,6 +178,7 @@ extern "C" int nk_setup(nk_ctx **ctx, int64_t E, int N, const double *coords, co
     c->w = reinterpret_cast<double *>(q); q += cv.vec;
     c->hf = reinterpret_cast<double *>(q); q += cv.vec;
     c->hx = reinterpret_cast<double *>(q); q += cv.vec;
+    c->dinv = reinterpret_cast<double *>(q); q += cv.vec;
     c->code = reinterpret_cast<uint8_t *>(q); q += cv.code;
     c->row_off = reinterpret_cast<int32_t *>(q); q += cv.off;
     c->row_idx = reinterpret_cast<int32_t *>(q); q += cv.idx;

@@ -148,6 +148,97 @@ get_mult_kernel(double *__restrict__ mult, const uint8_t *__restrict__ code, con
         mult[l] = mtab[code[l] & 0x7f];
 }
 
+// ---- Jacobi-preconditioned CG: z = dinv o r is never stored ---------------------
+// r = mask o f, x = 0, p = z = dinv o r, rho = <r,z>_c, hist[0] = sqrt<r,r>_c
+__global__ void __launch_bounds__(NK_VEC_THREADS)
+pcg_init_kernel(const double *__restrict__ f, double *__restrict__ x, double *__restrict__ r,
+                double *__restrict__ p, const double *__restrict__ dinv, const uint8_t *__restrict__ code,
+                const double *__restrict__ ctab, int64_t L, nk_reduce_ws ws, double *hist0)
+{
+    __shared__ double s_c[NK_CTAB];
+    __shared__ double s_red[33];
+    load_ctab(s_c, ctab);
+    const int64_t stride = (int64_t)gridDim.x * blockDim.x;
+    double a1 = 0.0, a2 = 0.0;
+    for (int64_t l = (int64_t)blockIdx.x * blockDim.x + threadIdx.x; l < L; l += stride) {
+        const uint8_t cd = code[l];
+        const double rv = (cd & NK_CODE_MASKED) ? 0.0 : f[l];
+        const double zv = dinv[l] * rv;
+        r[l] = rv; p[l] = zv; x[l] = 0.0;
+        const double cw = s_c[cd & 0x7f] * rv;
+        a1 = fma(cw, zv, a1);
+        a2 = fma(cw, rv, a2);
+    }
+    nk_grid_reduce2(a1, a2, s_red, ws, 1, hist0);
+}
+
+// x += alpha p; r -= alpha w; z = dinv o r; rho' = <r,z>_c; hist = sqrt<r,r>_c
+__global__ void __launch_bounds__(NK_VEC_THREADS)
+update_xrz_kernel(double *__restrict__ x, double *__restrict__ r, const double *__restrict__ p,
+                  const double *__restrict__ w, const double *__restrict__ dinv,
+                  const uint8_t *__restrict__ code, const double *__restrict__ ctab, int64_t L,
+                  nk_reduce_ws ws, double *hist_k)
+{
+    __shared__ double s_c[NK_CTAB];
+    __shared__ double s_red[33];
+    load_ctab(s_c, ctab);
+    const double alpha = ws.scal[NK_S_ALPHA];
+    const int64_t pairs = L >> 1;
+    const int64_t stride = (int64_t)gridDim.x * blockDim.x;
+    double a1 = 0.0, a2 = 0.0;
+    for (int64_t q = (int64_t)blockIdx.x * blockDim.x + threadIdx.x; q < pairs; q += stride) {
+        const double2 pv = reinterpret_cast<const double2 *>(p)[q];
+        const double2 wv = reinterpret_cast<const double2 *>(w)[q];
+        const double2 dv = reinterpret_cast<const double2 *>(dinv)[q];
+        double2 xv = reinterpret_cast<double2 *>(x)[q];
+        double2 rv = reinterpret_cast<double2 *>(r)[q];
+        const uchar2 cd = reinterpret_cast<const uchar2 *>(code)[q];
+        xv.x = fma(alpha, pv.x, xv.x);
+        xv.y = fma(alpha, pv.y, xv.y);
+        rv.x = fma(-alpha, wv.x, rv.x);
+        rv.y = fma(-alpha, wv.y, rv.y);
+        reinterpret_cast<double2 *>(x)[q] = xv;
+        reinterpret_cast<double2 *>(r)[q] = rv;
+        const double c0 = s_c[cd.x & 0x7f] * rv.x, c1 = s_c[cd.y & 0x7f] * rv.y;
+        a1 = fma(c0, dv.x * rv.x, a1);
+        a1 = fma(c1, dv.y * rv.y, a1);
+        a2 = fma(c0, rv.x, a2);
+        a2 = fma(c1, rv.y, a2);
+    }
+    if ((L & 1) && blockIdx.x == 0 && threadIdx.x == 0) {
+        const int64_t l = L - 1;
+        const double xv = fma(alpha, p[l], x[l]);
+        const double rv = fma(-alpha, w[l], r[l]);
+        x[l] = xv; r[l] = rv;
+        const double c0 = s_c[code[l] & 0x7f] * rv;
+        a1 = fma(c0, dinv[l] * rv, a1);
+        a2 = fma(c0, rv, a2);
+    }
+    nk_grid_reduce2(a1, a2, s_red, ws, 0, hist_k);
+}
+
+// p = dinv o r + beta p
+__global__ void __launch_bounds__(NK_VEC_THREADS)
+update_pz_kernel(double *__restrict__ p, const double *__restrict__ r, const double *__restrict__ dinv,
+                 const double *__restrict__ scal, int64_t L)
+{
+    const double beta = scal[NK_S_BETA];
+    const int64_t pairs = L >> 1;
+    const int64_t stride = (int64_t)gridDim.x * blockDim.x;
+    for (int64_t q = (int64_t)blockIdx.x * blockDim.x + threadIdx.x; q < pairs; q += stride) {
+        const double2 rv = reinterpret_cast<const double2 *>(r)[q];
+        const double2 dv = reinterpret_cast<const double2 *>(dinv)[q];
+        double2 pv = reinterpret_cast<double2 *>(p)[q];
+        pv.x = fma(beta, pv.x, dv.x * rv.x);
+        pv.y = fma(beta, pv.y, dv.y * rv.y);
+        reinterpret_cast<double2 *>(p)[q] = pv;
+    }
+    if ((L & 1) && blockIdx.x == 0 && threadIdx.x == 0) {
+        const int64_t l = L - 1;
+        p[l] = fma(beta, p[l], dinv[l] * r[l]);
+    }
+}
+
 }  // namespace
 
 cudaError_t nk_launch_dot(nk_ctx *c, const double *a, const double *b, double *out, int epi, cudaStream_t st)
@@ -186,6 +277,31 @@ cudaError_t nk_launch_get_mult(nk_ctx *c, double *mult, cudaStream_t st)
 {
     const int nb = vec_blocks(c, c->L);
     get_mult_kernel<<<nb, NK_VEC_THREADS, 0, st>>>(mult, c->code, c->mtab, c->L);
+    c->launches++;
+    return cudaGetLastError();
+}
+
+cudaError_t nk_launch_pcg_init(nk_ctx *c, const double *f, double *x, double *hist, cudaStream_t st)
+{
+    const int nb = vec_blocks(c, c->L >> 1);
+    pcg_init_kernel<<<nb, NK_VEC_THREADS, 0, st>>>(f, x, c->r, c->p, c->dinv, c->code, c->ctab, c->L, c->red, hist);
+    c->launches++;
+    return cudaGetLastError();
+}
+
+cudaError_t nk_launch_update_xrz(nk_ctx *c, double *x, double *hist_k, cudaStream_t st)
+{
+    const int nb = vec_blocks(c, c->L >> 1);
+    update_xrz_kernel<<<nb, NK_VEC_THREADS, 0, st>>>(x, c->r, c->p, c->w, c->dinv, c->code, c->ctab, c->L,
+                                                      c->red, hist_k);
+    c->launches++;
+    return cudaGetLastError();
+}
+
+cudaError_t nk_launch_update_pz(nk_ctx *c, cudaStream_t st)
+{
+    const int nb = vec_blocks(c, c->L >> 1);
+    update_pz_kernel<<<nb, NK_VEC_THREADS, 0, st>>>(c->p, c->r, c->dinv, c->red.scal, c->L);
     c->launches++;
     return cudaGetLastError();
 }

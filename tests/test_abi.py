@@ -44,8 +44,9 @@ def test_workspace_bytes(lib):
     from paper_2606_12650_b200 import workspace_bytes, NkError
     L = 512 * 8 ** 3
     b = workspace_bytes(512, 7)
-    # G (48 B/pt) + 5 vectors (40 B/pt) + code (1) + CSR worst case (8) and small tables
-    assert 97 * L <= b <= 97 * L + (1 << 20) + 4096
+    # G (48 B/pt) + 6 vectors (48 B/pt: r, p, w, two host-call staging vectors, the Jacobi diagonal)
+    # + code (1) + CSR worst case (8) and small tables
+    assert 105 * L <= b <= 105 * L + (1 << 20) + 4096
     assert workspace_bytes(1, 1) > 0
     for E, N in [(0, 3), (-1, 3), (8, 0), (8, 16), (1 << 31, 15)]:
         with pytest.raises(NkError) as ei:

@@ -185,3 +185,29 @@ def test_graph_default_and_pointer_change():
     assert bool((xa == xd).all()) and bool((ha == hd).all())
     assert bool((xb == xd).all()) and bool((hb == hd).all())
     assert bool((xc == xe).all()) and bool((hc == he).all())
+
+
+# ---- NEXT row f-3: Jacobi-preconditioned CG ------------------------------------------------------------
+@pytest.mark.parametrize("name", ["config1", "config2"])
+def test_jacobi_diag_and_pcg(name):
+    from paper_2606_12650_b200 import Nekbone
+    pr = pair_for_config(name)
+    gpu = Nekbone.from_mesh(pr.mesh)
+    niter = CONFIGS[name]["niter"]
+    f = config_rhs(name, pr.mesh)
+    assert elem_err(to_np(gpu.diag()), pr.orc.diag(), pr.P) <= TOL_OP
+    xo, ho = pr.orc.pcg(f, niter)
+    for fuse_pap in (1, 0):
+        gpu.set_option("fuse_pap", fuse_pap)
+        xg, hg = gpu.pcg(to_dev(f), niter)
+        xg, hg = to_np(xg), to_np(hg)
+        assert np.all(np.abs(hg - ho) <= TOL_CG * ho), np.abs(hg / ho - 1).max()
+        assert elem_err(xg, xo, pr.P) <= TOL_CG
+        assert np.all(xg[pr.mesh.mask == 0.0] == 0.0)
+    # guards and reproducibility
+    import torch
+    x0, h0 = gpu.pcg(torch.zeros(pr.L, dtype=torch.float64, device="cuda"), 4)
+    assert not bool(x0.any()) and not bool(h0.any())
+    xa, ha = gpu.pcg(to_dev(f), 10)
+    xb, hb = gpu.pcg(to_dev(f), 10)
+    assert bool((xa == xb).all()) and bool((ha == hb).all())

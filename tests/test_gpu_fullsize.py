@@ -116,3 +116,19 @@ def test_free_running_cg_full_size(name):
         assert np.all(np.abs(hg - ho) <= TOL_CG * ho), float(np.abs(hg / ho - 1).max())
         assert elem_err(xg, xo, P) <= TOL_CG
     assert np.all(xg[mesh.mask == 0.0] == 0.0)
+
+
+def test_jacobi_pcg_config3_early_iterations():
+    """NEXT row f-3 at full size: the diagonal everywhere, and PCG through iteration 60 (well inside the
+    stable part of config 3's trajectory, see the band protocol above)."""
+    from oracle.nko import Oracle
+    mesh, gpu = _gpu("config3")
+    P = mesh.n ** 3
+    orc = Oracle.from_mesh(mesh)
+    assert elem_err(to_np(gpu.diag()), orc.diag(), P) <= TOL_OP
+    f = config_rhs("config3", mesh)
+    xo, ho = orc.pcg(f, 60)
+    orc.close()
+    xg, hg = gpu.pcg(to_dev(f), 60)
+    assert np.all(np.abs(to_np(hg) - ho) <= TOL_CG * ho), float(np.abs(to_np(hg) / ho - 1).max())
+    assert elem_err(to_np(xg), xo, P) <= TOL_CG
