@@ -62,6 +62,10 @@ struct nk_ctx {
     int32_t *row_off;            // n_rows + 1
     int32_t *row_idx;            // n_listed local indices, rows in [0,n_sum_rows) are summed,
                                  // rows in [n_sum_rows, n_rows) are masked nodes
+    // the summed rows once more, packed by length (2, 4, 8 copies: faces, edges, corners of a conforming
+    // hex mesh) so that a thread fetches its indices with one vector load and no offset lookup
+    int32_t *pk2, *pk4, *pk8, *other_rows;
+    int64_t n2, n4, n8, n_other;
     double *ctab;                // NK_CTAB doubles: 1/multiplicity
     double *mtab;                // NK_CTAB doubles: multiplicity
     double *hist;                // NK_HIST_MAX doubles (nk_cg_host)
