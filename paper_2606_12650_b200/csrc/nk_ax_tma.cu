@@ -98,6 +98,10 @@ struct TmaCfg {
     static constexpr int WORK_BYTES = work_bytes(NW);
     static constexpr int SMEM = R * STAGE_BYTES + WORK_BYTES + BAR_BYTES;
     static_assert(R >= 2, "ring too small");
+#ifndef NK_TMA_IB
+#define NK_TMA_IB 2
+#endif
+    static constexpr int IB = NK_TMA_IB;                      // table rows advanced together in lines_apply
     // where the next batch's u pencil is requested: 1 = after P3, 2 = after P4 (measured per order)
 #ifdef NK_TMA_PF12
     static constexpr int PF = (n == 12) ? NK_TMA_PF12 : 1;
@@ -198,6 +202,67 @@ __device__ __forceinline__ void line_apply(const double (&ln)[n], Store store)
                     store(n - 1 - i, A[j] - S[j]);
                 } else {
                     store(i, A[j]);          // middle row of an odd n: its even part vanishes
+                }
+            }
+    }
+}
+
+// The same transform applied to NL grid lines at once (a thread's row, column and pencil): every table
+// entry is fetched once per phase and feeds NL DFMAs, and 2 IB NL independent chains are in flight.
+// (Three separate line_apply calls made ptxas keep the table of the first call alive for the next ones:
+// uniform registers spilled to vector registers and back, ~1 extra instruction per DFMA.)
+template <int n, int MOFF, int NL, int IB, class Store>
+__device__ __forceinline__ void lines_apply(const double (&ln)[NL][n], Store store)
+{
+    constexpr int h = n / 2, H = (n + 1) / 2, ROW = eo_row(n);
+    double ev[NL][H], od[NL][h > 0 ? h : 1];
+#pragma unroll
+    for (int q = 0; q < NL; ++q) {
+#pragma unroll
+        for (int m = 0; m < h; ++m) {
+            ev[q][m] = ln[q][m] + ln[q][n - 1 - m];
+            od[q][m] = ln[q][m] - ln[q][n - 1 - m];
+        }
+        if (n & 1) ev[q][H - 1] = ln[q][H - 1];
+    }
+#pragma unroll
+    for (int i0 = 0; i0 < H; i0 += IB) {
+        double S[IB][NL], A[IB][NL];
+#pragma unroll
+        for (int j = 0; j < IB; ++j)
+            if (i0 + j < H) {
+                const double *row = c_Dt + MOFF + (i0 + j) * ROW;
+#pragma unroll
+                for (int q = 0; q < NL; ++q) {
+                    A[j][q] = (h > 0) ? row[0] * od[q][0] : 0.0;
+                    S[j][q] = row[h] * ev[q][0];
+                }
+            }
+#pragma unroll
+        for (int m = 1; m < H; ++m) {
+#pragma unroll
+            for (int j = 0; j < IB; ++j)
+                if (i0 + j < H) {
+                    const double *row = c_Dt + MOFF + (i0 + j) * ROW;
+#pragma unroll
+                    for (int q = 0; q < NL; ++q) {
+                        if (m < h) A[j][q] = fma(row[m], od[q][m], A[j][q]);
+                        S[j][q] = fma(row[h + m], ev[q][m], S[j][q]);
+                    }
+                }
+        }
+#pragma unroll
+        for (int j = 0; j < IB; ++j)
+            if (i0 + j < H) {
+                const int i = i0 + j;
+#pragma unroll
+                for (int q = 0; q < NL; ++q) {
+                    if (n - 1 - i != i) {
+                        store(q, i, A[j][q] + S[j][q]);
+                        store(q, n - 1 - i, A[j][q] - S[j][q]);
+                    } else {
+                        store(q, i, A[j][q]);
+                    }
                 }
             }
     }
@@ -305,31 +370,32 @@ ax_tma_kernel(double *__restrict__ u_rw, const double *__restrict__ u_ro, const 
                 for (int k = 0; k < n; ++k) u_rw[gbase + k * n2] = ru[k];
             }
             group_sync<GTH>(grp);
-            // P2: r derivative along rows (A -> B), s derivative along columns (A -> C)
+            // P2: D along the thread's row (A -> B), column (A -> C) and pencil (registers -> wt), one pass
+            double wt[n];
             {
-                double ln[n];
+                double ln[3][n], cres[NW == 2 ? n : 1];
 #pragma unroll
-                for (int m = 0; m < n; ++m) ln[m] = sA[rbase + m];
-                line_apply<n, DOFF>(ln, [&](int i, double v) { if (mapped) sB[rbase + i] = v; });
-            }
-            if (NW == 2) {
-                double ln[n];                           // columns overwrite A in place: read, barrier, write
+                for (int m = 0; m < n; ++m) {
+                    ln[0][m] = sA[rbase + m];
+                    ln[1][m] = sA[cbase + m * S1];
+                    ln[2][m] = ru[m];
+                }
+                lines_apply<n, DOFF, 3, C::IB>(ln, [&](int q, int i, double v) {
+                    if (q == 0) { if (mapped) sB[rbase + i] = v; }
+                    else if (q == 1) { if (NW == 2) cres[NW == 2 ? i : 0] = v; else if (mapped) sC[cbase + i * S1] = v; }
+                    else wt[i] = v;
+                });
+                if (NW == 2) {                          // columns overwrite A in place: all reads of A are done
+                    group_sync<GTH>(grp);
+                    if (mapped) {
 #pragma unroll
-                for (int m = 0; m < n; ++m) ln[m] = sA[cbase + m * S1];
-                group_sync<GTH>(grp);
-                line_apply<n, DOFF>(ln, [&](int j, double v) { if (mapped) sC[cbase + j * S1] = v; });
-            } else {
-                double ln[n];
-#pragma unroll
-                for (int m = 0; m < n; ++m) ln[m] = sA[cbase + m * S1];
-                line_apply<n, DOFF>(ln, [&](int j, double v) { if (mapped) sC[cbase + j * S1] = v; });
+                        for (int j = 0; j < n; ++j) sC[cbase + j * S1] = cres[j];
+                    }
+                }
             }
             group_sync<GTH>(grp);
-            // P3: t derivative in registers; G from the ring; t transpose in registers
-            double rw[n];
+            // P3: the geometric factors from the ring, point by point along the pencil
             {
-                double wt[n];
-                line_apply<n, DOFF>(ru, [&](int k, double v) { wt[k] = v; });
                 // planes are waited for, used and handed back KG at a time, so that the loads and
                 // the 15 flops of several planes interleave (the waits are compiler barriers)
                 constexpr int KG = (KP == 1) ? NK_TMA_KG : n;
@@ -373,7 +439,6 @@ ax_tma_kernel(double *__restrict__ u_rw, const double *__restrict__ u_ro, const 
                     }
                     if (KP != 1) { if (++stage == R) { stage = 0; phase ^= 1u; } }
                 }
-                line_apply<n, TOFF>(wt, [&](int m, double v) { rw[m] = v; });
             }
             group_sync<GTH>(grp);
             auto prefetch = [&]() {
@@ -389,15 +454,21 @@ ax_tma_kernel(double *__restrict__ u_rw, const double *__restrict__ u_ro, const 
                 }
             };
             if (C::PF == 1) prefetch();
-            // P4: D^T along rows (B in place) and columns (C in place)
+            // P4: D^T along the row (B in place), the column (C in place) and the pencil (wt -> rw), one pass
+            double rw[n];
             {
-                double ln[n];
+                double ln[3][n];
 #pragma unroll
-                for (int m = 0; m < n; ++m) ln[m] = sB[rbase + m];
-                line_apply<n, TOFF>(ln, [&](int i, double v) { if (mapped) sB[rbase + i] = v; });
-#pragma unroll
-                for (int m = 0; m < n; ++m) ln[m] = sC[cbase + m * S1];
-                line_apply<n, TOFF>(ln, [&](int j, double v) { if (mapped) sC[cbase + j * S1] = v; });
+                for (int m = 0; m < n; ++m) {
+                    ln[0][m] = sB[rbase + m];
+                    ln[1][m] = sC[cbase + m * S1];
+                    ln[2][m] = wt[m];
+                }
+                lines_apply<n, TOFF, 3, C::IB>(ln, [&](int q, int i, double v) {
+                    if (q == 0) { if (mapped) sB[rbase + i] = v; }
+                    else if (q == 1) { if (mapped) sC[cbase + i * S1] = v; }
+                    else rw[i] = v;
+                });
             }
             group_sync<GTH>(grp);
             if (C::PF == 2) prefetch();
