@@ -106,8 +106,8 @@ int nk_cg_get_state(nk_ctx *ctx, double *r, double *p, double *w, void *stream);
 int nk_get_scalars(nk_ctx *ctx, double *out5_host, void *stream);
 
 /* Options (all default 0 unless stated):
- *   "ax_variant"   0 = auto, 1 = line kernel (thread per grid line, D as constant operands),
- *                  2 = slab kernel (2-D slab, k loop, D rows in registers)
+ *   "ax_variant"   0 (default) = TMA-pipelined persistent kernel (nk_ax_tma.cu); 1 = the round's first
+ *                  kernel, one CTA per element batch without pipelining (nk_ax.cu), kept for A/B runs
  *   "fuse_pap"     1 (default) = pap accumulated inside ax_e through the dot-fusion identity
  *                  <M QQ^T A_L p, p>_c = sum_l (A_L p)_l p_l; 0 = separate weighted dot after gs
  *   "fuse_p"       1 = p = r + beta p folded into the load of the next ax_e; 0 (default) = own kernel

@@ -301,7 +301,7 @@ int nk_get_scalars(nk_ctx *c, double *out5_host, void *stream)
 
 static int *option_slot(nk_ctx *c, const char *name, int *lo, int *hi)
 {
-    if (!std::strcmp(name, "ax_variant")) { *lo = 0; *hi = 2; return &c->opt_ax_variant; }
+    if (!std::strcmp(name, "ax_variant")) { *lo = 0; *hi = 1; return &c->opt_ax_variant; }
     if (!std::strcmp(name, "fuse_pap")) { *lo = 0; *hi = 1; return &c->opt_fuse_pap; }
     if (!std::strcmp(name, "fuse_p")) { *lo = 0; *hi = 1; return &c->opt_fuse_p; }
     if (!std::strcmp(name, "graph")) { *lo = 0; *hi = 2; return &c->opt_graph; }
