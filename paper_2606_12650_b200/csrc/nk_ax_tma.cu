@@ -399,6 +399,7 @@ ax_tma_kernel(double *__restrict__ u_rw, const double *__restrict__ u_ro, const 
                 // planes are waited for, used and handed back KG at a time, so that the loads and
                 // the 15 flops of several planes interleave (the waits are compiler barriers)
                 constexpr int KG = (KP == 1) ? NK_TMA_KG : n;
+                double dloc = 0.0;
 #pragma unroll
                 for (int k0 = 0; k0 < n; k0 += KG) {
                     int st[KG];
@@ -428,7 +429,7 @@ ax_tma_kernel(double *__restrict__ u_rw, const double *__restrict__ u_ro, const 
                             }
                             wt[k] = wk;
                             // <u, A_L u> = sum over points of grad(u)^T G grad(u): the fused pap needs no u later on
-                            dsum += active ? fma(ur, wr, fma(us, ws, ut * wk)) : 0.0;
+                            dloc += fma(ur, wr, fma(us, ws, ut * wk));
                         }
                     }
                     __syncwarp();                    // this warp is done with these stages: hand them back
@@ -439,6 +440,7 @@ ax_tma_kernel(double *__restrict__ u_rw, const double *__restrict__ u_ro, const 
                     }
                     if (KP != 1) { if (++stage == R) { stage = 0; phase ^= 1u; } }
                 }
+                dsum += active ? dloc : 0.0;        // threads without an element computed on stale data
             }
             group_sync<GTH>(grp);
             auto prefetch = [&]() {
