@@ -363,7 +363,8 @@ def run_ours(args) -> dict | None:
     if ax_n > 0:
         # bytes the ax_e launch moves by the S 8(d) model: u 8 + G 48 + w 8 = 64 B/pt, plus, when the
         # direction update is folded in, r 8 read + p 8 written (the update's own 24 B/pt kernel is gone)
-        bpp = 64.0 + (16.0 if args.fuse_p else 0.0)
+        fused_p = args.fuse_p == 1 or (args.fuse_p == 2 and L <= (1 << 24))
+        bpp = 64.0 + (16.0 if fused_p else 0.0)
         avg = ax_ms / ax_n
         ach = bpp * L / (avg * 1e-3) / 1e9
         traffic = args.traffic
@@ -373,7 +374,7 @@ def run_ours(args) -> dict | None:
                     traffic = float(json.load(fh)[args.workload]["dram_bytes_per_launch"])
             except Exception:
                 traffic = None
-        out["roofline"] = {"kernel": "ax_tma_kernel (ax_e" + (" + fused p=r+beta*p" if args.fuse_p else "")
+        out["roofline"] = {"kernel": "ax_tma_kernel (ax_e" + (" + fused p=r+beta*p" if fused_p else "")
                                      + (" + fused pap" if args.fuse_pap else "") + ")",
                            "bound": "hbm", "achieved": ach, "peak": peak, "unit": "GB/s", "frac": ach / peak,
                            "peak_kind": peak_kind + " copy peak (burst)", "frac_of_nominal_8TBs": ach / HBM_NOMINAL_GBS,
@@ -400,7 +401,7 @@ def main():
     ap.add_argument("--impl", default="ours", choices=["ours", "reference"])
     ap.add_argument("--workload", default="config5", choices=["config1", "config2", "config3", "config5"])
     ap.add_argument("--fuse-pap", type=int, default=1)
-    ap.add_argument("--fuse-p", type=int, default=0)
+    ap.add_argument("--fuse-p", type=int, default=2, help="0 off, 1 on, 2 library default (on up to 2^24 points)")
     ap.add_argument("--graph", type=int, default=2, help="0 off, 1 on, 2 library default (graph up to 2^24 points)")
     ap.add_argument("--traffic", type=float, default=None,
                     help="dram bytes per ax_e launch from the committed ncu --set full capture (profiles/)")

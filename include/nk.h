@@ -110,7 +110,8 @@ int nk_get_scalars(nk_ctx *ctx, double *out5_host, void *stream);
  *                  kernel, one CTA per element batch without pipelining (nk_ax.cu), kept for A/B runs
  *   "fuse_pap"     1 (default) = pap accumulated inside ax_e through the dot-fusion identity
  *                  <M QQ^T A_L p, p>_c = sum_l (A_L p)_l p_l; 0 = separate weighted dot after gs
- *   "fuse_p"       1 = p = r + beta p folded into the load of the next ax_e; 0 (default) = own kernel
+ *   "fuse_p"       1 = p = r + beta p folded into the load of the next ax_e; 0 = own kernel;
+ *                  2 (default) = 1 for meshes of up to 2^24 local points (one launch fewer), else 0
  *   "graph"        0 = nk_cg enqueues its launches one by one; 1 = records them into a CUDA graph
  *                  (cached per f, x, res_hist, niter; updated in place when the pointers change) and
  *                  replays it; 2 (default) = 1 for meshes of up to 2^24 local points, where launch gaps
