@@ -1,4 +1,8 @@
-// nk_ax.cu -- ax_e: w = A_L u, the element-local matrix-free Laplacian ("the action of the
+// nk_ax.cu -- ax_e, the round's FIRST kernel ("ax_variant" = 1; the default is nk_ax_tma.cu): one CTA
+// per element batch, load -> compute -> store with nothing in flight while it computes (39 % of the
+// copy peak at config 5).  Kept for A/B runs and as a second implementation under the parity tests.
+//
+// ax_e: w = A_L u, the element-local matrix-free Laplacian ("the action of the
 // Poisson operator", the most expensive kernel; S 8(a) a1, S 8(c) O3; BJ north_star (1)).
 //
 //   u_r = D u along r, u_s = D u along s, u_t = D u along t            (3 x (N+1) fma per point)

@@ -10,10 +10,12 @@
 //   * a producer warp: one lane streams the geometric factors -- 75 % of the bytes -- into a
 //     shared-memory ring with cp.async.bulk (TMA bulk copies, SASS UBLKCP) completing on mbarriers,
 //     k-plane by k-plane, running up to a whole element batch ahead of the arithmetic;
-//   * compute warps: the "line" scheme (every thread owns a whole grid line in each of the three
-//     directions, D entries are compile-time-indexed __constant__ operands of the DFMAs, 16
-//     shared-memory accesses per point) on the batch whose G has landed, while the next batch's
-//     u pencil is already on its way into registers.
+//   * compute warps: the "line" scheme.  A thread owns the pencil (i,j) of u in registers, a whole
+//     row (j,k) and a whole column (i,k) of the padded shared cube: 16 shared-memory accesses per
+//     point.  Phases per batch: P1 pencil -> cube; P2 D along row, column and pencil in ONE pass over
+//     the even-odd table (lines_apply: every entry fetched once through the uniform datapath, feeding
+//     three DFMAs); P3 the 3x3 G per point from the ring (+ the fused pap); P4 D^T likewise; P5 sum
+//     and store.  The next batch's u pencil is requested into registers while this one finishes.
 // G never touches registers before it is used and u is read exactly once, so DRAM traffic equals
 // the algorithmic bytes, and the bytes in flight per SM (ring of ~110-170 KB) exceed the ~30 KB
 // that 5.6 TB/s x ~0.8 us of latency asks for.
