@@ -382,7 +382,10 @@ def run_ours(args) -> dict | None:
                            "traffic": traffic, "algorithmic_bytes_per_launch": bpp * L,
                            "share_of_step": ax_ms * (args.steps if graphed else 1) / ms_for_share,
                            "timed_by": ktimes_from}
-        kb = {"gs": gs_bytes(sizes) / L, "dot": 24.0, "update_xr": 56.0 + 1.0 - 8.0, "update_p": 24.0}
+        # real bytes per point of the vector kernels: fused-p path = update x,r (49) [+ p inside ax_e];
+        # otherwise update_r (w, r, code in; r out = 25) and update_px (r, p, x in; p, x out = 40)
+        kb = {"gs": gs_bytes(sizes) / L, "dot": 17.0,
+              "update_xr": 49.0 if fused_p else 25.0, "update_p": 24.0 if fused_p else 40.0}
         out["kernels"] = {k: {"avg_us": 1e3 * t / n, "launches": n, "share_of_step": t * (args.steps if graphed else 1) / ms_for_share,
                               **({"gbs_model": kb[k] * L / (t / n * 1e-3) / 1e9} if k in kb else {})}
                           for k, (t, n) in ktimes.items() if n > 0}

@@ -110,11 +110,13 @@ cudaError_t enqueue_iteration(nk_ctx *c, double *x, double *hist_k, cudaStream_t
     }
     NK_LAUNCH(NK_K_GS, nk_launch_gs(c, c->w, 1, st));
     if (!fuse_pap) NK_LAUNCH(NK_K_DOT, nk_launch_dot(c, c->w, c->p, nullptr, NK_EPI_PAP, st));
-    NK_LAUNCH(NK_K_UPDATE_XR, nk_launch_update_xr(c, x, hist_k, st));
     if (fuse_p_on(c)) {
+        NK_LAUNCH(NK_K_UPDATE_XR, nk_launch_update_xr(c, x, hist_k, st));
         c->p_pending = 1;
     } else {
-        NK_LAUNCH(NK_K_UPDATE_P, nk_launch_update_p(c, st));
+        // r first, then x and p together: p is read once per iteration instead of twice (65 vs 73 B/pt)
+        NK_LAUNCH(NK_K_UPDATE_XR, nk_launch_update_r(c, hist_k, st));
+        NK_LAUNCH(NK_K_UPDATE_P, nk_launch_update_px(c, x, st));
     }
     return cudaSuccess;
 }
@@ -452,7 +454,7 @@ int nk_pcg(nk_ctx *c, const double *f, double *x, int niter, double *res_hist, v
         }
         NK_CUDA(nk_launch_update_xrz(c, x, res_hist + k, st));
         NK_CUDA(prof_mark(c, NK_K_UPDATE_XR, st));
-        NK_CUDA(nk_launch_update_pz(c, st));
+        NK_CUDA(nk_launch_update_pz(c, x, st));
         NK_CUDA(prof_mark(c, NK_K_UPDATE_P, st));
     }
     (void)e;

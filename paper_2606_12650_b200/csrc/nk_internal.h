@@ -110,10 +110,12 @@ cudaError_t nk_launch_dot(nk_ctx *c, const double *a, const double *b, double *o
 cudaError_t nk_launch_cg_init(nk_ctx *c, const double *f, double *x, double *hist, cudaStream_t st);
 cudaError_t nk_launch_update_xr(nk_ctx *c, double *x, double *hist_k, cudaStream_t st);
 cudaError_t nk_launch_update_p(nk_ctx *c, cudaStream_t st);
+cudaError_t nk_launch_update_r(nk_ctx *c, double *hist_k, cudaStream_t st);     // r -= alpha w, rho'
+cudaError_t nk_launch_update_px(nk_ctx *c, double *x, cudaStream_t st);         // x += alpha p; p = r + beta p
 cudaError_t nk_launch_get_mult(nk_ctx *c, double *mult, cudaStream_t st);
 // preconditioned CG
 cudaError_t nk_launch_diag(nk_ctx *c, double *diag, cudaStream_t st);          // nk_geom.cu: diag(A_L), local
 cudaError_t nk_launch_invert_diag(nk_ctx *c, double *d, cudaStream_t st);      // d = masked ? 0 : 1/d
 cudaError_t nk_launch_pcg_init(nk_ctx *c, const double *f, double *x, double *hist, cudaStream_t st);
 cudaError_t nk_launch_update_xrz(nk_ctx *c, double *x, double *hist_k, cudaStream_t st);
-cudaError_t nk_launch_update_pz(nk_ctx *c, cudaStream_t st);
+cudaError_t nk_launch_update_pz(nk_ctx *c, double *x, cudaStream_t st);   // x += alpha p; p = dinv r + beta p
