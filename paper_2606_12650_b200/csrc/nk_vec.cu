@@ -154,7 +154,28 @@ update_r_kernel(double *__restrict__ r, const double *__restrict__ w, const uint
     const int64_t pairs = L >> 1;
     const int64_t stride = (int64_t)gridDim.x * blockDim.x;
     double acc = 0.0;
-    for (int64_t q = (int64_t)blockIdx.x * blockDim.x + threadIdx.x; q < pairs; q += stride) {
+    // four pairs per step, all loads before the stores (r is loaded and stored through one pointer, so
+    // the compiler will not overlap the next step's loads with this step's store on its own)
+    int64_t q = (int64_t)blockIdx.x * blockDim.x + threadIdx.x;
+    for (; q + 3 * stride < pairs; q += 4 * stride) {
+        double2 wv[4], rv[4];
+        uchar2 cd[4];
+#pragma unroll
+        for (int j = 0; j < 4; ++j) {
+            wv[j] = reinterpret_cast<const double2 *>(w)[q + j * stride];
+            rv[j] = reinterpret_cast<double2 *>(r)[q + j * stride];
+            cd[j] = reinterpret_cast<const uchar2 *>(code)[q + j * stride];
+        }
+#pragma unroll
+        for (int j = 0; j < 4; ++j) {
+            rv[j].x = fma(-alpha, wv[j].x, rv[j].x);
+            rv[j].y = fma(-alpha, wv[j].y, rv[j].y);
+            reinterpret_cast<double2 *>(r)[q + j * stride] = rv[j];
+            acc = fma(s_c[cd[j].x & 0x7f] * rv[j].x, rv[j].x, acc);
+            acc = fma(s_c[cd[j].y & 0x7f] * rv[j].y, rv[j].y, acc);
+        }
+    }
+    for (; q < pairs; q += stride) {
         const double2 wv = reinterpret_cast<const double2 *>(w)[q];
         double2 rv = reinterpret_cast<double2 *>(r)[q];
         const uchar2 cd = reinterpret_cast<const uchar2 *>(code)[q];
