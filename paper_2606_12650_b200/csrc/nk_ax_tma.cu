@@ -45,9 +45,6 @@ __host__ __device__ constexpr int eo_off(int n) { int s = 0; for (int q = 2; q <
 constexpr int D_TOTAL = eo_off(17);
 __constant__ double c_Dt[D_TOTAL];
 
-#ifndef NK_TMA_KG
-#define NK_TMA_KG 1
-#endif
 constexpr int SMEM_CAP = 232448 - 1024;     // 227 KB opt-in limit minus this kernel's static shared memory
 constexpr int BAR_BYTES = 1024;             // 2 x 64 mbarriers
 
@@ -81,7 +78,7 @@ struct TmaCfg {
     static constexpr int S2 = n * S1, SE = n * S2;            // padded plane / cube (doubles)
     // a ring stage holds KP k-planes of every element of the batch: whole elements for small n
     // (one bulk copy per batch), single k-planes otherwise (one bulk copy per element and plane)
-    static constexpr int KP = (n <= 6) ? n : 1;
+    static constexpr int KP = (n <= 6) ? n : 1;            // (2 or 3 planes per stage at n = 12: measured 1.5 % slower)
     static constexpr int STAGE_D2 = EPB * KP * 3 * n2;        // double2 per stage
     static constexpr int STAGE_BYTES = STAGE_D2 * 16;
     static constexpr int SPB = n / KP;                        // stages per batch
@@ -312,10 +309,10 @@ ax_tma_kernel(double *__restrict__ u_rw, const double *__restrict__ u_ro, const 
                     if (KP == n) {       // whole elements: the batch is one contiguous chunk
                         mbar_expect_tx(fb, (uint32_t)ne * P * 48);
                         bulk_g2s(dst, g + nk_g_index(e0, 0, 0, 0, n), (uint32_t)ne * P * 48, fb);
-                    } else {             // one k-plane of every element of the batch
-                        mbar_expect_tx(fb, (uint32_t)ne * n2 * 48);
+                    } else {             // KP consecutive k-planes (contiguous in HBM) of every element of the batch
+                        mbar_expect_tx(fb, (uint32_t)ne * KP * n2 * 48);
                         for (int q = 0; q < ne; ++q)
-                            bulk_g2s(dst + q * n2 * 48, g + nk_g_index(e0 + q, ks, 0, 0, n), n2 * 48, fb);
+                            bulk_g2s(dst + q * KP * n2 * 48, g + nk_g_index(e0 + q, ks * KP, 0, 0, n), KP * n2 * 48, fb);
                     }
                     if (++stage == R) { stage = 0; phase ^= 1u; }
                 }
@@ -398,49 +395,31 @@ ax_tma_kernel(double *__restrict__ u_rw, const double *__restrict__ u_ro, const 
             group_sync<GTH>(grp);
             // P3: the geometric factors from the ring, point by point along the pencil
             {
-                // planes are waited for, used and handed back KG at a time, so that the loads and
-                // the 15 flops of several planes interleave (the waits are compiler barriers)
-                constexpr int KG = (KP == 1) ? NK_TMA_KG : n;
+                // a stage (KP planes) is waited for when its first plane comes up and handed back after its
+                // last one.  (Waiting for several stages at once was tried and is slower: the register
+                // pressure of interleaved planes costs more than the waits.)
                 double dloc = 0.0;
 #pragma unroll
-                for (int k0 = 0; k0 < n; k0 += KG) {
-                    int st[KG];
-#pragma unroll
-                    for (int j = 0; j < KG; ++j) {
-                        if (k0 + j < n && (KP == 1 || j == 0)) {
-                            mbar_wait_warp(full0 + 8 * stage, phase);
-                            st[j] = stage;
-                            if (KP == 1) { if (++stage == R) { stage = 0; phase ^= 1u; } }
-                        } else {
-                            st[j] = st[0];
-                        }
+                for (int k = 0; k < n; ++k) {
+                    if (k % KP == 0) mbar_wait_warp(full0 + 8 * stage, phase);
+                    const double2 *gs = gslot + (size_t)stage * C::STAGE_D2 + (k % KP) * 3 * n2;
+                    const double2 ga = gs[0], gb = gs[n2], gc = gs[2 * n2];
+                    const double ur = sB[pbase + k * S2], us = sC[pbase + k * S2], ut = wt[k];
+                    const double wr = fma(ga.x, ur, fma(ga.y, us, gb.x * ut));  // w_r = rr ur + rs us + rt ut
+                    const double ws = fma(ga.y, ur, fma(gb.y, us, gc.x * ut));  // w_s = rs ur + ss us + st ut
+                    const double wk = fma(gb.x, ur, fma(gc.x, us, gc.y * ut));  // w_t = rt ur + st us + tt ut
+                    if (mapped) {
+                        sB[pbase + k * S2] = wr;
+                        sC[pbase + k * S2] = ws;
                     }
-#pragma unroll
-                    for (int j = 0; j < KG; ++j) {
-                        const int k = k0 + j;
-                        if (k < n) {
-                            const double2 *gs = gslot + (size_t)st[j] * C::STAGE_D2 + (k % KP) * 3 * n2;
-                            const double2 ga = gs[0], gb = gs[n2], gc = gs[2 * n2];
-                            const double ur = sB[pbase + k * S2], us = sC[pbase + k * S2], ut = wt[k];
-                            const double wr = fma(ga.x, ur, fma(ga.y, us, gb.x * ut));  // w_r = rr ur + rs us + rt ut
-                            const double ws = fma(ga.y, ur, fma(gb.y, us, gc.x * ut));  // w_s = rs ur + ss us + st ut
-                            const double wk = fma(gb.x, ur, fma(gc.x, us, gc.y * ut));  // w_t = rt ur + st us + tt ut
-                            if (mapped) {
-                                sB[pbase + k * S2] = wr;
-                                sC[pbase + k * S2] = ws;
-                            }
-                            wt[k] = wk;
-                            // <u, A_L u> = sum over points of grad(u)^T G grad(u): the fused pap needs no u later on
-                            dloc += fma(ur, wr, fma(us, ws, ut * wk));
-                        }
+                    wt[k] = wk;
+                    // <u, A_L u> = sum over points of grad(u)^T G grad(u): the fused pap needs no u later on
+                    dloc += fma(ur, wr, fma(us, ws, ut * wk));
+                    if (k % KP == KP - 1) {          // this warp is done with the stage: hand it back
+                        __syncwarp();
+                        if (lane == 0) mbar_arrive(empty0 + 8 * stage);
+                        if (++stage == R) { stage = 0; phase ^= 1u; }
                     }
-                    __syncwarp();                    // this warp is done with these stages: hand them back
-                    if (lane == 0) {
-#pragma unroll
-                        for (int j = 0; j < KG; ++j)
-                            if (k0 + j < n && (KP == 1 || j == 0)) mbar_arrive(empty0 + 8 * st[j]);
-                    }
-                    if (KP != 1) { if (++stage == R) { stage = 0; phase ^= 1u; } }
                 }
                 dsum += active ? dloc : 0.0;        // threads without an element computed on stale data
             }
