@@ -72,7 +72,16 @@ struct TmaCfg {
     static constexpr int GTH = (SG * n2 + 31) / 32 * 32;      // threads per group
     static constexpr int CT = NG * GTH;                       // compute threads
     static constexpr int CW = CT / 32;                        // compute warps
-    static constexpr int THREADS = CT + 32;                   // + producer warp
+    // Warp-specialised register budget (n >= 15: eight full compute warps): the producer sits in a
+    // warpgroup of its own, which gives its registers back (setmaxnreg.dec) so that the two compute
+    // warpgroups can take 232 each (setmaxnreg.inc).  Without it nine warps cap every thread at 168
+    // registers (the register file is split per scheduler) and the n = 15, 16 kernels spill to L2.
+#ifdef NK_TMA_NO_SETMAXNREG
+    static constexpr bool WGP = false;
+#else
+    static constexpr bool WGP = (n >= 15) && (CW % 4 == 0);
+#endif
+    static constexpr int THREADS = CT + (WGP ? 128 : 32);     // + producer warp (or warpgroup)
     static_assert(EPB % SG == 0 && NG <= 15, "sync groups");
     static constexpr int S1 = (n & 1) ? n : n + 1;            // odd row stride: conflict-free lines
     static constexpr int S2 = n * S1, SE = n * S2;            // padded plane / cube (doubles)
@@ -294,6 +303,10 @@ ax_tma_kernel(double *__restrict__ u_rw, const double *__restrict__ u_ro, const 
     const int nit = (nb > (int64_t)blockIdx.x) ? (int)((nb - blockIdx.x + gridDim.x - 1) / gridDim.x) : 0;
     double dsum = 0.0;
 
+    if (C::WGP) {
+        if (tid >= CTHREADS) asm volatile("setmaxnreg.dec.sync.aligned.u32 24;");
+        else asm volatile("setmaxnreg.inc.sync.aligned.u32 240;");
+    }
     if (tid >= CTHREADS) {
         // ---- producer warp: one lane streams G into the ring ----------------------------------------
         if (tid == CTHREADS) {

@@ -211,3 +211,19 @@ def test_jacobi_diag_and_pcg(name):
     xa, ha = gpu.pcg(to_dev(f), 10)
     xb, hb = gpu.pcg(to_dev(f), 10)
     assert bool((xa == xb).all()) and bool((ha == hb).all())
+
+
+@pytest.mark.parametrize("N", [6, 10, 12, 14, 15])
+def test_cg_high_and_odd_orders(N):
+    """CG through the fused-pap path of every kernel configuration family: sync groups per slot (N = 10),
+    one work-array pair (N = 11 is config 5), single-element batches (N = 12), and the warp-specialised
+    register budget with the producer in its own warpgroup (N = 14, 15)."""
+    pr = pair_for_brick(3, 2, 2, N, 0.1)
+    f = rhs_unique(pr.mesh, 40 + N)
+    xo, ho = pr.orc.cg(f, 12)
+    for graph in (0, 1):
+        pr.gpu.set_option("graph", graph)
+        xg, hg = pr.gpu.cg(to_dev(f), 12)
+        assert np.all(np.abs(to_np(hg) - ho) <= TOL_CG * ho), (N, graph)
+        assert elem_err(to_np(xg), xo, pr.P) <= TOL_CG, (N, graph)
+    pr.gpu.set_option("graph", 2)
