@@ -49,55 +49,68 @@ __device__ __forceinline__ void gs_row(double *__restrict__ v, const int32_t *__
 }
 
 struct gs_plan {
-    const int32_t *pk2, *pk4, *pk8, *other, *off, *idx;
-    int n2, n4, n8, n_other;          // summed rows by length class
+    const int32_t *pk, *desc, *off, *idx;
+    int n_chunks;                     // chunks of NK_GS_CHUNK summed rows, BPC blocks each
     int n_sum_rows, n_rows;           // CSR: rows [0, n_sum_rows) summed, [n_sum_rows, n_rows) masked nodes
     int masked_begin, n_listed;       // the masked nodes' copies are idx[masked_begin, n_listed)
 };
 
+constexpr int BPC = NK_GS_CHUNK / GS_THREADS;     // blocks per chunk
+
 // Rows of 2, 4 and 8 copies (faces, edges, corners) come from the packed arrays: one vector load
 // of the indices, no offset lookup -- one dependent memory round trip less than the CSR walk, on
 // a kernel that is pure latency (ncu: 52 % of DRAM peak at 82 % occupancy, all long-scoreboard).
-// Sums run in ascending local index, as in gs_row.
+// Packing is per chunk of consecutive rows, so that rows of different length that share 32-byte
+// sectors are still worked on at about the same time (packing the whole mesh by length made
+// DRAM traffic grow from 0.90 to 1.11 GB at config 5).  Sums run in ascending local index, as in gs_row.
 __global__ void __launch_bounds__(GS_THREADS)
 gs_kernel(double *__restrict__ v, gs_plan pl, int with_mask)
 {
-    int t = blockIdx.x * GS_THREADS + threadIdx.x;
-    if (t < pl.n2) {
-        const int2 ii = reinterpret_cast<const int2 *>(pl.pk2)[t];
-        const double s = v[ii.x] + v[ii.y];
-        v[ii.x] = s; v[ii.y] = s;
-        return;
-    }
-    t -= pl.n2;
-    if (t < pl.n4) {
-        const int4 ii = reinterpret_cast<const int4 *>(pl.pk4)[t];
-        const double a0 = v[ii.x], a1 = v[ii.y], a2 = v[ii.z], a3 = v[ii.w];
-        const double s = ((a0 + a1) + a2) + a3;
-        v[ii.x] = s; v[ii.y] = s; v[ii.z] = s; v[ii.w] = s;
-        return;
-    }
-    t -= pl.n4;
-    if (t < pl.n8) {
-        const int4 ia = reinterpret_cast<const int4 *>(pl.pk8)[2 * t], ib = reinterpret_cast<const int4 *>(pl.pk8)[2 * t + 1];
-        const int ii[8] = {ia.x, ia.y, ia.z, ia.w, ib.x, ib.y, ib.z, ib.w};
-        double a[8];
+    const int chunk = blockIdx.x / BPC;
+    if (chunk < pl.n_chunks) {
+        const int4 d = reinterpret_cast<const int4 *>(pl.desc)[2 * chunk];       // offset, n2, n4, n8
+        const int n_other = pl.desc[8 * chunk + 4];
+        int t = (blockIdx.x - chunk * BPC) * GS_THREADS + threadIdx.x;
+        const int32_t *pk2 = pl.pk + d.x;
+        const int32_t *pk4 = pk2 + ((2 * d.y + 3) & ~3);
+        const int32_t *pk8 = pk4 + 4 * d.z;
+        const int32_t *oth = pk8 + 8 * d.w;
+        if (t < d.y) {
+            const int2 ii = reinterpret_cast<const int2 *>(pk2)[t];
+            const double s = v[ii.x] + v[ii.y];
+            v[ii.x] = s; v[ii.y] = s;
+            return;
+        }
+        t -= d.y;
+        if (t < d.z) {
+            const int4 ii = reinterpret_cast<const int4 *>(pk4)[t];
+            const double a0 = v[ii.x], a1 = v[ii.y], a2 = v[ii.z], a3 = v[ii.w];
+            const double s = ((a0 + a1) + a2) + a3;
+            v[ii.x] = s; v[ii.y] = s; v[ii.z] = s; v[ii.w] = s;
+            return;
+        }
+        t -= d.z;
+        if (t < d.w) {
+            const int4 ia = reinterpret_cast<const int4 *>(pk8)[2 * t], ib = reinterpret_cast<const int4 *>(pk8)[2 * t + 1];
+            const int ii[8] = {ia.x, ia.y, ia.z, ia.w, ib.x, ib.y, ib.z, ib.w};
+            double a[8];
 #pragma unroll
-        for (int j = 0; j < 8; ++j) a[j] = v[ii[j]];
-        double s = a[0];
+            for (int j = 0; j < 8; ++j) a[j] = v[ii[j]];
+            double s = a[0];
 #pragma unroll
-        for (int j = 1; j < 8; ++j) s += a[j];
+            for (int j = 1; j < 8; ++j) s += a[j];
 #pragma unroll
-        for (int j = 0; j < 8; ++j) v[ii[j]] = s;
+            for (int j = 0; j < 8; ++j) v[ii[j]] = s;
+            return;
+        }
+        t -= d.w;
+        if (t < n_other) {
+            const int row = oth[t];
+            gs_row(v, pl.idx, pl.off[row], pl.off[row + 1]);
+        }
         return;
     }
-    t -= pl.n8;
-    if (t < pl.n_other) {
-        const int row = pl.other[t];
-        gs_row(v, pl.idx, pl.off[row], pl.off[row + 1]);
-        return;
-    }
-    t -= pl.n_other;
+    const int t = (blockIdx.x - pl.n_chunks * BPC) * GS_THREADS + threadIdx.x;
     if (with_mask) {
         const int q = pl.masked_begin + t;
         if (q < pl.n_listed) v[pl.idx[q]] = 0.0;
@@ -116,16 +129,14 @@ cudaError_t nk_launch_gs(nk_ctx *c, double *v, int with_mask, cudaStream_t st)
 {
     const int64_t masked_listed = c->n_listed - c->n_sum_listed;
     const int64_t tail = with_mask ? masked_listed : c->n_rows - c->n_sum_rows;
-    const int64_t work = c->n_sum_rows + tail;
-    if (work <= 0) return cudaSuccess;
+    const int64_t nb = c->n_gs_chunks * BPC + (tail + GS_THREADS - 1) / GS_THREADS;
+    if (nb <= 0) return cudaSuccess;
     gs_plan pl;
-    pl.pk2 = c->pk2; pl.pk4 = c->pk4; pl.pk8 = c->pk8; pl.other = c->other_rows;
-    pl.off = c->row_off; pl.idx = c->row_idx;
-    pl.n2 = (int)c->n2; pl.n4 = (int)c->n4; pl.n8 = (int)c->n8; pl.n_other = (int)c->n_other;
+    pl.pk = c->pk; pl.desc = c->gs_desc; pl.off = c->row_off; pl.idx = c->row_idx;
+    pl.n_chunks = (int)c->n_gs_chunks;
     pl.n_sum_rows = (int)c->n_sum_rows; pl.n_rows = (int)c->n_rows;
     pl.masked_begin = (int)c->n_sum_listed; pl.n_listed = (int)c->n_listed;
-    const int nb = (int)((work + GS_THREADS - 1) / GS_THREADS);
-    gs_kernel<<<nb, GS_THREADS, 0, st>>>(v, pl, with_mask);
+    gs_kernel<<<(unsigned)nb, GS_THREADS, 0, st>>>(v, pl, with_mask);
     c->launches++;
     return cudaGetLastError();
 }

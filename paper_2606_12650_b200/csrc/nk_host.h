@@ -34,7 +34,8 @@ inline nk_carve nk_carve_sizes(int64_t L)
     c.code = nk_align_up((size_t)L, 256);
     c.off = nk_align_up(((size_t)L + 1) * sizeof(int32_t), 256);
     c.idx = nk_align_up((size_t)L * sizeof(int32_t), 256);
-    c.pk = nk_align_up(((size_t)L + 64) * sizeof(int32_t), 256);      // packed rows of length 2/4/8 + other row ids
+    // packed rows (<= L indices + 16 padding ints per chunk) and 8 ints of descriptor per chunk
+    c.pk = nk_align_up(((size_t)L + 24 * ((size_t)L / (2 * NK_GS_CHUNK) + 2) + 256) * sizeof(int32_t), 256);
     c.tabs = nk_align_up(2 * NK_CTAB * sizeof(double) + (16 * 16 + 16) * sizeof(double), 256);
     c.partials = nk_align_up(NK_MAX_PARTIALS * sizeof(double), 256);
     c.hist = nk_align_up(NK_HIST_MAX * sizeof(double), 256);

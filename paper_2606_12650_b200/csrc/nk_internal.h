@@ -22,6 +22,7 @@ enum { NK_EPI_STORE = 0,   // out[0] = total
 #define NK_CODE_MASKED 0x80u       // bit 7 of the per-point code: Dirichlet node
 #define NK_HIST_MAX 8192               // residual-history capacity of nk_cg_host
 #define NK_GRAPH_AUTO_MAX_L (1 << 24)   // "graph" = 2: nk_cg replays a CUDA graph up to this many local points
+#define NK_GS_CHUNK 32768          // rows per gs chunk (128 blocks of 256 threads)
 #define NK_CTAB 128                // code & 0x7f indexes ctab[] = 1/multiplicity
 
 // kernel classes of nk_get_kernel_times
@@ -62,10 +63,11 @@ struct nk_ctx {
     int32_t *row_off;            // n_rows + 1
     int32_t *row_idx;            // n_listed local indices, rows in [0,n_sum_rows) are summed,
                                  // rows in [n_sum_rows, n_rows) are masked nodes
-    // the summed rows once more, packed by length (2, 4, 8 copies: faces, edges, corners of a conforming
-    // hex mesh) so that a thread fetches its indices with one vector load and no offset lookup
-    int32_t *pk2, *pk4, *pk8, *other_rows;
-    int64_t n2, n4, n8, n_other;
+    // the summed rows once more, in chunks of NK_GS_CHUNK rows, packed by length inside a chunk (2, 4, 8
+    // copies: faces, edges, corners of a conforming hex mesh): a thread fetches its indices with one
+    // vector load and no offset lookup, and a chunk stays in one neighbourhood of memory
+    int32_t *pk, *gs_desc;
+    int64_t n_gs_chunks;
     double *ctab;                // NK_CTAB doubles: 1/multiplicity
     double *mtab;                // NK_CTAB doubles: multiplicity
     double *hist;                // NK_HIST_MAX doubles (nk_cg_host)

@@ -114,28 +114,39 @@ int setup_impl(nk_ctx *c, const double *coords, const int64_t *glo_num, const do
             }
         off[row] = (int32_t)pos;
     }
-    // packed copy of the summed rows by length (order inside a class: ascending first local index)
-    std::vector<int32_t> pk((size_t)n_sum_listed + 64), other;
-    {
-        int64_t cnt[3] = {0, 0, 0};
-        for (const Row &r : sum_rows) {
-            if (r.len == 2) ++cnt[0]; else if (r.len == 4) ++cnt[1]; else if (r.len == 8) ++cnt[2];
+    // packed copy of the summed rows: chunks of NK_GS_CHUNK consecutive rows (ascending first local index,
+    // so a chunk works on one neighbourhood of memory), inside a chunk the rows of 2, 4 and 8 copies
+    // packed by length, rows of any other length as row ids into the CSR.  Descriptor per chunk:
+    // {offset into pk, n2, n4, n8, n_other, 0, 0, 0}.
+    const int64_t n_chunks = (n_sum_rows + NK_GS_CHUNK - 1) / NK_GS_CHUNK;
+    std::vector<int32_t> pk, desc((size_t)std::max<int64_t>(n_chunks, 1) * 8, 0);
+    pk.reserve((size_t)n_sum_listed + 4 * (size_t)n_chunks + 64);
+    for (int64_t ch = 0; ch < n_chunks; ++ch) {
+        const int64_t r0 = ch * NK_GS_CHUNK, r1 = std::min<int64_t>(r0 + NK_GS_CHUNK, n_sum_rows);
+        int32_t *d = &desc[(size_t)ch * 8];
+        d[0] = (int32_t)pk.size();
+        for (int len : {2, 4, 8}) {
+            int32_t cnt = 0;
+            for (int64_t r = r0; r < r1; ++r) {
+                const Row &row = sum_rows[(size_t)r];
+                if ((int)row.len != len) continue;
+                for (uint32_t q = 0; q < row.len; ++q) pk.push_back((int32_t)loc[row.begin + q]);
+                ++cnt;
+            }
+            while (pk.size() % 4) pk.push_back(0);                     // 16-byte aligned class starts
+            d[len == 2 ? 1 : len == 4 ? 2 : 3] = cnt;
         }
-        auto up4 = [](int64_t x) { return (x + 3) / 4 * 4; };            // 16-byte aligned class starts
-        const int64_t o2 = 0, o4 = up4(2 * cnt[0]), o8 = o4 + up4(4 * cnt[1]), oo = o8 + up4(8 * cnt[2]);
-        int64_t w2 = o2, w4 = o4, w8 = o8, row = 0;
-        for (const Row &r : sum_rows) {
-            int64_t *w = r.len == 2 ? &w2 : r.len == 4 ? &w4 : r.len == 8 ? &w8 : nullptr;
-            if (w) for (uint32_t q = 0; q < r.len; ++q) pk[(*w)++] = (int32_t)loc[r.begin + q];
-            else other.push_back((int32_t)row);
-            ++row;
+        int32_t no = 0;
+        for (int64_t r = r0; r < r1; ++r) {
+            const uint32_t len = sum_rows[(size_t)r].len;
+            if (len != 2 && len != 4 && len != 8) { pk.push_back((int32_t)r); ++no; }
         }
-        c->n2 = cnt[0]; c->n4 = cnt[1]; c->n8 = cnt[2]; c->n_other = (int64_t)other.size();
-        c->pk4 = c->pk2 + o4; c->pk8 = c->pk2 + o8; c->other_rows = c->pk2 + oo;
-        if (oo + (int64_t)other.size() > (int64_t)pk.size()) pk.resize((size_t)(oo + other.size()));
-        for (size_t t = 0; t < other.size(); ++t) pk[(size_t)oo + t] = other[t];
-        pk.resize((size_t)(oo + other.size()) > 0 ? (size_t)(oo + other.size()) : 1);
+        while (pk.size() % 4) pk.push_back(0);
+        d[4] = no;
     }
+    if (pk.empty()) pk.push_back(0);
+    c->n_gs_chunks = n_chunks;
+    c->gs_desc = c->pk + nk_align_up(pk.size(), 64);
     c->n_unique = n_unique; c->n_shared_unique = n_shared; c->n_masked_unique = n_masked;
     c->n_rows = n_rows; c->n_listed = n_listed; c->n_sum_rows = n_sum_rows; c->n_sum_listed = n_sum_listed;
 
@@ -146,7 +157,8 @@ int setup_impl(nk_ctx *c, const double *coords, const int64_t *glo_num, const do
     NK_CUDA(cudaMemcpyAsync(c->row_off, off.data(), off.size() * sizeof(int32_t), cudaMemcpyHostToDevice, st));
     if (n_listed > 0)
         NK_CUDA(cudaMemcpyAsync(c->row_idx, idx.data(), (size_t)n_listed * sizeof(int32_t), cudaMemcpyHostToDevice, st));
-    NK_CUDA(cudaMemcpyAsync(c->pk2, pk.data(), pk.size() * sizeof(int32_t), cudaMemcpyHostToDevice, st));
+    NK_CUDA(cudaMemcpyAsync(c->pk, pk.data(), pk.size() * sizeof(int32_t), cudaMemcpyHostToDevice, st));
+    NK_CUDA(cudaMemcpyAsync(c->gs_desc, desc.data(), desc.size() * sizeof(int32_t), cudaMemcpyHostToDevice, st));
     NK_CUDA(cudaMemcpyAsync(c->ctab, ctab, sizeof(ctab), cudaMemcpyHostToDevice, st));
     NK_CUDA(cudaMemcpyAsync(c->mtab, mtab, sizeof(mtab), cudaMemcpyHostToDevice, st));
     NK_CUDA(cudaMemcpyAsync(D_dev, c->D, sizeof(double) * c->n * c->n, cudaMemcpyHostToDevice, st));
@@ -205,7 +217,7 @@ extern "C" int nk_setup(nk_ctx **ctx, int64_t E, int N, const double *coords, co
     c->code = reinterpret_cast<uint8_t *>(q); q += cv.code;
     c->row_off = reinterpret_cast<int32_t *>(q); q += cv.off;
     c->row_idx = reinterpret_cast<int32_t *>(q); q += cv.idx;
-    c->pk2 = reinterpret_cast<int32_t *>(q); q += cv.pk;
+    c->pk = reinterpret_cast<int32_t *>(q); q += cv.pk;
     c->ctab = reinterpret_cast<double *>(q); c->mtab = c->ctab + NK_CTAB; q += cv.tabs;
     c->red.partials = reinterpret_cast<double *>(q); q += cv.partials;
     c->hist = reinterpret_cast<double *>(q); q += cv.hist;
