@@ -474,7 +474,8 @@ ax_tma_kernel(double *__restrict__ u_rw, const double *__restrict__ u_ro, const 
                 const double wv = rw[k] + (sB[pbase + k * S2] + sC[pbase + k * S2]);
                 if (active) w[gbase + k * n2] = wv;
             }
-            if (NW == 2) group_sync<GTH>(grp);      // next P1 writes A, which P5 still reads as C
+            // (no barrier here even when C aliases A: P5 reads and the next P1 writes the same pencil
+            //  positions, by the same thread)
             if (C::PF == 0) prefetch();
         }
     }
