@@ -105,7 +105,7 @@ int nk_cg_step(nk_ctx *ctx, double *x, void *stream);
 int nk_cg_get_state(nk_ctx *ctx, double *r, double *p, double *w, void *stream);
 int nk_get_scalars(nk_ctx *ctx, double *out5_host, void *stream);
 
-/* Options (all default 0 unless stated):
+/* Options:
  *   "ax_variant"   0 (default) = TMA-pipelined persistent kernel (nk_ax_tma.cu); 1 = the round's first
  *                  kernel, one CTA per element batch without pipelining (nk_ax.cu), kept for A/B runs
  *   "fuse_pap"     1 (default) = pap accumulated inside ax_e through the dot-fusion identity
@@ -135,7 +135,9 @@ int nk_get_D(nk_ctx *ctx, double *D_host, double *xi_host, double *w_host);
 /* Device time per kernel class since the last call, measured with CUDA events on the launching
  * stream while the "profile" option is 1 (S 8(d): per-kernel time inside the timed region).
  * HOST out: ms[6], count[6], classes NK_K_*: 0 ax_e (with whatever is fused into it), 1 gs(+mask),
- * 2 dot, 3 update x,r + rtr, 4 update p, 5 cg init.  Synchronises `stream`; resets the record. */
+ * 2 dot, 3 the residual update with rtr (update_r; update x,r on the fuse_p path), 4 the direction
+ * update (update_px: x and p; update p on the fuse_p path), 5 cg init.  Synchronises `stream`; resets
+ * the record. */
 #define NK_K_CLASSES 6
 int nk_get_kernel_times(nk_ctx *ctx, double *ms_host, int64_t *count_host, void *stream);
 /* Kernel launches enqueued by this context so far (for bench.py's gpu_launches). */
