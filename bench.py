@@ -255,7 +255,7 @@ def run_ours(args) -> dict | None:
     t0 = time.perf_counter()
     nk = Nekbone.from_mesh(mesh)
     setup_s = time.perf_counter() - t0
-    for k, v in (("fuse_pap", args.fuse_pap), ("fuse_p", args.fuse_p), ("graph", args.graph)):
+    for k, v in (("fuse_pap", args.fuse_pap), ("fuse_p", args.fuse_p), ("graph", args.graph), ("pdl", args.pdl)):
         nk.set_option(k, v)
     sizes = {**nk.sizes(), **nk.gs_sizes()}
     L = mesh.L
@@ -349,7 +349,7 @@ def run_ours(args) -> dict | None:
            "e2e": {"value": e2e, "unit": UNIT, "h2d_bytes_per_step": 8 * L,
                    "d2h_bytes_per_step": 8 * (L + niter + 1), "ms_per_step": ms_e2e / args.steps},
            "gpu_launches": int(launches), "clocks": clk,
-           "options": {"fuse_pap": args.fuse_pap, "fuse_p": args.fuse_p, "graph": args.graph, "graph_used": graphed},
+           "options": {"fuse_pap": args.fuse_pap, "fuse_p": args.fuse_p, "graph": args.graph, "graph_used": graphed, "pdl": args.pdl},
            "setup_s": setup_s, "final_residual": res_final}
 
     # ---- iteration-level and kernel-level bandwidth ---------------------------------------------------
@@ -404,6 +404,7 @@ def main():
     ap.add_argument("--impl", default="ours", choices=["ours", "reference"])
     ap.add_argument("--workload", default="config5", choices=["config1", "config2", "config3", "config5"])
     ap.add_argument("--fuse-pap", type=int, default=1)
+    ap.add_argument("--pdl", type=int, default=1, help="programmatic dependent launch inside nk_cg (library default 1)")
     ap.add_argument("--fuse-p", type=int, default=2, help="0 off, 1 on, 2 library default (on up to 2^24 points)")
     ap.add_argument("--graph", type=int, default=2, help="0 off, 1 on, 2 library default (graph up to 2^24 points)")
     ap.add_argument("--traffic", type=float, default=None,

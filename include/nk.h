@@ -116,6 +116,12 @@ int nk_get_scalars(nk_ctx *ctx, double *out5_host, void *stream);
  *                  (cached per f, x, res_hist, niter; updated in place when the pointers change) and
  *                  replays it; 2 (default) = 1 for meshes of up to 2^24 local points, where launch gaps
  *                  matter, else 0
+ *   "pdl"          1 (default) = inside nk_cg, ax_e and the vector kernels are launched as programmatic
+ *                  dependents of their predecessor (cudaLaunchAttributeProgrammaticStreamSerialization):
+ *                  each runs its prologue early and executes griddepcontrol.wait before the first read of
+ *                  anything the predecessor wrote, so results are bit-identical to 0 = plain launches.
+ *                  gs is always launched plainly (its gathers need the L1 that ax_e's shared-memory
+ *                  carve-out takes away).  Ignored under "profile".
  *   "profile"      1 = record a CUDA event on `stream` between consecutive launches so that
  *                  nk_get_kernel_times can report device time per kernel class (nk_cg then
  *                  enqueues its launches directly whatever "graph" says)

@@ -127,6 +127,10 @@ cudaError_t enqueue_cg(nk_ctx *c, const double *f, double *x, int niter, double 
     c->p_pending = 0;
     if ((e = prof_mark(c, -1, st)) != cudaSuccess) return e;
     NK_LAUNCH(NK_K_INIT, nk_launch_cg_init(c, f, x, res_hist, st));
+    // "pdl": every kernel of the loop waits (griddepcontrol.wait) before it reads what its predecessor
+    // wrote, so the launches may overlap tail and prologue; the event pairs of "profile" would serialise them
+    struct pdl_scope { nk_ctx *c; ~pdl_scope() { c->pdl_now = 0; } } scope{c};
+    c->pdl_now = c->opt_profile ? 0 : c->opt_pdl;
     for (int k = 1; k <= niter; ++k)
         if ((e = enqueue_iteration(c, x, res_hist + k, st)) != cudaSuccess) return e;
     if (c->p_pending) {          // leave the context with p up to date
@@ -191,7 +195,7 @@ int nk_cg(nk_ctx *c, const double *f, double *x, int niter, double *res_hist, vo
     }
     // Record the launch sequence once per (f, x, res_hist, niter, options) and replay it: the CG
     // loop of the small configs is launch-bound (S 7 hard part 4).
-    const int key = c->opt_fuse_pap | (c->opt_fuse_p << 1) | (c->opt_ax_variant << 3);
+    const int key = c->opt_fuse_pap | (c->opt_fuse_p << 1) | (c->opt_ax_variant << 3) | (c->opt_pdl << 4);
     if (!c->graph_exec || c->graph_f != f || c->graph_x != x || c->graph_hist != res_hist ||
         c->graph_niter != niter || c->graph_key != key) {
         cudaStream_t cap;
@@ -314,6 +318,7 @@ static int *option_slot(nk_ctx *c, const char *name, int *lo, int *hi)
     if (!std::strcmp(name, "fuse_pap")) { *lo = 0; *hi = 1; return &c->opt_fuse_pap; }
     if (!std::strcmp(name, "fuse_p")) { *lo = 0; *hi = 2; return &c->opt_fuse_p; }
     if (!std::strcmp(name, "graph")) { *lo = 0; *hi = 2; return &c->opt_graph; }
+    if (!std::strcmp(name, "pdl")) { *lo = 0; *hi = 1; return &c->opt_pdl; }
     if (!std::strcmp(name, "profile")) { *lo = 0; *hi = 1; return &c->opt_profile; }
     return nullptr;
 }

@@ -350,6 +350,7 @@ ax_tma_kernel(double *__restrict__ u_rw, const double *__restrict__ u_ro, const 
         const int rbase = (a + n * b) * S1;             // row (j,k) = (a,b): + i
         const int cbase = a + b * S2;                   // column (i,k) = (a,b): + j*S1
         const double2 *gslot = ring + slot * KP * 3 * n2 + t2;
+        nk_pdl_wait();                                  // u, r, beta come from the preceding kernels
         const double beta = FUSEP ? red.scal[NK_S_BETA] : 0.0;
         int stage = 0;
         uint32_t phase = 0;
@@ -489,12 +490,15 @@ cudaError_t launch_tma(nk_ctx *c, double *u_rw, const double *u_ro, const double
     using C = TmaCfg<N>;
     const int64_t nb = (c->E + C::EPB - 1) / C::EPB;
     const unsigned grid = (unsigned)(nb < (int64_t)c->sm_count ? nb : (int64_t)c->sm_count);   // one CTA per SM
+    cudaError_t e;
     if (r_in != nullptr)
-        ax_tma_kernel<N, true><<<grid, C::THREADS, C::SMEM, st>>>(u_rw, nullptr, r_in, w, c->g, c->E, dot, c->red);
+        e = nk_launch(ax_tma_kernel<N, true>, grid, C::THREADS, C::SMEM, st, c->pdl_now, u_rw, (const double *)nullptr, r_in, w,
+                      (const double2 *)c->g, c->E, dot, c->red);
     else
-        ax_tma_kernel<N, false><<<grid, C::THREADS, C::SMEM, st>>>(nullptr, u_ro, nullptr, w, c->g, c->E, dot, c->red);
+        e = nk_launch(ax_tma_kernel<N, false>, grid, C::THREADS, C::SMEM, st, c->pdl_now, (double *)nullptr, u_ro,
+                      (const double *)nullptr, w, (const double2 *)c->g, c->E, dot, c->red);
     c->launches++;
-    return cudaGetLastError();
+    return e != cudaSuccess ? e : cudaGetLastError();
 }
 
 template <int N>

@@ -78,7 +78,8 @@ struct nk_ctx {
     int64_t n_unique, n_shared_unique, n_masked_unique;
     int64_t n_rows, n_listed, n_sum_rows, n_sum_listed;
     // options / state
-    int opt_ax_variant, opt_fuse_pap, opt_fuse_p, opt_graph, opt_profile;
+    int opt_ax_variant, opt_fuse_pap, opt_fuse_p, opt_graph, opt_profile, opt_pdl;
+    int pdl_now;                 // opt_pdl while nk_cg enqueues its loop (every kernel there waits), else 0
     int p_pending;               // 1: p = r + beta p has not been applied yet (fuse_p)
     int64_t launches;
     // per-kernel-class device timing ("profile" option): chained events, interval i = kernel class cls[i]
@@ -87,6 +88,27 @@ struct nk_ctx {
     cudaGraphExec_t graph_exec;
     const double *graph_f; double *graph_x; double *graph_hist; int graph_niter; int graph_key;
 };
+
+// Programmatic dependent launch (PDL): a kernel launched with `pdl` may start while its predecessor on
+// the stream is still draining; it runs its prologue (shared tables, mbarrier set-up, the first TMA
+// requests for the STATIC geometric factors) and then waits (nk_pdl_wait) before it touches anything the
+// predecessor wrote.  Without the attribute the two device calls are no-ops.
+#ifdef __CUDACC__
+__device__ __forceinline__ void nk_pdl_launch_dependents() { asm volatile("griddepcontrol.launch_dependents;" ::: "memory"); }
+__device__ __forceinline__ void nk_pdl_wait() { asm volatile("griddepcontrol.wait;" ::: "memory"); }
+template <typename... KArgs, typename... Args>
+inline cudaError_t nk_launch(void (*kernel)(KArgs...), dim3 grid, dim3 block, size_t smem, cudaStream_t st, int pdl,
+                             Args... args)
+{
+    cudaLaunchConfig_t cfg = {};
+    cfg.gridDim = grid; cfg.blockDim = block; cfg.dynamicSmemBytes = smem; cfg.stream = st;
+    cudaLaunchAttribute at[1];
+    at[0].id = cudaLaunchAttributeProgrammaticStreamSerialization;
+    at[0].val.programmaticStreamSerializationAllowed = 1;
+    cfg.attrs = at; cfg.numAttrs = pdl ? 1 : 0;
+    return cudaLaunchKernelEx(&cfg, kernel, KArgs(args)...);
+}
+#endif
 
 // ---- kernels' host launchers (each returns a cudaError_t from the launch) -----------------------
 // nk_basis.cpp

@@ -96,7 +96,9 @@ update_xr_kernel(double *__restrict__ x, double *__restrict__ r, const double *_
 {
     __shared__ double s_c[NK_CTAB];
     __shared__ double s_red[33];
+    nk_pdl_launch_dependents();
     load_ctab(s_c, ctab);
+    nk_pdl_wait();
     const double alpha = ws.scal[NK_S_ALPHA];
     const int64_t pairs = L >> 1;
     const int64_t stride = (int64_t)gridDim.x * blockDim.x;
@@ -130,6 +132,8 @@ update_xr_kernel(double *__restrict__ x, double *__restrict__ r, const double *_
 __global__ void __launch_bounds__(NK_VEC_THREADS)
 update_p_kernel(double *__restrict__ p, const double *__restrict__ r, const double *__restrict__ scal, int64_t L)
 {
+    nk_pdl_launch_dependents();
+    nk_pdl_wait();
     const double beta = scal[NK_S_BETA];
     const int64_t pairs = L >> 1;
     const int64_t stride = (int64_t)gridDim.x * blockDim.x;
@@ -155,7 +159,9 @@ update_r_kernel(double *__restrict__ r, const double *__restrict__ w, const uint
 {
     __shared__ double s_c[NK_CTAB];
     __shared__ double s_red[33];
+    nk_pdl_launch_dependents();
     load_ctab(s_c, ctab);
+    nk_pdl_wait();
     const double alpha = ws.scal[NK_S_ALPHA];
     const int64_t pairs = L >> 1;
     const int64_t stride = (int64_t)gridDim.x * blockDim.x;
@@ -205,6 +211,8 @@ __global__ void __launch_bounds__(NK_VEC_THREADS)
 update_px_kernel(double *__restrict__ x, double *__restrict__ p, const double *__restrict__ r,
                  const double *__restrict__ scal, int64_t L)
 {
+    nk_pdl_launch_dependents();
+    nk_pdl_wait();
     const double alpha = scal[NK_S_ALPHA], beta = scal[NK_S_BETA];
     const int64_t pairs = L >> 1;
     const int64_t stride = (int64_t)gridDim.x * blockDim.x;
@@ -344,7 +352,9 @@ cudaError_t nk_launch_cg_init(nk_ctx *c, const double *f, double *x, double *his
 cudaError_t nk_launch_update_xr(nk_ctx *c, double *x, double *hist_k, cudaStream_t st)
 {
     const int nb = vec_blocks(c, c->L >> 1);
-    update_xr_kernel<<<nb, NK_VEC_THREADS, 0, st>>>(x, c->r, c->p, c->w, c->code, c->ctab, c->L, c->red, hist_k);
+    const cudaError_t e = nk_launch(update_xr_kernel, nb, NK_VEC_THREADS, 0, st, c->pdl_now, x, c->r, c->p, c->w, c->code,
+                                    c->ctab, c->L, c->red, hist_k);
+    if (e != cudaSuccess) return e;
     c->launches++;
     return cudaGetLastError();
 }
@@ -352,7 +362,8 @@ cudaError_t nk_launch_update_xr(nk_ctx *c, double *x, double *hist_k, cudaStream
 cudaError_t nk_launch_update_p(nk_ctx *c, cudaStream_t st)
 {
     const int nb = vec_blocks(c, c->L >> 1);
-    update_p_kernel<<<nb, NK_VEC_THREADS, 0, st>>>(c->p, c->r, c->red.scal, c->L);
+    const cudaError_t e = nk_launch(update_p_kernel, nb, NK_VEC_THREADS, 0, st, c->pdl_now, c->p, c->r, c->red.scal, c->L);
+    if (e != cudaSuccess) return e;
     c->launches++;
     return cudaGetLastError();
 }
@@ -393,7 +404,9 @@ cudaError_t nk_launch_update_pz(nk_ctx *c, double *x, cudaStream_t st)
 cudaError_t nk_launch_update_r(nk_ctx *c, double *hist_k, cudaStream_t st)
 {
     const int nb = vec_blocks(c, c->L >> 1);
-    update_r_kernel<<<nb, NK_VEC_THREADS, 0, st>>>(c->r, c->w, c->code, c->ctab, c->L, c->red, hist_k);
+    const cudaError_t e = nk_launch(update_r_kernel, nb, NK_VEC_THREADS, 0, st, c->pdl_now, c->r, c->w, c->code, c->ctab,
+                                    c->L, c->red, hist_k);
+    if (e != cudaSuccess) return e;
     c->launches++;
     return cudaGetLastError();
 }
@@ -401,7 +414,8 @@ cudaError_t nk_launch_update_r(nk_ctx *c, double *hist_k, cudaStream_t st)
 cudaError_t nk_launch_update_px(nk_ctx *c, double *x, cudaStream_t st)
 {
     const int nb = vec_blocks(c, c->L >> 1);
-    update_px_kernel<<<nb, NK_VEC_THREADS, 0, st>>>(x, c->p, c->r, c->red.scal, c->L);
+    const cudaError_t e = nk_launch(update_px_kernel, nb, NK_VEC_THREADS, 0, st, c->pdl_now, x, c->p, c->r, c->red.scal, c->L);
+    if (e != cudaSuccess) return e;
     c->launches++;
     return cudaGetLastError();
 }

@@ -187,6 +187,34 @@ def test_graph_default_and_pointer_change():
     assert bool((xc == xe).all()) and bool((hc == he).all())
 
 
+@pytest.mark.parametrize("name", ["config1", "config2", "config3"])
+@pytest.mark.parametrize("fuse_p", [0, 1])
+def test_programmatic_dependent_launch_is_bitwise_neutral(name, fuse_p):
+    """"pdl" = 1 (default) overlaps each kernel's prologue with its predecessor's tail; every read of the
+    predecessor's output sits behind griddepcontrol.wait, so x and the residual history must be bitwise those
+    of plain launches, graphed or not, with p folded into ax_e or not."""
+    import torch
+    from paper_2606_12650_b200 import Nekbone
+    from workloads import config_mesh
+    mesh = config_mesh(name)
+    gpu = Nekbone.from_mesh(mesh)
+    assert gpu.get_option("pdl") == 1
+    gpu.set_option("fuse_p", fuse_p)
+    f = to_dev(config_rhs(name, mesh))
+    out = {}
+    for graph in (0, 1):
+        for pdl in (0, 1):
+            gpu.set_option("graph", graph)
+            gpu.set_option("pdl", pdl)
+            for rep in range(3):                       # replays too: the waits must hold on every run
+                out[graph, pdl, rep] = gpu.cg(f, 40)
+    torch.cuda.synchronize()
+    x0, h0 = out[0, 0, 0]
+    for key, (x, h) in out.items():
+        assert bool((x == x0).all()) and bool((h == h0).all()), key
+    gpu.close()
+
+
 # ---- NEXT row f-3: Jacobi-preconditioned CG ------------------------------------------------------------
 @pytest.mark.parametrize("name", ["config1", "config2"])
 def test_jacobi_diag_and_pcg(name):
