@@ -105,6 +105,45 @@ int nk_cg_step(nk_ctx *ctx, double *x, void *stream);
 int nk_cg_get_state(nk_ctx *ctx, double *r, double *p, double *w, void *stream);
 int nk_get_scalars(nk_ctx *ctx, double *out5_host, void *stream);
 
+/* ---- Distributed gs / CG over an element partition, one rank per GPU ------------------------------
+ * (PAPER.md:336 lists multi-rank runs as future work; the original
+ * Nekbone is MPI.)  The context is set up on the rank's OWN elements with GLOBAL node ids.
+ * Interface nodes (ids held by more than one rank) get one slot each in an exchange buffer; the plan
+ * (paper_2606_12650_b200/dist.py builds it) is
+ *   pack[n_slots]        local index of one copy of the slot's node, or -1 if this rank does not hold it
+ *   unpack_loc/slot[n_unpack]   every local copy of an interface node and its slot
+ * and the buffers are send[n_slots + 1], gathered[world * (n_slots + 1)] (rank-major), scalar_send[1],
+ * scalar_gathered[world].  All DEVICE, owned by the caller, alive as long as the context is used this way.
+ * The library enqueues kernels only; where a line says [all-gather A -> B] the caller runs that collective
+ * on the same stream before the next call (NCCL all-gather through torch.distributed; every rank then holds
+ * every rank's contribution and adds them in rank order, so results are bitwise equal across ranks and
+ * reproducible).  Errors as elsewhere; NK_ERR_ARG before nk_dist_attach.
+ *
+ *   nk_dist_set_mult   replaces the LOCAL multiplicities by the given global ones (integers 1..127 as
+ *                      doubles, L of them): the weights c = 1/mult of every dot product.  Synchronises.
+ *   gs:    nk_dist_gs_begin(v)  [all-gather send -> gathered]  nk_dist_gs_end(v)
+ *   dot:   nk_dist_dot_begin(a, b)  [all-gather scalar_send -> scalar_gathered]  nk_dist_dot_end(out)
+ *   CG:    nk_dist_cg_begin(f, x)  [all-gather scalar]  nk_dist_cg_begin_end(hist0)
+ *          per iteration k:  nk_dist_iter_a()            w = A_L p (pap partial in send[n_slots]), local gs + mask, pack
+ *                            [all-gather send -> gathered]
+ *                            nk_dist_iter_b()            w totals, alpha = rho / pap, r -= alpha w, rho' partial
+ *                            [all-gather scalar]
+ *                            nk_dist_iter_c(x, hist_k)   beta, sqrt(rho') -> hist_k, x += alpha p, p = r + beta p
+ */
+int nk_dist_attach(nk_ctx *ctx, int rank, int world, int64_t n_slots, const int32_t *pack_dev, int64_t n_unpack,
+                   const int32_t *unpack_loc_dev, const int32_t *unpack_slot_dev, double *send_dev,
+                   double *gathered_dev, double *scalar_send_dev, double *scalar_gathered_dev);
+int nk_dist_set_mult(nk_ctx *ctx, const double *mult_dev, void *stream);
+int nk_dist_gs_begin(nk_ctx *ctx, double *v, int with_mask, void *stream);
+int nk_dist_gs_end(nk_ctx *ctx, double *v, void *stream);
+int nk_dist_dot_begin(nk_ctx *ctx, const double *a, const double *b, void *stream);
+int nk_dist_dot_end(nk_ctx *ctx, double *out_dev, void *stream);
+int nk_dist_cg_begin(nk_ctx *ctx, const double *f, double *x, void *stream);
+int nk_dist_cg_begin_end(nk_ctx *ctx, double *hist0_dev, void *stream);
+int nk_dist_iter_a(nk_ctx *ctx, void *stream);
+int nk_dist_iter_b(nk_ctx *ctx, void *stream);
+int nk_dist_iter_c(nk_ctx *ctx, double *x, double *hist_k_dev, void *stream);
+
 /* Options:
  *   "ax_variant"   0 (default) = TMA-pipelined persistent kernel (nk_ax_tma.cu); 1 = the round's first
  *                  kernel, one CTA per element batch without pipelining (nk_ax.cu), kept for A/B runs

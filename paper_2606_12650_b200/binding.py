@@ -45,6 +45,17 @@ SIGNATURES = {
     "nk_get_geom": (_i, [_vp, _vp, _vp]),
     "nk_get_D": (_i, [_vp, _vp, _vp, _vp]),
     "nk_get_kernel_times": (_i, [_vp, _vp, _vp, _vp]),
+    "nk_dist_attach": (_i, [_vp, _i, _i, _i64, _vp, _i64, _vp, _vp, _vp, _vp, _vp, _vp]),
+    "nk_dist_set_mult": (_i, [_vp, _vp, _vp]),
+    "nk_dist_gs_begin": (_i, [_vp, _vp, _i, _vp]),
+    "nk_dist_gs_end": (_i, [_vp, _vp, _vp]),
+    "nk_dist_dot_begin": (_i, [_vp, _vp, _vp, _vp]),
+    "nk_dist_dot_end": (_i, [_vp, _vp, _vp]),
+    "nk_dist_cg_begin": (_i, [_vp, _vp, _vp, _vp]),
+    "nk_dist_cg_begin_end": (_i, [_vp, _vp, _vp]),
+    "nk_dist_iter_a": (_i, [_vp, _vp]),
+    "nk_dist_iter_b": (_i, [_vp, _vp]),
+    "nk_dist_iter_c": (_i, [_vp, _vp, _vp, _vp]),
     "nk_get_launch_count": (_i, [_vp, C.POINTER(_i64)]),
     "nk_strerror": (C.c_char_p, [_i]),
     "nk_last_cuda_error": (_i, []),

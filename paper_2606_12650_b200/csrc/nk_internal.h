@@ -41,6 +41,7 @@ struct nk_reduce_ws {
     double *partials;      // NK_MAX_PARTIALS doubles
     unsigned *counter;     // one ticket counter, self-resetting (atomicInc wrap)
     double *scal;          // NK_S_COUNT doubles
+    double *raw;           // NULL, or (distributed CG) where the rank-local total goes INSTEAD of the epilogue
 };
 
 struct nk_ctx {
@@ -84,6 +85,12 @@ struct nk_ctx {
     int64_t launches;
     // per-kernel-class device timing ("profile" option): chained events, interval i = kernel class cls[i]
     nk_prof *prof;
+    // distributed gs / CG (nk_dist.cu; S 8(e), 8(f) f-4): interface plan and exchange buffers, all DEVICE
+    // and owned by the caller (nk_dist_attach)
+    int dist_rank, dist_world;
+    int64_t dist_slots, dist_n_unpack;
+    const int32_t *dist_pack, *dist_uloc, *dist_uslot;
+    double *dist_send, *dist_gath, *dist_ssend, *dist_sgath;
     // cached graph for nk_cg
     cudaGraphExec_t graph_exec;
     const double *graph_f; double *graph_x; double *graph_hist; int graph_niter; int graph_key;

@@ -75,7 +75,10 @@ __device__ __forceinline__ void nk_grid_reduce(double v, double *sm, nk_reduce_w
     double t = 0.0;
     for (unsigned i = threadIdx.x; i < nb; i += blockDim.x) t += __ldcg(ws.partials + i);
     t = nk_block_sum(t, sm);
-    if (threadIdx.x == 0) nk_epilogue(epi, t, ws.scal, out);
+    if (threadIdx.x == 0) {
+        if (ws.raw) ws.raw[0] = t;              // distributed: the epilogue runs after the all-gather (nk_dist.cu)
+        else nk_epilogue(epi, t, ws.scal, out);
+    }
 }
 
 // Two sums at once (preconditioned CG: <r,z>_c and <r,r>_c in one pass).  Partials of the second sum

@@ -223,6 +223,7 @@ extern "C" int nk_setup(nk_ctx **ctx, int64_t E, int N, const double *coords, co
     c->hist = reinterpret_cast<double *>(q); q += cv.hist;
     c->red.scal = reinterpret_cast<double *>(q); q += cv.scal;
     c->red.counter = reinterpret_cast<unsigned *>(q);
+    c->red.raw = nullptr;
     c->errflag = reinterpret_cast<int *>(q + 64);
     c->res_dummy = reinterpret_cast<double *>(q + 128);
     int rc;
