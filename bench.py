@@ -396,6 +396,104 @@ def run_ours(args) -> dict | None:
     return out
 
 
+# ---- our arm, sharded: ONE mesh over all ranks ------------------------------------------
+def run_sharded(args) -> dict | None:
+    """`--sharded`: the workload's mesh is partitioned by elements over the ranks (paper_2606_12650_b200.dist:
+    one all-gather for gs and two scalar all-gathers per iteration over NCCL), so total work is fixed: "strong"
+    scaling.  The default without the flag stays N independent replicas.  Needs a process group
+    also at N = 1 (then it measures what the split-phase path costs against the fused nk_cg)."""
+    import torch
+    import torch.distributed as dist
+    from paper_2606_12650_b200.dist import DistNekbone, TorchComm
+    from workloads import CONFIGS, config_mesh, rhs_unique
+
+    rank = int(os.environ.get("RANK", "0"))
+    world = int(os.environ.get("WORLD_SIZE", "1"))
+    local = int(os.environ.get("LOCAL_RANK", "0"))
+    if not torch.cuda.is_available():
+        raise SystemExit("bench.py: no CUDA device (there is no CPU fallback; use --impl reference for the oracle)")
+    torch.cuda.set_device(local)
+    if world == 1:
+        os.environ.setdefault("MASTER_ADDR", "127.0.0.1")
+        os.environ.setdefault("MASTER_PORT", str(29400 + os.getpid() % 500))
+    dist.init_process_group("nccl", rank=rank, world_size=world, device_id=torch.device("cuda", local))
+    cfg = CONFIGS[args.workload]
+    niter, N = cfg["niter"], cfg["N"]
+    mesh = config_mesh(args.workload)
+    f_np = rhs_unique(mesh, cfg["seed"])                                  # one RHS for the whole mesh
+    d = DistNekbone.from_mesh(mesh, TorchComm())
+    L = mesh.L
+    U = int(np.unique(mesh.glo_num).size)
+    flops_step = flops_per_point_iter(N, float(L - U) / L) * L * niter    # of the WHOLE mesh
+    stream = torch.cuda.current_stream()
+    f_loc = d.local(f_np)
+    f = torch.from_numpy(f_loc).cuda()
+    x = d.empty()
+    hist = torch.empty(niter + 1, dtype=torch.float64, device="cuda")
+    small = d.L * 8 * 11 <= 2 * 126e6
+    flush = torch.empty(256 << 20, dtype=torch.uint8, device="cuda") if small else None
+
+    def barrier():
+        dist.barrier()
+        torch.cuda.synchronize()
+
+    def timed(fn):
+        e = [torch.cuda.Event(enable_timing=True) for _ in range(2 * args.steps)]
+        barrier()
+        for s in range(args.steps):
+            if flush is not None:
+                flush.fill_(1)
+            e[2 * s].record(stream)
+            fn()
+            e[2 * s + 1].record(stream)
+        barrier()
+        return sum(e[2 * s].elapsed_time(e[2 * s + 1]) for s in range(args.steps))
+
+    for _ in range(args.warmup):
+        d.cg(f, niter, x=x, res_hist=hist)
+    launches0 = d.nk.launch_count()
+    clocks = ClockSampler(local)
+    clocks.start()
+    time.sleep(0.25)
+    w0 = time.time()
+    ms = timed(lambda: d.cg(f, niter, x=x, res_hist=hist))
+    w1 = time.time()
+    clk = clocks.stop(w0, w1)
+    launches = d.nk.launch_count() - launches0
+    f_pin = torch.from_numpy(f_loc).pin_memory()
+    x_pin = torch.empty(d.L, dtype=torch.float64).pin_memory()
+    h_pin = torch.empty(niter + 1, dtype=torch.float64).pin_memory()
+
+    def e2e_step():
+        f.copy_(f_pin, non_blocking=True)
+        d.cg(f, niter, x=x, res_hist=hist)
+        x_pin.copy_(x, non_blocking=True)
+        h_pin.copy_(hist, non_blocking=True)
+        stream.synchronize()
+
+    e2e_step()
+    ms_e2e = timed(e2e_step)
+    ms, ms_e2e = max_over_ranks(dist, [ms, ms_e2e], "cuda")
+    res_final = float(hist[-1])
+    n_slots = d.n_slots
+    dist.barrier()
+    dist.destroy_process_group()
+    if rank != 0:
+        return None
+    out = {"metric": METRIC, "value": flops_step * args.steps / (ms * 1e-3) / 1e9, "unit": UNIT, "n_gpus": world,
+           "steps": args.steps, "warmup": args.warmup, "ms_per_step": ms / args.steps, "higher_is_better": True,
+           "scaling": "strong", "vs_baseline": None, "dtype": "f64", "data": "synthetic",
+           "config": {**workload_config(args.workload, cfg, world),
+                      "parallelism": f"element partition over {world} rank(s); gs interface all-gather ({n_slots} slots) + "
+                                     "2 scalar all-gathers per iteration (NCCL)"},
+           "e2e": {"value": flops_step * args.steps / (ms_e2e * 1e-3) / 1e9, "unit": UNIT,
+                   "h2d_bytes_per_step": 8 * d.L, "d2h_bytes_per_step": 8 * (d.L + niter + 1),
+                   "ms_per_step": ms_e2e / args.steps},
+           "gpu_launches": int(launches), "clocks": clk, "final_residual": res_final,
+           "roofline": None, "note": "sharded mode: see the default (replica) line for roofline and cpu_baseline"}
+    return out
+
+
 def main():
     ap = argparse.ArgumentParser()
     ap.add_argument("--gpus", type=int, default=1)
@@ -410,6 +508,8 @@ def main():
     ap.add_argument("--traffic", type=float, default=None,
                     help="dram bytes per ax_e launch from the committed ncu --set full capture (profiles/)")
     ap.add_argument("--no-cpu-baseline", action="store_true")
+    ap.add_argument("--sharded", action="store_true",
+                    help="partition ONE mesh over the ranks (distributed gs / CG) instead of N replicas")
     args = ap.parse_args()
     args.warmup = max(args.warmup, 3) if args.impl == "ours" else args.warmup
     rank = int(os.environ.get("RANK", "0"))
@@ -417,7 +517,7 @@ def main():
         if rank == 0:
             print(json.dumps(run_reference(args)), flush=True)
         return
-    out = run_ours(args)
+    out = run_sharded(args) if args.sharded else run_ours(args)
     if out is not None:
         print(json.dumps(out), flush=True)
 
