@@ -448,6 +448,8 @@ int nk_pcg(nk_ctx *c, const double *f, double *x, int niter, double *res_hist, v
     NK_CUDA(prof_mark(c, -1, st));
     NK_CUDA(nk_launch_pcg_init(c, f, x, res_hist, st));
     NK_CUDA(prof_mark(c, NK_K_INIT, st));
+    struct pdl_scope { nk_ctx *c; ~pdl_scope() { c->pdl_now = 0; } } scope{c};
+    c->pdl_now = c->opt_profile ? 0 : c->opt_pdl;      // as in nk_cg: every kernel of the loop waits before its first dependent read
     for (int k = 1; k <= niter; ++k) {
         NK_CUDA(nk_launch_ax_e(c, nullptr, c->p, nullptr, c->w, c->opt_fuse_pap, c->opt_ax_variant, st));
         NK_CUDA(prof_mark(c, NK_K_AX, st));

@@ -274,7 +274,9 @@ update_rz_kernel(double *__restrict__ r, const double *__restrict__ w, const dou
 {
     __shared__ double s_c[NK_CTAB];
     __shared__ double s_red[33];
+    nk_pdl_launch_dependents();
     load_ctab(s_c, ctab);
+    nk_pdl_wait();
     const double alpha = ws.scal[NK_S_ALPHA];
     const int64_t pairs = L >> 1;
     const int64_t stride = (int64_t)gridDim.x * blockDim.x;
@@ -309,6 +311,8 @@ __global__ void __launch_bounds__(NK_VEC_THREADS)
 update_pxz_kernel(double *__restrict__ x, double *__restrict__ p, const double *__restrict__ r,
                   const double *__restrict__ dinv, const double *__restrict__ scal, int64_t L)
 {
+    nk_pdl_launch_dependents();
+    nk_pdl_wait();
     const double alpha = scal[NK_S_ALPHA], beta = scal[NK_S_BETA];
     const int64_t pairs = L >> 1;
     const int64_t stride = (int64_t)gridDim.x * blockDim.x;
@@ -388,7 +392,9 @@ cudaError_t nk_launch_update_xrz(nk_ctx *c, double *x, double *hist_k, cudaStrea
 {
     const int nb = vec_blocks(c, c->L >> 1);
     (void)x;
-    update_rz_kernel<<<nb, NK_VEC_THREADS, 0, st>>>(c->r, c->w, c->dinv, c->code, c->ctab, c->L, c->red, hist_k);
+    const cudaError_t e = nk_launch(update_rz_kernel, nb, NK_VEC_THREADS, 0, st, c->pdl_now, c->r, c->w, c->dinv, c->code,
+                                    c->ctab, c->L, c->red, hist_k);
+    if (e != cudaSuccess) return e;
     c->launches++;
     return cudaGetLastError();
 }
@@ -396,7 +402,9 @@ cudaError_t nk_launch_update_xrz(nk_ctx *c, double *x, double *hist_k, cudaStrea
 cudaError_t nk_launch_update_pz(nk_ctx *c, double *x, cudaStream_t st)
 {
     const int nb = vec_blocks(c, c->L >> 1);
-    update_pxz_kernel<<<nb, NK_VEC_THREADS, 0, st>>>(x, c->p, c->r, c->dinv, c->red.scal, c->L);
+    const cudaError_t e = nk_launch(update_pxz_kernel, nb, NK_VEC_THREADS, 0, st, c->pdl_now, x, c->p, c->r, c->dinv,
+                                    c->red.scal, c->L);
+    if (e != cudaSuccess) return e;
     c->launches++;
     return cudaGetLastError();
 }

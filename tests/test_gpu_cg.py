@@ -241,6 +241,31 @@ def test_jacobi_diag_and_pcg(name):
     assert bool((xa == xb).all()) and bool((ha == hb).all())
 
 
+@pytest.mark.parametrize("name", ["config1", "config2", "config3"])
+@pytest.mark.parametrize("fuse_pap", [1, 0])
+def test_pcg_programmatic_dependent_launch_is_bitwise_neutral(name, fuse_pap):
+    """nk_pcg's loop launches ax_e, update_rz and update_pz as programmatic dependents too: same iterates,
+    bit for bit, as plain launches, on repeated calls."""
+    import torch
+    from paper_2606_12650_b200 import Nekbone
+    from workloads import config_mesh
+    mesh = config_mesh(name)
+    gpu = Nekbone.from_mesh(mesh)
+    gpu.set_option("fuse_pap", fuse_pap)
+    f = to_dev(config_rhs(name, mesh))
+    out = {}
+    for pdl in (0, 1):
+        gpu.set_option("pdl", pdl)
+        for rep in range(3):
+            x, h = gpu.pcg(f, 40)
+            out[pdl, rep] = (x.clone(), h.clone())
+    torch.cuda.synchronize()
+    x0, h0 = out[0, 0]
+    for key, (x, h) in out.items():
+        assert bool((x == x0).all()) and bool((h == h0).all()), key
+    gpu.close()
+
+
 @pytest.mark.parametrize("N", [6, 10, 12, 14, 15])
 def test_cg_high_and_odd_orders(N):
     """CG through the fused-pap path of every kernel configuration family: sync groups per slot (N = 10),
