@@ -155,8 +155,9 @@ class OracleSample:
 
     def calibrate(self, budget_s: float) -> int:
         self.time_iters(1)                                # first call: thread pool, page faults
-        t3 = self.time_iters(3)
-        return int(max(3, min(400, round(3 * budget_s / max(t3, 1e-6)))))
+        t3, t23 = self.time_iters(3), self.time_iters(23)  # a call has a fixed part (set-up, first residual)
+        per = max((t23 - t3) / 20.0, 1e-6)
+        return int(max(3, min(4000, round((budget_s - max(t3 - 3 * per, 0.0)) / per))))
 
     def gflops(self, k: int, seconds: float) -> float:
         return self.fpp * self.mesh.L * k / seconds / 1e9
