@@ -503,7 +503,7 @@ def main():
     ap.add_argument("--impl", default="ours", choices=["ours", "reference"])
     ap.add_argument("--workload", default="config5", choices=["config1", "config2", "config3", "config5"])
     ap.add_argument("--fuse-pap", type=int, default=1)
-    ap.add_argument("--pdl", type=int, default=1, help="programmatic dependent launch inside nk_cg (library default 1)")
+    ap.add_argument("--pdl", type=int, default=3, help="programmatic dependent launch inside nk_cg: 0 off, 1 all but gs, 2 gs too, 3 library default (2 up to 2^24 points, else 1)")
     ap.add_argument("--fuse-p", type=int, default=2, help="0 off, 1 on, 2 library default (on up to 2^24 points)")
     ap.add_argument("--graph", type=int, default=2, help="0 off, 1 on, 2 library default (graph up to 2^24 points)")
     ap.add_argument("--traffic", type=float, default=None,

@@ -155,12 +155,13 @@ int nk_dist_iter_c(nk_ctx *ctx, double *x, double *hist_k_dev, void *stream);
  *                  (cached per f, x, res_hist, niter; updated in place when the pointers change) and
  *                  replays it; 2 (default) = 1 for meshes of up to 2^24 local points, where launch gaps
  *                  matter, else 0
- *   "pdl"          1 (default) = inside nk_cg, ax_e and the vector kernels are launched as programmatic
+ *   "pdl"          1 = inside nk_cg, ax_e and the vector kernels are launched as programmatic
  *                  dependents of their predecessor (cudaLaunchAttributeProgrammaticStreamSerialization):
  *                  each runs its prologue early and executes griddepcontrol.wait before the first read of
  *                  anything the predecessor wrote, so results are bit-identical to 0 = plain launches.
- *                  gs is always launched plainly (its gathers need the L1 that ax_e's shared-memory
- *                  carve-out takes away).  Ignored under "profile".
+ *                  2 = gs as well (on large meshes slower: its gathers need the L1 that ax_e's
+ *                  shared-memory carve-out takes away); 3 (default) = 2 for meshes of up to 2^24 local
+ *                  points, else 1.  Ignored under "profile".
  *   "profile"      1 = record a CUDA event on `stream` between consecutive launches so that
  *                  nk_get_kernel_times can report device time per kernel class (nk_cg then
  *                  enqueues its launches directly whatever "graph" says)

@@ -130,7 +130,7 @@ cudaError_t enqueue_cg(nk_ctx *c, const double *f, double *x, int niter, double 
     // "pdl": every kernel of the loop waits (griddepcontrol.wait) before it reads what its predecessor
     // wrote, so the launches may overlap tail and prologue; the event pairs of "profile" would serialise them
     struct pdl_scope { nk_ctx *c; ~pdl_scope() { c->pdl_now = 0; } } scope{c};
-    c->pdl_now = c->opt_profile ? 0 : c->opt_pdl;
+    c->pdl_now = c->opt_profile ? 0 : nk_pdl_mode(c);
     for (int k = 1; k <= niter; ++k)
         if ((e = enqueue_iteration(c, x, res_hist + k, st)) != cudaSuccess) return e;
     if (c->p_pending) {          // leave the context with p up to date
@@ -318,7 +318,7 @@ static int *option_slot(nk_ctx *c, const char *name, int *lo, int *hi)
     if (!std::strcmp(name, "fuse_pap")) { *lo = 0; *hi = 1; return &c->opt_fuse_pap; }
     if (!std::strcmp(name, "fuse_p")) { *lo = 0; *hi = 2; return &c->opt_fuse_p; }
     if (!std::strcmp(name, "graph")) { *lo = 0; *hi = 2; return &c->opt_graph; }
-    if (!std::strcmp(name, "pdl")) { *lo = 0; *hi = 1; return &c->opt_pdl; }
+    if (!std::strcmp(name, "pdl")) { *lo = 0; *hi = 3; return &c->opt_pdl; }
     if (!std::strcmp(name, "profile")) { *lo = 0; *hi = 1; return &c->opt_profile; }
     return nullptr;
 }
@@ -449,7 +449,7 @@ int nk_pcg(nk_ctx *c, const double *f, double *x, int niter, double *res_hist, v
     NK_CUDA(nk_launch_pcg_init(c, f, x, res_hist, st));
     NK_CUDA(prof_mark(c, NK_K_INIT, st));
     struct pdl_scope { nk_ctx *c; ~pdl_scope() { c->pdl_now = 0; } } scope{c};
-    c->pdl_now = c->opt_profile ? 0 : c->opt_pdl;      // as in nk_cg: every kernel of the loop waits before its first dependent read
+    c->pdl_now = c->opt_profile ? 0 : nk_pdl_mode(c);      // as in nk_cg: every kernel of the loop waits before its first dependent read
     for (int k = 1; k <= niter; ++k) {
         NK_CUDA(nk_launch_ax_e(c, nullptr, c->p, nullptr, c->w, c->opt_fuse_pap, c->opt_ax_variant, st));
         NK_CUDA(prof_mark(c, NK_K_AX, st));

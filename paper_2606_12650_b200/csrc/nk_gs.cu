@@ -76,6 +76,7 @@ gs_kernel(double *__restrict__ v, gs_plan pl, int with_mask)
         const int32_t *pk4 = pk2 + ((2 * d.y + 3) & ~3);
         const int32_t *pk8 = pk4 + 4 * d.z;
         const int32_t *oth = pk8 + 8 * d.w;
+        nk_pdl_wait();                     // the plan is static; v is what the predecessor wrote
         if (t < d.y) {
             const int2 ii = reinterpret_cast<const int2 *>(pk2)[t];
             const double s = v[ii.x] + v[ii.y];
@@ -112,6 +113,7 @@ gs_kernel(double *__restrict__ v, gs_plan pl, int with_mask)
         return;
     }
     const int t = (blockIdx.x - pl.n_chunks * BPC) * GS_THREADS + threadIdx.x;
+    nk_pdl_wait();
     if (with_mask) {
         const int q = pl.masked_begin + t;
         if (q < pl.n_listed) v[pl.idx[q]] = 0.0;
@@ -139,7 +141,7 @@ cudaError_t nk_launch_gs(nk_ctx *c, double *v, int with_mask, cudaStream_t st)
     pl.masked_begin = (int)c->n_sum_listed; pl.n_listed = (int)c->n_listed;
     // never a programmatic dependent: its blocks would land on SMs still carved out for ax_e's 227 KB of shared
     // memory (L1 of ~1 KB) and the gathers would miss it (measured: +95 us at config 5)
-    gs_kernel<<<(unsigned)nb, GS_THREADS, 0, st>>>(v, pl, with_mask);
+    cudaError_t e = nk_launch(gs_kernel, (unsigned)nb, GS_THREADS, 0, st, c->pdl_now == 2, v, pl, with_mask);
     c->launches++;
-    return cudaGetLastError();
+    return e != cudaSuccess ? e : cudaGetLastError();
 }

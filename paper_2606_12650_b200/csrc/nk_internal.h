@@ -80,7 +80,7 @@ struct nk_ctx {
     int64_t n_rows, n_listed, n_sum_rows, n_sum_listed;
     // options / state
     int opt_ax_variant, opt_fuse_pap, opt_fuse_p, opt_graph, opt_profile, opt_pdl;
-    int pdl_now;                 // opt_pdl while nk_cg enqueues its loop (every kernel there waits), else 0
+    int pdl_now;                 // nk_pdl_mode while nk_cg enqueues its loop (every kernel there waits), else 0
     int p_pending;               // 1: p = r + beta p has not been applied yet (fuse_p)
     int64_t launches;
     // per-kernel-class device timing ("profile" option): chained events, interval i = kernel class cls[i]
@@ -95,6 +95,10 @@ struct nk_ctx {
     cudaGraphExec_t graph_exec;
     const double *graph_f; double *graph_x; double *graph_hist; int graph_niter; int graph_key;
 };
+// "pdl" resolved: 0 = plain launches, 1 = ax_e and the vector kernels are programmatic dependents, 2 = gs too.
+// gs as a dependent saves a launch gap where gaps matter (config 1: -5 % per solve) and costs 95 us at
+// config 5 (its gathers land on SMs whose L1 is still carved out for ax_e): auto = 2 up to 2^24 points.
+static inline int nk_pdl_mode(const nk_ctx *c) { return c->opt_pdl == 3 ? (c->L <= NK_GRAPH_AUTO_MAX_L ? 2 : 1) : c->opt_pdl; }
 
 // Programmatic dependent launch (PDL): a kernel launched with `pdl` may start while its predecessor on
 // the stream is still draining; it runs its prologue (shared tables, mbarrier set-up, the first TMA

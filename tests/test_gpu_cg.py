@@ -190,7 +190,7 @@ def test_graph_default_and_pointer_change():
 @pytest.mark.parametrize("name", ["config1", "config2", "config3"])
 @pytest.mark.parametrize("fuse_p", [0, 1])
 def test_programmatic_dependent_launch_is_bitwise_neutral(name, fuse_p):
-    """"pdl" = 1 (default) overlaps each kernel's prologue with its predecessor's tail; every read of the
+    """"pdl" (default 3: gs too on meshes up to 2^24 points) overlaps each kernel's prologue with its predecessor's tail; every read of the
     predecessor's output sits behind griddepcontrol.wait, so x and the residual history must be bitwise those
     of plain launches, graphed or not, with p folded into ax_e or not."""
     import torch
@@ -198,12 +198,12 @@ def test_programmatic_dependent_launch_is_bitwise_neutral(name, fuse_p):
     from workloads import config_mesh
     mesh = config_mesh(name)
     gpu = Nekbone.from_mesh(mesh)
-    assert gpu.get_option("pdl") == 1
+    assert gpu.get_option("pdl") == 3
     gpu.set_option("fuse_p", fuse_p)
     f = to_dev(config_rhs(name, mesh))
     out = {}
     for graph in (0, 1):
-        for pdl in (0, 1):
+        for pdl in (0, 1, 2, 3):
             gpu.set_option("graph", graph)
             gpu.set_option("pdl", pdl)
             for rep in range(3):                       # replays too: the waits must hold on every run
@@ -254,7 +254,7 @@ def test_pcg_programmatic_dependent_launch_is_bitwise_neutral(name, fuse_pap):
     gpu.set_option("fuse_pap", fuse_pap)
     f = to_dev(config_rhs(name, mesh))
     out = {}
-    for pdl in (0, 1):
+    for pdl in (0, 1, 2):
         gpu.set_option("pdl", pdl)
         for rep in range(3):
             x, h = gpu.pcg(f, 40)
