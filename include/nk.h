@@ -145,8 +145,6 @@ int nk_dist_iter_b(nk_ctx *ctx, void *stream);
 int nk_dist_iter_c(nk_ctx *ctx, double *x, double *hist_k_dev, void *stream);
 
 /* Options:
- *   "ax_variant"   0 (default) = TMA-pipelined persistent kernel (nk_ax_tma.cu); 1 = the round's first
- *                  kernel, one CTA per element batch without pipelining (nk_ax.cu), kept for A/B runs
  *   "fuse_pap"     1 (default) = pap accumulated inside ax_e through the dot-fusion identity
  *                  <M QQ^T A_L p, p>_c = sum_l (A_L p)_l p_l; 0 = separate weighted dot after gs
  *   "fuse_p"       1 = p = r + beta p folded into the load of the next ax_e; 0 = own kernel;
@@ -186,6 +184,15 @@ int nk_get_D(nk_ctx *ctx, double *D_host, double *xi_host, double *w_host);
  * the record. */
 #define NK_K_CLASSES 6
 int nk_get_kernel_times(nk_ctx *ctx, double *ms_host, int64_t *count_host, void *stream);
+/* How ax_e is scheduled (for tests and reports): the persistent kernel works on batches of
+ * nk_ax_batch_elements(N) elements (a compile-time constant per order; NK_ERR_ARG for N outside [1,15]);
+ * nk_get_ax_launch gives that number, the CTAs one launch uses on this context's device and the number
+ * of batches the busiest CTA runs (> 1: the shared-memory ring wraps and its mbarrier phases flip). */
+int nk_ax_batch_elements(int N);
+int nk_get_ax_launch(nk_ctx *ctx, int *batch_elements, int *ctas, int64_t *max_batches_per_cta);
+/* Which way nk_cg runs with the current options on this mesh: 0 = its kernels enqueued one by one
+ * (programmatic dependent launches unless "pdl" = 0), 1 = the same launches replayed as one CUDA graph. */
+int nk_get_cg_path(nk_ctx *ctx, int *path);
 /* Kernel launches enqueued by this context so far (for bench.py's gpu_launches). */
 int nk_get_launch_count(nk_ctx *ctx, int64_t *count);
 

@@ -349,6 +349,7 @@ int nko_gs(nko_ctx *c, double *v)
 int nko_mask(nko_ctx *c, double *v)
 {
     if (!c || !v) return NKO_ERR_ARG;
+#pragma omp parallel for schedule(static)
     for (int64_t l = 0; l < c->L; ++l) v[l] = c->mask[l] * v[l];
     return NKO_OK;
 }
@@ -397,6 +398,7 @@ int nko_dot(nko_ctx *c, const double *a, const double *b, double *out)
 int nko_cg_init(nko_ctx *c, const double *f, double *x, double *r, double *p, double *rho)
 {
     if (!c || !f || !x || !r || !p || !rho) return NKO_ERR_ARG;
+#pragma omp parallel for schedule(static)
     for (int64_t l = 0; l < c->L; ++l) {
         r[l] = c->mask[l] * f[l];
         x[l] = 0.0;
@@ -418,12 +420,15 @@ int nko_cg_step(nko_ctx *c, double *x, double *r, double *p, double *w, double *
     rc = nko_dot(c, w, p, &pap);
     if (rc != NKO_OK) return rc;
     const double alpha = (rho == 0.0 || pap == 0.0) ? 0.0 : rho / pap;
+#pragma omp parallel for schedule(static)
     for (int64_t l = 0; l < L; ++l) x[l] = x[l] + alpha * p[l];
+#pragma omp parallel for schedule(static)
     for (int64_t l = 0; l < L; ++l) r[l] = r[l] - alpha * w[l];
     double rho1;
     rc = nko_dot(c, r, r, &rho1);
     if (rc != NKO_OK) return rc;
     const double beta = (rho == 0.0 || pap == 0.0) ? 0.0 : rho1 / rho;
+#pragma omp parallel for schedule(static)
     for (int64_t l = 0; l < L; ++l) p[l] = r[l] + beta * p[l];
     scal[1] = pap;
     scal[2] = alpha;
@@ -501,6 +506,7 @@ int nko_pcg(nko_ctx *c, const double *f, double *x, int niter, double *res_hist)
     int rc = (r && p && w && z && dg) ? nko_diag(c, dg) : NKO_ERR_ALLOC;
     double rho = 0.0, rr = 0.0;
     if (rc == NKO_OK) {
+#pragma omp parallel for schedule(static)
         for (int64_t l = 0; l < L; ++l) {
             r[l] = c->mask[l] * f[l];
             x[l] = 0.0;
@@ -517,13 +523,17 @@ int nko_pcg(nko_ctx *c, const double *f, double *x, int niter, double *res_hist)
         if (rc == NKO_OK) rc = nko_dot(c, w, p, &pap);
         if (rc != NKO_OK) break;
         const double alpha = (rho == 0.0 || pap == 0.0) ? 0.0 : rho / pap;
+#pragma omp parallel for schedule(static)
         for (int64_t l = 0; l < L; ++l) x[l] = x[l] + alpha * p[l];
+#pragma omp parallel for schedule(static)
         for (int64_t l = 0; l < L; ++l) r[l] = r[l] - alpha * w[l];
+#pragma omp parallel for schedule(static)
         for (int64_t l = 0; l < L; ++l) z[l] = (c->mask[l] == 0.0) ? 0.0 : r[l] / dg[l];
         rc = nko_dot(c, r, z, &rho1);
         if (rc == NKO_OK) rc = nko_dot(c, r, r, &rr);
         res_hist[k] = sqrt(rr);
         const double beta = (rho == 0.0 || pap == 0.0) ? 0.0 : rho1 / rho;
+#pragma omp parallel for schedule(static)
         for (int64_t l = 0; l < L; ++l) p[l] = z[l] + beta * p[l];
         rho = rho1;
     }

@@ -57,6 +57,9 @@ SIGNATURES = {
     "nk_dist_iter_b": (_i, [_vp, _vp]),
     "nk_dist_iter_c": (_i, [_vp, _vp, _vp, _vp]),
     "nk_get_launch_count": (_i, [_vp, C.POINTER(_i64)]),
+    "nk_get_cg_path": (_i, [_vp, C.POINTER(_i)]),
+    "nk_ax_batch_elements": (_i, [_i]),
+    "nk_get_ax_launch": (_i, [_vp, C.POINTER(_i), C.POINTER(_i), C.POINTER(_i64)]),
     "nk_strerror": (C.c_char_p, [_i]),
     "nk_last_cuda_error": (_i, []),
     "nk_version": (C.c_char_p, []),
@@ -97,6 +100,14 @@ def workspace_bytes(E: int, N: int) -> int:
     out = _sz()
     _check(load().nk_workspace_bytes(int(E), int(N), C.byref(out)))
     return int(out.value)
+
+
+def ax_batch_elements(N: int) -> int:
+    """Elements per batch of the persistent ax_e kernel of order N (a compile-time constant)."""
+    rc = load().nk_ax_batch_elements(int(N))
+    if rc <= 0:
+        _check(rc if rc < 0 else NK_ERR_ARG)
+    return int(rc)
 
 
 def _np_ptr(a: np.ndarray):
@@ -280,6 +291,20 @@ class Nekbone:
         ms, cnt = np.zeros(6), np.zeros(6, dtype=np.int64)
         _check(self._lib.nk_get_kernel_times(self._ctx, _np_ptr(ms), _np_ptr(cnt), _stream()))
         return {k: (float(ms[i]), int(cnt[i])) for i, k in enumerate(self.KERNEL_CLASSES)}
+
+    def ax_launch(self) -> dict:
+        """How ax_e is scheduled here: elements per batch, persistent CTAs, batches of the busiest CTA."""
+        e, g, b = _i(), _i(), _i64()
+        _check(self._lib.nk_get_ax_launch(self._ctx, C.byref(e), C.byref(g), C.byref(b)))
+        return dict(batch_elements=int(e.value), ctas=int(g.value), max_batches_per_cta=int(b.value))
+
+    CG_PATHS = ("launches", "graph")
+
+    def solve_path(self) -> str:
+        """How nk_cg runs with the current options: "launches" (one by one) or "graph" (CUDA graph replay)."""
+        v = _i()
+        _check(self._lib.nk_get_cg_path(self._ctx, C.byref(v)))
+        return self.CG_PATHS[int(v.value)]
 
     def launch_count(self) -> int:
         v = _i64()

@@ -1,5 +1,5 @@
 // nk_api.cu -- the C-ABI of include/nk.h: argument checks, context, set-up (host side of the
-// gather-scatter plan), the CG driver.  Every numerical step runs in the kernels of nk_ax.cu,
+// gather-scatter plan), the CG driver.  Every numerical step runs in the kernels of nk_ax_tma.cu,
 // nk_gs.cu, nk_vec.cu, nk_geom.cu; nothing here computes on vectors and there is no CPU fallback.
 #include <cmath>
 #include <cstdlib>
@@ -103,10 +103,10 @@ cudaError_t enqueue_iteration(nk_ctx *c, double *x, double *hist_k, cudaStream_t
     cudaError_t e;
     const int fuse_pap = c->opt_fuse_pap;
     if (c->p_pending) {          // p = r + beta p folded into this ax_e's load
-        NK_LAUNCH(NK_K_AX, nk_launch_ax_e(c, c->p, nullptr, c->r, c->w, fuse_pap, c->opt_ax_variant, st));
+        NK_LAUNCH(NK_K_AX, nk_launch_ax_tma(c, c->p, nullptr, c->r, c->w, fuse_pap, st));
         c->p_pending = 0;
     } else {
-        NK_LAUNCH(NK_K_AX, nk_launch_ax_e(c, nullptr, c->p, nullptr, c->w, fuse_pap, c->opt_ax_variant, st));
+        NK_LAUNCH(NK_K_AX, nk_launch_ax_tma(c, nullptr, c->p, nullptr, c->w, fuse_pap, st));
     }
     NK_LAUNCH(NK_K_GS, nk_launch_gs(c, c->w, 1, st));
     if (!fuse_pap) NK_LAUNCH(NK_K_DOT, nk_launch_dot(c, c->w, c->p, nullptr, NK_EPI_PAP, st));
@@ -148,7 +148,7 @@ int nk_ax_e(nk_ctx *c, const double *u, double *w, void *stream)
 {
     if (!c || !u || !w || u == w || !nk_aligned16(u) || !nk_aligned16(w)) return NK_ERR_ARG;
     NK_CUDA(prof_mark(c, -1, S(stream)));
-    NK_CUDA(nk_launch_ax_e(c, nullptr, u, nullptr, w, 0, c->opt_ax_variant, S(stream)));
+    NK_CUDA(nk_launch_ax_tma(c, nullptr, u, nullptr, w, 0, S(stream)));
     NK_CUDA(prof_mark(c, NK_K_AX, S(stream)));
     return NK_OK;
 }
@@ -166,7 +166,7 @@ int nk_ax(nk_ctx *c, const double *u, double *w, void *stream)
 {
     if (!c || !u || !w || u == w || !nk_aligned16(u) || !nk_aligned16(w)) return NK_ERR_ARG;
     NK_CUDA(prof_mark(c, -1, S(stream)));
-    NK_CUDA(nk_launch_ax_e(c, nullptr, u, nullptr, w, 0, c->opt_ax_variant, S(stream)));
+    NK_CUDA(nk_launch_ax_tma(c, nullptr, u, nullptr, w, 0, S(stream)));
     NK_CUDA(prof_mark(c, NK_K_AX, S(stream)));
     NK_CUDA(nk_launch_gs(c, w, 1, S(stream)));
     NK_CUDA(prof_mark(c, NK_K_GS, S(stream)));
@@ -180,22 +180,33 @@ int nk_dot(nk_ctx *c, const double *a, const double *b, double *out, void *strea
     return NK_OK;
 }
 
+// "graph" = 2 (default): replay a CUDA graph where launch gaps matter (measured: config 2 3.8 -> 1.9 ms,
+// config 3 15.0 -> 13.0 ms per 100 iterations), enqueue directly on large meshes
+static bool cg_uses_graph(const nk_ctx *c)
+{
+    return !c->opt_profile && (c->opt_graph == 1 || (c->opt_graph == 2 && c->L <= NK_GRAPH_AUTO_MAX_L));
+}
+
+int nk_get_cg_path(nk_ctx *c, int *path)
+{
+    if (!c || !path) return NK_ERR_ARG;
+    *path = cg_uses_graph(c) ? 1 : 0;
+    return NK_OK;
+}
+
 int nk_cg(nk_ctx *c, const double *f, double *x, int niter, double *res_hist, void *stream)
 {
     if (!c || !f || !x || !res_hist || niter < 0 || f == x || !nk_aligned16(f) || !nk_aligned16(x))
         return NK_ERR_ARG;
     cudaStream_t st = S(stream);
-    // "graph" = 2 (default): replay a CUDA graph where launch gaps matter (measured: config 2 3.8 -> 1.9 ms,
-    // config 3 15.0 -> 13.0 ms per 100 iterations), enqueue directly on large meshes
-    const bool use_graph = !c->opt_profile && niter > 0 &&
-                           (c->opt_graph == 1 || (c->opt_graph == 2 && c->L <= NK_GRAPH_AUTO_MAX_L));
+    const bool use_graph = niter > 0 && cg_uses_graph(c);
     if (!use_graph) {
         NK_CUDA(enqueue_cg(c, f, x, niter, res_hist, st));
         return NK_OK;
     }
     // Record the launch sequence once per (f, x, res_hist, niter, options) and replay it: the CG
     // loop of the small configs is launch-bound (S 7 hard part 4).
-    const int key = c->opt_fuse_pap | (c->opt_fuse_p << 1) | (c->opt_ax_variant << 3) | (c->opt_pdl << 4);
+    const int key = c->opt_fuse_pap | (c->opt_fuse_p << 1) | (c->opt_pdl << 4);
     if (!c->graph_exec || c->graph_f != f || c->graph_x != x || c->graph_hist != res_hist ||
         c->graph_niter != niter || c->graph_key != key) {
         cudaStream_t cap;
@@ -314,7 +325,6 @@ int nk_get_scalars(nk_ctx *c, double *out5_host, void *stream)
 
 static int *option_slot(nk_ctx *c, const char *name, int *lo, int *hi)
 {
-    if (!std::strcmp(name, "ax_variant")) { *lo = 0; *hi = 1; return &c->opt_ax_variant; }
     if (!std::strcmp(name, "fuse_pap")) { *lo = 0; *hi = 1; return &c->opt_fuse_pap; }
     if (!std::strcmp(name, "fuse_p")) { *lo = 0; *hi = 2; return &c->opt_fuse_p; }
     if (!std::strcmp(name, "graph")) { *lo = 0; *hi = 2; return &c->opt_graph; }
@@ -404,6 +414,24 @@ int nk_get_kernel_times(nk_ctx *c, double *ms_host, int64_t *count_host, void *s
     return NK_OK;
 }
 
+int nk_ax_batch_elements(int N)
+{
+    const int epb = nk_ax_tma_epb(N);
+    return epb > 0 ? epb : NK_ERR_ARG;
+}
+
+int nk_get_ax_launch(nk_ctx *c, int *batch_elements, int *ctas, int64_t *max_batches_per_cta)
+{
+    if (!c) return NK_ERR_ARG;
+    const int epb = nk_ax_tma_epb(c->N);
+    const int64_t nb = (c->E + epb - 1) / epb;
+    const int64_t grid = nb < (int64_t)c->sm_count ? nb : (int64_t)c->sm_count;
+    if (batch_elements) *batch_elements = epb;
+    if (ctas) *ctas = (int)grid;
+    if (max_batches_per_cta) *max_batches_per_cta = (nb + grid - 1) / grid;
+    return NK_OK;
+}
+
 int nk_get_launch_count(nk_ctx *c, int64_t *count)
 {
     if (!c || !count) return NK_ERR_ARG;
@@ -451,7 +479,7 @@ int nk_pcg(nk_ctx *c, const double *f, double *x, int niter, double *res_hist, v
     struct pdl_scope { nk_ctx *c; ~pdl_scope() { c->pdl_now = 0; } } scope{c};
     c->pdl_now = c->opt_profile ? 0 : nk_pdl_mode(c);      // as in nk_cg: every kernel of the loop waits before its first dependent read
     for (int k = 1; k <= niter; ++k) {
-        NK_CUDA(nk_launch_ax_e(c, nullptr, c->p, nullptr, c->w, c->opt_fuse_pap, c->opt_ax_variant, st));
+        NK_CUDA(nk_launch_ax_tma(c, nullptr, c->p, nullptr, c->w, c->opt_fuse_pap, st));
         NK_CUDA(prof_mark(c, NK_K_AX, st));
         NK_CUDA(nk_launch_gs(c, c->w, 1, st));
         NK_CUDA(prof_mark(c, NK_K_GS, st));

@@ -545,6 +545,11 @@ cudaError_t nk_upload_D_tables_tma(void)
     return cudaSuccess;
 }
 
+int nk_ax_tma_epb(int N)
+{
+    return (N >= 1 && N <= NK_MAX_ORDER) ? tma_epb(N + 1) : 0;
+}
+
 cudaError_t nk_launch_ax_tma(nk_ctx *c, double *u_rw, const double *u_ro, const double *r_in, double *w, int dot,
                              cudaStream_t st)
 {

@@ -190,7 +190,7 @@ int nk_dist_iter_a(nk_ctx *c, void *stream)
     cudaStream_t st = S(stream);
     // pap = sum over ALL ranks' elements of grad(p)^T G grad(p): element-local, so the rank totals just add
     NK_CUDA(with_raw(c, c->dist_send + c->dist_slots,
-                     [&] { return nk_launch_ax_e(c, nullptr, c->p, nullptr, c->w, 1, c->opt_ax_variant, st); }));
+                     [&] { return nk_launch_ax_tma(c, nullptr, c->p, nullptr, c->w, 1, st); }));
     NK_CUDA(nk_launch_gs(c, c->w, 1, st));
     NK_CUDA(launch_pack(c, c->w, st));
     return NK_OK;

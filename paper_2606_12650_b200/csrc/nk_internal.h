@@ -79,7 +79,7 @@ struct nk_ctx {
     int64_t n_unique, n_shared_unique, n_masked_unique;
     int64_t n_rows, n_listed, n_sum_rows, n_sum_listed;
     // options / state
-    int opt_ax_variant, opt_fuse_pap, opt_fuse_p, opt_graph, opt_profile, opt_pdl;
+    int opt_fuse_pap, opt_fuse_p, opt_graph, opt_profile, opt_pdl;
     int pdl_now;                 // nk_pdl_mode while nk_cg enqueues its loop (every kernel there waits), else 0
     int p_pending;               // 1: p = r + beta p has not been applied yet (fuse_p)
     int64_t launches;
@@ -125,15 +125,12 @@ inline cudaError_t nk_launch(void (*kernel)(KArgs...), dim3 grid, dim3 block, si
 // nk_basis.cpp
 void nk_host_basis(int N, double *xi, double *w, double *D);
 void nk_host_basis_dd(int N, double *xi, double *w, double *D, double *Dlo);   // D = D + Dlo (long double split)
-// nk_ax.cu : w = A_L u.  If r_in != NULL: u := r_in + beta*u is applied first and written back to u.
-// If dot: sum_l u_l w_l is reduced with epilogue NK_EPI_PAP.
-cudaError_t nk_launch_ax_e(nk_ctx *c, double *u_rw, const double *u_ro, const double *r_in, double *w,
-                           int dot, int variant, cudaStream_t st);
-cudaError_t nk_upload_D_tables(void);
-// nk_ax_tma.cu : same contract, TMA-pipelined persistent kernel (the default variant)
+// nk_ax_tma.cu : w = A_L u (TMA-pipelined persistent kernel).  If r_in != NULL: u := r_in + beta*u is applied
+// first and written back to u.  If dot: sum_l u_l w_l is reduced with epilogue NK_EPI_PAP.
 cudaError_t nk_launch_ax_tma(nk_ctx *c, double *u_rw, const double *u_ro, const double *r_in, double *w,
                              int dot, cudaStream_t st);
 cudaError_t nk_upload_D_tables_tma(void);
+int nk_ax_tma_epb(int N);                       // elements per batch of order N, 0 if N is out of range
 // nk_geom.cu
 cudaError_t nk_launch_geom(nk_ctx *c, const double *coords_dev, const double *D_dev, const double *Dlo_dev,
                            const double *wq_dev, cudaStream_t st);

@@ -173,7 +173,6 @@ int setup_impl(nk_ctx *c, const double *coords, const int64_t *glo_num, const do
     // coordinates (x|y|z planes at stride L) are staged in the r|p|w block, which is >= 3L doubles
     double *coords_dev = c->r;
     NK_CUDA(cudaMemcpyAsync(coords_dev, coords, 3 * (size_t)L * sizeof(double), cudaMemcpyHostToDevice, st));
-    NK_CUDA(nk_upload_D_tables());
     NK_CUDA(nk_upload_D_tables_tma());
     NK_CUDA(nk_launch_geom(c, coords_dev, D_dev, Dlo_dev, wq_dev, st));
     int err = 0;

@@ -1,15 +1,21 @@
-"""Roofline sweep of ax_e, gs and ax (BASELINE.json configs[3]).
+"""Roofline sweeps of ax_e, gs, ax and the CG iteration (BASELINE.json configs[3]).
 
-    python -m paper_2606_12650_b200.sweep [--which e|n|both|paper] [--reps 50] [--out sweep.csv]
+    python -m paper_2606_12650_b200.sweep [--which e|n|both|big|paper] [--reps 50] [--out sweep.csv]
 
-4a: brick meshes with E = 2^10 .. 2^17 at N = 7;  4b: N = 3 .. 15 at E = 4096 (16^3); perturbed
+4a (e): brick meshes with E = 2^10 .. 2^17 at N = 7;  4b (n): N = 3 .. 15 at E = 4096 (16^3); perturbed
 geometry (amplitude 0.05), u uniform[-1,1) per LOCAL point (seed 1004), `reps` back-to-back
 applications timed with CUDA events after 3 untimed ones, best and median of 5 repeats.
+big: N = 7 .. 11 at E = 2^15 (32^3, working sets 1.2 - 4.1 GB, far beyond L2): the three operators plus
+the CG iteration (20 iterations per call), for the ">= 70 % at N = 7-11" target of BASELINE.json.
 Reported per point: us per application, model GB/s (ax_e 64 B/pt; gs 20 B per listed copy + 4 B per
-row; ax = both), model GFLOP/s (12(N+1)+15 per point), fraction of the measured copy peak
-(MEASURED_PEAKS.json, else the guide's fallback) and of the nominal 8 TB/s, and whether the working
+row; ax = both; CG iteration: the canonical unfused 168 B/pt + gs), model GFLOP/s, fraction of the measured
+copy peak (MEASURED_PEAKS.json, else the guide's fallback) and of the nominal 8 TB/s, and whether the working
 set fits in L2 ("L2-resident": effective GB/s can then exceed the HBM peak; the >= 70 % claim is made
-on the other points only).  No oracle here: parity is the tests' job.
+on the other points only).
+paper: the paper's own sweep: N in {4, 6, 8}, E = 2^1 .. 2^14, CG 100 iterations, GDOFS.
+
+This tool only times.  Parity of every point against the oracle is `python tests/sweep_parity.py`, which
+calls the generators below and appends its columns (the product never imports the oracle).
 """
 from __future__ import annotations
 
@@ -25,6 +31,7 @@ if ROOT not in sys.path:
     sys.path.insert(0, ROOT)
 
 L2_BYTES = 126e6
+BIG_SWEEP = [dict(brick=(32, 32, 32), N=N) for N in range(7, 12)]
 
 
 def _peak():
@@ -52,11 +59,11 @@ def _time(fn, reps, repeats=5):
     return min(out), float(np.median(out))
 
 
-def run_point(point, reps):
+def run_point(mesh, reps, with_cg=False):
     import torch
     from paper_2606_12650_b200 import Nekbone
-    from workloads import sweep_mesh, sweep_field
-    mesh = sweep_mesh(point)
+    from workloads import sweep_field, rhs_unique
+    from workloads.configs import SWEEP_SEED
     nk = Nekbone.from_mesh(mesh)
     u = torch.from_numpy(sweep_field(mesh)).cuda()
     w = nk.empty()
@@ -67,13 +74,23 @@ def run_point(point, reps):
     b_gs = 20.0 * s["n_listed"] + 4.0 * s["n_rows"]
     fl = (12.0 * (N + 1) + 15.0) * L
     rows = []
-    for name, fn, nbytes, flops in (("ax_e", lambda: nk.ax_e(u, w), b_ax_e, fl),
-                                    ("gs", lambda: nk.gs(v), b_gs, 0.0),
-                                    ("ax", lambda: nk.ax(u, w), b_ax_e + b_gs, fl)):
+    jobs = [("ax_e", lambda: nk.ax_e(u, w), b_ax_e, fl, reps),
+            ("gs", lambda: nk.gs(v), b_gs, 0.0, reps),
+            ("ax", lambda: nk.ax(u, w), b_ax_e + b_gs, fl, reps)]
+    if with_cg:
+        f = torch.from_numpy(rhs_unique(mesh, SWEEP_SEED)).cuda()
+        x = nk.empty()
+        hist = torch.empty(21, dtype=torch.float64, device="cuda")
+        gs_adds = float(L - nk.sizes()["n_unique"])
+        # one call = cg_init + 20 iterations; per iteration: the canonical unfused model
+        jobs.append(("cg_iteration", lambda: nk.cg(f, 20, x=x, res_hist=hist), 20 * (168.0 * L + b_gs),
+                     20 * ((12.0 * (N + 1) + 27.0) * L + gs_adds), max(1, reps // 10)))
+    for name, fn, nbytes, flops, r in jobs:
         if name == "gs":
             v.copy_(u)                                         # 50 in-place gs scale shared entries by <= 8^50: finite
-        best, med = _time(fn, reps)
-        rows.append(dict(kernel=name, E=mesh.E, N=N, L=L, us_best=best, us_median=med,
+        best, med = _time(fn, r)
+        per = 20.0 if name == "cg_iteration" else 1.0
+        rows.append(dict(kernel=name, E=mesh.E, N=N, L=L, us_best=best / per, us_median=med / per,
                          gbs=nbytes / best / 1e3, gflops=flops / best / 1e3,
                          working_set_mb=(72.0 * L) / 1e6, l2_resident=bool(72.0 * L <= L2_BYTES)))
     nk.close()
@@ -82,21 +99,50 @@ def run_point(point, reps):
     return rows
 
 
-def run_paper_sweep(out):
+def config4_points(which, reps=None):
+    """(csv header, generator of (csv rows of one point, its mesh))."""
+    from workloads import E_SWEEP, N_SWEEP, SWEEP_REPEATS, sweep_mesh
+    reps = reps or SWEEP_REPEATS
+    peak, kind = _peak()
+    points = []
+    if which in ("e", "both"):
+        points += [("4a", p) for p in E_SWEEP]
+    if which in ("n", "both"):
+        points += [("4b", p) for p in N_SWEEP]
+    if which == "big":
+        points += [("big", p) for p in BIG_SWEEP]
+    header = ("sweep,kernel,E,N,L,us_best,us_median,model_GBs,frac_of_%s_copy_peak,frac_of_8TBs,model_GFLOPs,"
+              "working_set_MB,l2_resident" % kind)
+
+    def gen():
+        for tag, p in points:
+            mesh = sweep_mesh(p)
+            rows = [f"{tag},{r['kernel']},{r['E']},{r['N']},{r['L']},{r['us_best']:.2f},{r['us_median']:.2f},"
+                    f"{r['gbs']:.1f},{r['gbs'] / peak:.4f},{r['gbs'] / 8000.0:.4f},{r['gflops']:.1f},"
+                    f"{r['working_set_mb']:.1f},{int(r['l2_resident'])}" for r in run_point(mesh, reps, tag == "big")]
+            yield rows, mesh
+    return header, gen()
+
+
+PAPER_HEADER = "N,E,n_local,dofs_E_N3,ms_per_100_iterations_mean_of_5,GDOFS,final_residual,solve_path"
+
+
+def paper_points():
     """The paper's own sweep (S 8(f) f-2, Figs 7-12): N in {4, 6, 8}, E = 2^1 .. 2^14,
     100 warm-up + 100 timed CG iterations, mean of 5 runs, GDOFS = E N^3 100 / (t 1e9) (Eq. 1) and the
     final residual.  Meshes and RHS are this repo's seeded bricks (amplitude 0.05, seed 1004): the
-    paper's own generator is not available, so only the SHAPE of its curves is comparable."""
+    paper's own generator is not available, so only the SHAPE of its curves is comparable.
+    Yields (csv row, mesh, f, residual history as numpy)."""
     import torch
     from paper_2606_12650_b200 import Nekbone
     from workloads import brick_mesh, rhs_unique, sweep_brick
     from workloads.configs import SWEEP_AMPLITUDE, SWEEP_SEED
-    lines = ["N,E,n_local,dofs_E_N3,ms_per_100_iterations_mean_of_5,GDOFS,final_residual,graph"]
     for N in (4, 6, 8):
         for k in range(1, 15):
             mesh = brick_mesh(*sweep_brick(k), N, SWEEP_AMPLITUDE)
             nk = Nekbone.from_mesh(mesh)
-            f = torch.from_numpy(rhs_unique(mesh, SWEEP_SEED)).cuda()
+            f_np = rhs_unique(mesh, SWEEP_SEED)
+            f = torch.from_numpy(f_np).cuda()
             x = nk.empty()
             hist = torch.empty(101, dtype=torch.float64, device="cuda")
             nk.cg(f, 100, x=x, res_hist=hist)                       # 100 warm-up iterations
@@ -111,36 +157,32 @@ def run_paper_sweep(out):
                 ts.append(e0.elapsed_time(e1))
             t = float(np.mean(ts))
             dofs = mesh.E * N ** 3
-            lines.append(f"{N},{mesh.E},{mesh.L},{dofs},{t:.4f},{dofs * 100 / (t * 1e-3) / 1e9:.4f},"
-                         f"{float(hist[-1]):.6e},{int(mesh.L <= (1 << 24))}")
-            print(lines[-1], flush=True)
+            h = hist.cpu().numpy()
+            row = (f"{N},{mesh.E},{mesh.L},{dofs},{t:.4f},{dofs * 100 / (t * 1e-3) / 1e9:.4f},"
+                   f"{float(h[-1]):.6e},{nk.solve_path()}")
             nk.close()
-    if out:
-        with open(out, "w") as fh:
-            fh.write("\n".join(lines) + "\n")
+            yield row, mesh, f_np, h
 
 
 def main():
     ap = argparse.ArgumentParser()
-    ap.add_argument("--which", default="both", choices=["e", "n", "both", "paper"])
+    ap.add_argument("--which", default="both", choices=["e", "n", "both", "big", "paper"])
     ap.add_argument("--reps", type=int, default=None)
     ap.add_argument("--out", default=None)
     args = ap.parse_args()
+    lines = []
     if args.which == "paper":
-        return run_paper_sweep(args.out)
-    from workloads import E_SWEEP, N_SWEEP, SWEEP_REPEATS
-    reps = args.reps or SWEEP_REPEATS
-    peak, kind = _peak()
-    points = (E_SWEEP if args.which in ("e", "both") else []) + (N_SWEEP if args.which in ("n", "both") else [])
-    lines = ["sweep,kernel,E,N,L,us_best,us_median,model_GBs,frac_of_%s_copy_peak,frac_of_8TBs,model_GFLOPs,"
-             "working_set_MB,l2_resident" % kind]
-    for p in points:
-        tag = "4a" if p in E_SWEEP else "4b"
-        for r in run_point(p, reps):
-            lines.append(f"{tag},{r['kernel']},{r['E']},{r['N']},{r['L']},{r['us_best']:.2f},{r['us_median']:.2f},"
-                         f"{r['gbs']:.1f},{r['gbs'] / peak:.4f},{r['gbs'] / 8000.0:.4f},{r['gflops']:.1f},"
-                         f"{r['working_set_mb']:.1f},{int(r['l2_resident'])}")
-            print(lines[-1], flush=True)
+        lines.append(PAPER_HEADER)
+        for row, _, _, _ in paper_points():
+            lines.append(row)
+            print(row, flush=True)
+    else:
+        header, points = config4_points(args.which, args.reps)
+        lines.append(header)
+        for rows, _ in points:
+            for row in rows:
+                lines.append(row)
+                print(row, flush=True)
     if args.out:
         with open(args.out, "w") as fh:
             fh.write("\n".join(lines) + "\n")

@@ -37,3 +37,24 @@ def maxnorm_rel(got, ref) -> float:
     d = np.abs(np.asarray(got) - np.asarray(ref)).max()
     s = np.abs(np.asarray(ref)).max()
     return float(d / s) if s > 0 else float(d)
+
+
+def history_parity(h_gpu, h_or, h_or_band, tol=1e-10, band_ok=1e-11, converged=1e-9):
+    """R15 protocol for a residual history (SURVEY.md 8(c) "CG sensitivity", parts 3-4).
+
+    h_or / h_or_band are the oracle's histories from its two builds (contraction off / on); their running
+    maximum relative difference is the oracle's own rounding band.  Returns (passed, worst, kstar):
+      * k with band <= band_ok:   |gpu - or| <= tol * or                      (the flat 1e-10)
+      * beyond:                   |gpu - or| <= max(tol, 10 band) * or, or both sides have converged
+                                  (<= converged * h[0]: the recursive residual is rounding noise there)
+    worst = max relative difference over the flat part, kstar = last index of the flat part."""
+    h_gpu, h_or, h_or_band = (np.asarray(a, dtype=np.float64) for a in (h_gpu, h_or, h_or_band))
+    den = np.where(h_or > 0, h_or, 1.0)
+    band = np.maximum.accumulate(np.abs(h_or_band - h_or) / den)
+    diff = np.abs(h_gpu - h_or) / den
+    flat = band <= band_ok
+    done = (h_gpu <= converged * h_or[0]) & (h_or <= converged * h_or[0])
+    ok = np.where(flat, diff <= tol, (diff <= np.maximum(tol, 10.0 * band)) | done)
+    kstar = int(np.nonzero(flat)[0].max()) if flat.any() else -1
+    worst = float(diff[flat].max()) if flat.any() else float("nan")
+    return bool(ok.all()), worst, kstar

@@ -50,11 +50,6 @@ def test_ax_e_every_order(nx, ny, nz, N):
     wo = pr.orc.ax_e(u)
     wg = to_np(pr.gpu.ax_e(to_dev(u)))
     assert elem_err(wg, wo, pr.P) <= TOL_OP, (N, elem_err(wg, wo, pr.P), maxnorm_rel(wg, wo))
-    # the round's first kernel stays selectable ("ax_variant" = 1) and must keep parity too
-    pr.gpu.set_option("ax_variant", 1)
-    w1 = to_np(pr.gpu.ax_e(to_dev(u)))
-    pr.gpu.set_option("ax_variant", 0)
-    assert elem_err(w1, wo, pr.P) <= TOL_OP, N
 
 
 @pytest.mark.parametrize("nx,ny,nz,N", ALL_N)

@@ -61,3 +61,21 @@ def test_field_local_differs_across_copies():
 def test_config_table():
     assert CONFIGS["config5"]["brick"] == (32, 32, 32) and CONFIGS["config5"]["N"] == 11
     assert CONFIGS["config3"]["amplitude"] == 0.1 and CONFIGS["config2"]["niter"] == 100
+
+
+def test_history_parity_protocol():
+    """The R15 protocol helper the GPU tests rely on: flat 1e-10 while the oracle's own band is small,
+    band-scaled or 'both converged' beyond."""
+    import sys, os
+    sys.path.insert(0, os.path.dirname(os.path.abspath(__file__)))
+    from parity import history_parity
+    k = np.arange(40)
+    ho = 10.0 ** (-0.5 * k)                                  # converges 20 decades in 40 iterations
+    hb = ho * (1 + np.where(k < 25, 1e-15, 1e-3))            # the oracle's two builds part ways at k = 25
+    good = ho * (1 + np.where(k < 25, 5e-12, 0.5))           # ... where everything is below 1e-9 h0
+    ok, worst, kstar = history_parity(good, ho, hb)
+    assert ok and kstar == 24 and 4e-12 < worst < 6e-12
+    bad = good.copy(); bad[10] *= 1 + 1e-9                   # a real disagreement inside the flat part
+    assert not history_parity(bad, ho, hb)[0]
+    notconv = ho.copy(); notconv[30] = 1e-3                  # beyond the band, but one side did not converge
+    assert not history_parity(notconv, ho, hb)[0]
