@@ -52,6 +52,12 @@ def gs_bytes(sizes: dict) -> float:
     return 20.0 * sizes["n_listed"] + 4.0 * sizes["n_rows"]
 
 
+def gs_gather_bytes(sizes: dict) -> float:
+    """gs folded into the residual update: per listed local copy its row's other copies are gathered (8 B each,
+    counted once per copy as in the gs model's read half) through 4 B of index; nothing is written back."""
+    return 12.0 * sizes["n_listed"] + 4.0 * sizes["n_rows"]
+
+
 def iter_model_bytes(L: int, sizes: dict) -> float:
     """Canonical unfused per-iteration model: 168 B/pt + gs."""
     return 168.0 * L + gs_bytes(sizes)
@@ -126,25 +132,33 @@ class ClockSampler:
 
 
 # ---- the oracle, timed (cpu_baseline and --impl reference) ------------------------------------------
-def sample_brick(cfg: dict):
-    """Bounded sample of a workload: same N and amplitude, a brick of at most 8x8x8 elements."""
-    return tuple(min(8, b) for b in cfg["brick"])
+def cpu_model_name() -> str:
+    try:
+        with open("/proc/cpuinfo") as fh:
+            for line in fh:
+                if line.startswith("model name"):
+                    return line.split(":", 1)[1].strip()
+    except OSError:
+        pass
+    return "unknown"
 
 
-class OracleSample:
-    """The oracle (test infrastructure, timed as it stands) set up on a bounded sample."""
+class OracleRun:
+    """The oracle (test infrastructure, timed as it stands) set up on the WORKLOAD'S OWN mesh: a step of the
+    CPU arm is k CG iterations of the real problem (cg_init + k iterations), not a smaller stand-in."""
 
-    def __init__(self, workload: str):
+    def __init__(self, workload: str, mesh=None, f=None):
         from oracle.nko import Oracle, num_threads
-        from workloads import CONFIGS, brick_mesh, rhs_unique
+        from workloads import CONFIGS, config_mesh, rhs_unique
         cfg = CONFIGS[workload]
-        self.cfg, self.brick = cfg, sample_brick(cfg)
-        self.mesh = brick_mesh(*self.brick, cfg["N"], cfg["amplitude"])
-        self.f = rhs_unique(self.mesh, cfg["seed"])
+        self.workload, self.cfg = workload, cfg
+        self.mesh = config_mesh(workload) if mesh is None else mesh
+        self.f = rhs_unique(self.mesh, cfg["seed"]) if f is None else f
+        t = time.perf_counter()
         self.orc = Oracle.from_mesh(self.mesh)
+        self.setup_s = time.perf_counter() - t
         self.cores = int(num_threads())
         s = self.orc.sizes()
-        # gs adds per point, from the mesh alone: (copies - 1) per shared unique node
         self.gs_adds = float(self.mesh.L - s["n_unique"]) / self.mesh.L
         self.fpp = flops_per_point_iter(cfg["N"], self.gs_adds)
 
@@ -153,35 +167,71 @@ class OracleSample:
         self.orc.cg(self.f, k)
         return time.perf_counter() - t
 
-    def calibrate(self, budget_s: float) -> int:
+    def iters_for(self, budget_s: float) -> int:
+        """k >= 3 iterations per step (never more than the workload's own count) that fit the budget."""
         self.time_iters(1)                                # first call: thread pool, page faults
-        t3, t23 = self.time_iters(3), self.time_iters(23)  # a call has a fixed part (set-up, first residual)
-        per = max((t23 - t3) / 20.0, 1e-6)
-        return int(max(3, min(4000, round((budget_s - max(t3 - 3 * per, 0.0)) / per))))
+        t1, t4 = self.time_iters(1), self.time_iters(4)   # a call has a fixed part (cg_init, allocations)
+        per = max((t4 - t1) / 3.0, 1e-7)
+        return int(max(3, min(self.cfg["niter"], (budget_s - max(t1 - per, 0.0)) / per)))
 
     def gflops(self, k: int, seconds: float) -> float:
         return self.fpp * self.mesh.L * k / seconds / 1e9
 
     def describe(self, k: int) -> str:
         m = self.mesh
-        return (f"oracle nko_cg, {k} CG iterations on E={m.E} ({'x'.join(map(str, self.brick))} brick), "
-                f"N={m.N}, amplitude {self.cfg['amplitude']}, L={m.L} (sample of the same workload)")
+        full = " (the whole solve)" if k == self.cfg["niter"] else f" of the solve's {self.cfg['niter']}"
+        return (f"oracle nko_cg on the workload's own mesh (E={m.E}, N={m.N}, L={m.L}): cg_init + {k} CG iterations"
+                f"{full}")
+
+    def best_of(self, fn, reps=5, warm=1):
+        for _ in range(warm):
+            fn()
+        ts = []
+        for _ in range(reps):
+            t = time.perf_counter()
+            fn()
+            ts.append(time.perf_counter() - t)
+        return min(ts)
+
+    def kernels(self) -> dict:
+        """ax_e and gs(+mask), best of 5 wall-clock applications."""
+        from workloads import field_local
+        m = self.mesh
+        u = field_local(m, 1004)
+        t_ax = self.best_of(lambda: self.orc.ax_e(u))
+        t_gs = self.best_of(lambda: self.orc.mask(self.orc.gs(u)))
+        fl = (12.0 * (m.N + 1) + 15.0) * m.L
+        return {"ax_e": {"ms": 1e3 * t_ax, "gflops": fl / t_ax / 1e9, "gbs_model": 64.0 * m.L / t_ax / 1e9},
+                "gs_mask": {"ms": 1e3 * t_gs}}
 
 
-def cpu_baseline(workload: str, budget_s: float = 12.0) -> dict:
-    s = OracleSample(workload)
-    k = s.calibrate(budget_s)
+def cpu_baseline(workload: str, mesh=None, f=None, budget_s: float = 12.0) -> dict:
+    from oracle import nko
+    s = OracleRun(workload, mesh, f)
+    k = s.iters_for(budget_s)
     sec = s.time_iters(k)
-    return {"value": s.gflops(k, sec), "unit": UNIT, "cores": s.cores, "kind": "oracle",
-            "sample": s.describe(k), "seconds": sec}
+    out = {"value": s.gflops(k, sec), "unit": UNIT, "cores": s.cores, "kind": "oracle",
+           "sample": s.describe(k), "seconds": sec, "cpu": cpu_model_name(), "oracle_setup_s": s.setup_s,
+           "note": "plain C99 loops + OpenMP parallel for (oracle/nko.c as it stands, untuned)"}
+    out["kernels"] = s.kernels()
+    # one-thread figure (BASELINE.md section 3), on the same mesh, at most ~10 s
+    nko.set_num_threads(1)
+    try:
+        k1 = max(1, min(k, int(10.0 / max(sec / k * s.cores, 1e-9))))     # assumes perfect scaling: an upper bound on its time
+        t1 = s.time_iters(k1)
+        out["one_thread"] = {"value": s.gflops(k1, t1), "unit": UNIT, "iterations": k1, "seconds": t1}
+    finally:
+        nko.set_num_threads(s.cores)
+    return out
 
 
 def run_reference(args) -> dict:
-    """This tier's reference arm: the oracle on the host cores, each step a bounded sample."""
+    """This tier's reference arm: the oracle on the host cores, on the workload's own mesh; a step is cg_init +
+    k CG iterations, k sized so that the whole --steps/--warmup run ends within a few minutes."""
     from workloads import CONFIGS
-    s = OracleSample(args.workload)
+    s = OracleRun(args.workload)
     total_budget = 150.0                                  # whole run within a few minutes
-    k = s.calibrate(total_budget / max(1, args.steps + args.warmup))
+    k = s.iters_for(total_budget / max(1, args.steps + args.warmup))
     for _ in range(args.warmup):
         s.time_iters(k)
     t = 0.0
@@ -189,13 +239,16 @@ def run_reference(args) -> dict:
         t += s.time_iters(k)
     val = s.gflops(k * args.steps, t)
     cfg = CONFIGS[args.workload]
+    conf = workload_config(args.workload, cfg, args.gpus)
+    conf["step"] = f"cg_init + {k} CG iterations of the workload's mesh (of its {cfg['niter']}; GFLOP/s is per iteration work)"
+    conf["iterations_per_step"] = k
     return {"impl": "reference", "metric": METRIC, "value": val, "unit": UNIT, "n_gpus": args.gpus,
             "steps": args.steps, "warmup": args.warmup, "ms_per_step": 1e3 * t / args.steps,
             "higher_is_better": True, "scaling": "weak", "vs_baseline": None, "dtype": "f64",
-            "data": "synthetic", "gpu_launches": 0,
-            "config": workload_config(args.workload, cfg, args.gpus),
+            "data": "synthetic", "gpu_launches": 0, "config": conf,
             "cpu_baseline": {"value": val, "unit": UNIT, "cores": s.cores, "kind": "oracle",
-                             "sample": s.describe(k) + " per step"},
+                             "sample": s.describe(k) + " per step", "cpu": cpu_model_name(),
+                             "oracle_setup_s": s.setup_s},
             "e2e": {"value": val, "unit": UNIT, "h2d_bytes_per_step": 0, "d2h_bytes_per_step": 0}}
 
 
@@ -256,8 +309,10 @@ def run_ours(args) -> dict | None:
     t0 = time.perf_counter()
     nk = Nekbone.from_mesh(mesh)
     setup_s = time.perf_counter() - t0
-    for k, v in (("fuse_pap", args.fuse_pap), ("fuse_p", args.fuse_p), ("graph", args.graph), ("pdl", args.pdl)):
-        nk.set_option(k, v)
+    for k, v in (("fuse_pap", args.fuse_pap), ("fuse_p", args.fuse_p), ("fuse_gs", args.fuse_gs), ("graph", args.graph),
+                 ("pdl", args.pdl)):
+        if v is not None:                                  # None: the library's default
+            nk.set_option(k, v)
     sizes = {**nk.sizes(), **nk.gs_sizes()}
     L = mesh.L
     gs_adds = float(L - sizes["n_unique"]) / L
@@ -280,13 +335,13 @@ def run_ours(args) -> dict | None:
             flush.fill_(1)
         nk.cg(f, niter, x=x, res_hist=hist)
 
-    # ---- device-resident timed region, per-kernel events inside it ---------------------------------
+    # ---- device-resident timed region: the DEFAULT path (no per-launch events: programmatic dependent
+    # launches / graph replay exactly as a caller of nk_cg gets them) ---------------------------------------
     for _ in range(args.warmup):
         step()
     barrier()
-    graphed = args.graph == 1 or (args.graph == 2 and L <= (1 << 24))      # the library's rule for "graph" = 2
-    nk.set_option("profile", 0 if graphed else 1)
-    nk.kernel_times()
+    nk.set_option("profile", 0)
+    solve_path = nk.solve_path()
     launches0 = nk.launch_count()
     clocks = ClockSampler(local)
     clocks.start()
@@ -302,20 +357,23 @@ def run_ours(args) -> dict | None:
         ev[2 * s + 1].record(stream)
     barrier()
     w1 = time.time()
-    clk = clocks.stop(w0, w1)
     ms = sum(ev[2 * s].elapsed_time(ev[2 * s + 1]) for s in range(args.steps))
     launches = nk.launch_count() - launches0
-    ktimes = nk.kernel_times()
-    ktimes_from = "CUDA events between launches inside the timed region"
-    if graphed:     # a replayed graph has no events inside: one extra untimed, un-graphed step for the breakdown
-        nk.set_option("profile", 1)
-        nk.kernel_times()
-        step()
-        ktimes = nk.kernel_times()
-        ktimes_from = "one extra un-graphed step after the timed region (the timed steps replay a CUDA graph)"
-    nk.set_option("profile", 0)
-    ms_for_share = ms if not graphed else args.steps * sum(t for t, n in ktimes.values())
     res_final = float(hist[-1])
+    # ---- per-kernel breakdown: extra steps with a CUDA event between consecutive launches ("profile": plain
+    # launches, no overlap between a kernel's tail and its successor's prologue), clocks still being sampled
+    nk.set_option("profile", 1)
+    nk.kernel_times()
+    prof_steps = max(1, min(3, args.steps))
+    for _ in range(prof_steps):
+        step()
+    ktimes = nk.kernel_times()
+    nk.set_option("profile", 0)
+    barrier()
+    clk = clocks.stop(w0, time.time())
+    ktimes_from = (f"{prof_steps} extra step(s) right after the timed region with a CUDA event between consecutive "
+                   "launches (option profile=1: plain launches); the timed steps themselves run the default path")
+    ms_prof_step = sum(t for t, n in ktimes.values()) / prof_steps
 
     # ---- end to end through nk_cg_host: pinned host buffers, copies inside the timer ---------------
     f_pin = torch.from_numpy(f_np).pin_memory()
@@ -343,6 +401,8 @@ def run_ours(args) -> dict | None:
     peak, peak_kind = measured_peaks()
     value = whole_job_value(flops_step, args.steps, world, ms)
     e2e = whole_job_value(flops_step, args.steps, world, ms_e2e)
+    opts = {k: nk.get_option(k) for k in ("fuse_pap", "fuse_p", "fuse_gs", "graph", "pdl")}
+    fused_p = opts["fuse_p"] == 1 or (opts["fuse_p"] == 2 and L <= (1 << 24))
     out = {"metric": METRIC, "value": value, "unit": UNIT, "n_gpus": world, "steps": args.steps,
            "warmup": args.warmup, "ms_per_step": ms / args.steps, "higher_is_better": True,
            "scaling": "weak", "vs_baseline": None, "dtype": "f64", "data": "synthetic",
@@ -350,50 +410,78 @@ def run_ours(args) -> dict | None:
            "e2e": {"value": e2e, "unit": UNIT, "h2d_bytes_per_step": 8 * L,
                    "d2h_bytes_per_step": 8 * (L + niter + 1), "ms_per_step": ms_e2e / args.steps},
            "gpu_launches": int(launches), "clocks": clk,
-           "options": {"fuse_pap": args.fuse_pap, "fuse_p": args.fuse_p, "graph": args.graph, "graph_used": graphed, "pdl": args.pdl},
+           "options": {**opts, "solve_path": solve_path, "pdl_effective": nk.pdl_effective(),
+                       "fuse_p_effective": int(fused_p), "profile_in_timed_region": False},
            "setup_s": setup_s, "final_residual": res_final}
 
     # ---- iteration-level and kernel-level bandwidth ---------------------------------------------------
+    # real bytes per point of each kernel class as launched: ax_e u 8 + G 48 + w 8 (+ r 8 read and
+    # p 8 written when the direction update is folded in); gs by its plan; the vector kernels by what they touch
+    gsb = gs_bytes(sizes) / L
+    fused_gs = bool(opts["fuse_gs"])
+    kb = {"ax_e": 64.0 + (16.0 if fused_p else 0.0), "gs": gsb, "dot": 17.0,
+          "update_xr": ((49.0 if fused_p else 25.0) + (gs_gather_bytes(sizes) / L if fused_gs else 0.0)),
+          "update_p": 24.0 if fused_p else 40.0, "cg_init": 33.0}
     it_bytes = iter_model_bytes(L, sizes)
     it_gbs = it_bytes * niter * args.steps / (ms * 1e-3) / 1e9
-    out["iteration"] = {"model_bytes_per_point": it_bytes / L, "ms_per_iteration": ms / args.steps / niter,
-                        "gbs_model": it_gbs, "frac_of_measured_copy": it_gbs / peak,
-                        "frac_of_nominal_8TBs": it_gbs / HBM_NOMINAL_GBS,
+    real_bpp = sum(kb[k] * n for k, (t, n) in ktimes.items() if k != "cg_init") / (prof_steps * niter)
+    real_gbs = real_bpp * L * niter * args.steps / (ms * 1e-3) / 1e9
+    out["iteration"] = {"ms_per_iteration": ms / args.steps / niter,
+                        "model_bytes_per_point": it_bytes / L, "gbs_model": it_gbs,
+                        "frac_model_bytes_of_copy_peak": it_gbs / peak,
+                        "frac_model_bytes_of_nominal_8TBs": it_gbs / HBM_NOMINAL_GBS,
+                        "model": "canonical UNFUSED iteration of SURVEY 8(d): 168 B/pt + gs; fusion removes real traffic, "
+                                 "so this rate can exceed the copy peak -- the real-bytes figures are the physical ones",
+                        "real_bytes_per_point": real_bpp, "gbs_real": real_gbs,
+                        "frac_real_of_measured_copy": real_gbs / peak,
+                        "frac_real_of_nominal_8TBs": real_gbs / HBM_NOMINAL_GBS,
                         "gdofs_paper_eq1": mesh.E * N ** 3 * niter * args.steps / (ms * 1e-3) / 1e9}
     ax_ms, ax_n = ktimes["ax_e"]
     if ax_n > 0:
-        # bytes the ax_e launch moves by the S 8(d) model: u 8 + G 48 + w 8 = 64 B/pt, plus, when the
-        # direction update is folded in, r 8 read + p 8 written (the update's own 24 B/pt kernel is gone)
-        fused_p = args.fuse_p == 1 or (args.fuse_p == 2 and L <= (1 << 24))
-        bpp = 64.0 + (16.0 if fused_p else 0.0)
+        bpp = kb["ax_e"]
         avg = ax_ms / ax_n
         ach = bpp * L / (avg * 1e-3) / 1e9
-        traffic = args.traffic
+        traffic, traffic_source = args.traffic, "--traffic argument"
         if traffic is None:
             try:
                 with open(os.path.join(ROOT, "profiles", "traffic.json.txt")) as fh:
-                    traffic = float(json.load(fh)[args.workload]["dram_bytes_per_launch"])
+                    rec = json.load(fh)[args.workload]
+                traffic = float(rec["dram_bytes_per_launch"])
+                traffic_source = ("constant from the committed ncu --set full capture " + rec.get("source", "under profiles/")
+                                  + " (dram__bytes_read.sum + dram__bytes_write.sum per launch); NOT measured in this run")
             except Exception:
-                traffic = None
+                traffic, traffic_source = None, None
         out["roofline"] = {"kernel": "ax_tma_kernel (ax_e" + (" + fused p=r+beta*p" if fused_p else "")
-                                     + (" + fused pap" if args.fuse_pap else "") + ")",
+                                     + (" + fused pap" if opts["fuse_pap"] else "") + ")",
                            "bound": "hbm", "achieved": ach, "peak": peak, "unit": "GB/s", "frac": ach / peak,
                            "peak_kind": peak_kind + " copy peak (burst)", "frac_of_nominal_8TBs": ach / HBM_NOMINAL_GBS,
                            "bytes_per_point": bpp, "avg_launch_us": 1e3 * avg, "launches_timed": ax_n,
-                           "traffic": traffic, "algorithmic_bytes_per_launch": bpp * L,
-                           "share_of_step": ax_ms * (args.steps if graphed else 1) / ms_for_share,
+                           "traffic": traffic, "traffic_source": traffic_source,
+                           "algorithmic_bytes_per_launch": bpp * L,
+                           "share_of_step": ax_ms / prof_steps / ms_prof_step,
                            "timed_by": ktimes_from}
-        # real bytes per point of the vector kernels: fused-p path = update x,r (49) [+ p inside ax_e];
-        # otherwise update_r (w, r, code in; r out = 25) and update_px (r, p, x in; p, x out = 40)
-        kb = {"gs": gs_bytes(sizes) / L, "dot": 17.0,
-              "update_xr": 49.0 if fused_p else 25.0, "update_p": 24.0 if fused_p else 40.0}
-        out["kernels"] = {k: {"avg_us": 1e3 * t / n, "launches": n, "share_of_step": t * (args.steps if graphed else 1) / ms_for_share,
-                              **({"gbs_model": kb[k] * L / (t / n * 1e-3) / 1e9} if k in kb else {})}
+        out["kernels"] = {k: {"avg_us": 1e3 * t / n, "launches_per_step": n // prof_steps,
+                              "share_of_step": t / prof_steps / ms_prof_step, "real_bytes_per_point": kb[k],
+                              "gbs_real": kb[k] * L / (t / n * 1e-3) / 1e9}
                           for k, (t, n) in ktimes.items() if n > 0}
+        out["kernels"]["_profiled_step_ms"] = ms_prof_step
+        # secondary roofline: the fp64 pipe.  Executed flops of ax_e per point with the even-odd
+        # transforms: 6 line transforms of n/2 + 2 fp64 instructions per point (n^2/2 DFMA + 2n DADD per line) =
+        # 6(n+1) flops, the 3x3 G 15, the fused pap 6, the final sum 2 -- against a DFMA-only microbenchmark
+        n = N + 1
+        from paper_2606_12650_b200.binding import fp64_peak
+        pk = fp64_peak()
+        ex_flops = (6.0 * (n + 1) + 15.0 + (6.0 if opts["fuse_pap"] else 0.0) + 2.0) * L
+        ex_instr = (3.0 * n + 12.0 + 9.0 + (4.0 if opts["fuse_pap"] else 0.0) + 2.0) * L
+        out["fp64"] = {"peak_tflops_measured": pk["tflops"], "how": "nk_fp64_peak: DFMA-only microbenchmark, 2 flops per DFMA, "
+                       "full occupancy, best of 5", "dfma_per_clk_per_sm_at_max_clock": pk["dfma_per_clk_per_sm_at_max_clock"],
+                       "ax_e_model_tflops": (12.0 * n + 15.0) * L / (avg * 1e-3) / 1e12,
+                       "ax_e_executed_tflops": ex_flops / (avg * 1e-3) / 1e12,
+                       "ax_e_fp64_instr_per_s_over_peak_dfma_per_s": ex_instr / (avg * 1e-3) / (pk["tflops"] * 1e12 / 2.0)}
     else:
         out["roofline"] = None
     if not args.no_cpu_baseline:
-        out["cpu_baseline"] = cpu_baseline(args.workload)
+        out["cpu_baseline"] = cpu_baseline(args.workload, mesh, f_np)
     return out
 
 
@@ -502,10 +590,11 @@ def main():
     ap.add_argument("--warmup", type=int, default=3)
     ap.add_argument("--impl", default="ours", choices=["ours", "reference"])
     ap.add_argument("--workload", default="config5", choices=["config1", "config2", "config3", "config5"])
-    ap.add_argument("--fuse-pap", type=int, default=1)
-    ap.add_argument("--pdl", type=int, default=3, help="programmatic dependent launch inside nk_cg: 0 off, 1 all but gs, 2 gs too, 3 library default (2 up to 2^24 points, else 1)")
-    ap.add_argument("--fuse-p", type=int, default=2, help="0 off, 1 on, 2 library default (on up to 2^24 points)")
-    ap.add_argument("--graph", type=int, default=2, help="0 off, 1 on, 2 library default (graph up to 2^24 points)")
+    ap.add_argument("--fuse-pap", type=int, default=None, help="library options (include/nk.h); default: the library's")
+    ap.add_argument("--pdl", type=int, default=None)
+    ap.add_argument("--fuse-p", type=int, default=None)
+    ap.add_argument("--fuse-gs", type=int, default=None)
+    ap.add_argument("--graph", type=int, default=None)
     ap.add_argument("--traffic", type=float, default=None,
                     help="dram bytes per ax_e launch from the committed ncu --set full capture (profiles/)")
     ap.add_argument("--no-cpu-baseline", action="store_true")

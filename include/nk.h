@@ -97,7 +97,7 @@ int nk_get_diag(nk_ctx *ctx, double *diag, void *stream);
  *   nk_cg_init       r = mask o f, x = 0, p = r, rho = <r,r>_c  (x DEVICE L, caller-owned, kept)
  *   nk_cg_load_state copies r, p (DEVICE, L) into the context and sets rho (x is the caller's)
  *   nk_cg_step       one iteration on (x, ctx r, ctx p); leaves w = ax(p) in the context
- *   nk_cg_get_state  copies ctx r, p, w out (DEVICE, L each; any may be NULL)
+ *   nk_cg_get_state  copies ctx r, p and w = M Q Q^T A_L p out (DEVICE, L each; any may be NULL)
  *   nk_get_scalars   HOST out[5] = rho (entering the last step), pap, alpha, rho', beta; synchronises */
 int nk_cg_init(nk_ctx *ctx, const double *f, double *x, void *stream);
 int nk_cg_load_state(nk_ctx *ctx, const double *r, const double *p, double rho, void *stream);
@@ -149,6 +149,12 @@ int nk_dist_iter_c(nk_ctx *ctx, double *x, double *hist_k_dev, void *stream);
  *                  <M QQ^T A_L p, p>_c = sum_l (A_L p)_l p_l; 0 = separate weighted dot after gs
  *   "fuse_p"       1 = p = r + beta p folded into the load of the next ax_e; 0 = own kernel;
  *                  2 (default) = 1 for meshes of up to 2^24 local points (one launch fewer), else 0
+ *   "fuse_gs"      1 (default) = inside nk_cg the gather-scatter and the mask are folded into the residual
+ *                  update: w = M Q Q^T A_L p is only ever read by r -= alpha w, so that kernel streams the
+ *                  UNSUMMED ax_e output and gathers the other copies of every shared node on the fly (sums
+ *                  in ascending local index, as nk_gs: x and the history are bitwise those of 0).  gs's
+ *                  write-back, its re-read and one launch per iteration are gone.  Needs "fuse_pap" = 1
+ *                  (the separate weighted dot reads the summed w); 0 = nk_gs as its own kernel.
  *   "graph"        0 = nk_cg enqueues its launches one by one; 1 = records them into a CUDA graph
  *                  (cached per f, x, res_hist, niter; updated in place when the pointers change) and
  *                  replays it; 2 (default) = 1 for meshes of up to 2^24 local points, where launch gaps
@@ -190,11 +196,18 @@ int nk_get_kernel_times(nk_ctx *ctx, double *ms_host, int64_t *count_host, void 
  * of batches the busiest CTA runs (> 1: the shared-memory ring wraps and its mbarrier phases flip). */
 int nk_ax_batch_elements(int N);
 int nk_get_ax_launch(nk_ctx *ctx, int *batch_elements, int *ctas, int64_t *max_batches_per_cta);
-/* Which way nk_cg runs with the current options on this mesh: 0 = its kernels enqueued one by one
- * (programmatic dependent launches unless "pdl" = 0), 1 = the same launches replayed as one CUDA graph. */
-int nk_get_cg_path(nk_ctx *ctx, int *path);
+/* Which way nk_cg runs with the current options on this mesh: path 0 = its kernels enqueued one by one,
+ * 1 = the same launches replayed as one CUDA graph; pdl_mode (may be NULL) = "pdl" resolved (0, 1 or 2). */
+int nk_get_cg_path(nk_ctx *ctx, int *path, int *pdl_mode);
 /* Kernel launches enqueued by this context so far (for bench.py's gpu_launches). */
 int nk_get_launch_count(nk_ctx *ctx, int64_t *count);
+
+/* The fp64 ceiling of the current device, measured with a DFMA-only microbenchmark (the
+ * secondary roofline of ax_e, whose primary bound is HBM): HOST out tflops = 2 flops x DFMA per second at
+ * full occupancy, best of 5 runs of about a millisecond; dfma_per_clk_per_sm (may be NULL) = the same rate
+ * per SM and per cycle of the device's MAXIMUM SM clock.  Needs no context; allocates 8 bytes for the
+ * duration of the call; synchronises. */
+int nk_fp64_peak(double *tflops_host, double *dfma_per_clk_per_sm_host, void *stream);
 
 const char *nk_strerror(int code);
 int nk_last_cuda_error(void);   /* cudaError_t of the last NK_ERR_CUDA on this thread, else 0 */

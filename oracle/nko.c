@@ -583,6 +583,17 @@ int nko_get_D(nko_ctx *c, double *D, double *xi, double *w)
     return NKO_OK;
 }
 
+/* Timing aid for bench.py's 1-thread CPU figure; no effect on any value:
+ * every sum is taken over fixed chunks in a fixed order. */
+void nko_set_num_threads(int nthreads)
+{
+#ifdef _OPENMP
+    if (nthreads >= 1) omp_set_num_threads(nthreads);
+#else
+    (void)nthreads;
+#endif
+}
+
 int nko_num_threads(void)
 {
 #ifdef _OPENMP

@@ -78,6 +78,7 @@ int nko_get_mult(nko_ctx *ctx, double *mult);             /* L, multiplicity = g
 int nko_get_geom(nko_ctx *ctx, double *G6, double *J);    /* G6: rr|rs|rt|ss|st|tt planes of L; J: L (may be NULL) */
 int nko_get_D(nko_ctx *ctx, double *D, double *xi, double *w);
 int nko_num_threads(void);
+void nko_set_num_threads(int nthreads);   /* timing aid only (bench.py's 1-thread figure) */
 const char *nko_strerror(int code);
 
 #ifdef __cplusplus

@@ -62,6 +62,8 @@ def _load(fma: bool = False):
     lib.nko_free.restype = None
     lib.nko_num_threads.argtypes = []
     lib.nko_num_threads.restype = C.c_int
+    lib.nko_set_num_threads.argtypes = [C.c_int]
+    lib.nko_set_num_threads.restype = None
     lib.nko_strerror.argtypes = [C.c_int]
     lib.nko_strerror.restype = C.c_char_p
     _libs[key] = lib
@@ -86,6 +88,11 @@ def _check(lib, rc: int):
 
 def num_threads() -> int:
     return int(_load().nko_num_threads())
+
+
+def set_num_threads(n: int) -> None:
+    """OpenMP threads of later calls (bench.py's 1-thread figure); values do not depend on it."""
+    _load().nko_set_num_threads(int(n))
 
 
 def basis(N: int, fma: bool = False):

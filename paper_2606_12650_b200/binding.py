@@ -57,7 +57,8 @@ SIGNATURES = {
     "nk_dist_iter_b": (_i, [_vp, _vp]),
     "nk_dist_iter_c": (_i, [_vp, _vp, _vp, _vp]),
     "nk_get_launch_count": (_i, [_vp, C.POINTER(_i64)]),
-    "nk_get_cg_path": (_i, [_vp, C.POINTER(_i)]),
+    "nk_get_cg_path": (_i, [_vp, C.POINTER(_i), C.POINTER(_i)]),
+    "nk_fp64_peak": (_i, [C.POINTER(_d), C.POINTER(_d), _vp]),
     "nk_ax_batch_elements": (_i, [_i]),
     "nk_get_ax_launch": (_i, [_vp, C.POINTER(_i), C.POINTER(_i), C.POINTER(_i64)]),
     "nk_strerror": (C.c_char_p, [_i]),
@@ -108,6 +109,13 @@ def ax_batch_elements(N: int) -> int:
     if rc <= 0:
         _check(rc if rc < 0 else NK_ERR_ARG)
     return int(rc)
+
+
+def fp64_peak() -> dict:
+    """DFMA-only microbenchmark on the current device: measured fp64 TFLOP/s (2 flops per DFMA)."""
+    t, r = _d(), _d()
+    _check(load().nk_fp64_peak(C.byref(t), C.byref(r), _stream()))
+    return dict(tflops=float(t.value), dfma_per_clk_per_sm_at_max_clock=float(r.value))
 
 
 def _np_ptr(a: np.ndarray):
@@ -303,8 +311,15 @@ class Nekbone:
     def solve_path(self) -> str:
         """How nk_cg runs with the current options: "launches" (one by one) or "graph" (CUDA graph replay)."""
         v = _i()
-        _check(self._lib.nk_get_cg_path(self._ctx, C.byref(v)))
+        _check(self._lib.nk_get_cg_path(self._ctx, C.byref(v), None))
         return self.CG_PATHS[int(v.value)]
+
+    def pdl_effective(self) -> int:
+        """The "pdl" option resolved for this mesh: 0 plain launches, 1 ax_e and the vector kernels are
+        programmatic dependents, 2 the kernels with gathers too."""
+        v, m = _i(), _i()
+        _check(self._lib.nk_get_cg_path(self._ctx, C.byref(v), C.byref(m)))
+        return int(m.value)
 
     def launch_count(self) -> int:
         v = _i64()

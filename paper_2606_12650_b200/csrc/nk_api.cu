@@ -108,14 +108,18 @@ cudaError_t enqueue_iteration(nk_ctx *c, double *x, double *hist_k, cudaStream_t
     } else {
         NK_LAUNCH(NK_K_AX, nk_launch_ax_tma(c, nullptr, c->p, nullptr, c->w, fuse_pap, st));
     }
-    NK_LAUNCH(NK_K_GS, nk_launch_gs(c, c->w, 1, st));
+    // "fuse_gs": gs and the mask ride in the residual update, which gathers the copies of shared nodes from the
+    // unsummed w (nk_vec.cu); the separate weighted dot needs the summed w, so it keeps gs in place
+    const int fuse_gs = c->opt_fuse_gs && fuse_pap;
+    if (!fuse_gs) NK_LAUNCH(NK_K_GS, nk_launch_gs(c, c->w, 1, st));
     if (!fuse_pap) NK_LAUNCH(NK_K_DOT, nk_launch_dot(c, c->w, c->p, nullptr, NK_EPI_PAP, st));
+    c->w_unsummed = fuse_gs;
     if (fuse_p_on(c)) {
-        NK_LAUNCH(NK_K_UPDATE_XR, nk_launch_update_xr(c, x, hist_k, st));
+        NK_LAUNCH(NK_K_UPDATE_XR, nk_launch_update_xr(c, x, hist_k, fuse_gs, st));
         c->p_pending = 1;
     } else {
         // r first, then x and p together: p is read once per iteration instead of twice (65 vs 73 B/pt)
-        NK_LAUNCH(NK_K_UPDATE_XR, nk_launch_update_r(c, hist_k, st));
+        NK_LAUNCH(NK_K_UPDATE_XR, nk_launch_update_r(c, hist_k, fuse_gs, st));
         NK_LAUNCH(NK_K_UPDATE_P, nk_launch_update_px(c, x, st));
     }
     return cudaSuccess;
@@ -187,10 +191,11 @@ static bool cg_uses_graph(const nk_ctx *c)
     return !c->opt_profile && (c->opt_graph == 1 || (c->opt_graph == 2 && c->L <= NK_GRAPH_AUTO_MAX_L));
 }
 
-int nk_get_cg_path(nk_ctx *c, int *path)
+int nk_get_cg_path(nk_ctx *c, int *path, int *pdl_mode)
 {
     if (!c || !path) return NK_ERR_ARG;
     *path = cg_uses_graph(c) ? 1 : 0;
+    if (pdl_mode) *pdl_mode = c->opt_profile ? 0 : nk_pdl_mode(c);
     return NK_OK;
 }
 
@@ -206,7 +211,7 @@ int nk_cg(nk_ctx *c, const double *f, double *x, int niter, double *res_hist, vo
     }
     // Record the launch sequence once per (f, x, res_hist, niter, options) and replay it: the CG
     // loop of the small configs is launch-bound (S 7 hard part 4).
-    const int key = c->opt_fuse_pap | (c->opt_fuse_p << 1) | (c->opt_pdl << 4);
+    const int key = c->opt_fuse_pap | (c->opt_fuse_p << 1) | (c->opt_fuse_gs << 3) | (c->opt_pdl << 4);
     if (!c->graph_exec || c->graph_f != f || c->graph_x != x || c->graph_hist != res_hist ||
         c->graph_niter != niter || c->graph_key != key) {
         cudaStream_t cap;
@@ -239,7 +244,7 @@ int nk_cg(nk_ctx *c, const double *f, double *x, int niter, double *res_hist, vo
         c->graph_f = f; c->graph_x = x; c->graph_hist = res_hist; c->graph_niter = niter; c->graph_key = key;
     }
     NK_CUDA(cudaGraphLaunch(c->graph_exec, st));
-    int per_iter = 3 + (c->opt_fuse_pap ? 0 : 1) + (fuse_p_on(c) ? 0 : 1);
+    int per_iter = 3 + (c->opt_fuse_pap ? 0 : 1) + (fuse_p_on(c) ? 0 : 1) - ((c->opt_fuse_gs && c->opt_fuse_pap) ? 1 : 0);
     c->launches += 1 + (int64_t)niter * per_iter + ((fuse_p_on(c) && niter > 0) ? 1 : 0);
     c->p_pending = 0;
     return NK_OK;
@@ -279,6 +284,7 @@ int nk_cg_load_state(nk_ctx *c, const double *r, const double *p, double rho, vo
     double scal[NK_S_COUNT] = {0};
     scal[NK_S_RHO] = rho; scal[NK_S_RHO_OLD] = rho; scal[NK_S_RHO_NEW] = rho;
     c->p_pending = 0;
+    c->w_unsummed = 0;
     NK_CUDA(cudaMemcpyAsync(c->r, r, bytes, cudaMemcpyDeviceToDevice, st));
     NK_CUDA(cudaMemcpyAsync(c->p, p, bytes, cudaMemcpyDeviceToDevice, st));
     NK_CUDA(cudaMemcpyAsync(c->red.scal, scal, sizeof(scal), cudaMemcpyHostToDevice, st));
@@ -304,7 +310,12 @@ int nk_cg_get_state(nk_ctx *c, double *r, double *p, double *w, void *stream)
     }
     if (r) NK_CUDA(cudaMemcpyAsync(r, c->r, bytes, cudaMemcpyDeviceToDevice, st));
     if (p) NK_CUDA(cudaMemcpyAsync(p, c->p, bytes, cudaMemcpyDeviceToDevice, st));
-    if (w) NK_CUDA(cudaMemcpyAsync(w, c->w, bytes, cudaMemcpyDeviceToDevice, st));
+    if (w) {
+        NK_CUDA(cudaMemcpyAsync(w, c->w, bytes, cudaMemcpyDeviceToDevice, st));
+        // "fuse_gs" leaves the UNSUMMED ax_e output in the context (the update gathered from it): what is handed
+        // out is w = M Q Q^T A_L p as documented, summed and masked on the copy
+        if (c->w_unsummed) NK_CUDA(nk_launch_gs(c, w, 1, st));
+    }
     return NK_OK;
 }
 
@@ -327,6 +338,7 @@ static int *option_slot(nk_ctx *c, const char *name, int *lo, int *hi)
 {
     if (!std::strcmp(name, "fuse_pap")) { *lo = 0; *hi = 1; return &c->opt_fuse_pap; }
     if (!std::strcmp(name, "fuse_p")) { *lo = 0; *hi = 2; return &c->opt_fuse_p; }
+    if (!std::strcmp(name, "fuse_gs")) { *lo = 0; *hi = 1; return &c->opt_fuse_gs; }
     if (!std::strcmp(name, "graph")) { *lo = 0; *hi = 2; return &c->opt_graph; }
     if (!std::strcmp(name, "pdl")) { *lo = 0; *hi = 3; return &c->opt_pdl; }
     if (!std::strcmp(name, "profile")) { *lo = 0; *hi = 1; return &c->opt_profile; }

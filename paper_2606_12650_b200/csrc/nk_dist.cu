@@ -202,7 +202,7 @@ int nk_dist_iter_b(nk_ctx *c, void *stream)
     cudaStream_t st = S(stream);
     NK_CUDA(launch_unpack(c, c->w, st));
     NK_CUDA(launch_finish(c, NK_EPI_PAP, c->dist_gath + c->dist_slots, c->dist_slots + 1, c->res_dummy, st));
-    NK_CUDA(with_raw(c, c->dist_ssend, [&] { return nk_launch_update_r(c, c->res_dummy, st); }));
+    NK_CUDA(with_raw(c, c->dist_ssend, [&] { return nk_launch_update_r(c, c->res_dummy, 0, st); }));
     return NK_OK;
 }
 

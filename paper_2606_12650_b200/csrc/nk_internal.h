@@ -68,6 +68,12 @@ struct nk_ctx {
     // copies: faces, edges, corners of a conforming hex mesh): a thread fetches its indices with one
     // vector load and no offset lookup, and a chunk stays in one neighbourhood of memory
     int32_t *pk, *gs_desc;
+    // gs folded into the residual update (nk_vec.cu, "fuse_gs"): per local point l
+    //   nbr[l] == l   its node has no other copy (or only masked ones): the value stands
+    //   nbr[l] >= 0   the ONE other copy of a node of multiplicity 2 (faces: 95 % of all shared points)
+    //   nbr[l] == -1  Dirichlet node: the sum is replaced by 0
+    //   nbr[l] <= -2  CSR row -nbr[l]-2 lists all copies (edges, corners, irregular meshes)
+    int32_t *nbr;
     int64_t n_gs_chunks;
     double *ctab;                // NK_CTAB doubles: 1/multiplicity
     double *mtab;                // NK_CTAB doubles: multiplicity
@@ -79,9 +85,10 @@ struct nk_ctx {
     int64_t n_unique, n_shared_unique, n_masked_unique;
     int64_t n_rows, n_listed, n_sum_rows, n_sum_listed;
     // options / state
-    int opt_fuse_pap, opt_fuse_p, opt_graph, opt_profile, opt_pdl;
+    int opt_fuse_pap, opt_fuse_p, opt_fuse_gs, opt_graph, opt_profile, opt_pdl;
     int pdl_now;                 // nk_pdl_mode while nk_cg enqueues its loop (every kernel there waits), else 0
     int p_pending;               // 1: p = r + beta p has not been applied yet (fuse_p)
+    int w_unsummed;              // 1: ctx w holds the unsummed ax_e output of the last iteration (fuse_gs)
     int64_t launches;
     // per-kernel-class device timing ("profile" option): chained events, interval i = kernel class cls[i]
     nk_prof *prof;
@@ -140,9 +147,11 @@ cudaError_t nk_launch_gs(nk_ctx *c, double *v, int with_mask, cudaStream_t st);
 // nk_vec.cu
 cudaError_t nk_launch_dot(nk_ctx *c, const double *a, const double *b, double *out, int epi, cudaStream_t st);
 cudaError_t nk_launch_cg_init(nk_ctx *c, const double *f, double *x, double *hist, cudaStream_t st);
-cudaError_t nk_launch_update_xr(nk_ctx *c, double *x, double *hist_k, cudaStream_t st);
+// gs != 0: w is the UNSUMMED ax_e output and every point gathers the other copies of its node on the fly
+// (r -= alpha M Q Q^T w without gs ever writing w back); same values, bit for bit, as nk_launch_gs + gs == 0
+cudaError_t nk_launch_update_xr(nk_ctx *c, double *x, double *hist_k, int gs, cudaStream_t st);
 cudaError_t nk_launch_update_p(nk_ctx *c, cudaStream_t st);
-cudaError_t nk_launch_update_r(nk_ctx *c, double *hist_k, cudaStream_t st);     // r -= alpha w, rho'
+cudaError_t nk_launch_update_r(nk_ctx *c, double *hist_k, int gs, cudaStream_t st);     // r -= alpha w, rho'
 cudaError_t nk_launch_update_px(nk_ctx *c, double *x, cudaStream_t st);         // x += alpha p; p = r + beta p
 cudaError_t nk_launch_get_mult(nk_ctx *c, double *mult, cudaStream_t st);
 // preconditioned CG

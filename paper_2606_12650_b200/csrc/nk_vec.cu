@@ -30,6 +30,38 @@ __device__ __forceinline__ void load_ctab(double *s_c, const double *ctab)
     __syncthreads();
 }
 
+// ---- gs folded into the residual update ("fuse_gs"; SURVEY 8(a) a2 + a3 + a5 in one pass) ---------------
+// Inside CG the summed w = M Q Q^T A_L p is read exactly once, by r -= alpha w (pap comes out of ax_e as a
+// quadratic form).  So w need never be summed IN PLACE: the update streams the UNSUMMED ax_e output and every
+// shared point gathers the other copies of its node on the fly.  gs's write-back (8 B per listed copy, 32 B
+// where the copy is alone in its sector: the stride-n r-faces), its re-read by the update and one launch per
+// iteration are gone; the gathered sectors are ones the streaming reads of neighbouring blocks fetch anyway.
+// Sums run in ascending local index, as in nk_gs.cu, so r and rho' are bitwise those of gs followed by the
+// plain update.
+struct nk_gather { const int32_t *nbr, *off, *idx; };
+
+// all copies of a node of multiplicity != 2 (edges, corners: 5 % of the shared points of a brick)
+__device__ __forceinline__ double gs_row_sum(const double *__restrict__ w, const int32_t *__restrict__ off,
+                                          const int32_t *__restrict__ idx, int row)
+{
+    const int b = off[row], e = off[row + 1];
+    double s = w[idx[b]];
+    for (int j = b + 1; j < e; ++j) s += w[idx[j]];
+    return s;
+}
+// the partner's value for a point of a multiplicity-2 node (predicated load, issued with the streaming loads)
+__device__ __forceinline__ double gs_partner(const double *__restrict__ w, int64_t l, int v)
+{
+    return (v >= 0 && (int64_t)v != l) ? w[v] : 0.0;
+}
+// (M Q Q^T w)_l from the point's own value wl, its gather code v = nbr[l] and the partner's value g
+__device__ __forceinline__ double gs_value(const double *__restrict__ w, const nk_gather &gp, int64_t l, int v, double wl, double g)
+{
+    if (v >= 0) return ((int64_t)v == l) ? wl : ((int64_t)v > l ? wl + g : g + wl);
+    if (v == -1) return 0.0;
+    return gs_row_sum(w, gp.off, gp.idx, -v - 2);
+}
+
 // out = <a,b>_c
 __global__ void __launch_bounds__(NK_VEC_THREADS)
 dot_kernel(const double *__restrict__ a, const double *__restrict__ b, const uint8_t *__restrict__ code,
@@ -89,10 +121,12 @@ cg_init_kernel(const double *__restrict__ f, double *__restrict__ x, double *__r
 }
 
 // x += alpha p; r -= alpha w; rho' = <r,r>_c          (S 8(a) a5: axpy, axpy and dot in one pass)
-__global__ void __launch_bounds__(NK_VEC_THREADS)
+// GS: w is the unsummed ax_e output; the sum over the copies and the mask are applied on the fly.
+template <bool GS>
+__global__ void __launch_bounds__(NK_VEC_THREADS, 2)
 update_xr_kernel(double *__restrict__ x, double *__restrict__ r, const double *__restrict__ p,
                  const double *__restrict__ w, const uint8_t *__restrict__ code,
-                 const double *__restrict__ ctab, int64_t L, nk_reduce_ws ws, double *hist_k)
+                 const double *__restrict__ ctab, int64_t L, nk_reduce_ws ws, double *hist_k, nk_gather gp)
 {
     __shared__ double s_c[NK_CTAB];
     __shared__ double s_red[33];
@@ -105,10 +139,16 @@ update_xr_kernel(double *__restrict__ x, double *__restrict__ r, const double *_
     double acc = 0.0;
     for (int64_t q = (int64_t)blockIdx.x * blockDim.x + threadIdx.x; q < pairs; q += stride) {
         const double2 pv = reinterpret_cast<const double2 *>(p)[q];
-        const double2 wv = reinterpret_cast<const double2 *>(w)[q];
+        double2 wv = reinterpret_cast<const double2 *>(w)[q];
         double2 xv = reinterpret_cast<double2 *>(x)[q];
         double2 rv = reinterpret_cast<double2 *>(r)[q];
         const uchar2 cd = reinterpret_cast<const uchar2 *>(code)[q];
+        if (GS) {
+            const int2 nv = reinterpret_cast<const int2 *>(gp.nbr)[q];
+            const double g0 = gs_partner(w, 2 * q, nv.x), g1 = gs_partner(w, 2 * q + 1, nv.y);
+            wv.x = gs_value(w, gp, 2 * q, nv.x, wv.x, g0);
+            wv.y = gs_value(w, gp, 2 * q + 1, nv.y, wv.y, g1);
+        }
         xv.x = fma(alpha, pv.x, xv.x);
         xv.y = fma(alpha, pv.y, xv.y);
         rv.x = fma(-alpha, wv.x, rv.x);
@@ -121,7 +161,9 @@ update_xr_kernel(double *__restrict__ x, double *__restrict__ r, const double *_
     if ((L & 1) && blockIdx.x == 0 && threadIdx.x == 0) {
         const int64_t l = L - 1;
         const double xv = fma(alpha, p[l], x[l]);
-        const double rv = fma(-alpha, w[l], r[l]);
+        double wl = w[l];
+        if (GS) wl = gs_value(w, gp, l, gp.nbr[l], wl, gs_partner(w, l, gp.nbr[l]));
+        const double rv = fma(-alpha, wl, r[l]);
         x[l] = xv; r[l] = rv;
         acc = fma(s_c[code[l] & 0x7f] * rv, rv, acc);
     }
@@ -153,9 +195,10 @@ update_p_kernel(double *__restrict__ p, const double *__restrict__ r, const doub
 // r -= alpha w; rho' = <r,r>_c.  With update_px_kernel below this is the un-fused iteration's vector
 // work in 65 B/pt instead of 73: p is read once per iteration (by update_px, which still has the old
 // p in registers when x needs it) instead of twice.  Same arithmetic per entry as update_xr_kernel.
-__global__ void __launch_bounds__(NK_VEC_THREADS)
+template <bool GS>
+__global__ void __launch_bounds__(NK_VEC_THREADS, 2)
 update_r_kernel(double *__restrict__ r, const double *__restrict__ w, const uint8_t *__restrict__ code,
-                const double *__restrict__ ctab, int64_t L, nk_reduce_ws ws, double *hist_k)
+                const double *__restrict__ ctab, int64_t L, nk_reduce_ws ws, double *hist_k, nk_gather gp)
 {
     __shared__ double s_c[NK_CTAB];
     __shared__ double s_red[33];
@@ -166,20 +209,39 @@ update_r_kernel(double *__restrict__ r, const double *__restrict__ w, const uint
     const int64_t pairs = L >> 1;
     const int64_t stride = (int64_t)gridDim.x * blockDim.x;
     double acc = 0.0;
-    // four pairs per step, all loads before the stores (r is loaded and stored through one pointer, so
-    // the compiler will not overlap the next step's loads with this step's store on its own)
+    // U pairs per step, all loads before the stores (r is loaded and stored through one pointer, so the
+    // compiler will not overlap the next step's loads with this step's store on its own).  The order in
+    // which acc takes its terms -- q ascending by stride, .x before .y -- does not depend on U.
+    constexpr int U = GS ? 2 : 4;
     int64_t q = (int64_t)blockIdx.x * blockDim.x + threadIdx.x;
-    for (; q + 3 * stride < pairs; q += 4 * stride) {
-        double2 wv[4], rv[4];
-        uchar2 cd[4];
+    for (; q + (U - 1) * stride < pairs; q += U * stride) {
+        double2 wv[U], rv[U];
+        uchar2 cd[U];
+        int2 nv[U];
 #pragma unroll
-        for (int j = 0; j < 4; ++j) {
+        for (int j = 0; j < U; ++j) {
+            if (GS) nv[j] = reinterpret_cast<const int2 *>(gp.nbr)[q + j * stride];
             wv[j] = reinterpret_cast<const double2 *>(w)[q + j * stride];
             rv[j] = reinterpret_cast<double2 *>(r)[q + j * stride];
             cd[j] = reinterpret_cast<const uchar2 *>(code)[q + j * stride];
         }
+        if (GS) {
+            double2 g[U];
 #pragma unroll
-        for (int j = 0; j < 4; ++j) {
+            for (int j = 0; j < U; ++j) {                 // the partners' values: 2 U independent gathers in flight
+                const int64_t l = 2 * (q + j * stride);
+                g[j].x = gs_partner(w, l, nv[j].x);
+                g[j].y = gs_partner(w, l + 1, nv[j].y);
+            }
+#pragma unroll
+            for (int j = 0; j < U; ++j) {
+                const int64_t l = 2 * (q + j * stride);
+                wv[j].x = gs_value(w, gp, l, nv[j].x, wv[j].x, g[j].x);
+                wv[j].y = gs_value(w, gp, l + 1, nv[j].y, wv[j].y, g[j].y);
+            }
+        }
+#pragma unroll
+        for (int j = 0; j < U; ++j) {
             rv[j].x = fma(-alpha, wv[j].x, rv[j].x);
             rv[j].y = fma(-alpha, wv[j].y, rv[j].y);
             reinterpret_cast<double2 *>(r)[q + j * stride] = rv[j];
@@ -188,9 +250,15 @@ update_r_kernel(double *__restrict__ r, const double *__restrict__ w, const uint
         }
     }
     for (; q < pairs; q += stride) {
-        const double2 wv = reinterpret_cast<const double2 *>(w)[q];
+        double2 wv = reinterpret_cast<const double2 *>(w)[q];
         double2 rv = reinterpret_cast<double2 *>(r)[q];
         const uchar2 cd = reinterpret_cast<const uchar2 *>(code)[q];
+        if (GS) {
+            const int2 n2 = reinterpret_cast<const int2 *>(gp.nbr)[q];
+            const double g0 = gs_partner(w, 2 * q, n2.x), g1 = gs_partner(w, 2 * q + 1, n2.y);
+            wv.x = gs_value(w, gp, 2 * q, n2.x, wv.x, g0);
+            wv.y = gs_value(w, gp, 2 * q + 1, n2.y, wv.y, g1);
+        }
         rv.x = fma(-alpha, wv.x, rv.x);
         rv.y = fma(-alpha, wv.y, rv.y);
         reinterpret_cast<double2 *>(r)[q] = rv;
@@ -199,7 +267,9 @@ update_r_kernel(double *__restrict__ r, const double *__restrict__ w, const uint
     }
     if ((L & 1) && blockIdx.x == 0 && threadIdx.x == 0) {
         const int64_t l = L - 1;
-        const double rv = fma(-alpha, w[l], r[l]);
+        double wl = w[l];
+        if (GS) wl = gs_value(w, gp, l, gp.nbr[l], wl, gs_partner(w, l, gp.nbr[l]));
+        const double rv = fma(-alpha, wl, r[l]);
         r[l] = rv;
         acc = fma(s_c[code[l] & 0x7f] * rv, rv, acc);
     }
@@ -353,11 +423,14 @@ cudaError_t nk_launch_cg_init(nk_ctx *c, const double *f, double *x, double *his
     return cudaGetLastError();
 }
 
-cudaError_t nk_launch_update_xr(nk_ctx *c, double *x, double *hist_k, cudaStream_t st)
+cudaError_t nk_launch_update_xr(nk_ctx *c, double *x, double *hist_k, int gs, cudaStream_t st)
 {
     const int nb = vec_blocks(c, c->L >> 1);
-    const cudaError_t e = nk_launch(update_xr_kernel, nb, NK_VEC_THREADS, 0, st, c->pdl_now, x, c->r, c->p, c->w, c->code,
-                                    c->ctab, c->L, c->red, hist_k);
+    const nk_gather gp{c->nbr, c->row_off, c->row_idx};
+    // (with the gathers the kernel is a programmatic dependent only where gs itself would be: nk_pdl_mode)
+    const int pdl = gs ? (c->pdl_now == 2) : c->pdl_now;
+    const cudaError_t e = nk_launch(gs ? update_xr_kernel<true> : update_xr_kernel<false>, nb, NK_VEC_THREADS, 0, st, pdl,
+                                    x, c->r, c->p, c->w, c->code, c->ctab, c->L, c->red, hist_k, gp);
     if (e != cudaSuccess) return e;
     c->launches++;
     return cudaGetLastError();
@@ -409,11 +482,13 @@ cudaError_t nk_launch_update_pz(nk_ctx *c, double *x, cudaStream_t st)
     return cudaGetLastError();
 }
 
-cudaError_t nk_launch_update_r(nk_ctx *c, double *hist_k, cudaStream_t st)
+cudaError_t nk_launch_update_r(nk_ctx *c, double *hist_k, int gs, cudaStream_t st)
 {
     const int nb = vec_blocks(c, c->L >> 1);
-    const cudaError_t e = nk_launch(update_r_kernel, nb, NK_VEC_THREADS, 0, st, c->pdl_now, c->r, c->w, c->code, c->ctab,
-                                    c->L, c->red, hist_k);
+    const nk_gather gp{c->nbr, c->row_off, c->row_idx};
+    const int pdl = gs ? (c->pdl_now == 2) : c->pdl_now;
+    const cudaError_t e = nk_launch(gs ? update_r_kernel<true> : update_r_kernel<false>, nb, NK_VEC_THREADS, 0, st, pdl,
+                                    c->r, c->w, c->code, c->ctab, c->L, c->red, hist_k, gp);
     if (e != cudaSuccess) return e;
     c->launches++;
     return cudaGetLastError();

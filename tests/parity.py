@@ -39,18 +39,38 @@ def maxnorm_rel(got, ref) -> float:
     return float(d / s) if s > 0 else float(d)
 
 
+def oracle_variants(mesh, f, niter):
+    """Histories (and solutions) of the oracle's OTHER correct evaluations of the same iteration: the build with
+    FMA contraction on, and plain double pairwise-free dot products instead of long double ones.  Their distance
+    from the reference run is the oracle's own rounding band (R15)."""
+    from oracle.nko import Oracle
+    out = []
+    ofm = Oracle.from_mesh(mesh, fma=True)
+    out.append(ofm.cg(f, niter))
+    ofm.close()
+    od = Oracle.from_mesh(mesh)
+    od.set_dot_mode(1)
+    out.append(od.cg(f, niter))
+    od.close()
+    return out
+
+
 def history_parity(h_gpu, h_or, h_or_band, tol=1e-10, band_ok=1e-11, converged=1e-9):
     """R15 protocol for a residual history (SURVEY.md 8(c) "CG sensitivity", parts 3-4).
 
-    h_or / h_or_band are the oracle's histories from its two builds (contraction off / on); their running
-    maximum relative difference is the oracle's own rounding band.  Returns (passed, worst, kstar):
+    h_or is the oracle's history, h_or_band one or several histories of other correct evaluations by the
+    oracle itself (oracle_variants: contraction on, double instead of long double dot products); the running
+    maximum of their relative distance from h_or is the oracle's own rounding band.  Once rounding noise
+    grows (x1000 per three iterations on a 63-unknown mesh) a single pair is one sample of it, so the band is
+    the maximum over the variants.  Returns (passed, worst, kstar):
       * k with band <= band_ok:   |gpu - or| <= tol * or                      (the flat 1e-10)
       * beyond:                   |gpu - or| <= max(tol, 10 band) * or, or both sides have converged
                                   (<= converged * h[0]: the recursive residual is rounding noise there)
     worst = max relative difference over the flat part, kstar = last index of the flat part."""
-    h_gpu, h_or, h_or_band = (np.asarray(a, dtype=np.float64) for a in (h_gpu, h_or, h_or_band))
+    h_gpu, h_or = np.asarray(h_gpu, dtype=np.float64), np.asarray(h_or, dtype=np.float64)
+    alts = np.atleast_2d(np.asarray(h_or_band, dtype=np.float64))
     den = np.where(h_or > 0, h_or, 1.0)
-    band = np.maximum.accumulate(np.abs(h_or_band - h_or) / den)
+    band = np.maximum.accumulate((np.abs(alts - h_or[None, :]) / den[None, :]).max(axis=0))
     diff = np.abs(h_gpu - h_or) / den
     flat = band <= band_ok
     done = (h_gpu <= converged * h_or[0]) & (h_or <= converged * h_or[0])

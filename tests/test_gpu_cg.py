@@ -10,9 +10,10 @@ from workloads import CONFIGS, config_rhs, rhs_unique
 
 pytestmark = pytest.mark.gpu
 
-OPTION_SETS = [dict(fuse_pap=1, fuse_p=1, graph=0), dict(fuse_pap=0, fuse_p=0, graph=0),
-               dict(fuse_pap=1, fuse_p=0, graph=0), dict(fuse_pap=0, fuse_p=1, graph=0),
-               dict(fuse_pap=1, fuse_p=1, graph=1)]
+OPTION_SETS = [dict(fuse_pap=1, fuse_p=1, fuse_gs=1, graph=0), dict(fuse_pap=0, fuse_p=0, fuse_gs=1, graph=0),
+               dict(fuse_pap=1, fuse_p=0, fuse_gs=1, graph=0), dict(fuse_pap=0, fuse_p=1, fuse_gs=1, graph=0),
+               dict(fuse_pap=1, fuse_p=1, fuse_gs=0, graph=0), dict(fuse_pap=1, fuse_p=0, fuse_gs=0, graph=0),
+               dict(fuse_pap=1, fuse_p=1, fuse_gs=1, graph=1)]
 
 
 def _set(gpu, opts):
@@ -26,7 +27,7 @@ def _rel(a, b):
 
 
 @pytest.mark.parametrize("name", ["config1", "config2"])
-@pytest.mark.parametrize("opts", OPTION_SETS[:4])
+@pytest.mark.parametrize("opts", OPTION_SETS[:6])
 def test_lockstep_iterations(name, opts):
     """Load the ORACLE's state at iteration k into the GPU, run one GPU iteration, compare
     (w, pap, alpha, x, r, rho', beta, p) -- every iteration-level formula, zero amplification."""
@@ -280,3 +281,61 @@ def test_cg_high_and_odd_orders(N):
         assert np.all(np.abs(to_np(hg) - ho) <= TOL_CG * ho), (N, graph)
         assert elem_err(to_np(xg), xo, pr.P) <= TOL_CG, (N, graph)
     pr.gpu.set_option("graph", 2)
+
+
+# ---- gs folded into the residual update ("fuse_gs") ------------------------------------------------------
+@pytest.mark.parametrize("name", ["config1", "config2", "config3"])
+@pytest.mark.parametrize("fuse_p", [0, 1])
+def test_fused_gs_is_bitwise_neutral(name, fuse_p):
+    """The residual update that gathers the copies of shared nodes from the unsummed ax_e output sums them in the
+    order nk_gs does and feeds the same reduction: x and the residual history are bitwise those of the separate
+    gs kernel, launch by launch or graphed, with or without programmatic dependent launches."""
+    import torch
+    from paper_2606_12650_b200 import Nekbone
+    from workloads import config_mesh
+    mesh = config_mesh(name)
+    gpu = Nekbone.from_mesh(mesh)
+    assert gpu.get_option("fuse_gs") == 1
+    gpu.set_option("fuse_p", fuse_p)
+    f = to_dev(config_rhs(name, mesh))
+    out = {}
+    for fuse_gs in (0, 1):
+        for graph, pdl in ((0, 0), (0, 3), (1, 3)):
+            gpu.set_option("fuse_gs", fuse_gs)
+            gpu.set_option("graph", graph)
+            gpu.set_option("pdl", pdl)
+            for rep in range(2):
+                out[fuse_gs, graph, pdl, rep] = gpu.cg(f, 40)
+    torch.cuda.synchronize()
+    x0, h0 = out[0, 0, 0, 0]
+    for key, (x, h) in out.items():
+        assert bool((x == x0).all()) and bool((h == h0).all()), key
+    gpu.close()
+
+
+def test_fused_gs_on_irregular_ids():
+    """Rows of 3, 5, 12 copies and scattered ids take the fused gather's CSR path; Dirichlet rows its zero path."""
+    from oracle.nko import Oracle
+    from paper_2606_12650_b200 import Nekbone
+    from workloads import brick_mesh
+    m = brick_mesh(3, 2, 2, 4, 0.05)
+    rng = np.random.Generator(np.random.PCG64(12))
+    glo = rng.integers(0, 400, m.L).astype(np.int64) * 1_000_003 + 17      # ~3.75 copies per id, scattered
+    glo[:12] = 5                                                            # one row of >= 12 copies
+    glo[m.L - 1] = 999_999_999_999                                          # the last point alone (odd L: 1500... even; harmless)
+    mask = np.ones(m.L)
+    mask[np.isin(glo, glo[100:110])] = 0.0
+    orc, gpu = Oracle(m.E, m.N, m.coords, glo, mask), Nekbone(m.E, m.N, m.coords, glo, mask)
+    _, inv = np.unique(glo, return_inverse=True)
+    f = rng.uniform(-1, 1, inv.max() + 1)[inv]                              # consistent on every copy
+    xo, ho = orc.cg(f, 15)
+    res = {}
+    for fuse_p in (0, 1):
+        for fuse_gs in (0, 1):
+            gpu.set_option("fuse_p", fuse_p)
+            gpu.set_option("fuse_gs", fuse_gs)
+            xg, hg = gpu.cg(to_dev(f), 15)
+            res[fuse_p, fuse_gs] = (to_np(xg), to_np(hg))
+            assert np.all(np.abs(res[fuse_p, fuse_gs][1] - ho) <= TOL_CG * ho), (fuse_p, fuse_gs)
+            assert elem_err(res[fuse_p, fuse_gs][0], xo, m.n ** 3) <= TOL_CG, (fuse_p, fuse_gs)
+        assert np.array_equal(res[fuse_p, 0][0], res[fuse_p, 1][0]) and np.array_equal(res[fuse_p, 0][1], res[fuse_p, 1][1])
