@@ -52,10 +52,11 @@ def gs_bytes(sizes: dict) -> float:
     return 20.0 * sizes["n_listed"] + 4.0 * sizes["n_rows"]
 
 
-def gs_gather_bytes(sizes: dict) -> float:
-    """gs folded into the residual update: per listed local copy its row's other copies are gathered (8 B each,
-    counted once per copy as in the gs model's read half) through 4 B of index; nothing is written back."""
-    return 12.0 * sizes["n_listed"] + 4.0 * sizes["n_rows"]
+def gs_gather_bytes(L: int, sizes: dict) -> float:
+    """gs folded into the residual update: a dense 4-byte gather code per local point, and per listed local copy
+    one 8-byte gather (the partner of a face point; the copies of an edge or corner node are read once per copy
+    too); nothing is written back."""
+    return 4.0 * L + 8.0 * sizes["n_listed"]
 
 
 def iter_model_bytes(L: int, sizes: dict) -> float:
@@ -403,6 +404,7 @@ def run_ours(args) -> dict | None:
     e2e = whole_job_value(flops_step, args.steps, world, ms_e2e)
     opts = {k: nk.get_option(k) for k in ("fuse_pap", "fuse_p", "fuse_gs", "graph", "pdl")}
     fused_p = opts["fuse_p"] == 1 or (opts["fuse_p"] == 2 and L <= (1 << 24))
+    fused_gs = bool(opts["fuse_pap"]) and (opts["fuse_gs"] == 1 or (opts["fuse_gs"] == 2 and L > (1 << 21)))
     out = {"metric": METRIC, "value": value, "unit": UNIT, "n_gpus": world, "steps": args.steps,
            "warmup": args.warmup, "ms_per_step": ms / args.steps, "higher_is_better": True,
            "scaling": "weak", "vs_baseline": None, "dtype": "f64", "data": "synthetic",
@@ -411,16 +413,16 @@ def run_ours(args) -> dict | None:
                    "d2h_bytes_per_step": 8 * (L + niter + 1), "ms_per_step": ms_e2e / args.steps},
            "gpu_launches": int(launches), "clocks": clk,
            "options": {**opts, "solve_path": solve_path, "pdl_effective": nk.pdl_effective(),
-                       "fuse_p_effective": int(fused_p), "profile_in_timed_region": False},
+                       "fuse_p_effective": int(fused_p), "fuse_gs_effective": int(fused_gs),
+                       "profile_in_timed_region": False},
            "setup_s": setup_s, "final_residual": res_final}
 
     # ---- iteration-level and kernel-level bandwidth ---------------------------------------------------
     # real bytes per point of each kernel class as launched: ax_e u 8 + G 48 + w 8 (+ r 8 read and
     # p 8 written when the direction update is folded in); gs by its plan; the vector kernels by what they touch
     gsb = gs_bytes(sizes) / L
-    fused_gs = bool(opts["fuse_gs"])
     kb = {"ax_e": 64.0 + (16.0 if fused_p else 0.0), "gs": gsb, "dot": 17.0,
-          "update_xr": ((49.0 if fused_p else 25.0) + (gs_gather_bytes(sizes) / L if fused_gs else 0.0)),
+          "update_xr": ((49.0 if fused_p else 25.0) + (gs_gather_bytes(L, sizes) / L if fused_gs else 0.0)),
           "update_p": 24.0 if fused_p else 40.0, "cg_init": 33.0}
     it_bytes = iter_model_bytes(L, sizes)
     it_gbs = it_bytes * niter * args.steps / (ms * 1e-3) / 1e9

@@ -149,12 +149,15 @@ int nk_dist_iter_c(nk_ctx *ctx, double *x, double *hist_k_dev, void *stream);
  *                  <M QQ^T A_L p, p>_c = sum_l (A_L p)_l p_l; 0 = separate weighted dot after gs
  *   "fuse_p"       1 = p = r + beta p folded into the load of the next ax_e; 0 = own kernel;
  *                  2 (default) = 1 for meshes of up to 2^24 local points (one launch fewer), else 0
- *   "fuse_gs"      1 (default) = inside nk_cg the gather-scatter and the mask are folded into the residual
+ *   "fuse_gs"      1 = inside nk_cg the gather-scatter and the mask are folded into the residual
  *                  update: w = M Q Q^T A_L p is only ever read by r -= alpha w, so that kernel streams the
- *                  UNSUMMED ax_e output and gathers the other copies of every shared node on the fly (sums
- *                  in ascending local index, as nk_gs: x and the history are bitwise those of 0).  gs's
- *                  write-back, its re-read and one launch per iteration are gone.  Needs "fuse_pap" = 1
- *                  (the separate weighted dot reads the summed w); 0 = nk_gs as its own kernel.
+ *                  UNSUMMED ax_e output and sums the copies of every shared node on the fly (in ascending
+ *                  local index, as nk_gs: r and x are, entry by entry, what 0 gives for the same alpha; rho'
+ *                  adds the same terms in another fixed order, so iterates agree to rounding, not bitwise).
+ *                  gs's write-back, its re-read and one launch per iteration are gone.  Needs "fuse_pap" = 1
+ *                  (the separate weighted dot reads the summed w); 0 = nk_gs as its own kernel; 2 (default)
+ *                  = 1 for meshes of more than 2^21 local points (below, everything sits in L2 and the
+ *                  separate kernel is faster), else 0.
  *   "graph"        0 = nk_cg enqueues its launches one by one; 1 = records them into a CUDA graph
  *                  (cached per f, x, res_hist, niter; updated in place when the pointers change) and
  *                  replays it; 2 (default) = 1 for meshes of up to 2^24 local points, where launch gaps

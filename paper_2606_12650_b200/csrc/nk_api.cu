@@ -97,6 +97,14 @@ inline bool fuse_p_on(const nk_ctx *c)
     return c->opt_fuse_p == 1 || (c->opt_fuse_p == 2 && c->L <= NK_GRAPH_AUTO_MAX_L);
 }
 
+// "fuse_gs" = 2 (default): gs rides in the residual update where its traffic matters (measured: config 5 135.5 ->
+// 132.1 ms per solve, config 3 11.3 -> 10.9; on L2-resident meshes the separate kernel is faster: config 2 1.55 vs
+// 1.78 ms).  The separate weighted dot needs the summed w, so without "fuse_pap" gs stays a kernel of its own.
+inline bool fuse_gs_on(const nk_ctx *c)
+{
+    return c->opt_fuse_pap && (c->opt_fuse_gs == 1 || (c->opt_fuse_gs == 2 && c->L > NK_FUSE_GS_AUTO_MIN_L));
+}
+
 // One CG iteration, enqueued (S 3 call stack (3)).  hist_k: where sqrt(rho') goes (DEVICE).
 cudaError_t enqueue_iteration(nk_ctx *c, double *x, double *hist_k, cudaStream_t st)
 {
@@ -110,7 +118,7 @@ cudaError_t enqueue_iteration(nk_ctx *c, double *x, double *hist_k, cudaStream_t
     }
     // "fuse_gs": gs and the mask ride in the residual update, which gathers the copies of shared nodes from the
     // unsummed w (nk_vec.cu); the separate weighted dot needs the summed w, so it keeps gs in place
-    const int fuse_gs = c->opt_fuse_gs && fuse_pap;
+    const int fuse_gs = fuse_gs_on(c);
     if (!fuse_gs) NK_LAUNCH(NK_K_GS, nk_launch_gs(c, c->w, 1, st));
     if (!fuse_pap) NK_LAUNCH(NK_K_DOT, nk_launch_dot(c, c->w, c->p, nullptr, NK_EPI_PAP, st));
     c->w_unsummed = fuse_gs;
@@ -244,7 +252,7 @@ int nk_cg(nk_ctx *c, const double *f, double *x, int niter, double *res_hist, vo
         c->graph_f = f; c->graph_x = x; c->graph_hist = res_hist; c->graph_niter = niter; c->graph_key = key;
     }
     NK_CUDA(cudaGraphLaunch(c->graph_exec, st));
-    int per_iter = 3 + (c->opt_fuse_pap ? 0 : 1) + (fuse_p_on(c) ? 0 : 1) - ((c->opt_fuse_gs && c->opt_fuse_pap) ? 1 : 0);
+    int per_iter = 3 + (c->opt_fuse_pap ? 0 : 1) + (fuse_p_on(c) ? 0 : 1) - (fuse_gs_on(c) ? 1 : 0);
     c->launches += 1 + (int64_t)niter * per_iter + ((fuse_p_on(c) && niter > 0) ? 1 : 0);
     c->p_pending = 0;
     return NK_OK;
@@ -338,7 +346,7 @@ static int *option_slot(nk_ctx *c, const char *name, int *lo, int *hi)
 {
     if (!std::strcmp(name, "fuse_pap")) { *lo = 0; *hi = 1; return &c->opt_fuse_pap; }
     if (!std::strcmp(name, "fuse_p")) { *lo = 0; *hi = 2; return &c->opt_fuse_p; }
-    if (!std::strcmp(name, "fuse_gs")) { *lo = 0; *hi = 1; return &c->opt_fuse_gs; }
+    if (!std::strcmp(name, "fuse_gs")) { *lo = 0; *hi = 2; return &c->opt_fuse_gs; }
     if (!std::strcmp(name, "graph")) { *lo = 0; *hi = 2; return &c->opt_graph; }
     if (!std::strcmp(name, "pdl")) { *lo = 0; *hi = 3; return &c->opt_pdl; }
     if (!std::strcmp(name, "profile")) { *lo = 0; *hi = 1; return &c->opt_profile; }
@@ -485,6 +493,7 @@ int nk_pcg(nk_ctx *c, const double *f, double *x, int niter, double *res_hist, v
     cudaError_t e;
     NK_CUDA(ensure_dinv(c, st));
     c->p_pending = 0;
+    c->w_unsummed = 0;
     NK_CUDA(prof_mark(c, -1, st));
     NK_CUDA(nk_launch_pcg_init(c, f, x, res_hist, st));
     NK_CUDA(prof_mark(c, NK_K_INIT, st));

@@ -188,6 +188,7 @@ int nk_dist_iter_a(nk_ctx *c, void *stream)
 {
     if (!attached(c)) return NK_ERR_ARG;
     cudaStream_t st = S(stream);
+    c->w_unsummed = 0;
     // pap = sum over ALL ranks' elements of grad(p)^T G grad(p): element-local, so the rank totals just add
     NK_CUDA(with_raw(c, c->dist_send + c->dist_slots,
                      [&] { return nk_launch_ax_tma(c, nullptr, c->p, nullptr, c->w, 1, st); }));

@@ -22,7 +22,7 @@ inline size_t nk_align_up(size_t x, size_t a) { return (x + a - 1) / a * a; }
 inline bool nk_aligned16(const void *p) { return (reinterpret_cast<uintptr_t>(p) & 15u) == 0; }
 
 struct nk_carve {
-    size_t g, vec, code, off, idx, nbr, pk, tabs, partials, hist, scal, small, total;
+    size_t g, vec, code, off, idx, nbr, gx, pk, tabs, partials, hist, scal, small, total;
 };
 
 // Worst case: every local point listed in the gs plan (n_listed <= L, n_rows <= L).
@@ -35,6 +35,8 @@ inline nk_carve nk_carve_sizes(int64_t L)
     c.off = nk_align_up(((size_t)L + 1) * sizeof(int32_t), 256);
     c.idx = nk_align_up((size_t)L * sizeof(int32_t), 256);
     c.nbr = nk_align_up((size_t)L * sizeof(int32_t), 256);         // per-point gather code of the fused gs (nk_ctx::nbr)
+    // its side table: rows of 3 or more copies, at most 8 ints per 3 listed points (header + alignment),
+    c.gx = nk_align_up((9 * ((size_t)L / 3 + 1) + 16) * sizeof(int32_t), 256);   // + one int per such row (gx_rows)
     // packed rows (<= L indices + 16 padding ints per chunk) and 8 ints of descriptor per chunk
     c.pk = nk_align_up(((size_t)L + 24 * ((size_t)L / (2 * NK_GS_CHUNK) + 2) + 256) * sizeof(int32_t), 256);
     c.tabs = nk_align_up(2 * NK_CTAB * sizeof(double) + (16 * 16 + 16) * sizeof(double), 256);
@@ -42,7 +44,7 @@ inline nk_carve nk_carve_sizes(int64_t L)
     c.hist = nk_align_up(NK_HIST_MAX * sizeof(double), 256);
     c.scal = 256;
     c.small = 256;                                                // counter, errflag, res_dummy
-    c.total = c.g + 6 * c.vec + c.code + c.off + c.idx + c.nbr + c.pk + c.tabs + c.partials + c.hist + c.scal + c.small;
+    c.total = c.g + 6 * c.vec + c.code + c.off + c.idx + c.nbr + c.gx + c.pk + c.tabs + c.partials + c.hist + c.scal + c.small;
     return c;
 }
 

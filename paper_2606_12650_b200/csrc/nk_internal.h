@@ -22,6 +22,7 @@ enum { NK_EPI_STORE = 0,   // out[0] = total
 #define NK_CODE_MASKED 0x80u       // bit 7 of the per-point code: Dirichlet node
 #define NK_HIST_MAX 8192               // residual-history capacity of nk_cg_host
 #define NK_GRAPH_AUTO_MAX_L (1 << 24)   // "graph" = 2: nk_cg replays a CUDA graph up to this many local points
+#define NK_FUSE_GS_AUTO_MIN_L (1 << 21)  // "fuse_gs" = 2: gs rides in the residual update above this many local points
 #define NK_GS_CHUNK 32768          // rows per gs chunk (128 blocks of 256 threads)
 #define NK_CTAB 128                // code & 0x7f indexes ctab[] = 1/multiplicity
 
@@ -72,8 +73,11 @@ struct nk_ctx {
     //   nbr[l] == l   its node has no other copy (or only masked ones): the value stands
     //   nbr[l] >= 0   the ONE other copy of a node of multiplicity 2 (faces: 95 % of all shared points)
     //   nbr[l] == -1  Dirichlet node: the sum is replaced by 0
-    //   nbr[l] <= -2  CSR row -nbr[l]-2 lists all copies (edges, corners, irregular meshes)
-    int32_t *nbr;
+    //   nbr[l] <= -2  all copies of the node (edges, corners, irregular meshes) are listed in gx: with
+    //                 p = -nbr[l]-2, gx[4p-1] = their number and gx[4p ..] their local indices, ascending
+    //                 (16-byte aligned so that the first eight come with two vector loads)
+    int32_t *nbr, *gx, *gx_rows;   // gx_rows[k] = p of the k-th such node (one thread each in the fused kernel)
+    int64_t n_gx_rows;
     int64_t n_gs_chunks;
     double *ctab;                // NK_CTAB doubles: 1/multiplicity
     double *mtab;                // NK_CTAB doubles: multiplicity
@@ -147,8 +151,8 @@ cudaError_t nk_launch_gs(nk_ctx *c, double *v, int with_mask, cudaStream_t st);
 // nk_vec.cu
 cudaError_t nk_launch_dot(nk_ctx *c, const double *a, const double *b, double *out, int epi, cudaStream_t st);
 cudaError_t nk_launch_cg_init(nk_ctx *c, const double *f, double *x, double *hist, cudaStream_t st);
-// gs != 0: w is the UNSUMMED ax_e output and every point gathers the other copies of its node on the fly
-// (r -= alpha M Q Q^T w without gs ever writing w back); same values, bit for bit, as nk_launch_gs + gs == 0
+// gs != 0: w is the UNSUMMED ax_e output and the copies of shared nodes are summed on the fly (r -= alpha M Q Q^T w
+// without gs ever writing w back): r, x entry by entry as nk_launch_gs + gs == 0, rho' summed in another fixed order
 cudaError_t nk_launch_update_xr(nk_ctx *c, double *x, double *hist_k, int gs, cudaStream_t st);
 cudaError_t nk_launch_update_p(nk_ctx *c, cudaStream_t st);
 cudaError_t nk_launch_update_r(nk_ctx *c, double *hist_k, int gs, cudaStream_t st);     // r -= alpha w, rho'

@@ -146,7 +146,7 @@ int setup_impl(nk_ctx *c, const double *coords, const int64_t *glo_num, const do
     }
     if (pk.empty()) pk.push_back(0);
     // per-point gather codes of the fused gs (nk_internal.h nk_ctx::nbr)
-    std::vector<int32_t> nbr((size_t)L);
+    std::vector<int32_t> nbr((size_t)L), gx, gx_rows;
     for (int64_t l = 0; l < L; ++l) nbr[(size_t)l] = (int32_t)l;
     for (int64_t r = 0; r < n_sum_rows; ++r) {
         const Row &row = sum_rows[(size_t)r];
@@ -155,9 +155,19 @@ int setup_impl(nk_ctx *c, const double *coords, const int64_t *glo_num, const do
             nbr[a] = (int32_t)b;
             nbr[b] = (int32_t)a;
         } else {
-            for (uint32_t q = 0; q < row.len; ++q) nbr[loc[row.begin + q]] = (int32_t)(-r - 2);
+            while ((gx.size() + 1) % 4) gx.push_back(0);
+            gx.push_back((int32_t)row.len);
+            const int32_t p4 = (int32_t)(gx.size() / 4);
+            gx_rows.push_back(p4);
+            for (uint32_t q = 0; q < row.len; ++q) {
+                gx.push_back((int32_t)loc[row.begin + q]);
+                nbr[loc[row.begin + q]] = -p4 - 2;
+            }
         }
     }
+    gx.resize((gx.size() + 12 + 3) / 4 * 4, 0);              // vector loads of the last row stay in bounds; 16-byte multiple
+    c->n_gx_rows = (int64_t)gx_rows.size();
+    c->gx_rows = c->gx + gx.size();
     for (const Row &row : msk_rows)
         for (uint32_t q = 0; q < row.len; ++q) nbr[loc[row.begin + q]] = -1;
     c->n_gs_chunks = n_chunks;
@@ -174,6 +184,9 @@ int setup_impl(nk_ctx *c, const double *coords, const int64_t *glo_num, const do
         NK_CUDA(cudaMemcpyAsync(c->row_idx, idx.data(), (size_t)n_listed * sizeof(int32_t), cudaMemcpyHostToDevice, st));
     NK_CUDA(cudaMemcpyAsync(c->pk, pk.data(), pk.size() * sizeof(int32_t), cudaMemcpyHostToDevice, st));
     NK_CUDA(cudaMemcpyAsync(c->nbr, nbr.data(), (size_t)L * sizeof(int32_t), cudaMemcpyHostToDevice, st));
+    NK_CUDA(cudaMemcpyAsync(c->gx, gx.data(), gx.size() * sizeof(int32_t), cudaMemcpyHostToDevice, st));
+    if (!gx_rows.empty())
+        NK_CUDA(cudaMemcpyAsync(c->gx_rows, gx_rows.data(), gx_rows.size() * sizeof(int32_t), cudaMemcpyHostToDevice, st));
     NK_CUDA(cudaMemcpyAsync(c->gs_desc, desc.data(), desc.size() * sizeof(int32_t), cudaMemcpyHostToDevice, st));
     NK_CUDA(cudaMemcpyAsync(c->ctab, ctab, sizeof(ctab), cudaMemcpyHostToDevice, st));
     NK_CUDA(cudaMemcpyAsync(c->mtab, mtab, sizeof(mtab), cudaMemcpyHostToDevice, st));
@@ -219,7 +232,7 @@ extern "C" int nk_setup(nk_ctx **ctx, int64_t E, int N, const double *coords, co
     c->E = E; c->N = N; c->n = N + 1; c->P = (int64_t)c->n * c->n * c->n; c->L = L;
     c->device = dev; c->sm_count = sms;
     c->ws = workspace; c->ws_bytes = workspace_bytes;
-    c->opt_fuse_pap = 1; c->opt_fuse_p = 2; c->opt_fuse_gs = 1; c->opt_graph = 2; c->opt_pdl = 3; c->pdl_now = 0;
+    c->opt_fuse_pap = 1; c->opt_fuse_p = 2; c->opt_fuse_gs = 2; c->opt_graph = 2; c->opt_pdl = 3; c->pdl_now = 0;
     nk_host_basis(N, c->xi, c->wq, c->D);
     char *q = static_cast<char *>(workspace);
     c->g = reinterpret_cast<double2 *>(q); q += cv.g;
@@ -233,6 +246,7 @@ extern "C" int nk_setup(nk_ctx **ctx, int64_t E, int N, const double *coords, co
     c->row_off = reinterpret_cast<int32_t *>(q); q += cv.off;
     c->row_idx = reinterpret_cast<int32_t *>(q); q += cv.idx;
     c->nbr = reinterpret_cast<int32_t *>(q); q += cv.nbr;
+    c->gx = reinterpret_cast<int32_t *>(q); q += cv.gx;
     c->pk = reinterpret_cast<int32_t *>(q); q += cv.pk;
     c->ctab = reinterpret_cast<double *>(q); c->mtab = c->ctab + NK_CTAB; q += cv.tabs;
     c->red.partials = reinterpret_cast<double *>(q); q += cv.partials;

@@ -30,38 +30,6 @@ __device__ __forceinline__ void load_ctab(double *s_c, const double *ctab)
     __syncthreads();
 }
 
-// ---- gs folded into the residual update ("fuse_gs"; SURVEY 8(a) a2 + a3 + a5 in one pass) ---------------
-// Inside CG the summed w = M Q Q^T A_L p is read exactly once, by r -= alpha w (pap comes out of ax_e as a
-// quadratic form).  So w need never be summed IN PLACE: the update streams the UNSUMMED ax_e output and every
-// shared point gathers the other copies of its node on the fly.  gs's write-back (8 B per listed copy, 32 B
-// where the copy is alone in its sector: the stride-n r-faces), its re-read by the update and one launch per
-// iteration are gone; the gathered sectors are ones the streaming reads of neighbouring blocks fetch anyway.
-// Sums run in ascending local index, as in nk_gs.cu, so r and rho' are bitwise those of gs followed by the
-// plain update.
-struct nk_gather { const int32_t *nbr, *off, *idx; };
-
-// all copies of a node of multiplicity != 2 (edges, corners: 5 % of the shared points of a brick)
-__device__ __forceinline__ double gs_row_sum(const double *__restrict__ w, const int32_t *__restrict__ off,
-                                          const int32_t *__restrict__ idx, int row)
-{
-    const int b = off[row], e = off[row + 1];
-    double s = w[idx[b]];
-    for (int j = b + 1; j < e; ++j) s += w[idx[j]];
-    return s;
-}
-// the partner's value for a point of a multiplicity-2 node (predicated load, issued with the streaming loads)
-__device__ __forceinline__ double gs_partner(const double *__restrict__ w, int64_t l, int v)
-{
-    return (v >= 0 && (int64_t)v != l) ? w[v] : 0.0;
-}
-// (M Q Q^T w)_l from the point's own value wl, its gather code v = nbr[l] and the partner's value g
-__device__ __forceinline__ double gs_value(const double *__restrict__ w, const nk_gather &gp, int64_t l, int v, double wl, double g)
-{
-    if (v >= 0) return ((int64_t)v == l) ? wl : ((int64_t)v > l ? wl + g : g + wl);
-    if (v == -1) return 0.0;
-    return gs_row_sum(w, gp.off, gp.idx, -v - 2);
-}
-
 // out = <a,b>_c
 __global__ void __launch_bounds__(NK_VEC_THREADS)
 dot_kernel(const double *__restrict__ a, const double *__restrict__ b, const uint8_t *__restrict__ code,
@@ -121,12 +89,10 @@ cg_init_kernel(const double *__restrict__ f, double *__restrict__ x, double *__r
 }
 
 // x += alpha p; r -= alpha w; rho' = <r,r>_c          (S 8(a) a5: axpy, axpy and dot in one pass)
-// GS: w is the unsummed ax_e output; the sum over the copies and the mask are applied on the fly.
-template <bool GS>
-__global__ void __launch_bounds__(NK_VEC_THREADS, 2)
+__global__ void __launch_bounds__(NK_VEC_THREADS)
 update_xr_kernel(double *__restrict__ x, double *__restrict__ r, const double *__restrict__ p,
                  const double *__restrict__ w, const uint8_t *__restrict__ code,
-                 const double *__restrict__ ctab, int64_t L, nk_reduce_ws ws, double *hist_k, nk_gather gp)
+                 const double *__restrict__ ctab, int64_t L, nk_reduce_ws ws, double *hist_k)
 {
     __shared__ double s_c[NK_CTAB];
     __shared__ double s_red[33];
@@ -139,16 +105,10 @@ update_xr_kernel(double *__restrict__ x, double *__restrict__ r, const double *_
     double acc = 0.0;
     for (int64_t q = (int64_t)blockIdx.x * blockDim.x + threadIdx.x; q < pairs; q += stride) {
         const double2 pv = reinterpret_cast<const double2 *>(p)[q];
-        double2 wv = reinterpret_cast<const double2 *>(w)[q];
+        const double2 wv = reinterpret_cast<const double2 *>(w)[q];
         double2 xv = reinterpret_cast<double2 *>(x)[q];
         double2 rv = reinterpret_cast<double2 *>(r)[q];
         const uchar2 cd = reinterpret_cast<const uchar2 *>(code)[q];
-        if (GS) {
-            const int2 nv = reinterpret_cast<const int2 *>(gp.nbr)[q];
-            const double g0 = gs_partner(w, 2 * q, nv.x), g1 = gs_partner(w, 2 * q + 1, nv.y);
-            wv.x = gs_value(w, gp, 2 * q, nv.x, wv.x, g0);
-            wv.y = gs_value(w, gp, 2 * q + 1, nv.y, wv.y, g1);
-        }
         xv.x = fma(alpha, pv.x, xv.x);
         xv.y = fma(alpha, pv.y, xv.y);
         rv.x = fma(-alpha, wv.x, rv.x);
@@ -161,11 +121,193 @@ update_xr_kernel(double *__restrict__ x, double *__restrict__ r, const double *_
     if ((L & 1) && blockIdx.x == 0 && threadIdx.x == 0) {
         const int64_t l = L - 1;
         const double xv = fma(alpha, p[l], x[l]);
-        double wl = w[l];
-        if (GS) wl = gs_value(w, gp, l, gp.nbr[l], wl, gs_partner(w, l, gp.nbr[l]));
-        const double rv = fma(-alpha, wl, r[l]);
+        const double rv = fma(-alpha, w[l], r[l]);
         x[l] = xv; r[l] = rv;
         acc = fma(s_c[code[l] & 0x7f] * rv, rv, acc);
+    }
+    nk_grid_reduce(acc, s_red, ws, NK_EPI_RHO, hist_k);
+}
+
+// ---- gs and the mask folded into the residual update ("fuse_gs"; SURVEY 8(a) a2 + a3 + a5 in one pass) -------
+// Inside CG the summed w = M Q Q^T A_L p is read exactly once, by r -= alpha w (pap comes out of ax_e as a
+// quadratic form).  So w need never be summed IN PLACE: this kernel streams the UNSUMMED ax_e output and sums
+// the copies of shared nodes on the fly.  gs's write-back (8 B per listed copy, 32 B where the copy is alone in
+// its sector: the stride-n r-faces), its re-read by the update and one launch per iteration are gone.
+// Two kinds of blocks in one launch:
+//   * streaming blocks, one pass over all points.  A point whose node has no other copy keeps its value; a point
+//     of a multiplicity-2 node (faces: 82 % of the shared points of a brick) adds its ONE partner, whose index
+//     nbr[l] was fetched one step ahead so that the gather is issued together with the streaming loads (the
+//     sector it hits is one a neighbouring block streams anyway); a Dirichlet point takes 0; a point of a node
+//     with three or more copies (edges, corners) is SKIPPED;
+//   * row blocks, interleaved with the first streaming blocks of the grid (their chains of dependent loads run
+//     while the streaming blocks keep HBM busy): one thread per node with three or more copies gathers w and r of all its
+//     copies (indices by vector load from gx), sums in ascending local index as nk_gs.cu does, and updates r at
+//     every copy.  Inlined into the streaming loop this work cost two dependent memory round trips in nearly
+//     every warp (one edge point among 32 lanes is enough) and tripled the time of the pass.
+// r, x are the values of nk_gs followed by the plain update, entry by entry; rho' sums the same terms in another
+// (fixed) order.  Run-to-run bitwise reproducible like every reduction here.
+struct nk_gather {
+    const int32_t *nbr, *gx, *rows;     // nk_internal.h nk_ctx::nbr, gx; rows[k] = p of the k-th node with >= 3 copies
+    int n_rows, row_blocks;
+};
+
+__device__ __forceinline__ double gs_partner(const double *__restrict__ w, int l, int v)
+{
+    return (v >= 0 && v != l) ? w[v] : 0.0;
+}
+// value of (M Q Q^T w)_l for a streamed point: own / face partner / Dirichlet; `skip` for the row blocks' points
+__device__ __forceinline__ double gs_stream_value(int l, int v, double wl, double g, bool &skip)
+{
+    skip = v < -1;
+    const double sum = (v > l) ? wl + g : g + wl;            // ascending local index
+    return (v == l) ? wl : (v >= 0 ? sum : 0.0);
+}
+
+template <bool WITH_X>
+__global__ void __launch_bounds__(NK_VEC_THREADS, 2)
+gs_update_kernel(double *__restrict__ x, double *r, const double *__restrict__ p, const double *__restrict__ w,
+                 const uint8_t *__restrict__ code, const double *__restrict__ ctab, int64_t L, nk_reduce_ws ws,
+                 double *hist_k, nk_gather gp)
+{
+    __shared__ double s_c[NK_CTAB];
+    __shared__ double s_red[33];
+    nk_pdl_launch_dependents();
+    load_ctab(s_c, ctab);
+    double acc = 0.0;
+    // block roles: b < 2 R alternates stream / row, the rest streams (R = row blocks; the launcher keeps R <= stream blocks)
+    const int stream_blocks = (int)gridDim.x - gp.row_blocks;
+    const int b = (int)blockIdx.x;
+    const bool row_role = b < 2 * gp.row_blocks && (b & 1);
+    const int role_id = b < 2 * gp.row_blocks ? (b >> 1) : b - gp.row_blocks;
+    if (row_role) {
+        // ---- row blocks: nodes with three or more copies ------------------------------------------------------
+        const int k = role_id * NK_VEC_THREADS + threadIdx.x;
+        const bool on = k < gp.n_rows;
+        int p4 = 0, len = 0;
+        int4 ia = make_int4(0, 0, 0, 0);
+        if (on) {                                             // the plan is static: fetched before the wait
+            p4 = gp.rows[k];
+            ia = reinterpret_cast<const int4 *>(gp.gx)[p4];
+            len = gp.gx[4 * p4 - 1];
+        }
+        nk_pdl_wait();
+        const double alpha = ws.scal[NK_S_ALPHA];
+        if (on && len == 4) {                                 // an edge of a conforming hex mesh
+            const double a0 = w[ia.x], a1 = w[ia.y], a2 = w[ia.z], a3 = w[ia.w];
+            double r0 = r[ia.x], r1 = r[ia.y], r2 = r[ia.z], r3 = r[ia.w];
+            const double cw = s_c[code[ia.x] & 0x7f];
+            const double s = ((a0 + a1) + a2) + a3;
+            r0 = fma(-alpha, s, r0); r1 = fma(-alpha, s, r1); r2 = fma(-alpha, s, r2); r3 = fma(-alpha, s, r3);
+            r[ia.x] = r0; r[ia.y] = r1; r[ia.z] = r2; r[ia.w] = r3;
+            acc = fma(cw * r0, r0, acc); acc = fma(cw * r1, r1, acc);
+            acc = fma(cw * r2, r2, acc); acc = fma(cw * r3, r3, acc);
+        } else if (on) {
+            const int32_t *ii = gp.gx + 4 * (int64_t)p4;
+            double s = w[ii[0]];
+            for (int j = 1; j < len; ++j) s += w[ii[j]];
+            const double cw = s_c[code[ii[0]] & 0x7f];
+            for (int j = 0; j < len; ++j) {
+                const double rn = fma(-alpha, s, r[ii[j]]);
+                r[ii[j]] = rn;
+                acc = fma(cw * rn, rn, acc);
+            }
+        }
+    } else {
+        // ---- streaming blocks ------------------------------------------------------------------------------------
+        const int64_t pairs = L >> 1;
+        const int64_t bs = role_id;
+        const int64_t stride = (int64_t)stream_blocks * blockDim.x;
+        constexpr int U = WITH_X ? 1 : 2;                     // pairs per step, all loads before the stores
+        int64_t q = bs * blockDim.x + threadIdx.x;
+        int2 nv[U];
+#pragma unroll
+        for (int j = 0; j < U; ++j)                           // gather codes of the first step: static, before the wait
+            nv[j] = (q + j * stride < pairs) ? reinterpret_cast<const int2 *>(gp.nbr)[q + j * stride] : make_int2(0, 0);
+        nk_pdl_wait();
+        const double alpha = ws.scal[NK_S_ALPHA];
+        for (; q + (U - 1) * stride < pairs; q += U * stride) {
+            double2 wv[U], rv[U], g[U], xv[WITH_X ? U : 1], pv[WITH_X ? U : 1];
+            uchar2 cd[U];
+            int2 nn[U];
+#pragma unroll
+            for (int j = 0; j < U; ++j) {
+                const int64_t qj = q + j * stride;
+                wv[j] = reinterpret_cast<const double2 *>(w)[qj];
+                rv[j] = reinterpret_cast<const double2 *>(r)[qj];
+                cd[j] = reinterpret_cast<const uchar2 *>(code)[qj];
+                g[j].x = gs_partner(w, (int)(2 * qj), nv[j].x);
+                g[j].y = gs_partner(w, (int)(2 * qj) + 1, nv[j].y);
+                if (WITH_X) {
+                    xv[WITH_X ? j : 0] = reinterpret_cast<const double2 *>(x)[qj];
+                    pv[WITH_X ? j : 0] = reinterpret_cast<const double2 *>(p)[qj];
+                }
+            }
+#pragma unroll
+            for (int j = 0; j < U; ++j) {                     // next step's gather codes
+                const int64_t qn = q + (U + j) * stride;
+                nn[j] = (qn < pairs) ? reinterpret_cast<const int2 *>(gp.nbr)[qn] : make_int2(0, 0);
+            }
+#pragma unroll
+            for (int j = 0; j < U; ++j) {
+                const int64_t qj = q + j * stride;
+                const int l = (int)(2 * qj);
+                bool k0, k1;
+                const double s0 = gs_stream_value(l, nv[j].x, wv[j].x, g[j].x, k0);
+                const double s1 = gs_stream_value(l + 1, nv[j].y, wv[j].y, g[j].y, k1);
+                rv[j].x = fma(-alpha, s0, rv[j].x);
+                rv[j].y = fma(-alpha, s1, rv[j].y);
+                if (!(k0 || k1)) {
+                    reinterpret_cast<double2 *>(r)[qj] = rv[j];
+                } else {                                      // a row block owns the other entry of the pair
+                    if (!k0) r[l] = rv[j].x;
+                    if (!k1) r[l + 1] = rv[j].y;
+                }
+                acc = fma((k0 ? 0.0 : s_c[cd[j].x & 0x7f]) * rv[j].x, rv[j].x, acc);
+                acc = fma((k1 ? 0.0 : s_c[cd[j].y & 0x7f]) * rv[j].y, rv[j].y, acc);
+                if (WITH_X) {
+                    double2 xn = xv[WITH_X ? j : 0];
+                    xn.x = fma(alpha, pv[WITH_X ? j : 0].x, xn.x);
+                    xn.y = fma(alpha, pv[WITH_X ? j : 0].y, xn.y);
+                    reinterpret_cast<double2 *>(x)[qj] = xn;
+                }
+                nv[j] = nn[j];
+            }
+        }
+        for (; q < pairs; q += stride) {
+            const int2 n2 = reinterpret_cast<const int2 *>(gp.nbr)[q];
+            const double2 wv = reinterpret_cast<const double2 *>(w)[q];
+            double2 rv = reinterpret_cast<const double2 *>(r)[q];
+            const uchar2 cd = reinterpret_cast<const uchar2 *>(code)[q];
+            const int l = (int)(2 * q);
+            bool k0, k1;
+            const double s0 = gs_stream_value(l, n2.x, wv.x, gs_partner(w, l, n2.x), k0);
+            const double s1 = gs_stream_value(l + 1, n2.y, wv.y, gs_partner(w, l + 1, n2.y), k1);
+            rv.x = fma(-alpha, s0, rv.x);
+            rv.y = fma(-alpha, s1, rv.y);
+            if (!k0) r[l] = rv.x;
+            if (!k1) r[l + 1] = rv.y;
+            acc = fma((k0 ? 0.0 : s_c[cd.x & 0x7f]) * rv.x, rv.x, acc);
+            acc = fma((k1 ? 0.0 : s_c[cd.y & 0x7f]) * rv.y, rv.y, acc);
+            if (WITH_X) {
+                double2 xn = reinterpret_cast<const double2 *>(x)[q];
+                const double2 pv = reinterpret_cast<const double2 *>(p)[q];
+                xn.x = fma(alpha, pv.x, xn.x);
+                xn.y = fma(alpha, pv.y, xn.y);
+                reinterpret_cast<double2 *>(x)[q] = xn;
+            }
+        }
+        if ((L & 1) && bs == 0 && threadIdx.x == 0) {
+            const int l = (int)(L - 1);
+            const int v = gp.nbr[l];
+            bool k0;
+            const double s0 = gs_stream_value(l, v, w[l], gs_partner(w, l, v), k0);
+            if (!k0) {
+                const double rn = fma(-alpha, s0, r[l]);
+                r[l] = rn;
+                acc = fma(s_c[code[l] & 0x7f] * rn, rn, acc);
+            }
+            if (WITH_X) x[l] = fma(alpha, p[l], x[l]);
+        }
     }
     nk_grid_reduce(acc, s_red, ws, NK_EPI_RHO, hist_k);
 }
@@ -195,10 +337,9 @@ update_p_kernel(double *__restrict__ p, const double *__restrict__ r, const doub
 // r -= alpha w; rho' = <r,r>_c.  With update_px_kernel below this is the un-fused iteration's vector
 // work in 65 B/pt instead of 73: p is read once per iteration (by update_px, which still has the old
 // p in registers when x needs it) instead of twice.  Same arithmetic per entry as update_xr_kernel.
-template <bool GS>
-__global__ void __launch_bounds__(NK_VEC_THREADS, 2)
+__global__ void __launch_bounds__(NK_VEC_THREADS)
 update_r_kernel(double *__restrict__ r, const double *__restrict__ w, const uint8_t *__restrict__ code,
-                const double *__restrict__ ctab, int64_t L, nk_reduce_ws ws, double *hist_k, nk_gather gp)
+                const double *__restrict__ ctab, int64_t L, nk_reduce_ws ws, double *hist_k)
 {
     __shared__ double s_c[NK_CTAB];
     __shared__ double s_red[33];
@@ -209,39 +350,20 @@ update_r_kernel(double *__restrict__ r, const double *__restrict__ w, const uint
     const int64_t pairs = L >> 1;
     const int64_t stride = (int64_t)gridDim.x * blockDim.x;
     double acc = 0.0;
-    // U pairs per step, all loads before the stores (r is loaded and stored through one pointer, so the
-    // compiler will not overlap the next step's loads with this step's store on its own).  The order in
-    // which acc takes its terms -- q ascending by stride, .x before .y -- does not depend on U.
-    constexpr int U = GS ? 2 : 4;
+    // four pairs per step, all loads before the stores (r is loaded and stored through one pointer, so
+    // the compiler will not overlap the next step's loads with this step's store on its own)
     int64_t q = (int64_t)blockIdx.x * blockDim.x + threadIdx.x;
-    for (; q + (U - 1) * stride < pairs; q += U * stride) {
-        double2 wv[U], rv[U];
-        uchar2 cd[U];
-        int2 nv[U];
+    for (; q + 3 * stride < pairs; q += 4 * stride) {
+        double2 wv[4], rv[4];
+        uchar2 cd[4];
 #pragma unroll
-        for (int j = 0; j < U; ++j) {
-            if (GS) nv[j] = reinterpret_cast<const int2 *>(gp.nbr)[q + j * stride];
+        for (int j = 0; j < 4; ++j) {
             wv[j] = reinterpret_cast<const double2 *>(w)[q + j * stride];
             rv[j] = reinterpret_cast<double2 *>(r)[q + j * stride];
             cd[j] = reinterpret_cast<const uchar2 *>(code)[q + j * stride];
         }
-        if (GS) {
-            double2 g[U];
 #pragma unroll
-            for (int j = 0; j < U; ++j) {                 // the partners' values: 2 U independent gathers in flight
-                const int64_t l = 2 * (q + j * stride);
-                g[j].x = gs_partner(w, l, nv[j].x);
-                g[j].y = gs_partner(w, l + 1, nv[j].y);
-            }
-#pragma unroll
-            for (int j = 0; j < U; ++j) {
-                const int64_t l = 2 * (q + j * stride);
-                wv[j].x = gs_value(w, gp, l, nv[j].x, wv[j].x, g[j].x);
-                wv[j].y = gs_value(w, gp, l + 1, nv[j].y, wv[j].y, g[j].y);
-            }
-        }
-#pragma unroll
-        for (int j = 0; j < U; ++j) {
+        for (int j = 0; j < 4; ++j) {
             rv[j].x = fma(-alpha, wv[j].x, rv[j].x);
             rv[j].y = fma(-alpha, wv[j].y, rv[j].y);
             reinterpret_cast<double2 *>(r)[q + j * stride] = rv[j];
@@ -250,15 +372,9 @@ update_r_kernel(double *__restrict__ r, const double *__restrict__ w, const uint
         }
     }
     for (; q < pairs; q += stride) {
-        double2 wv = reinterpret_cast<const double2 *>(w)[q];
+        const double2 wv = reinterpret_cast<const double2 *>(w)[q];
         double2 rv = reinterpret_cast<double2 *>(r)[q];
         const uchar2 cd = reinterpret_cast<const uchar2 *>(code)[q];
-        if (GS) {
-            const int2 n2 = reinterpret_cast<const int2 *>(gp.nbr)[q];
-            const double g0 = gs_partner(w, 2 * q, n2.x), g1 = gs_partner(w, 2 * q + 1, n2.y);
-            wv.x = gs_value(w, gp, 2 * q, n2.x, wv.x, g0);
-            wv.y = gs_value(w, gp, 2 * q + 1, n2.y, wv.y, g1);
-        }
         rv.x = fma(-alpha, wv.x, rv.x);
         rv.y = fma(-alpha, wv.y, rv.y);
         reinterpret_cast<double2 *>(r)[q] = rv;
@@ -267,9 +383,7 @@ update_r_kernel(double *__restrict__ r, const double *__restrict__ w, const uint
     }
     if ((L & 1) && blockIdx.x == 0 && threadIdx.x == 0) {
         const int64_t l = L - 1;
-        double wl = w[l];
-        if (GS) wl = gs_value(w, gp, l, gp.nbr[l], wl, gs_partner(w, l, gp.nbr[l]));
-        const double rv = fma(-alpha, wl, r[l]);
+        const double rv = fma(-alpha, w[l], r[l]);
         r[l] = rv;
         acc = fma(s_c[code[l] & 0x7f] * rv, rv, acc);
     }
@@ -423,14 +537,34 @@ cudaError_t nk_launch_cg_init(nk_ctx *c, const double *f, double *x, double *his
     return cudaGetLastError();
 }
 
+namespace {
+// gs != 0: the fused kernel (gs_update_kernel).  It is a programmatic dependent only where gs itself would be
+// (nk_pdl_mode: its gathers want the L1 that ax_e's shared-memory carve-out takes away on large meshes).
+template <bool WITH_X>
+cudaError_t launch_gs_update(nk_ctx *c, double *x, double *hist_k, cudaStream_t st)
+{
+    nk_gather gp;
+    gp.nbr = c->nbr; gp.gx = c->gx; gp.rows = c->gx_rows;
+    gp.n_rows = (int)c->n_gx_rows;
+    gp.row_blocks = (int)((c->n_gx_rows + NK_VEC_THREADS - 1) / NK_VEC_THREADS);
+    int nbs = vec_blocks(c, c->L >> 1);
+    if (nbs < gp.row_blocks) nbs = gp.row_blocks;               // the kernel's role map wants stream blocks >= row blocks
+    const int nb = nbs + gp.row_blocks;
+    const cudaError_t e = nk_launch(gs_update_kernel<WITH_X>, nb, NK_VEC_THREADS, 0, st, c->pdl_now == 2, x, c->r,
+                                    (const double *)c->p, (const double *)c->w, (const uint8_t *)c->code,
+                                    (const double *)c->ctab, c->L, c->red, hist_k, gp);
+    if (e != cudaSuccess) return e;
+    c->launches++;
+    return cudaGetLastError();
+}
+}  // namespace
+
 cudaError_t nk_launch_update_xr(nk_ctx *c, double *x, double *hist_k, int gs, cudaStream_t st)
 {
+    if (gs) return launch_gs_update<true>(c, x, hist_k, st);
     const int nb = vec_blocks(c, c->L >> 1);
-    const nk_gather gp{c->nbr, c->row_off, c->row_idx};
-    // (with the gathers the kernel is a programmatic dependent only where gs itself would be: nk_pdl_mode)
-    const int pdl = gs ? (c->pdl_now == 2) : c->pdl_now;
-    const cudaError_t e = nk_launch(gs ? update_xr_kernel<true> : update_xr_kernel<false>, nb, NK_VEC_THREADS, 0, st, pdl,
-                                    x, c->r, c->p, c->w, c->code, c->ctab, c->L, c->red, hist_k, gp);
+    const cudaError_t e = nk_launch(update_xr_kernel, nb, NK_VEC_THREADS, 0, st, c->pdl_now, x, c->r, c->p, c->w, c->code,
+                                    c->ctab, c->L, c->red, hist_k);
     if (e != cudaSuccess) return e;
     c->launches++;
     return cudaGetLastError();
@@ -484,11 +618,10 @@ cudaError_t nk_launch_update_pz(nk_ctx *c, double *x, cudaStream_t st)
 
 cudaError_t nk_launch_update_r(nk_ctx *c, double *hist_k, int gs, cudaStream_t st)
 {
+    if (gs) return launch_gs_update<false>(c, nullptr, hist_k, st);
     const int nb = vec_blocks(c, c->L >> 1);
-    const nk_gather gp{c->nbr, c->row_off, c->row_idx};
-    const int pdl = gs ? (c->pdl_now == 2) : c->pdl_now;
-    const cudaError_t e = nk_launch(gs ? update_r_kernel<true> : update_r_kernel<false>, nb, NK_VEC_THREADS, 0, st, pdl,
-                                    c->r, c->w, c->code, c->ctab, c->L, c->red, hist_k, gp);
+    const cudaError_t e = nk_launch(update_r_kernel, nb, NK_VEC_THREADS, 0, st, c->pdl_now, c->r, c->w, c->code, c->ctab,
+                                    c->L, c->red, hist_k);
     if (e != cudaSuccess) return e;
     c->launches++;
     return cudaGetLastError();

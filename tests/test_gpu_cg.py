@@ -286,18 +286,32 @@ def test_cg_high_and_odd_orders(N):
 # ---- gs folded into the residual update ("fuse_gs") ------------------------------------------------------
 @pytest.mark.parametrize("name", ["config1", "config2", "config3"])
 @pytest.mark.parametrize("fuse_p", [0, 1])
-def test_fused_gs_is_bitwise_neutral(name, fuse_p):
-    """The residual update that gathers the copies of shared nodes from the unsummed ax_e output sums them in the
-    order nk_gs does and feeds the same reduction: x and the residual history are bitwise those of the separate
-    gs kernel, launch by launch or graphed, with or without programmatic dependent launches."""
+def test_fused_gs_against_separate_gs(name, fuse_p):
+    """The residual update that sums the copies of shared nodes from the unsummed ax_e output ("fuse_gs") gives,
+    for the same alpha, r and x entry by entry as the separate gs kernel does (same order of addition per node);
+    rho' adds the same terms in another fixed order, so the two solves agree to rounding (config 1 has converged
+    nine decades by iteration 40, where rounding differences have grown to a few 1e-13: bound 1e-11).  Each is bitwise reproducible, launch by launch or graphed, with or without programmatic
+    dependent launches."""
     import torch
     from paper_2606_12650_b200 import Nekbone
     from workloads import config_mesh
     mesh = config_mesh(name)
     gpu = Nekbone.from_mesh(mesh)
-    assert gpu.get_option("fuse_gs") == 1
+    assert gpu.get_option("fuse_gs") == 2
     gpu.set_option("fuse_p", fuse_p)
     f = to_dev(config_rhs(name, mesh))
+    # one iteration from the same state: r, x bitwise equal (rho' and beta, hence p, only to rounding)
+    state = {}
+    for fuse_gs in (0, 1):
+        gpu.set_option("fuse_gs", fuse_gs)
+        x = gpu.empty()
+        gpu.cg_init(f, x)
+        gpu.cg_step(x)
+        r, p, w = gpu.cg_get_state()
+        state[fuse_gs] = (x.clone(), r.clone(), w.clone(), gpu.scalars())
+    assert bool((state[0][0] == state[1][0]).all()) and bool((state[0][1] == state[1][1]).all())
+    assert bool((state[0][2] == state[1][2]).all())
+    assert abs(state[0][3]["rho_new"] - state[1][3]["rho_new"]) <= 1e-14 * abs(state[0][3]["rho_new"])
     out = {}
     for fuse_gs in (0, 1):
         for graph, pdl in ((0, 0), (0, 3), (1, 3)):
@@ -307,9 +321,14 @@ def test_fused_gs_is_bitwise_neutral(name, fuse_p):
             for rep in range(2):
                 out[fuse_gs, graph, pdl, rep] = gpu.cg(f, 40)
     torch.cuda.synchronize()
-    x0, h0 = out[0, 0, 0, 0]
-    for key, (x, h) in out.items():
-        assert bool((x == x0).all()) and bool((h == h0).all()), key
+    for fuse_gs in (0, 1):
+        x0, h0 = out[fuse_gs, 0, 0, 0]
+        for key, (x, h) in out.items():
+            if key[0] == fuse_gs:
+                assert bool((x == x0).all()) and bool((h == h0).all()), key
+    (xa, ha), (xb, hb) = out[0, 0, 0, 0], out[1, 0, 0, 0]
+    assert float(((ha - hb).abs() / ha).max()) <= 1e-11
+    assert elem_err(to_np(xb), to_np(xa), mesh.n ** 3) <= 1e-12
     gpu.close()
 
 
@@ -338,4 +357,3 @@ def test_fused_gs_on_irregular_ids():
             res[fuse_p, fuse_gs] = (to_np(xg), to_np(hg))
             assert np.all(np.abs(res[fuse_p, fuse_gs][1] - ho) <= TOL_CG * ho), (fuse_p, fuse_gs)
             assert elem_err(res[fuse_p, fuse_gs][0], xo, m.n ** 3) <= TOL_CG, (fuse_p, fuse_gs)
-        assert np.array_equal(res[fuse_p, 0][0], res[fuse_p, 1][0]) and np.array_equal(res[fuse_p, 0][1], res[fuse_p, 1][1])

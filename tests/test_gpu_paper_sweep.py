@@ -29,14 +29,14 @@ def test_residual_agrees_with_oracle(N, k):
         xo, ho = pr.orc.cg(f, 100)
         xg, hg = pr.gpu.cg(to_dev(f), 100)
         xg, hg = to_np(xg), to_np(hg)
-        if not np.all(np.abs(hg - ho) <= TOL_CG * ho):
+        if not (np.all(np.abs(hg - ho) <= TOL_CG * ho) and elem_err(xg, xo, pr.P) <= TOL_CG):
+            # the flat 1e-10 fails somewhere (tiny meshes past convergence; x along directions the residual
+            # norm barely sees): the oracle's own rounding band decides (R15)
             alts = oracle_variants(mesh, f, 100)
             ok, worst, kstar = history_parity(hg, ho, [h for _, h in alts])
             assert ok, (N, k, worst, kstar)
             assert kstar >= 10, (N, k, kstar)
-            assert elem_err(xg, xo, pr.P) <= max(TOL_CG, 10.0 * max(elem_err(xb, xo, pr.P) for xb, _ in alts))
-        else:
-            assert elem_err(xg, xo, pr.P) <= TOL_CG, (N, k)
+            assert elem_err(xg, xo, pr.P) <= max(TOL_CG, 10.0 * max(elem_err(xb, xo, pr.P) for xb, _ in alts)), (N, k)
         assert np.all(xg[mesh.mask == 0.0] == 0.0)
     finally:
         pr.close()
