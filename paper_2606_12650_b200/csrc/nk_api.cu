@@ -152,6 +152,16 @@ cudaError_t enqueue_cg(nk_ctx *c, const double *f, double *x, int niter, double 
     return cudaSuccess;
 }
 
+// The operator calls launch their kernels as programmatic dependents too (unless "pdl" = 0 or "profile"): every
+// kernel here executes griddepcontrol.wait before it touches a vector, so whatever precedes it on the stream --
+// one of ours or anybody's -- has completed and flushed by then; what overlaps is the launch latency and, in
+// ax_e, the producer warp's first bulk copies of the (static) geometric factors.
+struct pdl_call_scope {
+    nk_ctx *c;
+    explicit pdl_call_scope(nk_ctx *ctx) : c(ctx) { c->pdl_now = c->opt_profile ? 0 : nk_pdl_mode(c); }
+    ~pdl_call_scope() { c->pdl_now = 0; }
+};
+
 }  // namespace
 
 extern "C" {
@@ -159,6 +169,7 @@ extern "C" {
 int nk_ax_e(nk_ctx *c, const double *u, double *w, void *stream)
 {
     if (!c || !u || !w || u == w || !nk_aligned16(u) || !nk_aligned16(w)) return NK_ERR_ARG;
+    pdl_call_scope scope(c);
     NK_CUDA(prof_mark(c, -1, S(stream)));
     NK_CUDA(nk_launch_ax_tma(c, nullptr, u, nullptr, w, 0, S(stream)));
     NK_CUDA(prof_mark(c, NK_K_AX, S(stream)));
@@ -168,6 +179,7 @@ int nk_ax_e(nk_ctx *c, const double *u, double *w, void *stream)
 int nk_gs(nk_ctx *c, double *v, void *stream)
 {
     if (!c || !v || !nk_aligned16(v)) return NK_ERR_ARG;
+    pdl_call_scope scope(c);
     NK_CUDA(prof_mark(c, -1, S(stream)));
     NK_CUDA(nk_launch_gs(c, v, 0, S(stream)));
     NK_CUDA(prof_mark(c, NK_K_GS, S(stream)));
@@ -177,6 +189,7 @@ int nk_gs(nk_ctx *c, double *v, void *stream)
 int nk_ax(nk_ctx *c, const double *u, double *w, void *stream)
 {
     if (!c || !u || !w || u == w || !nk_aligned16(u) || !nk_aligned16(w)) return NK_ERR_ARG;
+    pdl_call_scope scope(c);
     NK_CUDA(prof_mark(c, -1, S(stream)));
     NK_CUDA(nk_launch_ax_tma(c, nullptr, u, nullptr, w, 0, S(stream)));
     NK_CUDA(prof_mark(c, NK_K_AX, S(stream)));
@@ -448,7 +461,8 @@ int nk_get_ax_launch(nk_ctx *c, int *batch_elements, int *ctas, int64_t *max_bat
     const int64_t grid = nb < (int64_t)c->sm_count ? nb : (int64_t)c->sm_count;
     if (batch_elements) *batch_elements = epb;
     if (ctas) *ctas = (int)grid;
-    if (max_batches_per_cta) *max_batches_per_cta = (nb + grid - 1) / grid;
+    // every CTA takes a contiguous range of floor or ceil(E / ctas) elements, in batches
+    if (max_batches_per_cta) *max_batches_per_cta = ((c->E + grid - 1) / grid + epb - 1) / epb;
     return NK_OK;
 }
 

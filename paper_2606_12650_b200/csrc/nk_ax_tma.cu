@@ -44,9 +44,39 @@ __host__ __device__ constexpr int eo_mat(int n) { return (n + 1) / 2 * eo_row(n)
 __host__ __device__ constexpr int eo_off(int n) { int s = 0; for (int q = 2; q < n; ++q) s += 2 * eo_mat(q); return s; }
 constexpr int D_TOTAL = eo_off(17);
 __constant__ double c_Dt[D_TOTAL];
+// which row and which column of its sync group a compute thread takes: offsets (doubles) from the group's first
+// cube, per order, [0] rows, [1] columns, indexed by the thread's index in the group (TmaCfg, line_tables)
+constexpr int LUT_MAX = 256;
+__constant__ uint16_t c_lut[NK_MAX_ORDER + 1][2][LUT_MAX];
 
 constexpr int SMEM_CAP = 232448 - 1024;     // 227 KB opt-in limit minus this kernel's static shared memory
 constexpr int BAR_BYTES = 1024;             // 2 x 64 mbarriers
+
+// plane padding (doubles) that spreads the starts of rows, n j + S2 k, and of columns, i + S2 k, most evenly over
+// the 16 eight-byte banks of a half-warp (0 .. 16 tried; ties go to the smaller cube)
+__host__ __device__ constexpr int plane_pad(int n)
+{
+    const int n2 = n * n, groups = (n2 + 15) / 16;
+    int best = 0, best_score = 1 << 30;
+    for (int pad = 0; pad <= 16; ++pad) {
+        const int S2 = n2 + pad;
+        int hr[16] = {}, hc[16] = {};
+        for (int k = 0; k < n; ++k)
+            for (int a = 0; a < n; ++a) { ++hr[(n * a + S2 * k) & 15]; ++hc[(a + S2 * k) & 15]; }
+        int mr = 0, mc = 0;
+        for (int b = 0; b < 16; ++b) { mr = hr[b] > mr ? hr[b] : mr; mc = hc[b] > mc ? hc[b] : mc; }
+        const int score = (mr > groups ? mr - groups : 0) + (mc > groups ? mc - groups : 0);
+        if (score < best_score) { best_score = score; best = pad; }
+    }
+    return best;
+}
+// cube padding with nw (se0 + pad) = n2 (mod 16), 0 if there is none
+__host__ __device__ constexpr int cube_pad(int nw, int se0, int n2)
+{
+    for (int pad = 0; pad < 16; ++pad)
+        if (((nw * (se0 + pad)) & 15) == (n2 & 15)) return pad;
+    return 0;
+}
 
 // elements per batch: ~256 compute threads, fewer where shared memory is the limit
 __host__ __device__ constexpr int tma_epb(int n)
@@ -54,8 +84,17 @@ __host__ __device__ constexpr int tma_epb(int n)
 #ifdef NK_TMA_EPB
     return NK_TMA_EPB;
 #else
-    return n <= 2 ? 32 : n == 3 ? 28 : n == 4 ? 16 : n == 5 ? 10 : n == 6 ? 7 : n == 7 ? 5 : n == 8 ? 4
-         : n == 9 ? 3 : n <= 12 ? 2 : 1;
+#ifndef NK_EPB_8
+#define NK_EPB_8 4
+#endif
+#ifndef NK_EPB_9
+#define NK_EPB_9 3
+#endif
+#ifndef NK_EPB_10
+#define NK_EPB_10 2
+#endif
+    return n <= 2 ? 32 : n == 3 ? 28 : n == 4 ? 16 : n == 5 ? 10 : n == 6 ? 7 : n == 7 ? 5 : n == 8 ? NK_EPB_8
+         : n == 9 ? NK_EPB_9 : n == 10 ? NK_EPB_10 : n <= 12 ? 2 : 1;
 #endif
 }
 
@@ -83,15 +122,24 @@ struct TmaCfg {
 #endif
     static constexpr int THREADS = CT + (WGP ? 128 : 32);     // + producer warp (or warpgroup)
     static_assert(EPB % SG == 0 && NG <= 15, "sync groups");
-    static constexpr int S1 = (n & 1) ? n : n + 1;            // odd row stride: conflict-free lines
-    static constexpr int S2 = n * S1, SE = n * S2;            // padded plane / cube (doubles)
+    // Shared-memory cube: rows dense (stride n), planes padded by PADK doubles, cubes by PADE.  A thread's pencil
+    // (i,j) then sits at its own thread index (+ k S2): consecutive lanes, consecutive doubles, never a bank
+    // conflict.  Rows (j,k) start at n j + S2 k and columns (i,k) at i + S2 k; PADK is chosen so that these starts
+    // spread evenly over the 16 eight-byte banks of a half-warp, and WHICH row / column a thread takes comes from a
+    // table (c_lut, built on the host by line_tables below) that gives every half-warp 16 different banks.  (The
+    // round-1 layout -- odd row stride, thread (a,b) takes row (a,b) -- had two-way conflicts on every pencil
+    // access for even n and on every column access for odd n: 29 % of all shared-memory wavefronts at n = 12.)
+    static constexpr int S1 = n;
+    static constexpr int PADK = plane_pad(n);
+    static constexpr int S2 = n2 + PADK;
+    static constexpr int SE0 = n * S2;
     // a ring stage holds KP k-planes of every element of the batch: whole elements for small n
     // (one bulk copy per batch), single k-planes otherwise (one bulk copy per element and plane)
     static constexpr int KP = (n <= 6) ? n : 1;            // (2 or 3 planes per stage at n = 12: measured 1.5 % slower)
     static constexpr int STAGE_D2 = EPB * KP * 3 * n2;        // double2 per stage
     static constexpr int STAGE_BYTES = STAGE_D2 * 16;
     static constexpr int SPB = n / KP;                        // stages per batch
-    static constexpr int work_bytes(int nw) { return nw * EPB * SE * 8; }
+    static constexpr int work_bytes(int nw) { return nw * EPB * (SE0 + 15) * 8; }   // (bound: SE = SE0 + PADE <= SE0 + 15)
     static constexpr int ring_for(int nw) { return (SMEM_CAP - BAR_BYTES - work_bytes(nw)) / STAGE_BYTES; }
     // three work arrays (4 barriers per batch) if the ring then still holds 1.5 batches, else two (6
     // barriers).  (At N = 11 the alternative -- three arrays and a 9-plane ring -- is 2 % faster for a
@@ -103,7 +151,11 @@ struct TmaCfg {
 #else
     static constexpr int R = RMAX > 64 ? 64 : RMAX;
 #endif
-    static constexpr int WORK_BYTES = work_bytes(NW);
+    // several slots per sync group: thread indices run on from slot to slot, so the slot stride NW SE continues
+    // the bank sequence where it can (NW SE = n^2 mod 16)
+    static constexpr int PADE = (SG > 1) ? cube_pad(NW, SE0, n2) : 0;
+    static constexpr int SE = SE0 + PADE;
+    static constexpr int WORK_BYTES = NW * EPB * SE * 8;
     static constexpr int SMEM = R * STAGE_BYTES + WORK_BYTES + BAR_BYTES;
     static_assert(R >= 2, "ring too small");
 #ifndef NK_TMA_IB
@@ -299,8 +351,11 @@ ax_tma_kernel(double *__restrict__ u_rw, const double *__restrict__ u_ro, const 
     }
     __syncthreads();
 
-    const int64_t nb = (E + EPB - 1) / EPB;
-    const int nit = (nb > (int64_t)blockIdx.x) ? (int)((nb - blockIdx.x + gridDim.x - 1) / gridDim.x) : 0;
+    // This CTA's elements: a contiguous range, equal over the CTAs to within one element (batches dealt round
+    // robin left the last round 1/4 full on a 16^3 mesh at N = 9: one batch time of 10 lost).  The last batch of
+    // a range may be partial.
+    const int64_t elo = E * (int64_t)blockIdx.x / gridDim.x, ehi = E * ((int64_t)blockIdx.x + 1) / gridDim.x;
+    const int nit = (int)((ehi - elo + EPB - 1) / EPB);
     double dsum = 0.0;
 
     if (C::WGP) {
@@ -313,8 +368,8 @@ ax_tma_kernel(double *__restrict__ u_rw, const double *__restrict__ u_ro, const 
             int stage = 0;
             uint32_t phase = 0;
             for (int it = 0; it < nit; ++it) {
-                const int64_t e0 = ((int64_t)blockIdx.x + (int64_t)it * gridDim.x) * EPB;
-                const int ne = (int)((E - e0 < EPB) ? (E - e0) : EPB);
+                const int64_t e0 = elo + (int64_t)it * EPB;
+                const int ne = (int)((ehi - e0 < EPB) ? (ehi - e0) : EPB);
 #pragma unroll 1
                 for (int ks = 0; ks < C::SPB; ++ks) {
                     mbar_wait(empty0 + 8 * stage, phase ^ 1u);
@@ -343,12 +398,13 @@ ax_tma_kernel(double *__restrict__ u_rw, const double *__restrict__ u_ro, const 
         const int a = t2 % n, b = t2 / n;
         const bool mapped = sl < SG;
         const int slot = grp * SG + (mapped ? sl : 0);
-        double *sA = work + (size_t)slot * NW * SE;     // u, then (NW = 2) the s direction
+        // work arrays of the sync group's first slot; slot s of the group sits s NW SE doubles further on
+        double *sA = work + (size_t)(grp * SG) * NW * SE;              // u, then (NW = 2) the s direction
         double *sB = sA + SE;                                          // r direction
         double *sC = (NW == 3) ? sB + SE : sA;                         // s direction
-        const int pbase = a + b * S1;                   // pencil (i,j) = (a,b): + k*S2
-        const int rbase = (a + n * b) * S1;             // row (j,k) = (a,b): + i
-        const int cbase = a + b * S2;                   // column (i,k) = (a,b): + j*S1
+        const int pbase = (mapped ? sl : 0) * NW * SE + t2;            // pencil (i,j) of the thread's slot: + k*S2
+        const int rbase = c_lut[N][0][lt];                             // a row (j,k) of the group: + i
+        const int cbase = c_lut[N][1][lt];                             // a column (i,k) of the group: + j*S1
         const double2 *gslot = ring + slot * KP * 3 * n2 + t2;
         nk_pdl_wait();                                  // u, r, beta come from the preceding kernels
         const double beta = FUSEP ? red.scal[NK_S_BETA] : 0.0;
@@ -357,8 +413,8 @@ ax_tma_kernel(double *__restrict__ u_rw, const double *__restrict__ u_ro, const 
 
         double nu[n], nr[FUSEP ? n : 1];               // next batch's pencil, in flight
         {
-            const int64_t e = (int64_t)blockIdx.x * EPB + slot;
-            const bool act = mapped && nit > 0 && e < E;
+            const int64_t e = elo + slot;
+            const bool act = mapped && e < ehi;
             const int64_t gb = act ? e * P + t2 : 0;
 #pragma unroll
             for (int k = 0; k < n; ++k) {
@@ -367,8 +423,8 @@ ax_tma_kernel(double *__restrict__ u_rw, const double *__restrict__ u_ro, const 
             }
         }
         for (int it = 0; it < nit; ++it) {
-            const int64_t e = ((int64_t)blockIdx.x + (int64_t)it * gridDim.x) * EPB + slot;
-            const bool active = mapped && e < E;
+            const int64_t e = elo + (int64_t)it * EPB + slot;
+            const bool active = mapped && e < ehi;
             const int64_t gbase = e * P + t2;
             double ru[n];
             // P1: pencil -> padded cube (and p = r + beta p written back)
@@ -441,8 +497,8 @@ ax_tma_kernel(double *__restrict__ u_rw, const double *__restrict__ u_ro, const 
             auto prefetch = [&]() {
                 // the next batch's pencil, in flight while this batch finishes (the register file is
                 // split four ways, so > 8 warps means <= 168 registers: not before P3, where pressure peaks)
-                const int64_t e1 = e + (int64_t)gridDim.x * EPB;
-                const bool act = mapped && it + 1 < nit && e1 < E;
+                const int64_t e1 = e + EPB;
+                const bool act = mapped && e1 < ehi;
                 const int64_t gb = act ? e1 * P + t2 : 0;
 #pragma unroll
                 for (int k = 0; k < n; ++k) {
@@ -501,6 +557,49 @@ cudaError_t launch_tma(nk_ctx *c, double *u_rw, const double *u_ro, const double
     return e != cudaSuccess ? e : cudaGetLastError();
 }
 
+// Row and column assignment of one order (TmaCfg: the layout it serves).  The lines of a sync group -- rows at
+// s NW SE + n j + S2 k, columns at s NW SE + i + S2 k, slot s of the group -- are dealt to the group's threads
+// half-warp by half-warp, each half-warp taking lines from the 16-bank residue classes that have most lines left:
+// 16 different banks as long as no class holds more lines than there are half-warps, which plane_pad arranges.
+template <int N>
+void line_tables(uint16_t (*lut)[LUT_MAX])
+{
+    using C = TmaCfg<N>;
+    constexpr int n = C::n, n2 = C::n2, lines = C::SG * n2;
+    static_assert(lines <= LUT_MAX && C::GTH <= LUT_MAX, "line table too small");
+    static_assert((C::SG - 1) * C::NW * C::SE + n * C::S2 < 65536, "line offsets exceed 16 bits");
+    for (int which = 0; which < 2; ++which) {
+        int start[LUT_MAX];
+        bool used[LUT_MAX] = {};
+        for (int s = 0; s < C::SG; ++s)
+            for (int k = 0; k < n; ++k)
+                for (int a = 0; a < n; ++a)
+                    start[(s * n + k) * n + a] = s * C::NW * C::SE + (which ? a : n * a) + C::S2 * k;
+        for (int t = 0; t < LUT_MAX; ++t) lut[which][t] = 0;
+        for (int h0 = 0; h0 < lines; h0 += 16) {
+            const int want = lines - h0 < 16 ? lines - h0 : 16;
+            bool bank_taken[16] = {};
+            for (int got = 0; got < want; ++got) {
+                int left[16] = {};
+                for (int q = 0; q < lines; ++q)
+                    if (!used[q]) ++left[start[q] & 15];
+                int bank = -1;
+                for (int b = 0; b < 16; ++b)
+                    if (left[b] > 0 && !bank_taken[b] && (bank < 0 || left[b] > left[bank])) bank = b;
+                if (bank < 0)                                   // every free bank is exhausted: accept a conflict
+                    for (int b = 0; b < 16; ++b)
+                        if (left[b] > 0 && (bank < 0 || left[b] > left[bank])) bank = b;
+                int pick = -1;
+                for (int q = 0; q < lines && pick < 0; ++q)
+                    if (!used[q] && (start[q] & 15) == bank) pick = q;
+                used[pick] = true;
+                bank_taken[bank] = true;
+                lut[which][h0 + got] = (uint16_t)start[pick];
+            }
+        }
+    }
+}
+
 template <int N>
 cudaError_t prepare_tma()
 {
@@ -538,6 +637,12 @@ cudaError_t nk_upload_D_tables_tma(void)
     }
     cudaError_t e = cudaMemcpyToSymbol(c_Dt, h, sizeof(h));
     if (e != cudaSuccess) return e;
+    static uint16_t lut[NK_MAX_ORDER + 1][2][LUT_MAX];
+#define NK_CASE(NN) line_tables<NN>(lut[NN]);
+    NK_CASE(1) NK_CASE(2) NK_CASE(3) NK_CASE(4) NK_CASE(5) NK_CASE(6) NK_CASE(7) NK_CASE(8)
+    NK_CASE(9) NK_CASE(10) NK_CASE(11) NK_CASE(12) NK_CASE(13) NK_CASE(14) NK_CASE(15)
+#undef NK_CASE
+    if ((e = cudaMemcpyToSymbol(c_lut, lut, sizeof(lut))) != cudaSuccess) return e;
 #define NK_CASE(NN) if ((e = prepare_tma<NN>()) != cudaSuccess) return e;
     NK_CASE(1) NK_CASE(2) NK_CASE(3) NK_CASE(4) NK_CASE(5) NK_CASE(6) NK_CASE(7) NK_CASE(8)
     NK_CASE(9) NK_CASE(10) NK_CASE(11) NK_CASE(12) NK_CASE(13) NK_CASE(14) NK_CASE(15)

@@ -66,7 +66,7 @@ constexpr int BPC = NK_GS_CHUNK / GS_THREADS;     // blocks per chunk
 __global__ void __launch_bounds__(GS_THREADS)
 gs_kernel(double *__restrict__ v, gs_plan pl, int with_mask)
 {
-    nk_pdl_launch_dependents();            // update_r may queue up behind us; this kernel itself is launched plainly
+    nk_pdl_launch_dependents();            // the next kernel may queue up behind us (we are a dependent ourselves in pdl mode 2)
     const int chunk = blockIdx.x / BPC;
     if (chunk < pl.n_chunks) {
         const int4 d = reinterpret_cast<const int4 *>(pl.desc)[2 * chunk];       // offset, n2, n4, n8
@@ -139,7 +139,8 @@ cudaError_t nk_launch_gs(nk_ctx *c, double *v, int with_mask, cudaStream_t st)
     pl.n_chunks = (int)c->n_gs_chunks;
     pl.n_sum_rows = (int)c->n_sum_rows; pl.n_rows = (int)c->n_rows;
     pl.masked_begin = (int)c->n_sum_listed; pl.n_listed = (int)c->n_listed;
-    // never a programmatic dependent: its blocks would land on SMs still carved out for ax_e's 227 KB of shared
+    // a programmatic dependent only in pdl mode 2 (the default up to 2^24 points, where the launch gap saved
+    // matters more): on large meshes its blocks would land on SMs still carved out for ax_e's 227 KB of shared
     // memory (L1 of ~1 KB) and the gathers would miss it (measured: +95 us at config 5)
     cudaError_t e = nk_launch(gs_kernel, (unsigned)nb, GS_THREADS, 0, st, c->pdl_now == 2, v, pl, with_mask);
     c->launches++;
