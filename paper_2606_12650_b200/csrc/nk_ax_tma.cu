@@ -46,7 +46,7 @@ constexpr int D_TOTAL = eo_off(17);
 __constant__ double c_Dt[D_TOTAL];
 // which row and which column of its sync group a compute thread takes: offsets (doubles) from the group's first
 // cube, per order, [0] rows, [1] columns, indexed by the thread's index in the group (TmaCfg, line_tables)
-constexpr int LUT_MAX = 256;
+constexpr int LUT_MAX = 384;
 __constant__ uint16_t c_lut[NK_MAX_ORDER + 1][2][LUT_MAX];
 
 constexpr int SMEM_CAP = 232448 - 1024;     // 227 KB opt-in limit minus this kernel's static shared memory
@@ -88,7 +88,7 @@ __host__ __device__ constexpr int tma_epb(int n)
 #define NK_EPB_8 4
 #endif
 #ifndef NK_EPB_9
-#define NK_EPB_9 3
+#define NK_EPB_9 4
 #endif
 #ifndef NK_EPB_10
 #define NK_EPB_10 2
@@ -105,7 +105,8 @@ struct TmaCfg {
     // Sync groups: the element slots of a batch that share one named barrier.  From n^2 >= 64 on every
     // slot is its own group of whole warps, so the elements of a batch drift apart and the
     // shared-memory-bound phases of one overlap the DFMA-bound phases of the other.
-    static constexpr int SG = (n == 8 || n == 10 || n == 11 || n == 12 || n == 16) ? 1 : EPB;   // slots per group
+    // (n = 9 with four slots of three warps each: 35.5 -> 34.0 us at 16^3, the one 4b point that was below 70 %)
+    static constexpr int SG = (n == 8 || n == 9 || n == 10 || n == 11 || n == 12 || n == 16) ? 1 : EPB;   // slots per group
     // (only where a slot fills whole warps well; elsewhere per-slot groups cost a warp and registers)
     static constexpr int NG = EPB / SG;                       // groups
     static constexpr int GTH = (SG * n2 + 31) / 32 * 32;      // threads per group
