@@ -158,6 +158,13 @@ int nk_dist_iter_c(nk_ctx *ctx, double *x, double *hist_k_dev, void *stream);
  *                  (the separate weighted dot reads the summed w); 0 = nk_gs as its own kernel; 2 (default)
  *                  = 1 for meshes of more than 2^21 local points (below, everything sits in L2 and the
  *                  separate kernel is faster), else 0.
+ *   "coop"         1 = nk_cg runs the whole solve as ONE cooperative launch: a persistent CTA per SM does all
+ *                  iterations (ax_e with pap and the p update folded in | grid barrier | x, r update with gs
+ *                  and the mask folded in, rho' | grid barrier), scalars never leave the chip.  For meshes
+ *                  that sit in L2, where launch gaps and kernel tails are most of an iteration.  Orders
+ *                  N <= 13; otherwise, and under "profile", the next rule applies.  Sums run in fixed but
+ *                  different orders than launch by launch: the two agree to rounding, each is bitwise
+ *                  reproducible.  0 = never; 2 (default) = 1 for meshes of up to 2^20 local points.
  *   "graph"        0 = nk_cg enqueues its launches one by one; 1 = records them into a CUDA graph
  *                  (cached per f, x, res_hist, niter; updated in place when the pointers change) and
  *                  replays it; 2 (default) = 1 for meshes of up to 2^24 local points, where launch gaps
@@ -200,7 +207,8 @@ int nk_get_kernel_times(nk_ctx *ctx, double *ms_host, int64_t *count_host, void 
 int nk_ax_batch_elements(int N);
 int nk_get_ax_launch(nk_ctx *ctx, int *batch_elements, int *ctas, int64_t *max_batches_per_cta);
 /* Which way nk_cg runs with the current options on this mesh: path 0 = its kernels enqueued one by one,
- * 1 = the same launches replayed as one CUDA graph; pdl_mode (may be NULL) = "pdl" resolved (0, 1 or 2). */
+ * 1 = the same launches replayed as one CUDA graph, 2 = one cooperative launch for the whole solve ("coop");
+ * pdl_mode (may be NULL) = "pdl" resolved (0, 1 or 2; paths 0 and 1). */
 int nk_get_cg_path(nk_ctx *ctx, int *path, int *pdl_mode);
 /* Kernel launches enqueued by this context so far (for bench.py's gpu_launches). */
 int nk_get_launch_count(nk_ctx *ctx, int64_t *count);

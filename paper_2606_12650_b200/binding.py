@@ -306,10 +306,11 @@ class Nekbone:
         _check(self._lib.nk_get_ax_launch(self._ctx, C.byref(e), C.byref(g), C.byref(b)))
         return dict(batch_elements=int(e.value), ctas=int(g.value), max_batches_per_cta=int(b.value))
 
-    CG_PATHS = ("launches", "graph")
+    CG_PATHS = ("launches", "graph", "cooperative")
 
     def solve_path(self) -> str:
-        """How nk_cg runs with the current options: "launches" (one by one) or "graph" (CUDA graph replay)."""
+        """How nk_cg runs with the current options: "launches" (one by one), "graph" (CUDA graph replay) or
+        "cooperative" (one persistent cooperative launch for the whole solve)."""
         v = _i()
         _check(self._lib.nk_get_cg_path(self._ctx, C.byref(v), None))
         return self.CG_PATHS[int(v.value)]

@@ -207,15 +207,24 @@ int nk_dot(nk_ctx *c, const double *a, const double *b, double *out, void *strea
 
 // "graph" = 2 (default): replay a CUDA graph where launch gaps matter (measured: config 2 3.8 -> 1.9 ms,
 // config 3 15.0 -> 13.0 ms per 100 iterations), enqueue directly on large meshes
+// "coop" = 2 (default): the whole solve as one cooperative launch on meshes that sit in L2, where an iteration is
+// a few microseconds of work and even a replayed graph of programmatic dependents costs 11-16 us per iteration
+static bool cg_uses_coop(const nk_ctx *c)
+{
+    return !c->opt_profile && c->coop_ok && nk_coop_supported(c->N) &&
+           (c->opt_coop == 1 || (c->opt_coop == 2 && c->L <= NK_COOP_AUTO_MAX_L));
+}
+
 static bool cg_uses_graph(const nk_ctx *c)
 {
-    return !c->opt_profile && (c->opt_graph == 1 || (c->opt_graph == 2 && c->L <= NK_GRAPH_AUTO_MAX_L));
+    return !c->opt_profile && !cg_uses_coop(c) &&
+           (c->opt_graph == 1 || (c->opt_graph == 2 && c->L <= NK_GRAPH_AUTO_MAX_L));
 }
 
 int nk_get_cg_path(nk_ctx *c, int *path, int *pdl_mode)
 {
     if (!c || !path) return NK_ERR_ARG;
-    *path = cg_uses_graph(c) ? 1 : 0;
+    *path = cg_uses_coop(c) ? 2 : cg_uses_graph(c) ? 1 : 0;
     if (pdl_mode) *pdl_mode = c->opt_profile ? 0 : nk_pdl_mode(c);
     return NK_OK;
 }
@@ -225,6 +234,12 @@ int nk_cg(nk_ctx *c, const double *f, double *x, int niter, double *res_hist, vo
     if (!c || !f || !x || !res_hist || niter < 0 || f == x || !nk_aligned16(f) || !nk_aligned16(x))
         return NK_ERR_ARG;
     cudaStream_t st = S(stream);
+    if (niter > 0 && cg_uses_coop(c)) {
+        NK_CUDA(nk_launch_cg_coop(c, f, x, niter, res_hist, st));
+        c->p_pending = 0;
+        c->w_unsummed = 1;
+        return NK_OK;
+    }
     const bool use_graph = niter > 0 && cg_uses_graph(c);
     if (!use_graph) {
         NK_CUDA(enqueue_cg(c, f, x, niter, res_hist, st));
@@ -361,6 +376,7 @@ static int *option_slot(nk_ctx *c, const char *name, int *lo, int *hi)
     if (!std::strcmp(name, "fuse_p")) { *lo = 0; *hi = 2; return &c->opt_fuse_p; }
     if (!std::strcmp(name, "fuse_gs")) { *lo = 0; *hi = 2; return &c->opt_fuse_gs; }
     if (!std::strcmp(name, "graph")) { *lo = 0; *hi = 2; return &c->opt_graph; }
+    if (!std::strcmp(name, "coop")) { *lo = 0; *hi = 2; return &c->opt_coop; }
     if (!std::strcmp(name, "pdl")) { *lo = 0; *hi = 3; return &c->opt_pdl; }
     if (!std::strcmp(name, "profile")) { *lo = 0; *hi = 1; return &c->opt_profile; }
     return nullptr;

@@ -329,215 +329,479 @@ __device__ __forceinline__ void lines_apply(const double (&ln)[NL][n], Store sto
     }
 }
 
-template <int N, bool FUSEP>
-__global__ void __launch_bounds__(TmaCfg<N>::THREADS, 1)
-ax_tma_kernel(double *__restrict__ u_rw, const double *__restrict__ u_ro, const double *__restrict__ r_in,
-              double *__restrict__ w, const double2 *__restrict__ g, int64_t E, int dot, nk_reduce_ws red)
+// ---- the two halves of one application of ax_e, as device functions ---------------------------------------
+// (ax_tma_kernel below runs them once; cg_coop_kernel once per CG iteration with the ring state carried over)
+struct RingState { int stage; uint32_t phase; };
+
+template <int N>
+struct AxSmem {                 // carve-up of the dynamic shared memory (the same in every kernel of this file)
+    using C = TmaCfg<N>;
+    const double2 *ring;
+    double *work;
+    uint32_t ring0, full0, empty0;
+    __device__ __forceinline__ explicit AxSmem(unsigned char *raw)
+    {
+        ring = reinterpret_cast<const double2 *>(raw);
+        work = reinterpret_cast<double *>(raw + (size_t)C::R * C::STAGE_BYTES);
+        ring0 = smem_u32(raw);
+        full0 = ring0 + C::R * C::STAGE_BYTES + C::WORK_BYTES;
+        empty0 = full0 + 8 * C::R;
+    }
+    __device__ __forceinline__ void init_barriers() const      // one thread, before the CTA's first barrier
+    {
+        for (int s = 0; s < C::R; ++s) { mbar_init(full0 + 8 * s, 1); mbar_init(empty0 + 8 * s, C::CW); }
+        asm volatile("fence.mbarrier_init.release.cluster;" ::: "memory");
+    }
+};
+
+// Producer lane: the geometric factors of elements [elo, ehi) into the ring, batch by batch.
+template <int N>
+__device__ __forceinline__ void ax_produce(const AxSmem<N> &sm, const double2 *__restrict__ g, int64_t elo, int64_t ehi,
+                                           RingState &rs)
+{
+    using C = TmaCfg<N>;
+    constexpr int n = C::n, n2 = C::n2, P = C::P, EPB = C::EPB, R = C::R, KP = C::KP;
+    const int nit = (int)((ehi - elo + EPB - 1) / EPB);
+    for (int it = 0; it < nit; ++it) {
+        const int64_t e0 = elo + (int64_t)it * EPB;
+        const int ne = (int)((ehi - e0 < EPB) ? (ehi - e0) : EPB);
+#pragma unroll 1
+        for (int ks = 0; ks < C::SPB; ++ks) {
+            mbar_wait(sm.empty0 + 8 * rs.stage, rs.phase ^ 1u);
+            const uint32_t fb = sm.full0 + 8 * rs.stage, dst = sm.ring0 + rs.stage * C::STAGE_BYTES;
+            if (KP == n) {       // whole elements: the batch is one contiguous chunk
+                mbar_expect_tx(fb, (uint32_t)ne * P * 48);
+                bulk_g2s(dst, g + nk_g_index(e0, 0, 0, 0, n), (uint32_t)ne * P * 48, fb);
+            } else {             // KP consecutive k-planes (contiguous in HBM) of every element of the batch
+                mbar_expect_tx(fb, (uint32_t)ne * KP * n2 * 48);
+                for (int q = 0; q < ne; ++q)
+                    bulk_g2s(dst + q * KP * n2 * 48, g + nk_g_index(e0 + q, ks * KP, 0, 0, n), KP * n2 * 48, fb);
+            }
+            if (++rs.stage == R) { rs.stage = 0; rs.phase ^= 1u; }
+        }
+    }
+}
+
+// vectors other SMs wrote earlier in the SAME launch (cg_coop_kernel) are read past the L1
+template <bool CG>
+__device__ __forceinline__ double ld_vec(const double *p) { return CG ? __ldcg(p) : *p; }
+
+// Compute warps: w = A_L u on elements [elo, ehi); returns the thread's share of sum_l u_l (A_L u)_l.
+// (u_rw, u_ro, r_in are what a predecessor wrote: no `const __restrict__` pair, or their loads could be hoisted
+//  above the caller's griddepcontrol.wait as invariant -- see nk_vec.cu.)
+// FUSEP: u = r_in + beta u is applied while loading and written back.  CG: see ld_vec.
+// No arithmetic below sits under a thread-dependent branch: D reaches the DFMAs through the uniform datapath
+// (LDCU -> UR operand), which ptxas only uses in warp-uniform code.  Threads without an element (ragged last
+// warp, tail batch) compute on stale shared memory and only their stores are predicated off.
+template <int N, bool FUSEP, bool CG>
+__device__ __forceinline__ double ax_compute(const AxSmem<N> &sm, double *u_rw, const double *u_ro,
+                                             const double *r_in, double *__restrict__ w, double beta,
+                                             int64_t elo, int64_t ehi, RingState &rs)
 {
     using C = TmaCfg<N>;
     constexpr int n = C::n, n2 = C::n2, P = C::P, S1 = C::S1, S2 = C::S2, SE = C::SE, EPB = C::EPB;
-    constexpr int R = C::R, KP = C::KP, NW = C::NW, CW = C::CW, CTHREADS = C::CT, GTH = C::GTH, SG = C::SG;
+    constexpr int R = C::R, KP = C::KP, NW = C::NW, GTH = C::GTH, SG = C::SG;
     constexpr int DOFF = eo_off(n), TOFF = DOFF + eo_mat(n);     // even-odd tables of D and D^T in c_Dt
+    const int tid = threadIdx.x;
+    const int lane = tid & 31;
+    const int grp = tid / GTH, lt = tid - grp * GTH;
+    const int sl = lt / n2, t2 = lt - sl * n2;
+    const bool mapped = sl < SG;
+    const int slot = grp * SG + (mapped ? sl : 0);
+    // work arrays of the sync group's first slot; slot s of the group sits s NW SE doubles further on
+    double *sA = sm.work + (size_t)(grp * SG) * NW * SE;           // u, then (NW = 2) the s direction
+    double *sB = sA + SE;                                          // r direction
+    double *sC = (NW == 3) ? sB + SE : sA;                         // s direction
+    const int pbase = (mapped ? sl : 0) * NW * SE + t2;            // pencil (i,j) of the thread's slot: + k*S2
+    const int rbase = c_lut[N][0][lt];                             // a row (j,k) of the group: + i
+    const int cbase = c_lut[N][1][lt];                             // a column (i,k) of the group: + j*S1
+    const double2 *gslot = sm.ring + slot * KP * 3 * n2 + t2;
+    const int nit = (int)((ehi - elo + EPB - 1) / EPB);
+    double dsum = 0.0;
+
+    double nu[n], nr[FUSEP ? n : 1];               // next batch's pencil, in flight
+    {
+        const int64_t e = elo + slot;
+        const bool act = mapped && e < ehi;
+        const int64_t gb = act ? e * P + t2 : 0;
+#pragma unroll
+        for (int k = 0; k < n; ++k) {
+            nu[k] = act ? ld_vec<CG>((FUSEP ? u_rw : u_ro) + gb + k * n2) : 0.0;
+            if (FUSEP) nr[k] = act ? ld_vec<CG>(r_in + gb + k * n2) : 0.0;
+        }
+    }
+    for (int it = 0; it < nit; ++it) {
+        const int64_t e = elo + (int64_t)it * EPB + slot;
+        const bool active = mapped && e < ehi;
+        const int64_t gbase = e * P + t2;
+        double ru[n];
+        // P1: pencil -> padded cube (and p = r + beta p written back)
+#pragma unroll
+        for (int k = 0; k < n; ++k) ru[k] = FUSEP ? fma(beta, nu[k], nr[k]) : nu[k];
+        if (mapped) {
+#pragma unroll
+            for (int k = 0; k < n; ++k) sA[pbase + k * S2] = ru[k];
+        }
+        if (FUSEP && active) {
+#pragma unroll
+            for (int k = 0; k < n; ++k) u_rw[gbase + k * n2] = ru[k];
+        }
+        group_sync<GTH>(grp);
+        // P2: D along the thread's row (A -> B), column (A -> C) and pencil (registers -> wt), one pass
+        double wt[n];
+        {
+            double ln[3][n], cres[NW == 2 ? n : 1];
+#pragma unroll
+            for (int m = 0; m < n; ++m) {
+                ln[0][m] = sA[rbase + m];
+                ln[1][m] = sA[cbase + m * S1];
+                ln[2][m] = ru[m];
+            }
+            lines_apply<n, DOFF, 3, C::IB>(ln, [&](int q, int i, double v) {
+                if (q == 0) { if (mapped) sB[rbase + i] = v; }
+                else if (q == 1) { if (NW == 2) cres[NW == 2 ? i : 0] = v; else if (mapped) sC[cbase + i * S1] = v; }
+                else wt[i] = v;
+            });
+            if (NW == 2) {                          // columns overwrite A in place: all reads of A are done
+                group_sync<GTH>(grp);
+                if (mapped) {
+#pragma unroll
+                    for (int j = 0; j < n; ++j) sC[cbase + j * S1] = cres[j];
+                }
+            }
+        }
+        group_sync<GTH>(grp);
+        // P3: the geometric factors from the ring, point by point along the pencil
+        {
+            // a stage (KP planes) is waited for when its first plane comes up and handed back after its
+            // last one.  (Waiting for several stages at once was tried and is slower: the register
+            // pressure of interleaved planes costs more than the waits.)
+            double dloc = 0.0;
+#pragma unroll
+            for (int k = 0; k < n; ++k) {
+                if (k % KP == 0) mbar_wait_warp(sm.full0 + 8 * rs.stage, rs.phase);
+                const double2 *gs = gslot + (size_t)rs.stage * C::STAGE_D2 + (k % KP) * 3 * n2;
+                const double2 ga = gs[0], gb = gs[n2], gc = gs[2 * n2];
+                const double ur = sB[pbase + k * S2], us = sC[pbase + k * S2], ut = wt[k];
+                const double wr = fma(ga.x, ur, fma(ga.y, us, gb.x * ut));  // w_r = rr ur + rs us + rt ut
+                const double ws = fma(ga.y, ur, fma(gb.y, us, gc.x * ut));  // w_s = rs ur + ss us + st ut
+                const double wk = fma(gb.x, ur, fma(gc.x, us, gc.y * ut));  // w_t = rt ur + st us + tt ut
+                if (mapped) {
+                    sB[pbase + k * S2] = wr;
+                    sC[pbase + k * S2] = ws;
+                }
+                wt[k] = wk;
+                // <u, A_L u> = sum over points of grad(u)^T G grad(u): the fused pap needs no u later on
+                dloc += fma(ur, wr, fma(us, ws, ut * wk));
+                if (k % KP == KP - 1) {          // this warp is done with the stage: hand it back
+                    __syncwarp();
+                    if (lane == 0) mbar_arrive(sm.empty0 + 8 * rs.stage);
+                    if (++rs.stage == R) { rs.stage = 0; rs.phase ^= 1u; }
+                }
+            }
+            dsum += active ? dloc : 0.0;        // threads without an element computed on stale data
+        }
+        group_sync<GTH>(grp);
+        auto prefetch = [&]() {
+            // the next batch's pencil, in flight while this batch finishes (the register file is
+            // split four ways, so > 8 warps means <= 168 registers: not before P3, where pressure peaks)
+            const int64_t e1 = e + EPB;
+            const bool act = mapped && e1 < ehi;
+            const int64_t gb = act ? e1 * P + t2 : 0;
+#pragma unroll
+            for (int k = 0; k < n; ++k) {
+                nu[k] = act ? ld_vec<CG>((FUSEP ? u_rw : u_ro) + gb + k * n2) : 0.0;
+                if (FUSEP) nr[k] = act ? ld_vec<CG>(r_in + gb + k * n2) : 0.0;
+            }
+        };
+        if (C::PF == 1) prefetch();
+        // P4: D^T along the row (B in place), the column (C in place) and the pencil (wt -> rw), one pass
+        double rw[n];
+        {
+            double ln[3][n];
+#pragma unroll
+            for (int m = 0; m < n; ++m) {
+                ln[0][m] = sB[rbase + m];
+                ln[1][m] = sC[cbase + m * S1];
+                ln[2][m] = wt[m];
+            }
+            lines_apply<n, TOFF, 3, C::IB>(ln, [&](int q, int i, double v) {
+                if (q == 0) { if (mapped) sB[rbase + i] = v; }
+                else if (q == 1) { if (mapped) sC[cbase + i * S1] = v; }
+                else rw[i] = v;
+            });
+        }
+        group_sync<GTH>(grp);
+        if (C::PF == 2) prefetch();
+        // P5: sum the three directions, store
+#pragma unroll
+        for (int k = 0; k < n; ++k) {
+            const double wv = rw[k] + (sB[pbase + k * S2] + sC[pbase + k * S2]);
+            if (active) w[gbase + k * n2] = wv;
+        }
+        // (no barrier here even when C aliases A: P5 reads and the next P1 writes the same pencil
+        //  positions, by the same thread)
+        if (C::PF == 0) prefetch();
+    }
+    return dsum;
+}
+
+template <int N, bool FUSEP>
+__global__ void __launch_bounds__(TmaCfg<N>::THREADS, 1)
+ax_tma_kernel(double *u_rw, const double *u_ro, const double *r_in,
+              double *__restrict__ w, const double2 *__restrict__ g, int64_t E, int dot, nk_reduce_ws red)
+{
+    using C = TmaCfg<N>;
     extern __shared__ __align__(128) unsigned char smem_raw[];
     __shared__ double s_red[33];
-    const double2 *ring = reinterpret_cast<const double2 *>(smem_raw);
-    double *work = reinterpret_cast<double *>(smem_raw + (size_t)R * C::STAGE_BYTES);
-    const uint32_t ring0 = smem_u32(smem_raw);
-    const uint32_t full0 = ring0 + R * C::STAGE_BYTES + C::WORK_BYTES, empty0 = full0 + 8 * R;
-
+    const AxSmem<N> sm(smem_raw);
     const int tid = threadIdx.x;
-    if (tid == 0) {
-        for (int s = 0; s < R; ++s) { mbar_init(full0 + 8 * s, 1); mbar_init(empty0 + 8 * s, CW); }
-        asm volatile("fence.mbarrier_init.release.cluster;" ::: "memory");
-    }
+    if (tid == 0) sm.init_barriers();
     __syncthreads();
 
     // This CTA's elements: a contiguous range, equal over the CTAs to within one element (batches dealt round
     // robin left the last round 1/4 full on a 16^3 mesh at N = 9: one batch time of 10 lost).  The last batch of
     // a range may be partial.
     const int64_t elo = E * (int64_t)blockIdx.x / gridDim.x, ehi = E * ((int64_t)blockIdx.x + 1) / gridDim.x;
-    const int nit = (int)((ehi - elo + EPB - 1) / EPB);
     double dsum = 0.0;
-
     if (C::WGP) {
-        if (tid >= CTHREADS) asm volatile("setmaxnreg.dec.sync.aligned.u32 24;");
+        if (tid >= C::CT) asm volatile("setmaxnreg.dec.sync.aligned.u32 24;");
         else asm volatile("setmaxnreg.inc.sync.aligned.u32 240;");
     }
-    if (tid >= CTHREADS) {
-        // ---- producer warp: one lane streams G into the ring ----------------------------------------
-        if (tid == CTHREADS) {
-            int stage = 0;
-            uint32_t phase = 0;
-            for (int it = 0; it < nit; ++it) {
-                const int64_t e0 = elo + (int64_t)it * EPB;
-                const int ne = (int)((ehi - e0 < EPB) ? (ehi - e0) : EPB);
-#pragma unroll 1
-                for (int ks = 0; ks < C::SPB; ++ks) {
-                    mbar_wait(empty0 + 8 * stage, phase ^ 1u);
-                    const uint32_t fb = full0 + 8 * stage, dst = ring0 + stage * C::STAGE_BYTES;
-                    if (KP == n) {       // whole elements: the batch is one contiguous chunk
-                        mbar_expect_tx(fb, (uint32_t)ne * P * 48);
-                        bulk_g2s(dst, g + nk_g_index(e0, 0, 0, 0, n), (uint32_t)ne * P * 48, fb);
-                    } else {             // KP consecutive k-planes (contiguous in HBM) of every element of the batch
-                        mbar_expect_tx(fb, (uint32_t)ne * KP * n2 * 48);
-                        for (int q = 0; q < ne; ++q)
-                            bulk_g2s(dst + q * KP * n2 * 48, g + nk_g_index(e0 + q, ks * KP, 0, 0, n), KP * n2 * 48, fb);
-                    }
-                    if (++stage == R) { stage = 0; phase ^= 1u; }
-                }
-            }
-        }
+    RingState rs{0, 0u};
+    if (tid >= C::CT) {
+        // ---- producer warp: one lane streams G into the ring (static data: no need to wait for the predecessor)
+        if (tid == C::CT) ax_produce<N>(sm, g, elo, ehi, rs);
     } else {
-        // ---- compute warps ----------------------------------------------------------------------------
-        // No arithmetic below sits under a thread-dependent branch: D reaches the DFMAs through the
-        // uniform datapath (LDCU -> UR operand), which ptxas only uses in warp-uniform code.  Threads
-        // without an element (ragged last warp, tail batch) compute on stale shared memory and only
-        // their stores are predicated off.
-        const int lane = tid & 31;
-        const int grp = tid / GTH, lt = tid - grp * GTH;
-        const int sl = lt / n2, t2 = lt - sl * n2;
-        const int a = t2 % n, b = t2 / n;
-        const bool mapped = sl < SG;
-        const int slot = grp * SG + (mapped ? sl : 0);
-        // work arrays of the sync group's first slot; slot s of the group sits s NW SE doubles further on
-        double *sA = work + (size_t)(grp * SG) * NW * SE;              // u, then (NW = 2) the s direction
-        double *sB = sA + SE;                                          // r direction
-        double *sC = (NW == 3) ? sB + SE : sA;                         // s direction
-        const int pbase = (mapped ? sl : 0) * NW * SE + t2;            // pencil (i,j) of the thread's slot: + k*S2
-        const int rbase = c_lut[N][0][lt];                             // a row (j,k) of the group: + i
-        const int cbase = c_lut[N][1][lt];                             // a column (i,k) of the group: + j*S1
-        const double2 *gslot = ring + slot * KP * 3 * n2 + t2;
         nk_pdl_wait();                                  // u, r, beta come from the preceding kernels
         const double beta = FUSEP ? red.scal[NK_S_BETA] : 0.0;
-        int stage = 0;
-        uint32_t phase = 0;
-
-        double nu[n], nr[FUSEP ? n : 1];               // next batch's pencil, in flight
-        {
-            const int64_t e = elo + slot;
-            const bool act = mapped && e < ehi;
-            const int64_t gb = act ? e * P + t2 : 0;
-#pragma unroll
-            for (int k = 0; k < n; ++k) {
-                nu[k] = act ? (FUSEP ? u_rw[gb + k * n2] : u_ro[gb + k * n2]) : 0.0;
-                if (FUSEP) nr[k] = act ? r_in[gb + k * n2] : 0.0;
-            }
-        }
-        for (int it = 0; it < nit; ++it) {
-            const int64_t e = elo + (int64_t)it * EPB + slot;
-            const bool active = mapped && e < ehi;
-            const int64_t gbase = e * P + t2;
-            double ru[n];
-            // P1: pencil -> padded cube (and p = r + beta p written back)
-#pragma unroll
-            for (int k = 0; k < n; ++k) ru[k] = FUSEP ? fma(beta, nu[k], nr[k]) : nu[k];
-            if (mapped) {
-#pragma unroll
-                for (int k = 0; k < n; ++k) sA[pbase + k * S2] = ru[k];
-            }
-            if (FUSEP && active) {
-#pragma unroll
-                for (int k = 0; k < n; ++k) u_rw[gbase + k * n2] = ru[k];
-            }
-            group_sync<GTH>(grp);
-            // P2: D along the thread's row (A -> B), column (A -> C) and pencil (registers -> wt), one pass
-            double wt[n];
-            {
-                double ln[3][n], cres[NW == 2 ? n : 1];
-#pragma unroll
-                for (int m = 0; m < n; ++m) {
-                    ln[0][m] = sA[rbase + m];
-                    ln[1][m] = sA[cbase + m * S1];
-                    ln[2][m] = ru[m];
-                }
-                lines_apply<n, DOFF, 3, C::IB>(ln, [&](int q, int i, double v) {
-                    if (q == 0) { if (mapped) sB[rbase + i] = v; }
-                    else if (q == 1) { if (NW == 2) cres[NW == 2 ? i : 0] = v; else if (mapped) sC[cbase + i * S1] = v; }
-                    else wt[i] = v;
-                });
-                if (NW == 2) {                          // columns overwrite A in place: all reads of A are done
-                    group_sync<GTH>(grp);
-                    if (mapped) {
-#pragma unroll
-                        for (int j = 0; j < n; ++j) sC[cbase + j * S1] = cres[j];
-                    }
-                }
-            }
-            group_sync<GTH>(grp);
-            // P3: the geometric factors from the ring, point by point along the pencil
-            {
-                // a stage (KP planes) is waited for when its first plane comes up and handed back after its
-                // last one.  (Waiting for several stages at once was tried and is slower: the register
-                // pressure of interleaved planes costs more than the waits.)
-                double dloc = 0.0;
-#pragma unroll
-                for (int k = 0; k < n; ++k) {
-                    if (k % KP == 0) mbar_wait_warp(full0 + 8 * stage, phase);
-                    const double2 *gs = gslot + (size_t)stage * C::STAGE_D2 + (k % KP) * 3 * n2;
-                    const double2 ga = gs[0], gb = gs[n2], gc = gs[2 * n2];
-                    const double ur = sB[pbase + k * S2], us = sC[pbase + k * S2], ut = wt[k];
-                    const double wr = fma(ga.x, ur, fma(ga.y, us, gb.x * ut));  // w_r = rr ur + rs us + rt ut
-                    const double ws = fma(ga.y, ur, fma(gb.y, us, gc.x * ut));  // w_s = rs ur + ss us + st ut
-                    const double wk = fma(gb.x, ur, fma(gc.x, us, gc.y * ut));  // w_t = rt ur + st us + tt ut
-                    if (mapped) {
-                        sB[pbase + k * S2] = wr;
-                        sC[pbase + k * S2] = ws;
-                    }
-                    wt[k] = wk;
-                    // <u, A_L u> = sum over points of grad(u)^T G grad(u): the fused pap needs no u later on
-                    dloc += fma(ur, wr, fma(us, ws, ut * wk));
-                    if (k % KP == KP - 1) {          // this warp is done with the stage: hand it back
-                        __syncwarp();
-                        if (lane == 0) mbar_arrive(empty0 + 8 * stage);
-                        if (++stage == R) { stage = 0; phase ^= 1u; }
-                    }
-                }
-                dsum += active ? dloc : 0.0;        // threads without an element computed on stale data
-            }
-            group_sync<GTH>(grp);
-            auto prefetch = [&]() {
-                // the next batch's pencil, in flight while this batch finishes (the register file is
-                // split four ways, so > 8 warps means <= 168 registers: not before P3, where pressure peaks)
-                const int64_t e1 = e + EPB;
-                const bool act = mapped && e1 < ehi;
-                const int64_t gb = act ? e1 * P + t2 : 0;
-#pragma unroll
-                for (int k = 0; k < n; ++k) {
-                    nu[k] = act ? (FUSEP ? u_rw[gb + k * n2] : u_ro[gb + k * n2]) : 0.0;
-                    if (FUSEP) nr[k] = act ? r_in[gb + k * n2] : 0.0;
-                }
-            };
-            if (C::PF == 1) prefetch();
-            // P4: D^T along the row (B in place), the column (C in place) and the pencil (wt -> rw), one pass
-            double rw[n];
-            {
-                double ln[3][n];
-#pragma unroll
-                for (int m = 0; m < n; ++m) {
-                    ln[0][m] = sB[rbase + m];
-                    ln[1][m] = sC[cbase + m * S1];
-                    ln[2][m] = wt[m];
-                }
-                lines_apply<n, TOFF, 3, C::IB>(ln, [&](int q, int i, double v) {
-                    if (q == 0) { if (mapped) sB[rbase + i] = v; }
-                    else if (q == 1) { if (mapped) sC[cbase + i * S1] = v; }
-                    else rw[i] = v;
-                });
-            }
-            group_sync<GTH>(grp);
-            if (C::PF == 2) prefetch();
-            // P5: sum the three directions, store
-#pragma unroll
-            for (int k = 0; k < n; ++k) {
-                const double wv = rw[k] + (sB[pbase + k * S2] + sC[pbase + k * S2]);
-                if (active) w[gbase + k * n2] = wv;
-            }
-            // (no barrier here even when C aliases A: P5 reads and the next P1 writes the same pencil
-            //  positions, by the same thread)
-            if (C::PF == 0) prefetch();
-        }
+        dsum = ax_compute<N, FUSEP, false>(sm, u_rw, u_ro, r_in, w, beta, elo, ehi, rs);
     }
     if (dot) nk_grid_reduce(dsum, s_red, red, NK_EPI_PAP, nullptr);
+}
+
+// ---- the whole CG solve as ONE cooperative launch (small, L2-resident meshes) ------------------------------
+// (S 8(f) f-1 "or a persistent cooperative kernel"; PAPER.md:320 performance only saturates from 4e6 DOFs on,
+// PAPER.md:328 per-call overhead separates the implementations below that.)  On meshes that fit in L2 an
+// iteration is a few microseconds of work; launched kernel by kernel -- even as a CUDA graph of programmatic
+// dependents -- it costs 11-16 us.  Here one persistent CTA per SM runs all `niter` iterations: per iteration
+//   phase A  ax_e on the CTA's elements with p = r + beta p folded into the load and pap as the quadratic form
+//   -- grid barrier; every CTA adds the per-CTA pap partials in the same order: alpha --
+//   phase B  on the CTA's share of the points: x += alpha p; r -= alpha (M Q Q^T w), the copies of shared nodes
+//            gathered on the fly from the unsummed w (nk_ctx::nbr, gx); rho' partial
+//   -- grid barrier; every CTA adds the rho' partials in the same order: beta, residual history --
+// Two barriers per iteration (hand-written: one monotone counter in global memory, arrive = atomicAdd, wait =
+// ld.acquire until the count reaches blocks x barriers passed).  The producer warp never joins a barrier: the
+// geometric factors are static, so it streams the NEXT iteration's first batches into the ring while the compute
+// warps are in phase B -- the ring is full when phase A starts.  Vectors another SM may have written during the
+// launch are read past the L1 (ld.global.cg).  Sums are deterministic (fixed ranges, fixed trees); the order
+// differs from the launch-by-launch path, so the two agree to rounding, not bitwise.
+struct nk_coop_args {
+    const double *f;
+    double *x, *r, *p, *w;
+    const double2 *g;
+    const uint8_t *code;
+    const double *ctab;
+    const int32_t *nbr, *gx;
+    double *hist, *part, *scal;        // part: 2 x gridDim partial sums (alternating); scal: nk_reduce_ws::scal
+    unsigned *bar;                     // barrier counter, zeroed by the host before the launch
+    int64_t E, L;
+    int niter;
+};
+
+template <int CT>
+__device__ __forceinline__ void coop_cta_sync() { asm volatile("bar.sync 15, %0;" ::"n"(CT) : "memory"); }
+
+// all compute threads of all CTAs; `passed` counts the barriers this CTA has been through
+template <int CT>
+__device__ __forceinline__ void coop_grid_barrier(unsigned *bar, unsigned &passed)
+{
+    coop_cta_sync<CT>();
+    if (threadIdx.x == 0) {
+        const unsigned target = gridDim.x * (passed + 1u);
+        __threadfence();
+        atomicAdd(bar, 1u);
+        unsigned seen;
+        do {
+            asm volatile("ld.acquire.gpu.global.u32 %0, [%1];" : "=r"(seen) : "l"(bar) : "memory");
+        } while (seen < target);
+        __threadfence();
+    }
+    coop_cta_sync<CT>();
+    ++passed;
+}
+
+// Sum of v over all compute threads of all CTAs, the same bits in every thread of every CTA.
+template <int CT>
+__device__ __forceinline__ double coop_grid_sum(double v, double *s_red, double *part, unsigned *bar, unsigned &passed)
+{
+    const int tid = threadIdx.x, lane = tid & 31, wid = tid >> 5;
+    constexpr int NWARP = CT / 32;
+    v = nk_warp_sum(v);
+    if (lane == 0) s_red[wid] = v;
+    coop_cta_sync<CT>();
+    double *mine = part + (size_t)(passed & 1u) * gridDim.x;
+    if (wid == 0) {
+        double t = (lane < NWARP) ? s_red[lane] : 0.0;
+        t = nk_warp_sum(t);
+        if (lane == 0) __stcg(mine + blockIdx.x, t);
+    }
+    coop_grid_barrier<CT>(bar, passed);            // (`mine` was picked before `passed` moved on)
+    if (wid == 0) {
+        double t = 0.0;
+        for (unsigned i = lane; i < gridDim.x; i += 32) t += __ldcg(mine + i);
+        t = nk_warp_sum(t);
+        if (lane == 0) s_red[32] = t;
+    }
+    coop_cta_sync<CT>();
+    const double total = s_red[32];
+    coop_cta_sync<CT>();                           // s_red is free again
+    return total;
+}
+
+// (M Q Q^T w)_l from the unsummed w, read past the L1: own value / face partner / Dirichlet / all copies of a row
+__device__ __forceinline__ double coop_gs_value(const double *__restrict__ w, const int32_t *__restrict__ gx, int l, int v,
+                                                double wl)
+{
+    if (v == l) return wl;
+    if (v >= 0) { const double g = __ldcg(w + v); return v > l ? wl + g : g + wl; }
+    if (v == -1) return 0.0;
+    const int32_t *ii = gx + 4 * (int64_t)(-v - 2);
+    const int len = ii[-1];
+    double s = __ldcg(w + ii[0]);
+    for (int j = 1; j < len; ++j) s += __ldcg(w + ii[j]);
+    return s;
+}
+
+template <int N>
+__global__ void __launch_bounds__(TmaCfg<N>::THREADS, 1)
+cg_coop_kernel(nk_coop_args a)
+{
+    using C = TmaCfg<N>;
+    constexpr int CT = C::CT;
+    extern __shared__ __align__(128) unsigned char smem_raw[];
+    __shared__ double s_red[33];
+    __shared__ double s_c[NK_CTAB];
+    const AxSmem<N> sm(smem_raw);
+    const int tid = threadIdx.x;
+    if (tid == 0) sm.init_barriers();
+    for (int t = tid; t < NK_CTAB; t += blockDim.x) s_c[t] = a.ctab[t];
+    __syncthreads();
+    const int64_t elo = a.E * (int64_t)blockIdx.x / gridDim.x, ehi = a.E * ((int64_t)blockIdx.x + 1) / gridDim.x;
+    RingState rs{0, 0u};
+    if (tid >= CT) {
+        // producer: free-running over the iterations, held back only by the ring
+        if (tid == CT)
+            for (int k = 0; k < a.niter; ++k) ax_produce<N>(sm, a.g, elo, ehi, rs);
+        return;
+    }
+    // this CTA's share of the vectors for the streaming phases: a contiguous range of pairs
+    const int64_t pairs = a.L >> 1;
+    const int64_t plo = pairs * (int64_t)blockIdx.x / gridDim.x, phi = pairs * ((int64_t)blockIdx.x + 1) / gridDim.x;
+    const bool odd_tail = (a.L & 1) && blockIdx.x == gridDim.x - 1 && tid == 0;       // the last point of an odd L
+    unsigned passed = 0;
+    double *x2 = a.x, *r2 = a.r, *p2 = a.p;
+    // ---- r = mask o f, x = 0, p = r, rho = <r,r>_c -------------------------------------------------------------
+    double acc = 0.0;
+    for (int64_t q = plo + tid; q < phi; q += CT) {
+        double2 fv = reinterpret_cast<const double2 *>(a.f)[q];
+        const uchar2 cd = reinterpret_cast<const uchar2 *>(a.code)[q];
+        if (cd.x & NK_CODE_MASKED) fv.x = 0.0;
+        if (cd.y & NK_CODE_MASKED) fv.y = 0.0;
+        reinterpret_cast<double2 *>(r2)[q] = fv;
+        reinterpret_cast<double2 *>(p2)[q] = fv;
+        reinterpret_cast<double2 *>(x2)[q] = make_double2(0.0, 0.0);
+        acc = fma(s_c[cd.x & 0x7f] * fv.x, fv.x, acc);
+        acc = fma(s_c[cd.y & 0x7f] * fv.y, fv.y, acc);
+    }
+    if (odd_tail) {
+        const int64_t l = a.L - 1;
+        const uint8_t cd = a.code[l];
+        const double fv = (cd & NK_CODE_MASKED) ? 0.0 : a.f[l];
+        r2[l] = fv; p2[l] = fv; x2[l] = 0.0;
+        acc = fma(s_c[cd & 0x7f] * fv, fv, acc);
+    }
+    double rho = coop_grid_sum<CT>(acc, s_red, a.part, a.bar, passed);
+    if (blockIdx.x == 0 && tid == 0) a.hist[0] = sqrt(rho);
+    double beta = 0.0, alpha = 0.0, pap = 0.0, rho_old = rho;
+    for (int k = 1; k <= a.niter; ++k) {
+        // ---- phase A: w = A_L p with p = r + beta p folded in; pap ------------------------------------------------
+        const double dsum = ax_compute<N, true, true>(sm, p2, nullptr, r2, a.w, beta, elo, ehi, rs);
+        pap = coop_grid_sum<CT>(dsum, s_red, a.part, a.bar, passed);
+        alpha = (rho == 0.0 || pap == 0.0) ? 0.0 : rho / pap;
+        // ---- phase B: x += alpha p; r -= alpha M Q Q^T w; rho' ----------------------------------------------------
+        acc = 0.0;
+        for (int64_t q = plo + tid; q < phi; q += CT) {
+            const double2 pv = __ldcg(reinterpret_cast<const double2 *>(p2) + q);
+            const double2 wv = __ldcg(reinterpret_cast<const double2 *>(a.w) + q);
+            double2 xv = reinterpret_cast<const double2 *>(x2)[q];
+            double2 rv = reinterpret_cast<const double2 *>(r2)[q];
+            const uchar2 cd = reinterpret_cast<const uchar2 *>(a.code)[q];
+            const int2 nv = reinterpret_cast<const int2 *>(a.nbr)[q];
+            const int l = (int)(2 * q);
+            const double s0 = coop_gs_value(a.w, a.gx, l, nv.x, wv.x);
+            const double s1 = coop_gs_value(a.w, a.gx, l + 1, nv.y, wv.y);
+            xv.x = fma(alpha, pv.x, xv.x);
+            xv.y = fma(alpha, pv.y, xv.y);
+            rv.x = fma(-alpha, s0, rv.x);
+            rv.y = fma(-alpha, s1, rv.y);
+            reinterpret_cast<double2 *>(x2)[q] = xv;
+            reinterpret_cast<double2 *>(r2)[q] = rv;
+            acc = fma(s_c[cd.x & 0x7f] * rv.x, rv.x, acc);
+            acc = fma(s_c[cd.y & 0x7f] * rv.y, rv.y, acc);
+        }
+        if (odd_tail) {
+            const int l = (int)(a.L - 1);
+            const double s0 = coop_gs_value(a.w, a.gx, l, a.nbr[l], __ldcg(a.w + l));
+            x2[l] = fma(alpha, __ldcg(p2 + l), x2[l]);
+            const double rn = fma(-alpha, s0, r2[l]);
+            r2[l] = rn;
+            acc = fma(s_c[a.code[l] & 0x7f] * rn, rn, acc);
+        }
+        const double rho_new = coop_grid_sum<CT>(acc, s_red, a.part, a.bar, passed);
+        beta = (rho == 0.0 || pap == 0.0) ? 0.0 : rho_new / rho;
+        rho_old = rho;
+        rho = rho_new;
+        if (blockIdx.x == 0 && tid == 0) a.hist[k] = sqrt(rho_new);
+    }
+    // ---- leave the context as the launch-by-launch path does: p = r + beta p applied, scalars of the last step ----
+    if (a.niter > 0) {
+        for (int64_t q = plo + tid; q < phi; q += CT) {
+            const double2 rv = reinterpret_cast<const double2 *>(r2)[q];
+            double2 pv = __ldcg(reinterpret_cast<const double2 *>(p2) + q);
+            pv.x = fma(beta, pv.x, rv.x);
+            pv.y = fma(beta, pv.y, rv.y);
+            reinterpret_cast<double2 *>(p2)[q] = pv;
+        }
+        if (odd_tail) { const int64_t l = a.L - 1; p2[l] = fma(beta, __ldcg(p2 + l), r2[l]); }
+    }
+    if (blockIdx.x == 0 && tid == 0) {
+        a.scal[NK_S_RHO] = rho; a.scal[NK_S_RHO_OLD] = rho_old; a.scal[NK_S_RHO_NEW] = rho;
+        a.scal[NK_S_PAP] = pap; a.scal[NK_S_ALPHA] = alpha; a.scal[NK_S_BETA] = beta;
+    }
+}
+
+template <int N>
+cudaError_t launch_coop(nk_ctx *c, const double *f, double *x, int niter, double *hist, cudaStream_t st)
+{
+    using C = TmaCfg<N>;
+    nk_coop_args a;
+    a.f = f; a.x = x; a.r = c->r; a.p = c->p; a.w = c->w; a.g = c->g;
+    a.code = c->code; a.ctab = c->ctab; a.nbr = c->nbr; a.gx = c->gx;
+    a.hist = hist; a.part = c->red.partials; a.scal = c->red.scal; a.bar = c->coop_bar;
+    a.E = c->E; a.L = c->L; a.niter = niter;
+    cudaError_t e = cudaMemsetAsync(c->coop_bar, 0, sizeof(unsigned), st);
+    if (e != cudaSuccess) return e;
+    cudaLaunchConfig_t cfg = {};
+    cfg.gridDim = dim3((unsigned)c->sm_count); cfg.blockDim = dim3(C::THREADS);
+    cfg.dynamicSmemBytes = C::SMEM; cfg.stream = st;
+    cudaLaunchAttribute at[1];
+    at[0].id = cudaLaunchAttributeCooperative;                 // all CTAs co-resident, or the launch fails
+    at[0].val.cooperative = 1;
+    cfg.attrs = at; cfg.numAttrs = 1;
+    e = cudaLaunchKernelEx(&cfg, cg_coop_kernel<N>, a);
+    c->launches++;
+    return e != cudaSuccess ? e : cudaGetLastError();
 }
 
 template <int N>
@@ -607,8 +871,11 @@ cudaError_t prepare_tma()
     cudaError_t e = cudaFuncSetAttribute(ax_tma_kernel<N, true>, cudaFuncAttributeMaxDynamicSharedMemorySize,
                                          TmaCfg<N>::SMEM);
     if (e != cudaSuccess) return e;
-    return cudaFuncSetAttribute(ax_tma_kernel<N, false>, cudaFuncAttributeMaxDynamicSharedMemorySize,
-                                TmaCfg<N>::SMEM);
+    e = cudaFuncSetAttribute(ax_tma_kernel<N, false>, cudaFuncAttributeMaxDynamicSharedMemorySize, TmaCfg<N>::SMEM);
+    if (e != cudaSuccess) return e;
+    if constexpr (N <= 13)           // nk_coop_supported
+        e = cudaFuncSetAttribute(cg_coop_kernel<N>, cudaFuncAttributeMaxDynamicSharedMemorySize, TmaCfg<N>::SMEM);
+    return e;
 }
 
 }  // namespace
@@ -649,6 +916,20 @@ cudaError_t nk_upload_D_tables_tma(void)
     NK_CASE(9) NK_CASE(10) NK_CASE(11) NK_CASE(12) NK_CASE(13) NK_CASE(14) NK_CASE(15)
 #undef NK_CASE
     return cudaSuccess;
+}
+
+// the whole solve as one cooperative launch (orders whose ax_e needs no register re-balancing: N <= 13)
+int nk_coop_supported(int N) { return N >= 1 && N <= 13; }
+
+cudaError_t nk_launch_cg_coop(nk_ctx *c, const double *f, double *x, int niter, double *hist, cudaStream_t st)
+{
+    switch (c->N) {
+#define NK_CASE(NN) case NN: return launch_coop<NN>(c, f, x, niter, hist, st);
+        NK_CASE(1) NK_CASE(2) NK_CASE(3) NK_CASE(4) NK_CASE(5) NK_CASE(6) NK_CASE(7) NK_CASE(8)
+        NK_CASE(9) NK_CASE(10) NK_CASE(11) NK_CASE(12) NK_CASE(13)
+#undef NK_CASE
+    }
+    return cudaErrorInvalidValue;
 }
 
 int nk_ax_tma_epb(int N)

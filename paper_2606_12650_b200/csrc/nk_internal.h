@@ -22,6 +22,7 @@ enum { NK_EPI_STORE = 0,   // out[0] = total
 #define NK_CODE_MASKED 0x80u       // bit 7 of the per-point code: Dirichlet node
 #define NK_HIST_MAX 8192               // residual-history capacity of nk_cg_host
 #define NK_GRAPH_AUTO_MAX_L (1 << 24)   // "graph" = 2: nk_cg replays a CUDA graph up to this many local points
+#define NK_COOP_AUTO_MAX_L (1 << 20)     // "coop" = 2: one cooperative launch per solve up to this many local points
 #define NK_FUSE_GS_AUTO_MIN_L (1 << 21)  // "fuse_gs" = 2: gs rides in the residual update above this many local points
 #define NK_GS_CHUNK 32768          // rows per gs chunk (128 blocks of 256 threads)
 #define NK_CTAB 128                // code & 0x7f indexes ctab[] = 1/multiplicity
@@ -84,12 +85,14 @@ struct nk_ctx {
     double *hist;                // NK_HIST_MAX doubles (nk_cg_host)
     double *res_dummy;           // 1 double (history sink for nk_cg_step)
     int *errflag;                // geometry error flag
+    unsigned *coop_bar;          // grid-barrier counter of the cooperative solve (nk_ax_tma.cu cg_coop_kernel)
+    int coop_ok;                 // the device supports cooperative launches
     nk_reduce_ws red;
     // sizes
     int64_t n_unique, n_shared_unique, n_masked_unique;
     int64_t n_rows, n_listed, n_sum_rows, n_sum_listed;
     // options / state
-    int opt_fuse_pap, opt_fuse_p, opt_fuse_gs, opt_graph, opt_profile, opt_pdl;
+    int opt_fuse_pap, opt_fuse_p, opt_fuse_gs, opt_coop, opt_graph, opt_profile, opt_pdl;
     int pdl_now;                 // nk_pdl_mode while nk_cg enqueues its loop (every kernel there waits), else 0
     int p_pending;               // 1: p = r + beta p has not been applied yet (fuse_p)
     int w_unsummed;              // 1: ctx w holds the unsummed ax_e output of the last iteration (fuse_gs)
@@ -141,7 +144,11 @@ void nk_host_basis_dd(int N, double *xi, double *w, double *D, double *Dlo);   /
 cudaError_t nk_launch_ax_tma(nk_ctx *c, double *u_rw, const double *u_ro, const double *r_in, double *w,
                              int dot, cudaStream_t st);
 cudaError_t nk_upload_D_tables_tma(void);
-int nk_ax_tma_epb(int N);                       // elements per batch of order N, 0 if N is out of range
+int nk_ax_tma_epb(int N);
+int nk_coop_supported(int N);
+// the whole CG solve as one cooperative launch (cg_coop_kernel): x, hist as nk_cg; leaves r, p, the unsummed w and
+// the scalars of the last iteration in the context
+cudaError_t nk_launch_cg_coop(nk_ctx *c, const double *f, double *x, int niter, double *hist, cudaStream_t st);                       // elements per batch of order N, 0 if N is out of range
 // nk_geom.cu
 cudaError_t nk_launch_geom(nk_ctx *c, const double *coords_dev, const double *D_dev, const double *Dlo_dev,
                            const double *wq_dev, cudaStream_t st);

@@ -232,7 +232,7 @@ extern "C" int nk_setup(nk_ctx **ctx, int64_t E, int N, const double *coords, co
     c->E = E; c->N = N; c->n = N + 1; c->P = (int64_t)c->n * c->n * c->n; c->L = L;
     c->device = dev; c->sm_count = sms;
     c->ws = workspace; c->ws_bytes = workspace_bytes;
-    c->opt_fuse_pap = 1; c->opt_fuse_p = 2; c->opt_fuse_gs = 2; c->opt_graph = 2; c->opt_pdl = 3; c->pdl_now = 0;
+    c->opt_fuse_pap = 1; c->opt_fuse_p = 2; c->opt_fuse_gs = 2; c->opt_coop = 2; c->opt_graph = 2; c->opt_pdl = 3; c->pdl_now = 0;
     nk_host_basis(N, c->xi, c->wq, c->D);
     char *q = static_cast<char *>(workspace);
     c->g = reinterpret_cast<double2 *>(q); q += cv.g;
@@ -256,6 +256,12 @@ extern "C" int nk_setup(nk_ctx **ctx, int64_t E, int N, const double *coords, co
     c->red.raw = nullptr;
     c->errflag = reinterpret_cast<int *>(q + 64);
     c->res_dummy = reinterpret_cast<double *>(q + 128);
+    c->coop_bar = reinterpret_cast<unsigned *>(q + 192);
+    {
+        int coop = 0;
+        NK_CUDA(cudaDeviceGetAttribute(&coop, cudaDevAttrCooperativeLaunch, dev));
+        c->coop_ok = coop;
+    }
     int rc;
     try {
         rc = setup_impl(c, coords, glo_num, mask, static_cast<cudaStream_t>(stream));

@@ -8,6 +8,13 @@
 
 namespace {
 
+// Pointer qualifiers in this file: a kernel launched as a PROGRAMMATIC DEPENDENT starts while its predecessor
+// still runs and reads the predecessor's output only after griddepcontrol.wait (nk_pdl_wait).  Such inputs (w, r,
+// p, the scalar block) are plain `const double *`, never `const ... __restrict__`: that pair lets the compiler use
+// non-coherent loads (LDG.CONSTANT), which it treats as invariant and hoists ABOVE the wait -- round 1's update_p
+// fetched beta before its predecessor had written it (found by the cooperative path's state comparison).  Static
+// set-up data (code, ctab, nbr, gx, dinv) keeps the qualifiers: fetching it before the wait is the point.
+//
 // Fixed grid => fixed partial sums => run-to-run bitwise reproducible.
 inline int vec_blocks(const nk_ctx *c, int64_t pairs)
 {
@@ -90,8 +97,8 @@ cg_init_kernel(const double *__restrict__ f, double *__restrict__ x, double *__r
 
 // x += alpha p; r -= alpha w; rho' = <r,r>_c          (S 8(a) a5: axpy, axpy and dot in one pass)
 __global__ void __launch_bounds__(NK_VEC_THREADS)
-update_xr_kernel(double *__restrict__ x, double *__restrict__ r, const double *__restrict__ p,
-                 const double *__restrict__ w, const uint8_t *__restrict__ code,
+update_xr_kernel(double *__restrict__ x, double *__restrict__ r, const double *p,
+                 const double *w, const uint8_t *__restrict__ code,
                  const double *__restrict__ ctab, int64_t L, nk_reduce_ws ws, double *hist_k)
 {
     __shared__ double s_c[NK_CTAB];
@@ -151,7 +158,7 @@ struct nk_gather {
     int n_rows, row_blocks;
 };
 
-__device__ __forceinline__ double gs_partner(const double *__restrict__ w, int l, int v)
+__device__ __forceinline__ double gs_partner(const double *w, int l, int v)
 {
     return (v >= 0 && v != l) ? w[v] : 0.0;
 }
@@ -165,7 +172,7 @@ __device__ __forceinline__ double gs_stream_value(int l, int v, double wl, doubl
 
 template <bool WITH_X>
 __global__ void __launch_bounds__(NK_VEC_THREADS, 2)
-gs_update_kernel(double *__restrict__ x, double *r, const double *__restrict__ p, const double *__restrict__ w,
+gs_update_kernel(double *__restrict__ x, double *r, const double *p, const double *w,
                  const uint8_t *__restrict__ code, const double *__restrict__ ctab, int64_t L, nk_reduce_ws ws,
                  double *hist_k, nk_gather gp)
 {
@@ -314,7 +321,7 @@ gs_update_kernel(double *__restrict__ x, double *r, const double *__restrict__ p
 
 // p = r + beta p                                       (S 8(a) a6)
 __global__ void __launch_bounds__(NK_VEC_THREADS)
-update_p_kernel(double *__restrict__ p, const double *__restrict__ r, const double *__restrict__ scal, int64_t L)
+update_p_kernel(double *__restrict__ p, const double *r, const double *scal, int64_t L)
 {
     nk_pdl_launch_dependents();
     nk_pdl_wait();
@@ -338,7 +345,7 @@ update_p_kernel(double *__restrict__ p, const double *__restrict__ r, const doub
 // work in 65 B/pt instead of 73: p is read once per iteration (by update_px, which still has the old
 // p in registers when x needs it) instead of twice.  Same arithmetic per entry as update_xr_kernel.
 __global__ void __launch_bounds__(NK_VEC_THREADS)
-update_r_kernel(double *__restrict__ r, const double *__restrict__ w, const uint8_t *__restrict__ code,
+update_r_kernel(double *__restrict__ r, const double *w, const uint8_t *__restrict__ code,
                 const double *__restrict__ ctab, int64_t L, nk_reduce_ws ws, double *hist_k)
 {
     __shared__ double s_c[NK_CTAB];
@@ -392,8 +399,8 @@ update_r_kernel(double *__restrict__ r, const double *__restrict__ w, const uint
 
 // x += alpha p (the OLD p); p = r + beta p
 __global__ void __launch_bounds__(NK_VEC_THREADS)
-update_px_kernel(double *__restrict__ x, double *__restrict__ p, const double *__restrict__ r,
-                 const double *__restrict__ scal, int64_t L)
+update_px_kernel(double *__restrict__ x, double *__restrict__ p, const double *r,
+                 const double *scal, int64_t L)
 {
     nk_pdl_launch_dependents();
     nk_pdl_wait();
@@ -452,7 +459,7 @@ pcg_init_kernel(const double *__restrict__ f, double *__restrict__ x, double *__
 
 // r -= alpha w; z = dinv o r; rho' = <r,z>_c; hist = sqrt<r,r>_c   (x rides with the p update below)
 __global__ void __launch_bounds__(NK_VEC_THREADS)
-update_rz_kernel(double *__restrict__ r, const double *__restrict__ w, const double *__restrict__ dinv,
+update_rz_kernel(double *__restrict__ r, const double *w, const double *__restrict__ dinv,
                   const uint8_t *__restrict__ code, const double *__restrict__ ctab, int64_t L,
                   nk_reduce_ws ws, double *hist_k)
 {
@@ -492,8 +499,8 @@ update_rz_kernel(double *__restrict__ r, const double *__restrict__ w, const dou
 
 // x += alpha p (the OLD p); p = dinv o r + beta p
 __global__ void __launch_bounds__(NK_VEC_THREADS)
-update_pxz_kernel(double *__restrict__ x, double *__restrict__ p, const double *__restrict__ r,
-                  const double *__restrict__ dinv, const double *__restrict__ scal, int64_t L)
+update_pxz_kernel(double *__restrict__ x, double *__restrict__ p, const double *r,
+                  const double *__restrict__ dinv, const double *scal, int64_t L)
 {
     nk_pdl_launch_dependents();
     nk_pdl_wait();

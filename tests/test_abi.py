@@ -105,3 +105,33 @@ def test_product_does_not_import_oracle():
                 assert not re.search(r"^\s*(from|import)\s+paper_2606_12650_b200", src, flags=re.M), fn
                 assert not re.search(r'#include\s+"[^"]*nk(_\w+)?\.(h|cuh)"', src), fn
                 assert "CDLL" not in src or "libnk.so" not in src, fn
+
+
+def test_no_dependent_load_is_hoisted_above_the_pdl_wait():
+    """A kernel launched as a programmatic dependent may read what its predecessor wrote only after
+    griddepcontrol.wait (SASS: ACQBULK).  `const T *__restrict__` parameters make such loads non-coherent and
+    invariant, and ptxas then hoists them above the wait (round 1: update_p fetched beta too early).  In the kernels
+    that fetch NOTHING static before the wait, no global load may precede ACQBULK."""
+    import shutil
+    import subprocess
+    cuobjdump = shutil.which("cuobjdump") or "/usr/local/cuda/bin/cuobjdump"
+    if not os.path.exists(cuobjdump):
+        pytest.skip("cuobjdump not available")
+    from paper_2606_12650_b200 import build
+    build.build()
+    sass = subprocess.run([cuobjdump, "-sass", os.path.join(build.OBJDIR, "nk_vec.o")], capture_output=True, text=True,
+                          check=True).stdout
+    seen = set()
+    cur, order = None, []
+    for line in sass.splitlines() + ["Function : end"]:
+        if "Function :" in line:
+            if cur is not None and any(k in cur for k in ("update_p_kernel", "update_px_kernel", "update_pxz_kernel")):
+                assert "ACQBULK" in order, cur
+                assert "LDG" not in order[:order.index("ACQBULK")], cur
+                seen.add(cur)
+            cur, order = line, []
+        elif "ACQBULK" in line:
+            order.append("ACQBULK")
+        elif "LDG" in line:
+            order.append("LDG")
+    assert len(seen) == 3, seen

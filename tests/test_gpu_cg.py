@@ -10,10 +10,12 @@ from workloads import CONFIGS, config_rhs, rhs_unique
 
 pytestmark = pytest.mark.gpu
 
-OPTION_SETS = [dict(fuse_pap=1, fuse_p=1, fuse_gs=1, graph=0), dict(fuse_pap=0, fuse_p=0, fuse_gs=1, graph=0),
-               dict(fuse_pap=1, fuse_p=0, fuse_gs=1, graph=0), dict(fuse_pap=0, fuse_p=1, fuse_gs=1, graph=0),
-               dict(fuse_pap=1, fuse_p=1, fuse_gs=0, graph=0), dict(fuse_pap=1, fuse_p=0, fuse_gs=0, graph=0),
-               dict(fuse_pap=1, fuse_p=1, fuse_gs=1, graph=1)]
+# launch-by-launch paths ("coop" = 0) with every fusion option, the graph replay, and the cooperative whole-solve launch
+OPTION_SETS = [dict(coop=0, fuse_pap=1, fuse_p=1, fuse_gs=1, graph=0), dict(coop=0, fuse_pap=0, fuse_p=0, fuse_gs=1, graph=0),
+               dict(coop=0, fuse_pap=1, fuse_p=0, fuse_gs=1, graph=0), dict(coop=0, fuse_pap=0, fuse_p=1, fuse_gs=1, graph=0),
+               dict(coop=0, fuse_pap=1, fuse_p=1, fuse_gs=0, graph=0), dict(coop=0, fuse_pap=1, fuse_p=0, fuse_gs=0, graph=0),
+               dict(coop=0, fuse_pap=1, fuse_p=1, fuse_gs=1, graph=1), dict(coop=1)]
+DEFAULTS = dict(coop=2, fuse_pap=1, fuse_p=2, fuse_gs=2, graph=2)
 
 
 def _set(gpu, opts):
@@ -53,7 +55,7 @@ def test_lockstep_iterations(name, opts):
             assert elem_err(rg, r, pr.P) <= TOL_OP, k
             assert elem_err(pg, p, pr.P) <= TOL_OP, k
         rho = so["rho_new"]
-    _set(pr.gpu, OPTION_SETS[0])
+    _set(pr.gpu, DEFAULTS)
 
 
 @pytest.mark.parametrize("name", ["config1", "config2"])
@@ -70,7 +72,7 @@ def test_free_running_cg(name, opts):
     assert np.all(np.abs(hg - ho) <= TOL_CG * ho), np.abs(hg / ho - 1).max()
     assert elem_err(xg, xo, pr.P) <= TOL_CG
     assert np.all(xg[pr.mesh.mask == 0.0] == 0.0)
-    _set(pr.gpu, OPTION_SETS[0])
+    _set(pr.gpu, DEFAULTS)
 
 
 def test_golden_history_config1():
@@ -172,7 +174,9 @@ def test_graph_default_and_pointer_change():
     from paper_2606_12650_b200 import Nekbone
     pr = pair_for_config("config2")
     gpu = Nekbone.from_mesh(pr.mesh)                  # a fresh context: the shared one has had options set
-    assert gpu.get_option("graph") == 2
+    assert gpu.get_option("graph") == 2 and gpu.solve_path() == "cooperative"
+    gpu.set_option("coop", 0)                         # below the cooperative launch the rule is: replay a graph
+    assert gpu.solve_path() == "graph"
     f1 = to_dev(config_rhs("config2", pr.mesh))
     f2 = f1.clone()
     xa, ha = gpu.cg(f1, 25)
@@ -200,6 +204,7 @@ def test_programmatic_dependent_launch_is_bitwise_neutral(name, fuse_p):
     mesh = config_mesh(name)
     gpu = Nekbone.from_mesh(mesh)
     assert gpu.get_option("pdl") == 3
+    gpu.set_option("coop", 0)
     gpu.set_option("fuse_p", fuse_p)
     f = to_dev(config_rhs(name, mesh))
     out = {}
@@ -275,12 +280,13 @@ def test_cg_high_and_odd_orders(N):
     pr = pair_for_brick(3, 2, 2, N, 0.1)
     f = rhs_unique(pr.mesh, 40 + N)
     xo, ho = pr.orc.cg(f, 12)
-    for graph in (0, 1):
+    for coop, graph in ((0, 0), (0, 1), (2, 2)):          # launches, graph replay, the default (cooperative up to N = 13)
+        pr.gpu.set_option("coop", coop)
         pr.gpu.set_option("graph", graph)
         xg, hg = pr.gpu.cg(to_dev(f), 12)
-        assert np.all(np.abs(to_np(hg) - ho) <= TOL_CG * ho), (N, graph)
-        assert elem_err(to_np(xg), xo, pr.P) <= TOL_CG, (N, graph)
-    pr.gpu.set_option("graph", 2)
+        assert np.all(np.abs(to_np(hg) - ho) <= TOL_CG * ho), (N, coop, graph)
+        assert elem_err(to_np(xg), xo, pr.P) <= TOL_CG, (N, coop, graph)
+    assert pr.gpu.solve_path() == ("cooperative" if N <= 13 else "graph")
 
 
 # ---- gs folded into the residual update ("fuse_gs") ------------------------------------------------------
@@ -298,6 +304,7 @@ def test_fused_gs_against_separate_gs(name, fuse_p):
     mesh = config_mesh(name)
     gpu = Nekbone.from_mesh(mesh)
     assert gpu.get_option("fuse_gs") == 2
+    gpu.set_option("coop", 0)
     gpu.set_option("fuse_p", fuse_p)
     f = to_dev(config_rhs(name, mesh))
     # one iteration from the same state: r, x bitwise equal (rho' and beta, hence p, only to rounding)
@@ -357,3 +364,93 @@ def test_fused_gs_on_irregular_ids():
             res[fuse_p, fuse_gs] = (to_np(xg), to_np(hg))
             assert np.all(np.abs(res[fuse_p, fuse_gs][1] - ho) <= TOL_CG * ho), (fuse_p, fuse_gs)
             assert elem_err(res[fuse_p, fuse_gs][0], xo, m.n ** 3) <= TOL_CG, (fuse_p, fuse_gs)
+
+
+# ---- the whole solve as one cooperative launch ("coop") -----------------------------------------------------
+COOP_MESHES = [(2, 2, 2, 3), (5, 3, 3, 1), (3, 3, 3, 2), (7, 6, 5, 4), (6, 5, 5, 6), (8, 8, 8, 7), (6, 5, 4, 8), (5, 4, 4, 9),
+               (4, 3, 3, 11), (3, 2, 2, 13), (300, 1, 1, 5)]
+
+
+@pytest.mark.parametrize("nx,ny,nz,N", COOP_MESHES)
+def test_cooperative_solve(nx, ny, nz, N):
+    """One persistent cooperative launch for the whole solve: against the oracle at 1e-10 (history and
+    x), against the launch-by-launch path to rounding, bitwise reproducible, context left as the other paths leave
+    it.  Meshes: fewer elements than CTAs (CTAs with no element still take their share of the vector phases and
+    of the barriers), more than one batch per CTA (300 elements at N = 5 on 148 CTAs... 2-3 elements each, the
+    8^3 mesh of config 2), odd L (N = 2: 27 points per element, 27 elements)."""
+    import torch
+    from paper_2606_12650_b200 import Nekbone
+    pr = pair_for_brick(nx, ny, nz, N, 0.05)
+    gpu = Nekbone.from_mesh(pr.mesh)
+    assert gpu.solve_path() == "cooperative"
+    f = rhs_unique(pr.mesh, 300 + N)
+    niter = 30
+    xo, ho = pr.orc.cg(f, niter)
+    fd = to_dev(f)
+    runs = [gpu.cg(fd, niter) for _ in range(3)]
+    torch.cuda.synchronize()
+    x0, h0 = runs[0]
+    for x, h in runs[1:]:
+        assert bool((x == x0).all()) and bool((h == h0).all())
+    xg, hg = to_np(x0), to_np(h0)
+    if not (np.all(np.abs(hg - ho) <= TOL_CG * ho) and elem_err(xg, xo, pr.P) <= TOL_CG):
+        from parity import history_parity, oracle_variants           # tiny meshes converge within the 30 iterations
+        alts = oracle_variants(pr.mesh, f, niter)
+        ok, worst, kstar = history_parity(hg, ho, [h for _, h in alts])
+        assert ok and kstar >= 8, (N, worst, kstar)
+        assert elem_err(xg, xo, pr.P) <= max(TOL_CG, 10.0 * max(elem_err(xb, xo, pr.P) for xb, _ in alts))
+    assert np.all(xg[pr.mesh.mask == 0.0] == 0.0)
+    # the context afterwards: r, p, w = M Q Q^T A_L p and the scalars of the last iteration, as the launch path leaves them
+    rc, pc, wc = (to_np(t) for t in gpu.cg_get_state())
+    sc = gpu.scalars()
+    gpu.set_option("coop", 0)
+    xl, hl = gpu.cg(fd, niter)
+    rl, pl, wl = (to_np(t) for t in gpu.cg_get_state())
+    sl = gpu.scalars()
+    k = int(np.nonzero(to_np(hl) > 1e-8 * to_np(hl)[0])[0].max())          # compare where rounding has not taken over
+    assert float(np.abs(hg[:k + 1] / to_np(hl)[:k + 1] - 1).max()) <= 1e-11
+    if k == niter:
+        assert elem_err(xg, to_np(xl), pr.P) <= 1e-11
+        assert elem_err(rc, rl, pr.P) <= 1e-9 and elem_err(pc, pl, pr.P) <= 1e-9 and elem_err(wc, wl, pr.P) <= 1e-9
+        for key in ("pap", "alpha", "rho_new", "beta"):
+            assert abs(sc[key] - sl[key]) <= 1e-9 * abs(sl[key]), key
+    # guards and degenerate calls on the cooperative path
+    gpu.set_option("coop", 1)
+    xz, hz = gpu.cg(torch.zeros(pr.L, dtype=torch.float64, device="cuda"), 5)
+    assert not bool(xz.any()) and not bool(hz.any())
+    x1, h1 = gpu.cg(fd, 1)
+    xo1, ho1 = pr.orc.cg(f, 1)
+    assert np.all(np.abs(to_np(h1) - ho1) <= TOL_OP * ho1) and elem_err(to_np(x1), xo1, pr.P) <= TOL_OP
+    xh, hh = gpu.cg_host(f, niter)
+    assert np.array_equal(xh, xg) and np.array_equal(hh, hg)
+    gpu.close()
+
+
+@pytest.mark.parametrize("fuse_p", [0, 1])
+@pytest.mark.parametrize("graph", [0, 1])
+def test_context_state_after_a_solve(graph, fuse_p):
+    """r, p, w = M Q Q^T A_L p and the scalars a solve leaves in the context (the direction update of the last
+    iteration applied) against the oracle's, on every launch path, with programmatic dependent launches on: the final
+    p = r + beta p once read beta before its predecessor had written it (a `const __restrict__` load hoisted above
+    griddepcontrol.wait)."""
+    from paper_2606_12650_b200 import Nekbone
+    pr = pair_for_config("config2")
+    gpu = Nekbone.from_mesh(pr.mesh)
+    gpu.set_option("coop", 0)
+    gpu.set_option("graph", graph)
+    gpu.set_option("fuse_p", fuse_p)
+    f = config_rhs("config2", pr.mesh)
+    x, r, p, rho = pr.orc.cg_init(f)
+    for k in range(3):
+        w, so = pr.orc.cg_step(x, r, p, rho)
+        rho = so["rho_new"]
+    for rep in range(3):
+        xg, hg = gpu.cg(to_dev(f), 3)
+        rg, pg, wg = (to_np(t) for t in gpu.cg_get_state())
+        assert elem_err(to_np(xg), x, pr.P) <= TOL_OP and elem_err(rg, r, pr.P) <= TOL_OP
+        assert elem_err(pg, p, pr.P) <= TOL_OP, rep
+        assert elem_err(wg, w, pr.P) <= TOL_OP
+        sg = gpu.scalars()
+        for key in ("pap", "alpha", "rho_new", "beta"):
+            assert abs(sg[key] - so[key]) <= TOL_OP * abs(so[key]), key
+    gpu.close()
