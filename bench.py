@@ -311,7 +311,7 @@ def run_ours(args) -> dict | None:
     nk = Nekbone.from_mesh(mesh)
     setup_s = time.perf_counter() - t0
     for k, v in (("fuse_pap", args.fuse_pap), ("fuse_p", args.fuse_p), ("fuse_gs", args.fuse_gs), ("graph", args.graph),
-                 ("pdl", args.pdl)):
+                 ("pdl", args.pdl), ("coop", args.coop)):
         if v is not None:                                  # None: the library's default
             nk.set_option(k, v)
     sizes = {**nk.sizes(), **nk.gs_sizes()}
@@ -402,7 +402,7 @@ def run_ours(args) -> dict | None:
     peak, peak_kind = measured_peaks()
     value = whole_job_value(flops_step, args.steps, world, ms)
     e2e = whole_job_value(flops_step, args.steps, world, ms_e2e)
-    opts = {k: nk.get_option(k) for k in ("fuse_pap", "fuse_p", "fuse_gs", "graph", "pdl")}
+    opts = {k: nk.get_option(k) for k in ("fuse_pap", "fuse_p", "fuse_gs", "graph", "pdl", "coop")}
     fused_p = opts["fuse_p"] == 1 or (opts["fuse_p"] == 2 and L <= (1 << 24))
     fused_gs = bool(opts["fuse_pap"]) and (opts["fuse_gs"] == 1 or (opts["fuse_gs"] == 2 and L > (1 << 21)))
     out = {"metric": METRIC, "value": value, "unit": UNIT, "n_gpus": world, "steps": args.steps,
@@ -597,6 +597,7 @@ def main():
     ap.add_argument("--fuse-p", type=int, default=None)
     ap.add_argument("--fuse-gs", type=int, default=None)
     ap.add_argument("--graph", type=int, default=None)
+    ap.add_argument("--coop", type=int, default=None)
     ap.add_argument("--traffic", type=float, default=None,
                     help="dram bytes per ax_e launch from the committed ncu --set full capture (profiles/)")
     ap.add_argument("--no-cpu-baseline", action="store_true")

@@ -164,7 +164,8 @@ int nk_dist_iter_c(nk_ctx *ctx, double *x, double *hist_k_dev, void *stream);
  *                  that sit in L2, where launch gaps and kernel tails are most of an iteration.  Orders
  *                  N <= 13; otherwise, and under "profile", the next rule applies.  Sums run in fixed but
  *                  different orders than launch by launch: the two agree to rounding, each is bitwise
- *                  reproducible.  0 = never; 2 (default) = 1 for meshes of up to 2^20 local points.
+ *                  reproducible.  0 = never; 2 (default) = 1 for meshes of up to 2^19 local points (1.1-1.3x the
+ *                  graph replay there; slower from about 0.8 M points on).
  *   "graph"        0 = nk_cg enqueues its launches one by one; 1 = records them into a CUDA graph
  *                  (cached per f, x, res_hist, niter; updated in place when the pointers change) and
  *                  replays it; 2 (default) = 1 for meshes of up to 2^24 local points, where launch gaps

@@ -208,7 +208,8 @@ int nk_dot(nk_ctx *c, const double *a, const double *b, double *out, void *strea
 // "graph" = 2 (default): replay a CUDA graph where launch gaps matter (measured: config 2 3.8 -> 1.9 ms,
 // config 3 15.0 -> 13.0 ms per 100 iterations), enqueue directly on large meshes
 // "coop" = 2 (default): the whole solve as one cooperative launch on meshes that sit in L2, where an iteration is
-// a few microseconds of work and even a replayed graph of programmatic dependents costs 11-16 us per iteration
+// a few microseconds of work and even a replayed graph of programmatic dependents costs 10-16 us per iteration
+// (measured: 7.8-13 us here, profiles/r2_coop_vs_graph.txt)
 static bool cg_uses_coop(const nk_ctx *c)
 {
     return !c->opt_profile && c->coop_ok && nk_coop_supported(c->N) &&

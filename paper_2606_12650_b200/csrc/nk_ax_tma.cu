@@ -27,6 +27,8 @@
 // Fusions on the CG path (S 8(f) f-1), as in nk_ax.cu:
 //   dot   : sum_l u_l w_l reduced in the same pass (dot-fusion identity), epilogue alpha = rho/pap;
 //   r_in  : p = r + beta p applied while loading (p written back).
+#include <cstdio>
+
 #include "nk_internal.h"
 #include "nk_reduce.cuh"
 
@@ -591,7 +593,9 @@ ax_tma_kernel(double *u_rw, const double *u_ro, const double *r_in,
 //            gathered on the fly from the unsummed w (nk_ctx::nbr, gx); rho' partial
 //   -- grid barrier; every CTA adds the rho' partials in the same order: beta, residual history --
 // Two barriers per iteration (hand-written: one monotone counter in global memory, arrive = atomicAdd, wait =
-// ld.acquire until the count reaches blocks x barriers passed).  The producer warp never joins a barrier: the
+// ld.acquire until the count reaches blocks x barriers passed; measured ~2 us each, as a grid.sync.  A variant
+// that carried the partial sums in the flag words themselves, LL-protocol style, polled by a whole warp, was
+// SLOWER: 4-5 us per exchange).  The producer warp never joins a barrier: the
 // geometric factors are static, so it streams the NEXT iteration's first batches into the ring while the compute
 // warps are in phase B -- the ring is full when phase A starts.  Vectors another SM may have written during the
 // launch are read past the L1 (ld.global.cg).  Sums are deterministic (fixed ranges, fixed trees); the order
@@ -602,7 +606,8 @@ struct nk_coop_args {
     const double2 *g;
     const uint8_t *code;
     const double *ctab;
-    const int32_t *nbr, *gx;
+    const int32_t *nbr, *gx, *gx_rows;   // nk_ctx: gather codes, index rows of nodes with >= 3 copies, their list
+    int64_t n_gx_rows;
     double *hist, *part, *scal;        // part: 2 x gridDim partial sums (alternating); scal: nk_reduce_ws::scal
     unsigned *bar;                     // barrier counter, zeroed by the host before the launch
     int64_t E, L;
@@ -659,18 +664,51 @@ __device__ __forceinline__ double coop_grid_sum(double v, double *s_red, double 
     return total;
 }
 
-// (M Q Q^T w)_l from the unsummed w, read past the L1: own value / face partner / Dirichlet / all copies of a row
-__device__ __forceinline__ double coop_gs_value(const double *__restrict__ w, const int32_t *__restrict__ gx, int l, int v,
-                                                double wl)
+// (M Q Q^T w)_l of a streamed point from the unsummed w: own value / face partner g / Dirichlet.  Points of nodes
+// with three or more copies (v < -1) are left to coop_row_update: `skip`.
+__device__ __forceinline__ double coop_gs_value(int l, int v, double wl, double g, bool &skip)
 {
-    if (v == l) return wl;
-    if (v >= 0) { const double g = __ldcg(w + v); return v > l ? wl + g : g + wl; }
-    if (v == -1) return 0.0;
-    const int32_t *ii = gx + 4 * (int64_t)(-v - 2);
+    skip = v < -1;
+    const double sum = v > l ? wl + g : g + wl;              // ascending local index
+    return (v == l) ? wl : (v >= 0 ? sum : 0.0);
+}
+
+// One node with three or more copies (edges, corners): gather w (past the L1) and r at all copies, sum in ascending
+// local index, r -= alpha sum at every copy; returns the node's share of rho'.  One thread per node, so that the
+// dependent loads of many nodes overlap (inlined per point they serialised behind each other: 10 us per phase).
+__device__ __forceinline__ double coop_row_update(const double *w, double *r, const int32_t *__restrict__ gx, int p4,
+                                                  double alpha, const double (&cw_of_len)[9])
+{
+    const int32_t *ii = gx + 4 * (int64_t)p4;
     const int len = ii[-1];
-    double s = __ldcg(w + ii[0]);
-    for (int j = 1; j < len; ++j) s += __ldcg(w + ii[j]);
-    return s;
+    const int4 ia = *reinterpret_cast<const int4 *>(ii);
+    double acc = 0.0;
+    if (len == 4) {
+        const double a0 = __ldcg(w + ia.x), a1 = __ldcg(w + ia.y), a2 = __ldcg(w + ia.z), a3 = __ldcg(w + ia.w);
+        double r0 = r[ia.x], r1 = r[ia.y], r2 = r[ia.z], r3 = r[ia.w];
+        const double s = ((a0 + a1) + a2) + a3, cw = cw_of_len[4];
+        r0 = fma(-alpha, s, r0); r1 = fma(-alpha, s, r1); r2 = fma(-alpha, s, r2); r3 = fma(-alpha, s, r3);
+        r[ia.x] = r0; r[ia.y] = r1; r[ia.z] = r2; r[ia.w] = r3;
+        acc = fma(cw * r0, r0, acc); acc = fma(cw * r1, r1, acc); acc = fma(cw * r2, r2, acc); acc = fma(cw * r3, r3, acc);
+        return acc;
+    }
+    const int4 ib = *reinterpret_cast<const int4 *>(ii + 4);
+    const int id[8] = {ia.x, ia.y, ia.z, ia.w, ib.x, ib.y, ib.z, ib.w};
+    double av[8], rr[8];
+#pragma unroll
+    for (int j = 0; j < 8; ++j) { av[j] = (j < len) ? __ldcg(w + id[j]) : 0.0; rr[j] = (j < len) ? r[id[j]] : 0.0; }
+    double s = av[0];
+#pragma unroll
+    for (int j = 1; j < 8; ++j) s = (j < len) ? s + av[j] : s;
+    for (int j = 8; j < len; ++j) s += __ldcg(w + ii[j]);
+    double cw = 1.0 / (double)len;
+#pragma unroll
+    for (int j = 1; j < 9; ++j) cw = (len == j) ? cw_of_len[j] : cw;
+#pragma unroll
+    for (int j = 0; j < 8; ++j)
+        if (j < len) { const double rn = fma(-alpha, s, rr[j]); r[id[j]] = rn; acc = fma(cw * rn, rn, acc); }
+    for (int j = 8; j < len; ++j) { const double rn = fma(-alpha, s, r[ii[j]]); r[ii[j]] = rn; acc = fma(cw * rn, rn, acc); }
+    return acc;
 }
 
 template <int N>
@@ -699,6 +737,11 @@ cg_coop_kernel(nk_coop_args a)
     const int64_t pairs = a.L >> 1;
     const int64_t plo = pairs * (int64_t)blockIdx.x / gridDim.x, phi = pairs * ((int64_t)blockIdx.x + 1) / gridDim.x;
     const bool odd_tail = (a.L & 1) && blockIdx.x == gridDim.x - 1 && tid == 0;       // the last point of an odd L
+    // ... and of the nodes with three or more copies (coop_row_update)
+    const int64_t rlo = a.n_gx_rows * (int64_t)blockIdx.x / gridDim.x, rhi = a.n_gx_rows * ((int64_t)blockIdx.x + 1) / gridDim.x;
+    double cw_of_len[9];
+#pragma unroll
+    for (int j = 0; j < 9; ++j) cw_of_len[j] = j ? 1.0 / (double)j : 0.0;      // = ctab of that multiplicity, bit for bit
     unsigned passed = 0;
     double *x2 = a.x, *r2 = a.r, *p2 = a.p;
     // ---- r = mask o f, x = 0, p = r, rho = <r,r>_c -------------------------------------------------------------
@@ -726,39 +769,88 @@ cg_coop_kernel(nk_coop_args a)
     double beta = 0.0, alpha = 0.0, pap = 0.0, rho_old = rho;
     for (int k = 1; k <= a.niter; ++k) {
         // ---- phase A: w = A_L p with p = r + beta p folded in; pap ------------------------------------------------
+#ifdef NK_COOP_TIMING
+        unsigned long long tt[5];
+        asm volatile("mov.u64 %0, %%globaltimer;" : "=l"(tt[0]));
+#endif
         const double dsum = ax_compute<N, true, true>(sm, p2, nullptr, r2, a.w, beta, elo, ehi, rs);
+#ifdef NK_COOP_TIMING
+        asm volatile("mov.u64 %0, %%globaltimer;" : "=l"(tt[1]));
+#endif
         pap = coop_grid_sum<CT>(dsum, s_red, a.part, a.bar, passed);
+#ifdef NK_COOP_TIMING
+        asm volatile("mov.u64 %0, %%globaltimer;" : "=l"(tt[2]));
+#endif
         alpha = (rho == 0.0 || pap == 0.0) ? 0.0 : rho / pap;
         // ---- phase B: x += alpha p; r -= alpha M Q Q^T w; rho' ----------------------------------------------------
         acc = 0.0;
-        for (int64_t q = plo + tid; q < phi; q += CT) {
-            const double2 pv = __ldcg(reinterpret_cast<const double2 *>(p2) + q);
-            const double2 wv = __ldcg(reinterpret_cast<const double2 *>(a.w) + q);
-            double2 xv = reinterpret_cast<const double2 *>(x2)[q];
-            double2 rv = reinterpret_cast<const double2 *>(r2)[q];
-            const uchar2 cd = reinterpret_cast<const uchar2 *>(a.code)[q];
-            const int2 nv = reinterpret_cast<const int2 *>(a.nbr)[q];
-            const int l = (int)(2 * q);
-            const double s0 = coop_gs_value(a.w, a.gx, l, nv.x, wv.x);
-            const double s1 = coop_gs_value(a.w, a.gx, l + 1, nv.y, wv.y);
-            xv.x = fma(alpha, pv.x, xv.x);
-            xv.y = fma(alpha, pv.y, xv.y);
-            rv.x = fma(-alpha, s0, rv.x);
-            rv.y = fma(-alpha, s1, rv.y);
-            reinterpret_cast<double2 *>(x2)[q] = xv;
-            reinterpret_cast<double2 *>(r2)[q] = rv;
-            acc = fma(s_c[cd.x & 0x7f] * rv.x, rv.x, acc);
-            acc = fma(s_c[cd.y & 0x7f] * rv.y, rv.y, acc);
+        for (int64_t q0 = plo + tid; q0 < phi; q0 += 4 * CT) {          // four pairs per thread in flight
+            double2 pv[4], wv[4], xv[4], rv[4], gv[4];
+            uchar2 cd[4];
+            int2 nv[4];
+#pragma unroll
+            for (int j = 0; j < 4; ++j) {
+                const int64_t q = q0 + j * CT;
+                const bool on = q < phi;
+                nv[j] = on ? reinterpret_cast<const int2 *>(a.nbr)[q] : make_int2(0, 0);
+                cd[j] = on ? reinterpret_cast<const uchar2 *>(a.code)[q] : make_uchar2(0, 0);
+                pv[j] = on ? __ldcg(reinterpret_cast<const double2 *>(p2) + q) : make_double2(0.0, 0.0);
+                wv[j] = on ? __ldcg(reinterpret_cast<const double2 *>(a.w) + q) : make_double2(0.0, 0.0);
+                xv[j] = on ? reinterpret_cast<const double2 *>(x2)[q] : make_double2(0.0, 0.0);
+                rv[j] = on ? reinterpret_cast<const double2 *>(r2)[q] : make_double2(0.0, 0.0);
+            }
+#pragma unroll
+            for (int j = 0; j < 4; ++j) {                                  // the face partners, all at once
+                const int l = (int)(2 * (q0 + j * CT));
+                gv[j].x = (q0 + j * CT < phi && nv[j].x >= 0 && nv[j].x != l) ? __ldcg(a.w + nv[j].x) : 0.0;
+                gv[j].y = (q0 + j * CT < phi && nv[j].y >= 0 && nv[j].y != l + 1) ? __ldcg(a.w + nv[j].y) : 0.0;
+            }
+#pragma unroll
+            for (int j = 0; j < 4; ++j) {
+                const int64_t q = q0 + j * CT;
+                if (q < phi) {
+                    const int l = (int)(2 * q);
+                    bool k0, k1;
+                    const double s0 = coop_gs_value(l, nv[j].x, wv[j].x, gv[j].x, k0);
+                    const double s1 = coop_gs_value(l + 1, nv[j].y, wv[j].y, gv[j].y, k1);
+                    xv[j].x = fma(alpha, pv[j].x, xv[j].x);
+                    xv[j].y = fma(alpha, pv[j].y, xv[j].y);
+                    rv[j].x = fma(-alpha, s0, rv[j].x);
+                    rv[j].y = fma(-alpha, s1, rv[j].y);
+                    reinterpret_cast<double2 *>(x2)[q] = xv[j];
+                    if (!(k0 || k1)) {
+                        reinterpret_cast<double2 *>(r2)[q] = rv[j];
+                    } else {                                           // coop_row_update owns the other entry
+                        if (!k0) r2[l] = rv[j].x;
+                        if (!k1) r2[l + 1] = rv[j].y;
+                    }
+                    acc = fma((k0 ? 0.0 : s_c[cd[j].x & 0x7f]) * rv[j].x, rv[j].x, acc);
+                    acc = fma((k1 ? 0.0 : s_c[cd[j].y & 0x7f]) * rv[j].y, rv[j].y, acc);
+                }
+            }
         }
+        for (int64_t kr = rlo + tid; kr < rhi; kr += CT) acc += coop_row_update(a.w, r2, a.gx, a.gx_rows[kr], alpha, cw_of_len);
         if (odd_tail) {
             const int l = (int)(a.L - 1);
-            const double s0 = coop_gs_value(a.w, a.gx, l, a.nbr[l], __ldcg(a.w + l));
+            const int vt = a.nbr[l];
+            bool k0;
+            const double s0 = coop_gs_value(l, vt, __ldcg(a.w + l), (vt >= 0 && vt != l) ? __ldcg(a.w + vt) : 0.0, k0);
             x2[l] = fma(alpha, __ldcg(p2 + l), x2[l]);
-            const double rn = fma(-alpha, s0, r2[l]);
-            r2[l] = rn;
-            acc = fma(s_c[a.code[l] & 0x7f] * rn, rn, acc);
+            if (!k0) {
+                const double rn = fma(-alpha, s0, r2[l]);
+                r2[l] = rn;
+                acc = fma(s_c[a.code[l] & 0x7f] * rn, rn, acc);
+            }
         }
+#ifdef NK_COOP_TIMING
+        asm volatile("mov.u64 %0, %%globaltimer;" : "=l"(tt[3]));
+#endif
         const double rho_new = coop_grid_sum<CT>(acc, s_red, a.part, a.bar, passed);
+#ifdef NK_COOP_TIMING
+        asm volatile("mov.u64 %0, %%globaltimer;" : "=l"(tt[4]));
+        if ((blockIdx.x == 0 || blockIdx.x == 77) && tid == 0 && (k == 5 || k == 6))
+            printf("cta %d it %d: A %llu  sum1 %llu  B %llu  sum2 %llu ns\n", blockIdx.x, k, tt[1] - tt[0], tt[2] - tt[1], tt[3] - tt[2], tt[4] - tt[3]);
+#endif
         beta = (rho == 0.0 || pap == 0.0) ? 0.0 : rho_new / rho;
         rho_old = rho;
         rho = rho_new;
@@ -787,7 +879,7 @@ cudaError_t launch_coop(nk_ctx *c, const double *f, double *x, int niter, double
     using C = TmaCfg<N>;
     nk_coop_args a;
     a.f = f; a.x = x; a.r = c->r; a.p = c->p; a.w = c->w; a.g = c->g;
-    a.code = c->code; a.ctab = c->ctab; a.nbr = c->nbr; a.gx = c->gx;
+    a.code = c->code; a.ctab = c->ctab; a.nbr = c->nbr; a.gx = c->gx; a.gx_rows = c->gx_rows; a.n_gx_rows = c->n_gx_rows;
     a.hist = hist; a.part = c->red.partials; a.scal = c->red.scal; a.bar = c->coop_bar;
     a.E = c->E; a.L = c->L; a.niter = niter;
     cudaError_t e = cudaMemsetAsync(c->coop_bar, 0, sizeof(unsigned), st);

@@ -22,7 +22,8 @@ enum { NK_EPI_STORE = 0,   // out[0] = total
 #define NK_CODE_MASKED 0x80u       // bit 7 of the per-point code: Dirichlet node
 #define NK_HIST_MAX 8192               // residual-history capacity of nk_cg_host
 #define NK_GRAPH_AUTO_MAX_L (1 << 24)   // "graph" = 2: nk_cg replays a CUDA graph up to this many local points
-#define NK_COOP_AUTO_MAX_L (1 << 20)     // "coop" = 2: one cooperative launch per solve up to this many local points
+#define NK_COOP_AUTO_MAX_L (1 << 19)     // "coop" = 2: one cooperative launch per solve up to this many local points
+                                        // (measured crossover against the graph replay: 0.7 - 0.9 M points, N = 3..11)
 #define NK_FUSE_GS_AUTO_MIN_L (1 << 21)  // "fuse_gs" = 2: gs rides in the residual update above this many local points
 #define NK_GS_CHUNK 32768          // rows per gs chunk (128 blocks of 256 threads)
 #define NK_CTAB 128                // code & 0x7f indexes ctab[] = 1/multiplicity
