@@ -209,7 +209,7 @@ int nk_dot(nk_ctx *c, const double *a, const double *b, double *out, void *strea
 // config 3 15.0 -> 13.0 ms per 100 iterations), enqueue directly on large meshes
 // "coop" = 2 (default): the whole solve as one cooperative launch on meshes that sit in L2, where an iteration is
 // a few microseconds of work and even a replayed graph of programmatic dependents costs 10-16 us per iteration
-// (measured: 7.8-13 us here, profiles/r2_coop_vs_graph.txt)
+// (measured: 7.8-13 us here, profiles/r2_sweep_coop.csv)
 static bool cg_uses_coop(const nk_ctx *c)
 {
     return !c->opt_profile && c->coop_ok && nk_coop_supported(c->N) &&

@@ -1,6 +1,6 @@
 """Roofline sweeps of ax_e, gs, ax and the CG iteration (BASELINE.json configs[3]).
 
-    python -m paper_2606_12650_b200.sweep [--which e|n|both|big|paper] [--reps 50] [--out sweep.csv]
+    python -m paper_2606_12650_b200.sweep [--which e|n|both|big|paper|coop] [--reps 50] [--out sweep.csv]
 
 4a (e): brick meshes with E = 2^10 .. 2^17 at N = 7;  4b (n): N = 3 .. 15 at E = 4096 (16^3); perturbed
 geometry (amplitude 0.05), u uniform[-1,1) per LOCAL point (seed 1004), `reps` back-to-back
@@ -13,6 +13,7 @@ copy peak (MEASURED_PEAKS.json, else the guide's fallback) and of the nominal 8 
 set fits in L2 ("L2-resident": effective GB/s can then exceed the HBM peak; the >= 70 % claim is made
 on the other points only).
 paper: the paper's own sweep: N in {4, 6, 8}, E = 2^1 .. 2^14, CG 100 iterations, GDOFS.
+coop: the CG iteration on small meshes, graph replay against the cooperative whole-solve launch.
 
 This tool only times.  Parity of every point against the oracle is `python tests/sweep_parity.py`, which
 calls the generators below and appends its columns (the product never imports the oracle).
@@ -164,14 +165,58 @@ def paper_points():
             yield row, mesh, f_np, h
 
 
+def coop_points():
+    """nk_cg per iteration on small meshes: CUDA graph replay ("coop" = 0) against the cooperative whole-solve launch
+    ("coop" = 1); the measurement behind NK_COOP_AUTO_MAX_L.  N in {3, 4, 6, 7, 8, 9, 11}, E = 2^1 .. 2^14 up to 2^22
+    points; mean of 5 timed solves of 100 iterations after a warm-up solve."""
+    import torch
+    from paper_2606_12650_b200 import Nekbone
+    from workloads import brick_mesh, rhs_unique, sweep_brick
+    from workloads.configs import SWEEP_AMPLITUDE, SWEEP_SEED
+
+    def timed(nk, f, x, h):
+        nk.cg(f, 100, x=x, res_hist=h)
+        torch.cuda.synchronize()
+        ts = []
+        for _ in range(5):
+            e0, e1 = torch.cuda.Event(enable_timing=True), torch.cuda.Event(enable_timing=True)
+            e0.record()
+            nk.cg(f, 100, x=x, res_hist=h)
+            e1.record()
+            torch.cuda.synchronize()
+            ts.append(e0.elapsed_time(e1))
+        return float(np.mean(ts))
+
+    yield "N,E,n_local,graph_us_per_iteration,cooperative_us_per_iteration,graph_over_cooperative,default_path"
+    for N in (3, 4, 6, 7, 8, 9, 11):
+        for k in range(1, 15):
+            mesh = brick_mesh(*sweep_brick(k), N, SWEEP_AMPLITUDE)
+            if mesh.L > (1 << 22):
+                break
+            nk = Nekbone.from_mesh(mesh)
+            default_path = nk.solve_path()
+            f = torch.from_numpy(rhs_unique(mesh, SWEEP_SEED)).cuda()
+            x, h = nk.empty(), torch.empty(101, dtype=torch.float64, device="cuda")
+            nk.set_option("coop", 0)
+            tg = timed(nk, f, x, h)
+            nk.set_option("coop", 1)
+            tc = timed(nk, f, x, h)
+            nk.close()
+            yield f"{N},{mesh.E},{mesh.L},{tg * 10:.2f},{tc * 10:.2f},{tg / tc:.3f},{default_path}"
+
+
 def main():
     ap = argparse.ArgumentParser()
-    ap.add_argument("--which", default="both", choices=["e", "n", "both", "big", "paper"])
+    ap.add_argument("--which", default="both", choices=["e", "n", "both", "big", "paper", "coop"])
     ap.add_argument("--reps", type=int, default=None)
     ap.add_argument("--out", default=None)
     args = ap.parse_args()
     lines = []
-    if args.which == "paper":
+    if args.which == "coop":
+        for row in coop_points():
+            lines.append(row)
+            print(row, flush=True)
+    elif args.which == "paper":
         lines.append(PAPER_HEADER)
         for row, _, _, _ in paper_points():
             lines.append(row)
