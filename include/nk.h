@@ -63,6 +63,10 @@ int nk_workspace_bytes(int64_t E, int N, size_t *bytes);
 int nk_setup(nk_ctx **ctx, int64_t E, int N, const double *coords, const int64_t *glo_num,
              const double *mask, void *workspace, size_t workspace_bytes, void *stream);
 void nk_free(nk_ctx *ctx);
+/* Host threads the set-up's plan building uses from now on (it runs on all cores by default: a parallel radix
+ * sort of (global id, local index), the group walk, the packing); n < 1 restores the default.  Every array
+ * nk_setup builds is independent of this number. */
+int nk_set_host_threads(int n);
 
 /* w = A_L u : element-local Laplacian, no gs, no mask (S 8(a) a1).  u, w DEVICE, L; u != w. */
 int nk_ax_e(nk_ctx *ctx, const double *u, double *w, void *stream);

@@ -24,6 +24,7 @@ SIGNATURES = {
     "nk_workspace_bytes": (_i, [_i64, _i, C.POINTER(_sz)]),
     "nk_setup": (_i, [C.POINTER(_vp), _i64, _i, _vp, _vp, _vp, _vp, _sz, _vp]),
     "nk_free": (None, [_vp]),
+    "nk_set_host_threads": (_i, [_i]),
     "nk_ax_e": (_i, [_vp, _vp, _vp, _vp]),
     "nk_gs": (_i, [_vp, _vp, _vp]),
     "nk_ax": (_i, [_vp, _vp, _vp, _vp]),
@@ -116,6 +117,11 @@ def fp64_peak() -> dict:
     t, r = _d(), _d()
     _check(load().nk_fp64_peak(C.byref(t), C.byref(r), _stream()))
     return dict(tflops=float(t.value), dfma_per_clk_per_sm_at_max_clock=float(r.value))
+
+
+def set_host_threads(n: int) -> None:
+    """Host threads of later set-ups (0 = all cores); the plan they build does not depend on it."""
+    _check(load().nk_set_host_threads(int(n)))
 
 
 def _np_ptr(a: np.ndarray):

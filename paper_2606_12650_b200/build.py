@@ -23,7 +23,7 @@ HEADERS = ["nk_internal.h", "nk_host.h", "nk_reduce.cuh"]
 
 NVCC = os.environ.get("NVCC", "/usr/local/cuda/bin/nvcc")
 ARCH = ["-gencode", "arch=compute_100a,code=sm_100a"]
-FLAGS = ["-O3", "-std=c++17", "-lineinfo", "-Xcompiler", "-fPIC", "-Xcompiler", "-Wall",
+FLAGS = ["-O3", "-std=c++17", "-lineinfo", "-Xcompiler", "-fPIC", "-Xcompiler", "-Wall", "-Xcompiler", "-fopenmp",
          "-Xptxas", "-v"]
 EXTRA = os.environ.get("NK_NVCC_EXTRA", "").split()
 
@@ -56,7 +56,7 @@ def build(force: bool = False, verbose: bool = False) -> str:
         results = list(ex.map(lambda s: _compile(s, force, verbose), SOURCES))
     objs = [o for o, _ in results]
     if force or not os.path.exists(LIB) or any(os.path.getmtime(o) > os.path.getmtime(LIB) for o in objs):
-        cmd = [NVCC, *ARCH, "-shared", "-o", LIB, *objs]
+        cmd = [NVCC, *ARCH, "-shared", "-o", LIB, *objs, "-lgomp"]
         if verbose:
             print(" ".join(cmd), file=sys.stderr)
         subprocess.run(cmd, check=True)

@@ -2,8 +2,13 @@
 // caller's workspace, build the gather-scatter plan on the host (sort (global id, local index)
 // pairs -> CSR of nodes that are shared or masked -> multiplicity codes), upload, run the geometry
 // kernel.  One-time cost; the paper discards set-up and warm-up from its timings too.
+// The host part runs on all cores (OpenMP: parallel radix sort, group walk cut at group boundaries, chunked
+// packing); every array it builds is independent of the thread count (tests/test_abi.py::test_plan_threads).
 #include <algorithm>
 #include <cmath>
+#ifdef _OPENMP
+#include <omp.h>
+#endif
 #include <cstring>
 #include <new>
 
@@ -11,23 +16,51 @@
 
 namespace {
 
-// Stable LSD radix sort of (key, payload) by key, 11 bits per pass, only the passes max_key needs.
+int g_host_threads = 0;          // nk_set_host_threads; 0 = all cores
+
+inline int host_threads()
+{
+#ifdef _OPENMP
+    return g_host_threads > 0 ? g_host_threads : omp_get_num_procs();
+#else
+    return 1;
+#endif
+}
+
+// Stable LSD radix sort of (key, payload) by key, 11 bits per pass, only the passes max_key needs; every pass
+// is parallel over contiguous chunks (per-thread histograms, bucket-major prefix, in-order scatter: stable).
 void radix_sort_pairs(std::vector<uint64_t> &key, std::vector<uint32_t> &val, uint64_t max_key)
 {
-    const size_t n = key.size();
-    std::vector<uint64_t> key2(n);
-    std::vector<uint32_t> val2(n);
+    const int64_t n = (int64_t)key.size();
+    std::vector<uint64_t> key2((size_t)n);
+    std::vector<uint32_t> val2((size_t)n);
     constexpr int BITS = 11, BUCKETS = 1 << BITS;
-    std::vector<size_t> count(BUCKETS);
+    const int T = host_threads();
+    std::vector<int64_t> count((size_t)T * BUCKETS);
     for (int shift = 0; shift < 64 && (max_key >> shift) != 0; shift += BITS) {
-        std::fill(count.begin(), count.end(), 0);
-        for (size_t i = 0; i < n; ++i) count[(key[i] >> shift) & (BUCKETS - 1)]++;
-        size_t run = 0;
-        for (int b = 0; b < BUCKETS; ++b) { const size_t c = count[b]; count[b] = run; run += c; }
-        for (size_t i = 0; i < n; ++i) {
-            const size_t d = count[(key[i] >> shift) & (BUCKETS - 1)]++;
-            key2[d] = key[i];
-            val2[d] = val[i];
+#pragma omp parallel num_threads(T)
+        {
+#ifdef _OPENMP
+            const int t = omp_get_thread_num(), TT = omp_get_num_threads();      // TT <= T: what the runtime gave us
+#else
+            const int t = 0, TT = 1;
+#endif
+            const int64_t lo = n * t / TT, hi = n * (t + 1) / TT;
+            int64_t *cnt = &count[(size_t)t * BUCKETS];
+            for (int b = 0; b < BUCKETS; ++b) cnt[b] = 0;
+            for (int64_t i = lo; i < hi; ++i) cnt[(key[(size_t)i] >> shift) & (BUCKETS - 1)]++;
+#pragma omp barrier
+#pragma omp single
+            {
+                int64_t run = 0;
+                for (int b = 0; b < BUCKETS; ++b)
+                    for (int u = 0; u < TT; ++u) { const int64_t c = count[(size_t)u * BUCKETS + b]; count[(size_t)u * BUCKETS + b] = run; run += c; }
+            }
+            for (int64_t i = lo; i < hi; ++i) {
+                const int64_t d = cnt[(key[(size_t)i] >> shift) & (BUCKETS - 1)]++;
+                key2[(size_t)d] = key[(size_t)i];
+                val2[(size_t)d] = val[(size_t)i];
+            }
         }
         key.swap(key2);
         val.swap(val2);
@@ -39,43 +72,64 @@ struct Row { uint32_t first, begin, len; };   // first local index, position in 
 int setup_impl(nk_ctx *c, const double *coords, const int64_t *glo_num, const double *mask, cudaStream_t st)
 {
     const int64_t L = c->L;
+    const int T = host_threads();
     // ---- validate ids and mask ------------------------------------------------------------------
     uint64_t max_id = 0;
+    int bad_id = 0, bad_mask = 0;
+#pragma omp parallel for schedule(static) num_threads(T) reduction(max : max_id) reduction(| : bad_id, bad_mask)
     for (int64_t l = 0; l < L; ++l) {
-        if (glo_num[l] < 0) return NK_ERR_ID;
+        if (glo_num[l] < 0) { bad_id = 1; continue; }
         if ((uint64_t)glo_num[l] > max_id) max_id = (uint64_t)glo_num[l];
-        if (!(mask[l] == 0.0 || mask[l] == 1.0)) return NK_ERR_MASK;
+        if (!(mask[l] == 0.0 || mask[l] == 1.0)) bad_mask = 1;
     }
+    if (bad_id) return NK_ERR_ID;
+    if (bad_mask) return NK_ERR_MASK;
     // ---- group local indices by global id (stable: ascending local index inside a group) ---------
     std::vector<uint64_t> key((size_t)L);
     std::vector<uint32_t> loc((size_t)L);
-    for (int64_t l = 0; l < L; ++l) { key[l] = (uint64_t)glo_num[l]; loc[l] = (uint32_t)l; }
+#pragma omp parallel for schedule(static) num_threads(T)
+    for (int64_t l = 0; l < L; ++l) { key[(size_t)l] = (uint64_t)glo_num[l]; loc[(size_t)l] = (uint32_t)l; }
     radix_sort_pairs(key, loc, max_id);
 
+    // ---- walk the groups, in parallel over chunks of the sorted list cut at group boundaries ------------------
     std::vector<uint8_t> code((size_t)L);
-    std::vector<Row> sum_rows, msk_rows;
-    std::vector<int64_t> mult_values;                 // distinct multiplicities, ascending after the walk
-    int64_t n_unique = 0, n_shared = 0, n_masked = 0;
-    // first pass over groups: sizes, mask consistency, distinct multiplicities
-    for (int64_t b = 0; b < L;) {
-        int64_t e = b + 1;
-        while (e < L && key[e] == key[b]) ++e;
-        const int64_t len = e - b;
-        const double m0 = mask[loc[b]];
-        for (int64_t q = b + 1; q < e; ++q)
-            if (mask[loc[q]] != m0) return NK_ERR_MASK;
-        ++n_unique;
-        if (len > 1) ++n_shared;
-        if (m0 == 0.0) ++n_masked;
-        if (std::find(mult_values.begin(), mult_values.end(), len) == mult_values.end()) {
-            if (mult_values.size() >= NK_CTAB) return NK_ERR_MULT;
-            mult_values.push_back(len);
-        }
-        Row r{loc[b], (uint32_t)b, (uint32_t)len};
-        if (m0 == 0.0) msk_rows.push_back(r);
-        else if (len > 1) sum_rows.push_back(r);
-        b = e;
+    std::vector<std::vector<Row>> sum_t((size_t)T), msk_t((size_t)T);
+    std::vector<std::vector<int64_t>> mult_t((size_t)T);
+    std::vector<int64_t> cut((size_t)T + 1);
+    for (int t = 0; t <= T; ++t) {
+        int64_t p = L * t / T;
+        while (p > 0 && p < L && key[(size_t)p] == key[(size_t)p - 1]) ++p;       // forward to the next group start
+        cut[(size_t)t] = p;
     }
+    int64_t n_unique = 0, n_shared = 0, n_masked = 0;
+    int mask_clash = 0;
+#pragma omp parallel for schedule(static, 1) num_threads(T) reduction(+ : n_unique, n_shared, n_masked) reduction(| : mask_clash)
+    for (int t = 0; t < T; ++t) {
+        std::vector<Row> &sr = sum_t[(size_t)t], &mr = msk_t[(size_t)t];
+        std::vector<int64_t> &mv = mult_t[(size_t)t];
+        for (int64_t b = cut[(size_t)t]; b < cut[(size_t)t + 1];) {
+            int64_t e = b + 1;
+            while (e < L && key[(size_t)e] == key[(size_t)b]) ++e;
+            const int64_t len = e - b;
+            const double m0 = mask[loc[(size_t)b]];
+            for (int64_t q = b + 1; q < e; ++q)
+                if (mask[loc[(size_t)q]] != m0) mask_clash = 1;
+            ++n_unique;
+            if (len > 1) ++n_shared;
+            if (m0 == 0.0) ++n_masked;
+            if (std::find(mv.begin(), mv.end(), len) == mv.end()) mv.push_back(len);
+            Row r{loc[(size_t)b], (uint32_t)b, (uint32_t)len};
+            if (m0 == 0.0) mr.push_back(r);
+            else if (len > 1) sr.push_back(r);
+            b = e;
+        }
+    }
+    if (mask_clash) return NK_ERR_MASK;
+    std::vector<int64_t> mult_values;                 // distinct multiplicities, ascending
+    for (const auto &mv : mult_t)
+        for (int64_t v : mv)
+            if (std::find(mult_values.begin(), mult_values.end(), v) == mult_values.end()) mult_values.push_back(v);
+    if (mult_values.size() > NK_CTAB) return NK_ERR_MULT;
     std::sort(mult_values.begin(), mult_values.end());
     double ctab[NK_CTAB], mtab[NK_CTAB];
     for (int t = 0; t < NK_CTAB; ++t) { ctab[t] = 0.0; mtab[t] = 0.0; }
@@ -84,92 +138,129 @@ int setup_impl(nk_ctx *c, const double *coords, const int64_t *glo_num, const do
         ctab[t] = 1.0 / (double)mult_values[t];
     }
     // second pass: per-point codes
-    for (int64_t b = 0; b < L;) {
-        int64_t e = b + 1;
-        while (e < L && key[e] == key[b]) ++e;
-        const int64_t len = e - b;
-        const int t = (int)(std::lower_bound(mult_values.begin(), mult_values.end(), len) - mult_values.begin());
-        const uint8_t cd = (uint8_t)(t | (mask[loc[b]] == 0.0 ? NK_CODE_MASKED : 0u));
-        for (int64_t q = b; q < e; ++q) code[loc[q]] = cd;
-        b = e;
-    }
+#pragma omp parallel for schedule(static, 1) num_threads(T)
+    for (int t = 0; t < T; ++t)
+        for (int64_t b = cut[(size_t)t]; b < cut[(size_t)t + 1];) {
+            int64_t e = b + 1;
+            while (e < L && key[(size_t)e] == key[(size_t)b]) ++e;
+            const int64_t len = e - b;
+            const int ti = (int)(std::lower_bound(mult_values.begin(), mult_values.end(), len) - mult_values.begin());
+            const uint8_t cd = (uint8_t)(ti | (mask[loc[(size_t)b]] == 0.0 ? NK_CODE_MASKED : 0u));
+            for (int64_t q = b; q < e; ++q) code[loc[(size_t)q]] = cd;
+            b = e;
+        }
     std::vector<uint64_t>().swap(key);
-    // ---- order rows by first local index so neighbouring threads touch neighbouring memory ------
-    auto by_first = [](const Row &x, const Row &y) { return x.first < y.first; };
-    std::sort(sum_rows.begin(), sum_rows.end(), by_first);
-    std::sort(msk_rows.begin(), msk_rows.end(), by_first);
+    // ---- order rows by first local index so neighbouring threads touch neighbouring memory (first indices are
+    // distinct, so the order does not depend on how the walk was cut) -------------------------------------------
+    auto gather_sorted = [&](std::vector<std::vector<Row>> &parts) {
+        size_t total = 0;
+        for (const auto &v : parts) total += v.size();
+        std::vector<Row> all;
+        all.reserve(total);
+        for (auto &v : parts) { all.insert(all.end(), v.begin(), v.end()); std::vector<Row>().swap(v); }
+        std::vector<uint64_t> k(total);
+        std::vector<uint32_t> id(total);
+#pragma omp parallel for schedule(static) num_threads(T)
+        for (int64_t i = 0; i < (int64_t)total; ++i) { k[(size_t)i] = all[(size_t)i].first; id[(size_t)i] = (uint32_t)i; }
+        radix_sort_pairs(k, id, (uint64_t)(L > 0 ? L - 1 : 0));
+        std::vector<Row> out(total);
+#pragma omp parallel for schedule(static) num_threads(T)
+        for (int64_t i = 0; i < (int64_t)total; ++i) out[(size_t)i] = all[id[(size_t)i]];
+        return out;
+    };
+    std::vector<Row> sum_rows = gather_sorted(sum_t), msk_rows = gather_sorted(msk_t);
     const int64_t n_sum_rows = (int64_t)sum_rows.size(), n_rows = n_sum_rows + (int64_t)msk_rows.size();
     std::vector<int32_t> off((size_t)n_rows + 1);
     int64_t n_listed = 0, n_sum_listed = 0;
-    for (const Row &r : sum_rows) n_sum_listed += r.len;
-    n_listed = n_sum_listed;
-    for (const Row &r : msk_rows) n_listed += r.len;
-    std::vector<int32_t> idx((size_t)std::max<int64_t>(n_listed, 1));
     {
         int64_t pos = 0, row = 0;
-        for (const std::vector<Row> *rows : {&sum_rows, &msk_rows})
-            for (const Row &r : *rows) {
-                off[row++] = (int32_t)pos;
-                for (uint32_t q = 0; q < r.len; ++q) idx[pos++] = (int32_t)loc[r.begin + q];
-            }
-        off[row] = (int32_t)pos;
+        for (const Row &r : sum_rows) { off[(size_t)row++] = (int32_t)pos; pos += r.len; }
+        n_sum_listed = pos;
+        for (const Row &r : msk_rows) { off[(size_t)row++] = (int32_t)pos; pos += r.len; }
+        off[(size_t)row] = (int32_t)pos;
+        n_listed = pos;
+    }
+    std::vector<int32_t> idx((size_t)std::max<int64_t>(n_listed, 1));
+#pragma omp parallel for schedule(static) num_threads(T)
+    for (int64_t row = 0; row < n_rows; ++row) {
+        const Row &r = row < n_sum_rows ? sum_rows[(size_t)row] : msk_rows[(size_t)(row - n_sum_rows)];
+        int32_t *dst = &idx[(size_t)off[(size_t)row]];
+        for (uint32_t q = 0; q < r.len; ++q) dst[q] = (int32_t)loc[r.begin + q];
     }
     // packed copy of the summed rows: chunks of NK_GS_CHUNK consecutive rows (ascending first local index,
     // so a chunk works on one neighbourhood of memory), inside a chunk the rows of 2, 4 and 8 copies
     // packed by length, rows of any other length as row ids into the CSR.  Descriptor per chunk:
-    // {offset into pk, n2, n4, n8, n_other, 0, 0, 0}.
+    // {offset into pk, n2, n4, n8, n_other, 0, 0, 0}.  Sizes first, then offsets, then the chunks in parallel.
     const int64_t n_chunks = (n_sum_rows + NK_GS_CHUNK - 1) / NK_GS_CHUNK;
-    std::vector<int32_t> pk, desc((size_t)std::max<int64_t>(n_chunks, 1) * 8, 0);
-    pk.reserve((size_t)n_sum_listed + 4 * (size_t)n_chunks + 64);
+    std::vector<int32_t> desc((size_t)std::max<int64_t>(n_chunks, 1) * 8, 0);
+    auto pad4 = [](int64_t v) { return (v + 3) / 4 * 4; };
+#pragma omp parallel for schedule(static) num_threads(T)
     for (int64_t ch = 0; ch < n_chunks; ++ch) {
         const int64_t r0 = ch * NK_GS_CHUNK, r1 = std::min<int64_t>(r0 + NK_GS_CHUNK, n_sum_rows);
-        int32_t *d = &desc[(size_t)ch * 8];
-        d[0] = (int32_t)pk.size();
-        for (int len : {2, 4, 8}) {
-            int32_t cnt = 0;
-            for (int64_t r = r0; r < r1; ++r) {
-                const Row &row = sum_rows[(size_t)r];
-                if ((int)row.len != len) continue;
-                for (uint32_t q = 0; q < row.len; ++q) pk.push_back((int32_t)loc[row.begin + q]);
-                ++cnt;
-            }
-            while (pk.size() % 4) pk.push_back(0);                     // 16-byte aligned class starts
-            d[len == 2 ? 1 : len == 4 ? 2 : 3] = cnt;
-        }
-        int32_t no = 0;
+        int32_t cnt[4] = {0, 0, 0, 0};
         for (int64_t r = r0; r < r1; ++r) {
             const uint32_t len = sum_rows[(size_t)r].len;
-            if (len != 2 && len != 4 && len != 8) { pk.push_back((int32_t)r); ++no; }
+            ++cnt[len == 2 ? 0 : len == 4 ? 1 : len == 8 ? 2 : 3];
         }
-        while (pk.size() % 4) pk.push_back(0);
-        d[4] = no;
+        int32_t *d = &desc[(size_t)ch * 8];
+        d[1] = cnt[0]; d[2] = cnt[1]; d[3] = cnt[2]; d[4] = cnt[3];
     }
-    if (pk.empty()) pk.push_back(0);
+    int64_t pk_size = 0;
+    for (int64_t ch = 0; ch < n_chunks; ++ch) {
+        int32_t *d = &desc[(size_t)ch * 8];
+        d[0] = (int32_t)pk_size;
+        pk_size += pad4(2 * (int64_t)d[1]) + pad4(4 * (int64_t)d[2]) + pad4(8 * (int64_t)d[3]) + pad4(d[4]);
+    }
+    std::vector<int32_t> pk((size_t)std::max<int64_t>(pk_size, 1), 0);
+#pragma omp parallel for schedule(static) num_threads(T)
+    for (int64_t ch = 0; ch < n_chunks; ++ch) {
+        const int64_t r0 = ch * NK_GS_CHUNK, r1 = std::min<int64_t>(r0 + NK_GS_CHUNK, n_sum_rows);
+        const int32_t *d = &desc[(size_t)ch * 8];
+        int32_t *p2 = &pk[(size_t)d[0]], *p4 = p2 + pad4(2 * (int64_t)d[1]), *p8 = p4 + pad4(4 * (int64_t)d[2]);
+        int32_t *po = p8 + pad4(8 * (int64_t)d[3]);
+        for (int64_t r = r0; r < r1; ++r) {
+            const Row &row = sum_rows[(size_t)r];
+            if (row.len == 2 || row.len == 4 || row.len == 8) {
+                int32_t *&dst = row.len == 2 ? p2 : row.len == 4 ? p4 : p8;
+                for (uint32_t q = 0; q < row.len; ++q) *dst++ = (int32_t)loc[row.begin + q];
+            } else {
+                *po++ = (int32_t)r;
+            }
+        }
+    }
     // per-point gather codes of the fused gs (nk_internal.h nk_ctx::nbr)
     std::vector<int32_t> nbr((size_t)L), gx, gx_rows;
+#pragma omp parallel for schedule(static) num_threads(T)
     for (int64_t l = 0; l < L; ++l) nbr[(size_t)l] = (int32_t)l;
+#pragma omp parallel for schedule(static) num_threads(T)
     for (int64_t r = 0; r < n_sum_rows; ++r) {
         const Row &row = sum_rows[(size_t)r];
         if (row.len == 2) {
             const uint32_t a = loc[row.begin], b = loc[row.begin + 1];
             nbr[a] = (int32_t)b;
             nbr[b] = (int32_t)a;
-        } else {
-            while ((gx.size() + 1) % 4) gx.push_back(0);
-            gx.push_back((int32_t)row.len);
-            const int32_t p4 = (int32_t)(gx.size() / 4);
-            gx_rows.push_back(p4);
-            for (uint32_t q = 0; q < row.len; ++q) {
-                gx.push_back((int32_t)loc[row.begin + q]);
-                nbr[loc[row.begin + q]] = -p4 - 2;
-            }
+        }
+    }
+    for (int64_t r = 0; r < n_sum_rows; ++r) {
+        const Row &row = sum_rows[(size_t)r];
+        if (row.len == 2) continue;
+        while ((gx.size() + 1) % 4) gx.push_back(0);
+        gx.push_back((int32_t)row.len);
+        const int32_t p4 = (int32_t)(gx.size() / 4);
+        gx_rows.push_back(p4);
+        for (uint32_t q = 0; q < row.len; ++q) {
+            gx.push_back((int32_t)loc[row.begin + q]);
+            nbr[loc[row.begin + q]] = -p4 - 2;
         }
     }
     gx.resize((gx.size() + 12 + 3) / 4 * 4, 0);              // vector loads of the last row stay in bounds; 16-byte multiple
     c->n_gx_rows = (int64_t)gx_rows.size();
     c->gx_rows = c->gx + gx.size();
-    for (const Row &row : msk_rows)
+#pragma omp parallel for schedule(static) num_threads(T)
+    for (int64_t r = 0; r < (int64_t)msk_rows.size(); ++r) {
+        const Row &row = msk_rows[(size_t)r];
         for (uint32_t q = 0; q < row.len; ++q) nbr[loc[row.begin + q]] = -1;
+    }
     c->n_gs_chunks = n_chunks;
     c->gs_desc = c->pk + nk_align_up(pk.size(), 64);
     c->n_unique = n_unique; c->n_shared_unique = n_shared; c->n_masked_unique = n_masked;
@@ -212,6 +303,12 @@ int setup_impl(nk_ctx *c, const double *coords, const int64_t *glo_num, const do
 }
 
 }  // namespace
+
+extern "C" int nk_set_host_threads(int n)
+{
+    g_host_threads = n > 0 ? n : 0;
+    return NK_OK;
+}
 
 extern "C" int nk_setup(nk_ctx **ctx, int64_t E, int N, const double *coords, const int64_t *glo_num,
                         const double *mask, void *workspace, size_t workspace_bytes, void *stream)

@@ -180,3 +180,39 @@ def test_rotation_invariance_through_the_gpu_path():
     g1 = to_np(Nekbone(m.E, m.N, R @ m.coords, m.glo_num, m.mask).geom())
     sc = np.repeat(np.abs(g0.reshape(6, -1, 216)).max(axis=(0, 2)), 216)
     assert max(scaled_err(g1[a], g0[a], sc) for a in range(6)) <= 1e-13
+
+
+def test_plan_does_not_depend_on_host_threads():
+    """nk_setup builds the gather-scatter plan on all host cores (parallel radix sort, group walk cut at group
+    boundaries, chunked packing); the plan -- hence gs, ax and a CG solve with the fused gs, bit for bit -- must be
+    the one a single thread builds.  Irregular ids (rows of 3, 5, 12 copies) and a brick with several gs chunks."""
+    from paper_2606_12650_b200 import Nekbone
+    from paper_2606_12650_b200.binding import set_host_threads
+    m1 = brick_mesh(3, 2, 2, 4, 0.05)
+    rng = np.random.Generator(np.random.PCG64(13))
+    glo = rng.integers(0, 400, m1.L).astype(np.int64) * 1_000_003 + 17
+    glo[:12] = 5
+    mask = np.ones(m1.L)
+    mask[np.isin(glo, glo[100:110])] = 0.0
+    m2 = brick_mesh(24, 20, 16, 3, 0.05)                      # 7680 elements, 116 K summed rows: four gs chunks
+    cases = [(m1.E, m1.N, m1.coords, glo, mask), (m2.E, m2.N, m2.coords, m2.glo_num, m2.mask)]
+    for E, N, co, g, mk in cases:
+        L = E * (N + 1) ** 3
+        v = to_dev(rng.uniform(-1, 1, L))
+        _, inv = np.unique(g, return_inverse=True)
+        f = to_dev(rng.uniform(-1, 1, inv.max() + 1)[inv])
+        out = []
+        for threads in (1, 3, 0):
+            set_host_threads(threads)
+            gpu = Nekbone(E, N, co, g, mk)
+            gpu.set_option("coop", 0)
+            gpu.set_option("fuse_gs", 1)
+            x, h = gpu.cg(f, 10)
+            out.append((gpu.sizes(), gpu.gs_sizes(), to_np(gpu.gs(v.clone())), to_np(gpu.ax(v)), to_np(gpu.mult()),
+                        to_np(x), to_np(h)))
+            gpu.close()
+        set_host_threads(0)
+        for o in out[1:]:
+            assert o[0] == out[0][0] and o[1] == out[0][1]
+            for a, b in zip(o[2:], out[0][2:]):
+                assert np.array_equal(a, b)
