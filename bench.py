@@ -489,9 +489,9 @@ def run_ours(args) -> dict | None:
 
 # ---- our arm, sharded: ONE mesh over all ranks ------------------------------------------
 def run_sharded(args) -> dict | None:
-    """`--sharded`: the workload's mesh is partitioned by elements over the ranks (paper_2606_12650_b200.dist:
-    one all-gather for gs and two scalar all-gathers per iteration over NCCL), so total work is fixed: "strong"
-    scaling.  The default without the flag stays N independent replicas.  Needs a process group
+    """`--sharded`: the workload's mesh is partitioned by elements over the ranks (paper_2606_12650_b200.dist /
+    nk_dist_cg: one neighbour-wise halo exchange and two all-gathers of a double per iteration over NCCL), so total
+    work is fixed: "strong" scaling.  The default without the flag stays N independent replicas.  Needs a process group
     also at N = 1 (then it measures what the split-phase path costs against the fused nk_cg)."""
     import torch
     import torch.distributed as dist
@@ -566,7 +566,7 @@ def run_sharded(args) -> dict | None:
     ms_e2e = timed(e2e_step)
     ms, ms_e2e = max_over_ranks(dist, [ms, ms_e2e], "cuda")
     res_final = float(hist[-1])
-    n_slots = d.n_slots
+    n_nbr, n_xch, n_if_el = d.n_neighbors, d.n_exchange, d.n_interface_elements
     dist.barrier()
     dist.destroy_process_group()
     if rank != 0:
@@ -575,8 +575,9 @@ def run_sharded(args) -> dict | None:
            "steps": args.steps, "warmup": args.warmup, "ms_per_step": ms / args.steps, "higher_is_better": True,
            "scaling": "strong", "vs_baseline": None, "dtype": "f64", "data": "synthetic",
            "config": {**workload_config(args.workload, cfg, world),
-                      "parallelism": f"element partition over {world} rank(s); gs interface all-gather ({n_slots} slots) + "
-                                     "2 scalar all-gathers per iteration (NCCL)"},
+                      "parallelism": f"element partition over {world} rank(s): per iteration one neighbour-wise halo exchange "
+                                     f"(rank 0: {n_nbr} neighbours, {n_xch} doubles each way, overlapped with ax_e on the "
+                                     f"{d.nk.E - n_if_el} interior elements) + 2 all-gathers of one double (NCCL)"},
            "e2e": {"value": flops_step * args.steps / (ms_e2e * 1e-3) / 1e9, "unit": UNIT,
                    "h2d_bytes_per_step": 8 * d.L, "d2h_bytes_per_step": 8 * (d.L + niter + 1),
                    "ms_per_step": ms_e2e / args.steps},

@@ -109,44 +109,61 @@ int nk_cg_step(nk_ctx *ctx, double *x, void *stream);
 int nk_cg_get_state(nk_ctx *ctx, double *r, double *p, double *w, void *stream);
 int nk_get_scalars(nk_ctx *ctx, double *out5_host, void *stream);
 
-/* ---- Distributed gs / CG over an element partition, one rank per GPU ------------------------------
- * (PAPER.md:336 lists multi-rank runs as future work; the original
- * Nekbone is MPI.)  The context is set up on the rank's OWN elements with GLOBAL node ids.
- * Interface nodes (ids held by more than one rank) get one slot each in an exchange buffer; the plan
- * (paper_2606_12650_b200/dist.py builds it) is
- *   pack[n_slots]        local index of one copy of the slot's node, or -1 if this rank does not hold it
- *   unpack_loc/slot[n_unpack]   every local copy of an interface node and its slot
- * and the buffers are send[n_slots + 1], gathered[world * (n_slots + 1)] (rank-major), scalar_send[1],
- * scalar_gathered[world].  All DEVICE, owned by the caller, alive as long as the context is used this way.
- * The library enqueues kernels only; where a line says [all-gather A -> B] the caller runs that collective
- * on the same stream before the next call (NCCL all-gather through torch.distributed; every rank then holds
- * every rank's contribution and adds them in rank order, so results are bitwise equal across ranks and
- * reproducible).  Errors as elsewhere; NK_ERR_ARG before nk_dist_attach.
+/* ---- Distributed gs / CG over an element partition, one rank per GPU ------------------------------------
+ * (PAPER.md:336 lists multi-rank runs as future work; the original Nekbone is MPI,
+ * PAPER.md:225.)  Every rank calls nk_setup on ITS OWN elements with GLOBAL node ids; ax_e and the vector kernels
+ * are rank-local.  gs needs one neighbour-wise exchange of the partial sums of INTERFACE nodes (nodes another rank
+ * holds too), each of the two dot products of an iteration one all-gather of a double; all sums over ranks run
+ * in ascending rank order, so every rank holds the same bits and reruns are bitwise equal.  The library builds the
+ * plan, enqueues every kernel and drives the sequence; the transfers are the caller's, through a callback.
  *
- *   nk_dist_set_mult   replaces the LOCAL multiplicities by the given global ones (integers 1..127 as
- *                      doubles, L of them): the weights c = 1/mult of every dot product.  Synchronises.
- *   gs:    nk_dist_gs_begin(v)  [all-gather send -> gathered]  nk_dist_gs_end(v)
- *   dot:   nk_dist_dot_begin(a, b)  [all-gather scalar_send -> scalar_gathered]  nk_dist_dot_end(out)
- *   CG:    nk_dist_cg_begin(f, x)  [all-gather scalar]  nk_dist_cg_begin_end(hist0)
- *          per iteration k:  nk_dist_iter_a()            w = A_L p (pap partial in send[n_slots]), local gs + mask, pack
- *                            [all-gather send -> gathered]
- *                            nk_dist_iter_b()            w totals, alpha = rho / pap, r -= alpha w, rho' partial
- *                            [all-gather scalar]
- *                            nk_dist_iter_c(x, hist_k)   beta, sqrt(rho') -> hist_k, x += alpha p, p = r + beta p
+ *   nk_dist_candidates  HOST: the distinct global ids of the points on element boundaries (i, j or k in {0, N}),
+ *                       ascending -- the only nodes another rank can hold.  ids_out needs room for
+ *                       E ((N+1)^3 - (N-1)^3) ids.  Needs no context and no device.
+ *   nk_dist_setup       builds the plan from ALL ranks' candidate lists (HOST: cand_ids = the lists concatenated in
+ *                       rank order, cand_counts[world] their lengths; the caller gathers them, e.g. all_gather).
+ *                       glo_num HOST, L, as given to nk_setup.  Plan arrays are device memory the LIBRARY allocates
+ *                       (cudaMalloc; the one exception to "the caller owns all device memory"), freed by nk_free.
+ *                       Synchronises.  For the halo exchange to overlap ax_e inside nk_dist_cg, put the elements
+ *                       that touch another rank's FIRST in the rank's element order (nk_dist_info reports how far
+ *                       elements holding an interface node reach).
+ *   nk_dist_info        neighbours, doubles in the send (= receive) buffer, interface nodes, leading elements that
+ *                       hold interface nodes.  Any out pointer may be NULL.
+ *   nk_dist_neighbors   HOST out, one entry per neighbour (ascending rank): its rank, and offset and count of its
+ *                       segment in BOTH the send and the receive buffer (the two ranks list the nodes they share in
+ *                       ascending global id, so the layouts agree).
+ *   nk_dist_set_buffers DEVICE, caller-owned: send, recv (n_exchange doubles each; may be NULL if 0), scalar_send (1),
+ *                       scalar_gathered (world).
+ *   nk_dist_set_mult    replaces the LOCAL multiplicities by the given global ones (integers 1..127 as doubles, L of
+ *                       them: nk_dist_gs of ones): the weights c = 1/mult of every dot product.  Synchronises.
+ *   nk_exchange_fn      the caller's transfers, enqueued on `stream` (a cudaStream_t; inside nk_dist_cg the halo
+ *                       exchange gets a stream of the library's own).  kind & 1: for every neighbour send its
+ *                       segment of `send` and receive its segment of `recv` (one grouped NCCL send/recv);
+ *                       kind & 2: all-gather scalar_send[0] into scalar_gathered[0..world).  Return 0 on success.
+ *                       Not called where there is nothing to move (one rank; no neighbour).
+ *   nk_dist_gs          v <- Q Q^T v over ALL ranks, in place (and the Dirichlet mask if with_mask).
+ *   nk_dist_dot         out_dev[0] = <a,b>_c over all ranks.
+ *   nk_dist_cg          as nk_cg, over all ranks: per iteration ax_e on the interface elements, their partial sums
+ *                       out on a second stream while ax_e runs on the interior elements; all-gather of pap; the
+ *                       rank's own gs and mask; totals over the holders; r update; all-gather of rho'; x, p update.
+ *                       Three transfers and eight launches per iteration, no host synchronisation.  With one rank
+ *                       it IS nk_cg.  Errors as elsewhere; NK_ERR_ARG before nk_dist_setup / nk_dist_set_buffers.
  */
-int nk_dist_attach(nk_ctx *ctx, int rank, int world, int64_t n_slots, const int32_t *pack_dev, int64_t n_unpack,
-                   const int32_t *unpack_loc_dev, const int32_t *unpack_slot_dev, double *send_dev,
-                   double *gathered_dev, double *scalar_send_dev, double *scalar_gathered_dev);
+typedef int (*nk_exchange_fn)(void *user, int kind, void *stream);
+int nk_dist_candidates(int64_t E, int N, const int64_t *glo_num_host, int64_t *ids_out_host, int64_t *n_out_host);
+int nk_dist_setup(nk_ctx *ctx, int rank, int world, const int64_t *glo_num_host, const int64_t *cand_ids_host,
+                  const int64_t *cand_counts_host, void *stream);
+int nk_dist_info(nk_ctx *ctx, int *n_neighbors, int64_t *n_exchange, int64_t *n_interface_nodes,
+                 int64_t *n_interface_elements);
+int nk_dist_neighbors(nk_ctx *ctx, int *ranks_host, int64_t *offsets_host, int64_t *counts_host);
+int nk_dist_set_buffers(nk_ctx *ctx, double *send_dev, double *recv_dev, double *scalar_send_dev,
+                        double *scalar_gathered_dev);
 int nk_dist_set_mult(nk_ctx *ctx, const double *mult_dev, void *stream);
-int nk_dist_gs_begin(nk_ctx *ctx, double *v, int with_mask, void *stream);
-int nk_dist_gs_end(nk_ctx *ctx, double *v, void *stream);
-int nk_dist_dot_begin(nk_ctx *ctx, const double *a, const double *b, void *stream);
-int nk_dist_dot_end(nk_ctx *ctx, double *out_dev, void *stream);
-int nk_dist_cg_begin(nk_ctx *ctx, const double *f, double *x, void *stream);
-int nk_dist_cg_begin_end(nk_ctx *ctx, double *hist0_dev, void *stream);
-int nk_dist_iter_a(nk_ctx *ctx, void *stream);
-int nk_dist_iter_b(nk_ctx *ctx, void *stream);
-int nk_dist_iter_c(nk_ctx *ctx, double *x, double *hist_k_dev, void *stream);
+int nk_dist_gs(nk_ctx *ctx, double *v, int with_mask, nk_exchange_fn exchange, void *user, void *stream);
+int nk_dist_dot(nk_ctx *ctx, const double *a, const double *b, double *out_dev, nk_exchange_fn exchange, void *user,
+                void *stream);
+int nk_dist_cg(nk_ctx *ctx, const double *f, double *x, int niter, double *res_hist, nk_exchange_fn exchange,
+               void *user, void *stream);
 
 /* Options:
  *   "fuse_pap"     1 (default) = pap accumulated inside ax_e through the dot-fusion identity

@@ -20,6 +20,7 @@ NK_ERR_GEOM, NK_ERR_CUDA, NK_ERR_ALLOC, NK_ERR_MULT = -5, -6, -7, -8
 
 # every symbol include/nk.h declares: name -> (restype, argtypes)
 _vp, _i, _i64, _sz, _d = C.c_void_p, C.c_int, C.c_int64, C.c_size_t, C.c_double
+EXCHANGE_FN = C.CFUNCTYPE(C.c_int, C.c_void_p, C.c_int, C.c_void_p)        # nk_exchange_fn
 SIGNATURES = {
     "nk_workspace_bytes": (_i, [_i64, _i, C.POINTER(_sz)]),
     "nk_setup": (_i, [C.POINTER(_vp), _i64, _i, _vp, _vp, _vp, _vp, _sz, _vp]),
@@ -46,17 +47,15 @@ SIGNATURES = {
     "nk_get_geom": (_i, [_vp, _vp, _vp]),
     "nk_get_D": (_i, [_vp, _vp, _vp, _vp]),
     "nk_get_kernel_times": (_i, [_vp, _vp, _vp, _vp]),
-    "nk_dist_attach": (_i, [_vp, _i, _i, _i64, _vp, _i64, _vp, _vp, _vp, _vp, _vp, _vp]),
+    "nk_dist_candidates": (_i, [_i64, _i, _vp, _vp, C.POINTER(_i64)]),
+    "nk_dist_setup": (_i, [_vp, _i, _i, _vp, _vp, _vp, _vp]),
+    "nk_dist_info": (_i, [_vp, C.POINTER(_i), C.POINTER(_i64), C.POINTER(_i64), C.POINTER(_i64)]),
+    "nk_dist_neighbors": (_i, [_vp, _vp, _vp, _vp]),
+    "nk_dist_set_buffers": (_i, [_vp, _vp, _vp, _vp, _vp]),
     "nk_dist_set_mult": (_i, [_vp, _vp, _vp]),
-    "nk_dist_gs_begin": (_i, [_vp, _vp, _i, _vp]),
-    "nk_dist_gs_end": (_i, [_vp, _vp, _vp]),
-    "nk_dist_dot_begin": (_i, [_vp, _vp, _vp, _vp]),
-    "nk_dist_dot_end": (_i, [_vp, _vp, _vp]),
-    "nk_dist_cg_begin": (_i, [_vp, _vp, _vp, _vp]),
-    "nk_dist_cg_begin_end": (_i, [_vp, _vp, _vp]),
-    "nk_dist_iter_a": (_i, [_vp, _vp]),
-    "nk_dist_iter_b": (_i, [_vp, _vp]),
-    "nk_dist_iter_c": (_i, [_vp, _vp, _vp, _vp]),
+    "nk_dist_gs": (_i, [_vp, _vp, _i, _vp, _vp, _vp]),
+    "nk_dist_dot": (_i, [_vp, _vp, _vp, _vp, _vp, _vp, _vp]),
+    "nk_dist_cg": (_i, [_vp, _vp, _vp, _i, _vp, _vp, _vp, _vp]),
     "nk_get_launch_count": (_i, [_vp, C.POINTER(_i64)]),
     "nk_get_cg_path": (_i, [_vp, C.POINTER(_i), C.POINTER(_i)]),
     "nk_fp64_peak": (_i, [C.POINTER(_d), C.POINTER(_d), _vp]),

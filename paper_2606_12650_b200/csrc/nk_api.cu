@@ -80,6 +80,7 @@ void nk_free(nk_ctx *c)
 {
     if (!c) return;
     if (c->graph_exec) cudaGraphExecDestroy(c->graph_exec);
+    nk_dist_release(c);
     delete c->prof;
     delete c;
 }
@@ -212,7 +213,7 @@ int nk_dot(nk_ctx *c, const double *a, const double *b, double *out, void *strea
 // (measured: 7.8-13 us here, profiles/r2_sweep_coop.csv)
 static bool cg_uses_coop(const nk_ctx *c)
 {
-    return !c->opt_profile && c->coop_ok && nk_coop_supported(c->N) &&
+    return !c->opt_profile && c->coop_ok && nk_coop_supported(c->N) && !c->dist_mult &&
            (c->opt_coop == 1 || (c->opt_coop == 2 && c->L <= NK_COOP_AUTO_MAX_L));
 }
 

@@ -551,7 +551,7 @@ __device__ __forceinline__ double ax_compute(const AxSmem<N> &sm, double *u_rw, 
 template <int N, bool FUSEP>
 __global__ void __launch_bounds__(TmaCfg<N>::THREADS, 1)
 ax_tma_kernel(double *u_rw, const double *u_ro, const double *r_in,
-              double *__restrict__ w, const double2 *__restrict__ g, int64_t E, int dot, nk_reduce_ws red)
+              double *__restrict__ w, const double2 *__restrict__ g, int64_t e_begin, int64_t E, int dot, nk_reduce_ws red)
 {
     using C = TmaCfg<N>;
     extern __shared__ __align__(128) unsigned char smem_raw[];
@@ -564,7 +564,8 @@ ax_tma_kernel(double *u_rw, const double *u_ro, const double *r_in,
     // This CTA's elements: a contiguous range, equal over the CTAs to within one element (batches dealt round
     // robin left the last round 1/4 full on a 16^3 mesh at N = 9: one batch time of 10 lost).  The last batch of
     // a range may be partial.
-    const int64_t elo = E * (int64_t)blockIdx.x / gridDim.x, ehi = E * ((int64_t)blockIdx.x + 1) / gridDim.x;
+    // (E elements starting at e_begin: the whole mesh, or the interface / interior part of a rank's share)
+    const int64_t elo = e_begin + E * (int64_t)blockIdx.x / gridDim.x, ehi = e_begin + E * ((int64_t)blockIdx.x + 1) / gridDim.x;
     double dsum = 0.0;
     if (C::WGP) {
         if (tid >= C::CT) asm volatile("setmaxnreg.dec.sync.aligned.u32 24;");
@@ -898,18 +899,19 @@ cudaError_t launch_coop(nk_ctx *c, const double *f, double *x, int niter, double
 
 template <int N>
 cudaError_t launch_tma(nk_ctx *c, double *u_rw, const double *u_ro, const double *r_in, double *w, int dot,
-                       cudaStream_t st)
+                       int64_t e_begin, int64_t e_count, cudaStream_t st)
 {
     using C = TmaCfg<N>;
-    const int64_t nb = (c->E + C::EPB - 1) / C::EPB;
+    if (e_count <= 0) return cudaSuccess;
+    const int64_t nb = (e_count + C::EPB - 1) / C::EPB;
     const unsigned grid = (unsigned)(nb < (int64_t)c->sm_count ? nb : (int64_t)c->sm_count);   // one CTA per SM
     cudaError_t e;
     if (r_in != nullptr)
         e = nk_launch(ax_tma_kernel<N, true>, grid, C::THREADS, C::SMEM, st, c->pdl_now, u_rw, (const double *)nullptr, r_in, w,
-                      (const double2 *)c->g, c->E, dot, c->red);
+                      (const double2 *)c->g, e_begin, e_count, dot, c->red);
     else
         e = nk_launch(ax_tma_kernel<N, false>, grid, C::THREADS, C::SMEM, st, c->pdl_now, (double *)nullptr, u_ro,
-                      (const double *)nullptr, w, (const double2 *)c->g, c->E, dot, c->red);
+                      (const double *)nullptr, w, (const double2 *)c->g, e_begin, e_count, dot, c->red);
     c->launches++;
     return e != cudaSuccess ? e : cudaGetLastError();
 }
@@ -1032,8 +1034,14 @@ int nk_ax_tma_epb(int N)
 cudaError_t nk_launch_ax_tma(nk_ctx *c, double *u_rw, const double *u_ro, const double *r_in, double *w, int dot,
                              cudaStream_t st)
 {
+    return nk_launch_ax_tma_range(c, u_rw, u_ro, r_in, w, dot, 0, c->E, st);
+}
+
+cudaError_t nk_launch_ax_tma_range(nk_ctx *c, double *u_rw, const double *u_ro, const double *r_in, double *w, int dot,
+                                   int64_t e_begin, int64_t e_count, cudaStream_t st)
+{
     switch (c->N) {
-#define NK_CASE(NN) case NN: return launch_tma<NN>(c, u_rw, u_ro, r_in, w, dot, st);
+#define NK_CASE(NN) case NN: return launch_tma<NN>(c, u_rw, u_ro, r_in, w, dot, e_begin, e_count, st);
         NK_CASE(1) NK_CASE(2) NK_CASE(3) NK_CASE(4) NK_CASE(5) NK_CASE(6) NK_CASE(7) NK_CASE(8)
         NK_CASE(9) NK_CASE(10) NK_CASE(11) NK_CASE(12) NK_CASE(13) NK_CASE(14) NK_CASE(15)
 #undef NK_CASE

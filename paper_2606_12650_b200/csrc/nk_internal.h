@@ -31,6 +31,7 @@ enum { NK_EPI_STORE = 0,   // out[0] = total
 // kernel classes of nk_get_kernel_times
 enum { NK_K_AX = 0, NK_K_GS = 1, NK_K_DOT = 2, NK_K_UPDATE_XR = 3, NK_K_UPDATE_P = 4, NK_K_INIT = 5, NK_K_COUNT = 6 };
 struct nk_prof;     // nk_api.cu
+struct nk_dist;     // nk_dist.cu
 
 // Layout of the geometric factors in HBM: G[e][k][c2][t2] as double2, c2 = 0 (rr,rs),
 // 1 (rt,ss), 2 (st,tt), t2 = i + n j.  One element is one contiguous 48 P-byte chunk and one k-plane
@@ -100,12 +101,9 @@ struct nk_ctx {
     int64_t launches;
     // per-kernel-class device timing ("profile" option): chained events, interval i = kernel class cls[i]
     nk_prof *prof;
-    // distributed gs / CG (nk_dist.cu; S 8(e), 8(f) f-4): interface plan and exchange buffers, all DEVICE
-    // and owned by the caller (nk_dist_attach)
-    int dist_rank, dist_world;
-    int64_t dist_slots, dist_n_unpack;
-    const int32_t *dist_pack, *dist_uloc, *dist_uslot;
-    double *dist_send, *dist_gath, *dist_ssend, *dist_sgath;
+    // distributed gs / CG (nk_dist.cu; S 8(e), 8(f) f-4): the interface plan, library-owned
+    struct nk_dist *dist;
+    int dist_mult;               // 1: the weights c = 1/multiplicity are GLOBAL (nk_dist_set_mult); rank-local shortcuts are off
     // cached graph for nk_cg
     cudaGraphExec_t graph_exec;
     const double *graph_f; double *graph_x; double *graph_hist; int graph_niter; int graph_key;
@@ -137,6 +135,8 @@ inline cudaError_t nk_launch(void (*kernel)(KArgs...), dim3 grid, dim3 block, si
 #endif
 
 // ---- kernels' host launchers (each returns a cudaError_t from the launch) -----------------------
+// nk_dist.cu
+void nk_dist_release(nk_ctx *c);              // frees the distributed plan (nk_free)
 // nk_basis.cpp
 void nk_host_basis(int N, double *xi, double *w, double *D);
 void nk_host_basis_dd(int N, double *xi, double *w, double *D, double *Dlo);   // D = D + Dlo (long double split)
@@ -144,6 +144,9 @@ void nk_host_basis_dd(int N, double *xi, double *w, double *D, double *Dlo);   /
 // first and written back to u.  If dot: sum_l u_l w_l is reduced with epilogue NK_EPI_PAP.
 cudaError_t nk_launch_ax_tma(nk_ctx *c, double *u_rw, const double *u_ro, const double *r_in, double *w,
                              int dot, cudaStream_t st);
+// the same on elements [e_begin, e_begin + e_count) only (distributed path: interface elements first, then the rest)
+cudaError_t nk_launch_ax_tma_range(nk_ctx *c, double *u_rw, const double *u_ro, const double *r_in, double *w, int dot,
+                                   int64_t e_begin, int64_t e_count, cudaStream_t st);
 cudaError_t nk_upload_D_tables_tma(void);
 int nk_ax_tma_epb(int N);
 int nk_coop_supported(int N);

@@ -1,6 +1,6 @@
 """Several ranks of paper_2606_12650_b200.dist inside ONE process (one GPU): every rank is a host thread
-running the same SPMD code as under torchrun; the communicator's all-gather is a device copy between the
-ranks' buffers, ordered by stream synchronisation and a host barrier (no kernel waits on another)."""
+running the same SPMD code as under torchrun; the communicator's all-gather and neighbour exchange are device copies
+between the ranks' buffers, ordered by stream synchronisation and a host barrier (no kernel waits on another)."""
 import threading
 
 
@@ -33,6 +33,25 @@ class ThreadComm:
         rows = out.view(self.world, -1)
         for r in range(self.world):
             rows[r].copy_(sh.slots[r])
+        if send.is_cuda:
+            torch.cuda.synchronize()
+        sh.barrier.wait()
+
+
+    def exchange(self, send, recv, neighbours):
+        """Segment [off, off + cnt) of `send` to, and of `recv` from, every neighbour: device copies between the ranks'
+        buffers (each rank publishes its buffer and where each neighbour's segment sits in it)."""
+        import torch
+        sh = self._sh
+        if send.is_cuda:
+            torch.cuda.synchronize()
+        sh.slots[self.rank] = (send, {r: (off, cnt) for r, off, cnt in neighbours})
+        sh.barrier.wait()
+        for r, off, cnt in neighbours:
+            theirs, table = sh.slots[r]
+            toff, tcnt = table[self.rank]
+            assert tcnt == cnt, "the two ranks disagree on how many nodes they share"
+            recv[off:off + cnt].copy_(theirs[toff:toff + tcnt])
         if send.is_cuda:
             torch.cuda.synchronize()
         sh.barrier.wait()
