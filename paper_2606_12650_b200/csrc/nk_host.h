@@ -36,7 +36,8 @@ inline nk_carve nk_carve_sizes(int64_t L)
     c.idx = nk_align_up((size_t)L * sizeof(int32_t), 256);
     c.nbr = nk_align_up((size_t)L * sizeof(int32_t), 256);         // per-point gather code of the fused gs (nk_ctx::nbr)
     // its side table: rows of 3 or more copies, at most 8 ints per 3 listed points (header + alignment),
-    c.gx = nk_align_up((9 * ((size_t)L / 3 + 1) + 16) * sizeof(int32_t), 256);   // + one int per such row (gx_rows)
+    c.gx = nk_align_up((9 * ((size_t)L / 3 + 1) + 16 + 65536 + 8) * sizeof(int32_t), 256);   // + one int per such row (gx_rows)
+                                                                                  // + the per-block cut of that list (gx_blk)
     // packed rows (<= L indices + 16 padding ints per chunk) and 8 ints of descriptor per chunk
     c.pk = nk_align_up(((size_t)L + 24 * ((size_t)L / (2 * NK_GS_CHUNK) + 2) + 256) * sizeof(int32_t), 256);
     c.tabs = nk_align_up(2 * NK_CTAB * sizeof(double) + (16 * 16 + 16) * sizeof(double), 256);

@@ -80,6 +80,7 @@ struct nk_ctx {
     //                 p = -nbr[l]-2, gx[4p-1] = their number and gx[4p ..] their local indices, ascending
     //                 (16-byte aligned so that the first eight come with two vector loads)
     int32_t *nbr, *gx, *gx_rows;   // gx_rows[k] = p of the k-th such node (one thread each in the fused kernel)
+    int32_t *gx_blk;               // nk_vec_blocks(L/2) + 1 ints: block b of the fused kernel takes nodes [gx_blk[b], gx_blk[b+1])
     int64_t n_gx_rows;
     int64_t n_gs_chunks;
     double *ctab;                // NK_CTAB doubles: 1/multiplicity
@@ -133,6 +134,22 @@ inline cudaError_t nk_launch(void (*kernel)(KArgs...), dim3 grid, dim3 block, si
     return cudaLaunchKernelEx(&cfg, kernel, KArgs(args)...);
 }
 #endif
+
+// Grid of the streaming kernels (nk_vec.cu) and of the row cut nk_setup makes for the fused gs (gx_blk): at least two
+// blocks per SM when there is work for them, then 8 pairs per thread (fewer, fatter blocks: less reduction tail on
+// mid-size meshes; config 3: 12.4 -> 11.7 ms per solve), capped at 4 resident blocks/SM x 4 waves.
+// Fixed grid => fixed partial sums => run-to-run bitwise reproducible.
+static inline int nk_vec_blocks(int sm_count, int64_t pairs)
+{
+    const int64_t one = (pairs + NK_VEC_THREADS - 1) / NK_VEC_THREADS;
+    const int64_t floor2 = (int64_t)sm_count * 2, cap = (int64_t)sm_count * 4 * 4;
+    int64_t want = (pairs + NK_VEC_THREADS * 8 - 1) / (NK_VEC_THREADS * 8);
+    const int64_t lo = one < floor2 ? one : floor2;
+    if (want < lo) want = lo;
+    if (want > cap) want = cap;
+    if (want < 1) want = 1;
+    return (int)want;
+}
 
 // ---- kernels' host launchers (each returns a cudaError_t from the launch) -----------------------
 // nk_dist.cu

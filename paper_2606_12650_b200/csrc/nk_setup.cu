@@ -256,6 +256,20 @@ int setup_impl(nk_ctx *c, const double *coords, const int64_t *glo_num, const do
     gx.resize((gx.size() + 12 + 3) / 4 * 4, 0);              // vector loads of the last row stay in bounds; 16-byte multiple
     c->n_gx_rows = (int64_t)gx_rows.size();
     c->gx_rows = c->gx + gx.size();
+    // the list cut by the chunks of the fused kernel's blocks: a node goes to the block whose chunk holds its first copy
+    const int nvb = nk_vec_blocks(c->sm_count, L >> 1);
+    std::vector<int32_t> gx_blk((size_t)nvb + 1);
+    {
+        const int64_t pairs = L >> 1;
+        size_t k = 0;
+        for (int b = 0; b <= nvb; ++b) {
+            const int64_t first_point = b == nvb ? L + 1 : 2 * (pairs * (int64_t)b / nvb);
+            while (k < gx_rows.size() && (int64_t)gx[4 * (size_t)gx_rows[k]] < first_point) ++k;
+            gx_blk[(size_t)b] = (int32_t)k;
+        }
+        gx_blk[0] = 0;
+    }
+    c->gx_blk = c->gx_rows + ((gx_rows.size() + 3) / 4 * 4);
 #pragma omp parallel for schedule(static) num_threads(T)
     for (int64_t r = 0; r < (int64_t)msk_rows.size(); ++r) {
         const Row &row = msk_rows[(size_t)r];
@@ -278,6 +292,7 @@ int setup_impl(nk_ctx *c, const double *coords, const int64_t *glo_num, const do
     NK_CUDA(cudaMemcpyAsync(c->gx, gx.data(), gx.size() * sizeof(int32_t), cudaMemcpyHostToDevice, st));
     if (!gx_rows.empty())
         NK_CUDA(cudaMemcpyAsync(c->gx_rows, gx_rows.data(), gx_rows.size() * sizeof(int32_t), cudaMemcpyHostToDevice, st));
+    NK_CUDA(cudaMemcpyAsync(c->gx_blk, gx_blk.data(), gx_blk.size() * sizeof(int32_t), cudaMemcpyHostToDevice, st));
     NK_CUDA(cudaMemcpyAsync(c->gs_desc, desc.data(), desc.size() * sizeof(int32_t), cudaMemcpyHostToDevice, st));
     NK_CUDA(cudaMemcpyAsync(c->ctab, ctab, sizeof(ctab), cudaMemcpyHostToDevice, st));
     NK_CUDA(cudaMemcpyAsync(c->mtab, mtab, sizeof(mtab), cudaMemcpyHostToDevice, st));

@@ -16,20 +16,7 @@ namespace {
 // set-up data (code, ctab, nbr, gx, dinv) keeps the qualifiers: fetching it before the wait is the point.
 //
 // Fixed grid => fixed partial sums => run-to-run bitwise reproducible.
-inline int vec_blocks(const nk_ctx *c, int64_t pairs)
-{
-    // at least two blocks per SM when there is work for them, then 8 pairs per thread (fewer, fatter
-    // blocks: less reduction tail on mid-size meshes; config 3: 12.4 -> 11.7 ms per solve), capped at
-    // 4 resident blocks/SM x 4 waves
-    const int64_t one = (pairs + NK_VEC_THREADS - 1) / NK_VEC_THREADS;
-    const int64_t floor2 = (int64_t)c->sm_count * 2, cap = (int64_t)c->sm_count * 4 * 4;
-    int64_t want = (pairs + NK_VEC_THREADS * 8 - 1) / (NK_VEC_THREADS * 8);
-    const int64_t lo = one < floor2 ? one : floor2;
-    if (want < lo) want = lo;
-    if (want > cap) want = cap;
-    if (want < 1) want = 1;
-    return (int)want;
-}
+inline int vec_blocks(const nk_ctx *c, int64_t pairs) { return nk_vec_blocks(c->sm_count, pairs); }
 
 __device__ __forceinline__ void load_ctab(double *s_c, const double *ctab)
 {
@@ -140,22 +127,23 @@ update_xr_kernel(double *__restrict__ x, double *__restrict__ r, const double *p
 // quadratic form).  So w need never be summed IN PLACE: this kernel streams the UNSUMMED ax_e output and sums
 // the copies of shared nodes on the fly.  gs's write-back (8 B per listed copy, 32 B where the copy is alone in
 // its sector: the stride-n r-faces), its re-read by the update and one launch per iteration are gone.
-// Two kinds of blocks in one launch:
-//   * streaming blocks, one pass over all points.  A point whose node has no other copy keeps its value; a point
-//     of a multiplicity-2 node (faces: 82 % of the shared points of a brick) adds its ONE partner, whose index
-//     nbr[l] was fetched one step ahead so that the gather is issued together with the streaming loads (the
-//     sector it hits is one a neighbouring block streams anyway); a Dirichlet point takes 0; a point of a node
-//     with three or more copies (edges, corners) is SKIPPED;
-//   * row blocks, interleaved with the first streaming blocks of the grid (their chains of dependent loads run
-//     while the streaming blocks keep HBM busy): one thread per node with three or more copies gathers w and r of all its
-//     copies (indices by vector load from gx), sums in ascending local index as nk_gs.cu does, and updates r at
-//     every copy.  Inlined into the streaming loop this work cost two dependent memory round trips in nearly
-//     every warp (one edge point among 32 lanes is enough) and tripled the time of the pass.
+// Every block takes a contiguous chunk of the vectors and does two things:
+//   * it streams the chunk.  A point whose node has no other copy keeps its value; a point of a multiplicity-2
+//     node (faces: 82 % of the shared points of a brick) adds its ONE partner, whose index nbr[l] was fetched one
+//     step ahead so that the gather is issued together with the streaming loads; a Dirichlet point takes 0; a
+//     point of a node with three or more copies (edges, corners) is SKIPPED;
+//   * it then handles the nodes with three or more copies whose first copy lies in the chunk, one thread each:
+//     gathers w and r of all copies (indices by vector load from gx), sums in ascending local index as nk_gs.cu
+//     does, and updates r at every copy.  (Inlined into the streaming loop this work cost two dependent memory
+//     round trips in nearly every warp -- one edge point among 32 lanes is enough -- and tripled the time of the
+//     pass; given to blocks of their own, far from where the chunk's data is in L2, it cost 0.3 GB of DRAM traffic.)
+// Blocks run in index order, so the resident ones form a window of some tens of MB that moves through the
+// vectors once: partners 14 KB (r-faces), 0.4 MB (s-faces) or 14 MB (t-faces, config 5) away are L2 hits.
 // r, x are the values of nk_gs followed by the plain update, entry by entry; rho' sums the same terms in another
 // (fixed) order.  Run-to-run bitwise reproducible like every reduction here.
 struct nk_gather {
     const int32_t *nbr, *gx, *rows;     // nk_internal.h nk_ctx::nbr, gx; rows[k] = p of the k-th node with >= 3 copies
-    int n_rows, row_blocks;
+    const int32_t *blk;                 // rows [blk[b], blk[b+1]) have their first copy in block b's chunk of the vector
 };
 
 __device__ __forceinline__ double gs_partner(const double *w, int l, int v)
@@ -170,6 +158,38 @@ __device__ __forceinline__ double gs_stream_value(int l, int v, double wl, doubl
     return (v == l) ? wl : (v >= 0 ? sum : 0.0);
 }
 
+// one node with three or more copies: r -= alpha sum at every copy; returns its share of rho'
+__device__ __forceinline__ double gs_row_update(const double *w, double *r, const uint8_t *__restrict__ code,
+                                                const double *s_c, const int32_t *__restrict__ gx, int p4, double alpha)
+{
+    const int4 ia = reinterpret_cast<const int4 *>(gx)[p4];
+    const int len = gx[4 * p4 - 1];
+    double acc = 0.0;
+    if (len == 4) {                                       // an edge of a conforming hex mesh
+        const double a0 = w[ia.x], a1 = w[ia.y], a2 = w[ia.z], a3 = w[ia.w];
+        double r0 = r[ia.x], r1 = r[ia.y], r2 = r[ia.z], r3 = r[ia.w];
+        const double cw = s_c[code[ia.x] & 0x7f];
+        const double s = ((a0 + a1) + a2) + a3;
+        r0 = fma(-alpha, s, r0); r1 = fma(-alpha, s, r1); r2 = fma(-alpha, s, r2); r3 = fma(-alpha, s, r3);
+        r[ia.x] = r0; r[ia.y] = r1; r[ia.z] = r2; r[ia.w] = r3;
+        acc = fma(cw * r0, r0, acc); acc = fma(cw * r1, r1, acc);
+        acc = fma(cw * r2, r2, acc); acc = fma(cw * r3, r3, acc);
+        return acc;
+    }
+    const int32_t *ii = gx + 4 * (int64_t)p4;
+    double s = w[ii[0]];
+    for (int j = 1; j < len; ++j) s += w[ii[j]];
+    const double cw = s_c[code[ii[0]] & 0x7f];
+    for (int j = 0; j < len; ++j) {
+        const double rn = fma(-alpha, s, r[ii[j]]);
+        r[ii[j]] = rn;
+        acc = fma(cw * rn, rn, acc);
+    }
+    return acc;
+}
+
+constexpr int GS_U = 2;                                   // pairs per thread and step of the large-mesh variant
+
 template <bool WITH_X>
 __global__ void __launch_bounds__(NK_VEC_THREADS, 2)
 gs_update_kernel(double *__restrict__ x, double *r, const double *p, const double *w,
@@ -181,141 +201,109 @@ gs_update_kernel(double *__restrict__ x, double *r, const double *p, const doubl
     nk_pdl_launch_dependents();
     load_ctab(s_c, ctab);
     double acc = 0.0;
-    // block roles: b < 2 R alternates stream / row, the rest streams (R = row blocks; the launcher keeps R <= stream blocks)
-    const int stream_blocks = (int)gridDim.x - gp.row_blocks;
-    const int b = (int)blockIdx.x;
-    const bool row_role = b < 2 * gp.row_blocks && (b & 1);
-    const int role_id = b < 2 * gp.row_blocks ? (b >> 1) : b - gp.row_blocks;
-    if (row_role) {
-        // ---- row blocks: nodes with three or more copies ------------------------------------------------------
-        const int k = role_id * NK_VEC_THREADS + threadIdx.x;
-        const bool on = k < gp.n_rows;
-        int p4 = 0, len = 0;
-        int4 ia = make_int4(0, 0, 0, 0);
-        if (on) {                                             // the plan is static: fetched before the wait
-            p4 = gp.rows[k];
-            ia = reinterpret_cast<const int4 *>(gp.gx)[p4];
-            len = gp.gx[4 * p4 - 1];
-        }
-        nk_pdl_wait();
-        const double alpha = ws.scal[NK_S_ALPHA];
-        if (on && len == 4) {                                 // an edge of a conforming hex mesh
-            const double a0 = w[ia.x], a1 = w[ia.y], a2 = w[ia.z], a3 = w[ia.w];
-            double r0 = r[ia.x], r1 = r[ia.y], r2 = r[ia.z], r3 = r[ia.w];
-            const double cw = s_c[code[ia.x] & 0x7f];
-            const double s = ((a0 + a1) + a2) + a3;
-            r0 = fma(-alpha, s, r0); r1 = fma(-alpha, s, r1); r2 = fma(-alpha, s, r2); r3 = fma(-alpha, s, r3);
-            r[ia.x] = r0; r[ia.y] = r1; r[ia.z] = r2; r[ia.w] = r3;
-            acc = fma(cw * r0, r0, acc); acc = fma(cw * r1, r1, acc);
-            acc = fma(cw * r2, r2, acc); acc = fma(cw * r3, r3, acc);
-        } else if (on) {
-            const int32_t *ii = gp.gx + 4 * (int64_t)p4;
-            double s = w[ii[0]];
-            for (int j = 1; j < len; ++j) s += w[ii[j]];
-            const double cw = s_c[code[ii[0]] & 0x7f];
-            for (int j = 0; j < len; ++j) {
-                const double rn = fma(-alpha, s, r[ii[j]]);
-                r[ii[j]] = rn;
-                acc = fma(cw * rn, rn, acc);
-            }
-        }
-    } else {
-        // ---- streaming blocks ------------------------------------------------------------------------------------
-        const int64_t pairs = L >> 1;
-        const int64_t bs = role_id;
-        const int64_t stride = (int64_t)stream_blocks * blockDim.x;
-        constexpr int U = WITH_X ? 1 : 2;                     // pairs per step, all loads before the stores
-        int64_t q = bs * blockDim.x + threadIdx.x;
-        int2 nv[U];
+    // this block's CONTIGUOUS chunk of pairs (blocks run in index order, so the resident blocks form one window
+    // that moves through the vectors: a partner a few KB or MB away is in L2 when it is gathered)
+    const int64_t pairs = L >> 1;
+    const int64_t plo = pairs * (int64_t)blockIdx.x / gridDim.x, phi = pairs * ((int64_t)blockIdx.x + 1) / gridDim.x;
+    const int64_t stride = blockDim.x;
+    constexpr int U = WITH_X ? 1 : GS_U;                      // pairs per step, all loads before the stores
+    int64_t q = plo + threadIdx.x;
+    int2 nv[U];
 #pragma unroll
-        for (int j = 0; j < U; ++j)                           // gather codes of the first step: static, before the wait
-            nv[j] = (q + j * stride < pairs) ? reinterpret_cast<const int2 *>(gp.nbr)[q + j * stride] : make_int2(0, 0);
-        nk_pdl_wait();
-        const double alpha = ws.scal[NK_S_ALPHA];
-        for (; q + (U - 1) * stride < pairs; q += U * stride) {
-            double2 wv[U], rv[U], g[U], xv[WITH_X ? U : 1], pv[WITH_X ? U : 1];
-            uchar2 cd[U];
-            int2 nn[U];
+    for (int j = 0; j < U; ++j)                               // gather codes of the first step: static, before the wait
+        nv[j] = (q + j * stride < phi) ? reinterpret_cast<const int2 *>(gp.nbr)[q + j * stride] : make_int2(0, 0);
+    nk_pdl_wait();
+    const double alpha = ws.scal[NK_S_ALPHA];
+    // (Staging the streamed operands through shared memory with cp.async, four pairs per thread in flight instead of
+    //  two, was measured SLOWER: 394 vs 369 us at config 5 -- the pass is bound by the gathers' sector requests, not by
+    //  bytes in flight.)
+    for (; q + (U - 1) * stride < phi; q += U * stride) {
+        double2 wv[U], rv[U], g[U], xv[WITH_X ? U : 1], pv[WITH_X ? U : 1];
+        uchar2 cd[U];
+        int2 nn[U];
 #pragma unroll
-            for (int j = 0; j < U; ++j) {
-                const int64_t qj = q + j * stride;
-                wv[j] = reinterpret_cast<const double2 *>(w)[qj];
-                rv[j] = reinterpret_cast<const double2 *>(r)[qj];
-                cd[j] = reinterpret_cast<const uchar2 *>(code)[qj];
-                g[j].x = gs_partner(w, (int)(2 * qj), nv[j].x);
-                g[j].y = gs_partner(w, (int)(2 * qj) + 1, nv[j].y);
-                if (WITH_X) {
-                    xv[WITH_X ? j : 0] = reinterpret_cast<const double2 *>(x)[qj];
-                    pv[WITH_X ? j : 0] = reinterpret_cast<const double2 *>(p)[qj];
-                }
-            }
-#pragma unroll
-            for (int j = 0; j < U; ++j) {                     // next step's gather codes
-                const int64_t qn = q + (U + j) * stride;
-                nn[j] = (qn < pairs) ? reinterpret_cast<const int2 *>(gp.nbr)[qn] : make_int2(0, 0);
-            }
-#pragma unroll
-            for (int j = 0; j < U; ++j) {
-                const int64_t qj = q + j * stride;
-                const int l = (int)(2 * qj);
-                bool k0, k1;
-                const double s0 = gs_stream_value(l, nv[j].x, wv[j].x, g[j].x, k0);
-                const double s1 = gs_stream_value(l + 1, nv[j].y, wv[j].y, g[j].y, k1);
-                rv[j].x = fma(-alpha, s0, rv[j].x);
-                rv[j].y = fma(-alpha, s1, rv[j].y);
-                if (!(k0 || k1)) {
-                    reinterpret_cast<double2 *>(r)[qj] = rv[j];
-                } else {                                      // a row block owns the other entry of the pair
-                    if (!k0) r[l] = rv[j].x;
-                    if (!k1) r[l + 1] = rv[j].y;
-                }
-                acc = fma((k0 ? 0.0 : s_c[cd[j].x & 0x7f]) * rv[j].x, rv[j].x, acc);
-                acc = fma((k1 ? 0.0 : s_c[cd[j].y & 0x7f]) * rv[j].y, rv[j].y, acc);
-                if (WITH_X) {
-                    double2 xn = xv[WITH_X ? j : 0];
-                    xn.x = fma(alpha, pv[WITH_X ? j : 0].x, xn.x);
-                    xn.y = fma(alpha, pv[WITH_X ? j : 0].y, xn.y);
-                    reinterpret_cast<double2 *>(x)[qj] = xn;
-                }
-                nv[j] = nn[j];
-            }
-        }
-        for (; q < pairs; q += stride) {
-            const int2 n2 = reinterpret_cast<const int2 *>(gp.nbr)[q];
-            const double2 wv = reinterpret_cast<const double2 *>(w)[q];
-            double2 rv = reinterpret_cast<const double2 *>(r)[q];
-            const uchar2 cd = reinterpret_cast<const uchar2 *>(code)[q];
-            const int l = (int)(2 * q);
-            bool k0, k1;
-            const double s0 = gs_stream_value(l, n2.x, wv.x, gs_partner(w, l, n2.x), k0);
-            const double s1 = gs_stream_value(l + 1, n2.y, wv.y, gs_partner(w, l + 1, n2.y), k1);
-            rv.x = fma(-alpha, s0, rv.x);
-            rv.y = fma(-alpha, s1, rv.y);
-            if (!k0) r[l] = rv.x;
-            if (!k1) r[l + 1] = rv.y;
-            acc = fma((k0 ? 0.0 : s_c[cd.x & 0x7f]) * rv.x, rv.x, acc);
-            acc = fma((k1 ? 0.0 : s_c[cd.y & 0x7f]) * rv.y, rv.y, acc);
+        for (int j = 0; j < U; ++j) {
+            const int64_t qj = q + j * stride;
+            wv[j] = reinterpret_cast<const double2 *>(w)[qj];
+            rv[j] = reinterpret_cast<const double2 *>(r)[qj];
+            cd[j] = reinterpret_cast<const uchar2 *>(code)[qj];
+            g[j].x = gs_partner(w, (int)(2 * qj), nv[j].x);
+            g[j].y = gs_partner(w, (int)(2 * qj) + 1, nv[j].y);
             if (WITH_X) {
-                double2 xn = reinterpret_cast<const double2 *>(x)[q];
-                const double2 pv = reinterpret_cast<const double2 *>(p)[q];
-                xn.x = fma(alpha, pv.x, xn.x);
-                xn.y = fma(alpha, pv.y, xn.y);
-                reinterpret_cast<double2 *>(x)[q] = xn;
+                xv[WITH_X ? j : 0] = reinterpret_cast<const double2 *>(x)[qj];
+                pv[WITH_X ? j : 0] = reinterpret_cast<const double2 *>(p)[qj];
             }
         }
-        if ((L & 1) && bs == 0 && threadIdx.x == 0) {
-            const int l = (int)(L - 1);
-            const int v = gp.nbr[l];
-            bool k0;
-            const double s0 = gs_stream_value(l, v, w[l], gs_partner(w, l, v), k0);
-            if (!k0) {
-                const double rn = fma(-alpha, s0, r[l]);
-                r[l] = rn;
-                acc = fma(s_c[code[l] & 0x7f] * rn, rn, acc);
+#pragma unroll
+        for (int j = 0; j < U; ++j) {                         // next step's gather codes
+            const int64_t qn = q + (U + j) * stride;
+            nn[j] = (qn < phi) ? reinterpret_cast<const int2 *>(gp.nbr)[qn] : make_int2(0, 0);
+        }
+#pragma unroll
+        for (int j = 0; j < U; ++j) {
+            const int64_t qj = q + j * stride;
+            const int l = (int)(2 * qj);
+            bool k0, k1;
+            const double s0 = gs_stream_value(l, nv[j].x, wv[j].x, g[j].x, k0);
+            const double s1 = gs_stream_value(l + 1, nv[j].y, wv[j].y, g[j].y, k1);
+            rv[j].x = fma(-alpha, s0, rv[j].x);
+            rv[j].y = fma(-alpha, s1, rv[j].y);
+            if (!(k0 || k1)) {
+                reinterpret_cast<double2 *>(r)[qj] = rv[j];
+            } else {                                          // gs_row_update owns the other entry of the pair
+                if (!k0) r[l] = rv[j].x;
+                if (!k1) r[l + 1] = rv[j].y;
             }
-            if (WITH_X) x[l] = fma(alpha, p[l], x[l]);
+            acc = fma((k0 ? 0.0 : s_c[cd[j].x & 0x7f]) * rv[j].x, rv[j].x, acc);
+            acc = fma((k1 ? 0.0 : s_c[cd[j].y & 0x7f]) * rv[j].y, rv[j].y, acc);
+            if (WITH_X) {
+                double2 xn = xv[WITH_X ? j : 0];
+                xn.x = fma(alpha, pv[WITH_X ? j : 0].x, xn.x);
+                xn.y = fma(alpha, pv[WITH_X ? j : 0].y, xn.y);
+                reinterpret_cast<double2 *>(x)[qj] = xn;
+            }
+            nv[j] = nn[j];
         }
     }
+    for (; q < phi; q += stride) {
+        const int2 n2 = reinterpret_cast<const int2 *>(gp.nbr)[q];
+        const double2 wv = reinterpret_cast<const double2 *>(w)[q];
+        double2 rv = reinterpret_cast<const double2 *>(r)[q];
+        const uchar2 cd = reinterpret_cast<const uchar2 *>(code)[q];
+        const int l = (int)(2 * q);
+        bool k0, k1;
+        const double s0 = gs_stream_value(l, n2.x, wv.x, gs_partner(w, l, n2.x), k0);
+        const double s1 = gs_stream_value(l + 1, n2.y, wv.y, gs_partner(w, l + 1, n2.y), k1);
+        rv.x = fma(-alpha, s0, rv.x);
+        rv.y = fma(-alpha, s1, rv.y);
+        if (!k0) r[l] = rv.x;
+        if (!k1) r[l + 1] = rv.y;
+        acc = fma((k0 ? 0.0 : s_c[cd.x & 0x7f]) * rv.x, rv.x, acc);
+        acc = fma((k1 ? 0.0 : s_c[cd.y & 0x7f]) * rv.y, rv.y, acc);
+        if (WITH_X) {
+            double2 xn = reinterpret_cast<const double2 *>(x)[q];
+            const double2 pv = reinterpret_cast<const double2 *>(p)[q];
+            xn.x = fma(alpha, pv.x, xn.x);
+            xn.y = fma(alpha, pv.y, xn.y);
+            reinterpret_cast<double2 *>(x)[q] = xn;
+        }
+    }
+    if ((L & 1) && blockIdx.x == gridDim.x - 1 && threadIdx.x == 0) {
+        const int l = (int)(L - 1);
+        const int v = gp.nbr[l];
+        bool k0;
+        const double s0 = gs_stream_value(l, v, w[l], gs_partner(w, l, v), k0);
+        if (!k0) {
+            const double rn = fma(-alpha, s0, r[l]);
+            r[l] = rn;
+            acc = fma(s_c[code[l] & 0x7f] * rn, rn, acc);
+        }
+        if (WITH_X) x[l] = fma(alpha, p[l], x[l]);
+    }
+    // the nodes with three or more copies whose FIRST copy lies in this block's chunk (their other copies sit in
+    // neighbouring chunks: in L2, just streamed or about to be), one thread each
+    for (int k = gp.blk[blockIdx.x] + (int)threadIdx.x; k < gp.blk[blockIdx.x + 1]; k += blockDim.x)
+        acc += gs_row_update(w, r, code, s_c, gp.gx, gp.rows[k], alpha);
     nk_grid_reduce(acc, s_red, ws, NK_EPI_RHO, hist_k);
 }
 
@@ -551,12 +539,8 @@ template <bool WITH_X>
 cudaError_t launch_gs_update(nk_ctx *c, double *x, double *hist_k, cudaStream_t st)
 {
     nk_gather gp;
-    gp.nbr = c->nbr; gp.gx = c->gx; gp.rows = c->gx_rows;
-    gp.n_rows = (int)c->n_gx_rows;
-    gp.row_blocks = (int)((c->n_gx_rows + NK_VEC_THREADS - 1) / NK_VEC_THREADS);
-    int nbs = vec_blocks(c, c->L >> 1);
-    if (nbs < gp.row_blocks) nbs = gp.row_blocks;               // the kernel's role map wants stream blocks >= row blocks
-    const int nb = nbs + gp.row_blocks;
+    gp.nbr = c->nbr; gp.gx = c->gx; gp.rows = c->gx_rows; gp.blk = c->gx_blk;
+    const int nb = vec_blocks(c, c->L >> 1);                      // the grid nk_setup cut the row list for (gx_blk)
     const cudaError_t e = nk_launch(gs_update_kernel<WITH_X>, nb, NK_VEC_THREADS, 0, st, c->pdl_now == 2, x, c->r,
                                     (const double *)c->p, (const double *)c->w, (const uint8_t *)c->code,
                                     (const double *)c->ctab, c->L, c->red, hist_k, gp);
