@@ -1,6 +1,6 @@
 """Build libnk.so in-tree with nvcc for sm_100a (cross-compiles without a GPU).
 
-    python -m paper_2606_12650_b200.build [--force] [--verbose]
+    python -m paper_2606_12650_b200.build [--force] [--verbose] | --census
 
 Objects are compiled in parallel (one nvcc per translation unit) into csrc/build/, then linked
 into paper_2606_12650_b200/libnk.so.  The .so is git-ignored but travels to the GPU box.
@@ -63,6 +63,73 @@ def build(force: bool = False, verbose: bool = False) -> str:
     return LIB
 
 
+def census() -> str:
+    """SASS / ptxas census of every kernel in libnk.so as a markdown table: registers and spill bytes (ptxas -v, kept
+    beside the objects), and from `cuobjdump -sass` the counts of UBLKCP (bulk-copy / TMA engine), SYNCS (mbarrier),
+    DFMA, DFMA with a uniform-register operand (D through the uniform datapath), LDL/STL (local memory), ACQBULK
+    (griddepcontrol.wait), LDGSTS, and tensor-core MMA opcodes (none expected: fp64, HBM-bound)."""
+    import re
+    build()
+    cuobjdump = os.path.join(os.path.dirname(NVCC), "cuobjdump")
+    rows = []
+    for src in SOURCES:
+        if not src.endswith(".cu"):
+            continue
+        obj = os.path.join(OBJDIR, os.path.splitext(src)[0] + ".o")
+        regs = {}
+        try:
+            txt = open(obj + ".ptxas.txt").read()
+        except OSError:
+            txt = ""
+        for m in re.finditer(r"Compiling entry function '(\S+)'.*?\n.*?\n\s*(\d+) bytes stack frame, (\d+) bytes spill stores, "
+                             r"(\d+) bytes spill loads\n.*?Used (\d+) registers", txt):
+            regs[m.group(1)] = (int(m.group(5)), int(m.group(3)), int(m.group(4)))
+        sass = subprocess.run([cuobjdump, "-sass", obj], capture_output=True, text=True).stdout
+        name, counts = None, None
+
+        def flush():
+            if name is None:
+                return
+            dem = subprocess.run(["c++filt", name], capture_output=True, text=True).stdout.strip() or name
+            dem = re.sub(r"\(anonymous namespace\)::", "", dem)
+            dem = re.sub(r"\(.*", "", dem)[:60]
+            r = regs.get(name, ("?", "?", "?"))
+            rows.append((src, dem, r[0], f"{r[1]}/{r[2]}", counts["UBLKCP"], counts["SYNCS"], counts["DFMA"], counts["DFMA_UR"],
+                         counts["LDL"] + counts["STL"], counts["ACQBULK"], counts["MMA"]))
+        for line in sass.splitlines():
+            m = re.search(r"Function : (\S+)", line)
+            if m:
+                flush()
+                name = m.group(1)
+                counts = dict(UBLKCP=0, SYNCS=0, DFMA=0, DFMA_UR=0, LDL=0, STL=0, ACQBULK=0, MMA=0)
+                continue
+            if counts is None or "/*" not in line:
+                continue
+            ins = line.split("*/", 1)[-1]
+            for key in ("UBLKCP", "SYNCS", "ACQBULK"):
+                if re.search(r"\b" + key, ins):
+                    counts[key] += 1
+            if re.search(r"\bDFMA\b", ins):
+                counts["DFMA"] += 1
+                if re.search(r"\bUR\d+", ins):
+                    counts["DFMA_UR"] += 1
+            if re.search(r"\bLDL\b|\bLDL\.", ins):
+                counts["LDL"] += 1
+            if re.search(r"\bSTL\b|\bSTL\.", ins):
+                counts["STL"] += 1
+            if re.search(r"\b(UTC\w*MMA|HMMA|DMMA|IMMA)\b", ins):
+                counts["MMA"] += 1
+        flush()
+    out = ["| file | kernel | registers | spill B (st/ld) | UBLKCP | SYNCS | DFMA | DFMA with UR operand | LDL+STL | ACQBULK | tensor MMA |",
+           "|---|---|---|---|---|---|---|---|---|---|---|"]
+    for r in rows:
+        out.append("| " + " | ".join(str(x) for x in r) + " |")
+    return "\n".join(out)
+
+
 if __name__ == "__main__":
-    build(force="--force" in sys.argv, verbose="--verbose" in sys.argv or "-v" in sys.argv)
-    print(LIB)
+    if "--census" in sys.argv:
+        print(census())
+    else:
+        build(force="--force" in sys.argv, verbose="--verbose" in sys.argv or "-v" in sys.argv)
+        print(LIB)
