@@ -665,6 +665,56 @@ __device__ __forceinline__ double coop_grid_sum(double v, double *s_red, double 
     return total;
 }
 
+// The same for ONE THREAD-BLOCK CLUSTER of CS CTAs (meshes of a few thousand points: a handful of CTAs has all the
+// parallelism there is, and a cluster exchange costs a fraction of a grid barrier).  Every CTA stores its partial sum
+// into slot [rank] of EVERY CTA's shared memory (distributed shared memory) and arrives, with release semantics at
+// cluster scope, on every CTA's mbarrier; each CTA waits on its own mbarrier (CS arrivals per phase) and adds the CS
+// partials in rank order.  Two slot arrays alternate as in coop_grid_sum.  No all-thread cluster barrier is used:
+// the producer lane never joins.
+constexpr int COOP_CS = 16;
+
+__device__ __forceinline__ uint32_t mapa_u32(uint32_t addr, uint32_t cta)
+{
+    uint32_t r;
+    asm volatile("mapa.shared::cluster.u32 %0, %1, %2;" : "=r"(r) : "r"(addr), "r"(cta));
+    return r;
+}
+
+template <int CT>
+__device__ __forceinline__ double coop_cluster_sum(double v, double *s_red, double *s_part, uint32_t cbar, unsigned &passed)
+{
+    const int tid = threadIdx.x, lane = tid & 31, wid = tid >> 5;
+    constexpr int NWARP = CT / 32;
+    v = nk_warp_sum(v);
+    if (lane == 0) s_red[wid] = v;
+    const unsigned e = passed++;                       // exchange number, from 0
+    double *mine = s_part + (e & 1u) * COOP_CS;
+    coop_cta_sync<CT>();                               // the CTA's writes of this phase happen-before the release below
+    if (wid == 0) {
+        double t = (lane < NWARP) ? s_red[lane] : 0.0;
+        t = nk_warp_sum(t);
+        if (lane < (int)gridDim.x) {
+            const uint32_t slot = mapa_u32(smem_u32(mine + blockIdx.x), (uint32_t)lane);
+            const uint32_t rbar = mapa_u32(cbar, (uint32_t)lane);
+            asm volatile("st.shared::cluster.f64 [%0], %1;" ::"r"(slot), "d"(t) : "memory");
+            asm volatile("mbarrier.arrive.release.cluster.shared::cluster.b64 _, [%0];" ::"r"(rbar) : "memory");
+        }
+        uint32_t done;
+        do {
+            asm volatile("{\n.reg .pred P1;\n"
+                         "mbarrier.try_wait.parity.acquire.cluster.shared::cta.b64 P1, [%1], %2;\n"
+                         "selp.u32 %0, 1, 0, P1;\n}\n" : "=r"(done) : "r"(cbar), "r"(e & 1u) : "memory");
+        } while (!__all_sync(0xffffffffu, done));
+        if (lane == 0) {
+            double sum = mine[0];
+            for (unsigned i = 1; i < gridDim.x; ++i) sum += mine[i];
+            s_red[32] = sum;
+        }
+    }
+    coop_cta_sync<CT>();
+    return s_red[32];
+}
+
 // (M Q Q^T w)_l of a streamed point from the unsummed w: own value / face partner g / Dirichlet.  Points of nodes
 // with three or more copies (v < -1) are left to coop_row_update: `skip`.
 __device__ __forceinline__ double coop_gs_value(int l, int v, double wl, double g, bool &skip)
@@ -712,20 +762,33 @@ __device__ __forceinline__ double coop_row_update(const double *w, double *r, co
     return acc;
 }
 
-template <int N>
+template <int N, bool CLUSTER>
 __global__ void __launch_bounds__(TmaCfg<N>::THREADS, 1)
 cg_coop_kernel(nk_coop_args a)
 {
     using C = TmaCfg<N>;
     constexpr int CT = C::CT;
+    __shared__ double s_part[2 * COOP_CS];
+    __shared__ __align__(8) unsigned long long s_cbar;
+    const uint32_t cbar = smem_u32(&s_cbar);
     extern __shared__ __align__(128) unsigned char smem_raw[];
     __shared__ double s_red[33];
     __shared__ double s_c[NK_CTAB];
     const AxSmem<N> sm(smem_raw);
     const int tid = threadIdx.x;
-    if (tid == 0) sm.init_barriers();
+    if (tid == 0) {
+        sm.init_barriers();
+        if (CLUSTER) { mbar_init(cbar, gridDim.x); asm volatile("fence.mbarrier_init.release.cluster;" ::: "memory"); }
+    }
     for (int t = tid; t < NK_CTAB; t += blockDim.x) s_c[t] = a.ctab[t];
     __syncthreads();
+    if (CLUSTER) {                                     // every CTA's mbarrier exists before anybody arrives on it
+        asm volatile("barrier.cluster.arrive.release.aligned;" ::: "memory");
+        asm volatile("barrier.cluster.wait.acquire.aligned;" ::: "memory");
+    }
+    auto grid_sum = [&](double v, unsigned &passed) {
+        return CLUSTER ? coop_cluster_sum<CT>(v, s_red, s_part, cbar, passed) : coop_grid_sum<CT>(v, s_red, a.part, a.bar, passed);
+    };
     const int64_t elo = a.E * (int64_t)blockIdx.x / gridDim.x, ehi = a.E * ((int64_t)blockIdx.x + 1) / gridDim.x;
     RingState rs{0, 0u};
     if (tid >= CT) {
@@ -765,7 +828,7 @@ cg_coop_kernel(nk_coop_args a)
         r2[l] = fv; p2[l] = fv; x2[l] = 0.0;
         acc = fma(s_c[cd & 0x7f] * fv, fv, acc);
     }
-    double rho = coop_grid_sum<CT>(acc, s_red, a.part, a.bar, passed);
+    double rho = grid_sum(acc, passed);
     if (blockIdx.x == 0 && tid == 0) a.hist[0] = sqrt(rho);
     double beta = 0.0, alpha = 0.0, pap = 0.0, rho_old = rho;
     for (int k = 1; k <= a.niter; ++k) {
@@ -778,7 +841,7 @@ cg_coop_kernel(nk_coop_args a)
 #ifdef NK_COOP_TIMING
         asm volatile("mov.u64 %0, %%globaltimer;" : "=l"(tt[1]));
 #endif
-        pap = coop_grid_sum<CT>(dsum, s_red, a.part, a.bar, passed);
+        pap = grid_sum(dsum, passed);
 #ifdef NK_COOP_TIMING
         asm volatile("mov.u64 %0, %%globaltimer;" : "=l"(tt[2]));
 #endif
@@ -846,7 +909,7 @@ cg_coop_kernel(nk_coop_args a)
 #ifdef NK_COOP_TIMING
         asm volatile("mov.u64 %0, %%globaltimer;" : "=l"(tt[3]));
 #endif
-        const double rho_new = coop_grid_sum<CT>(acc, s_red, a.part, a.bar, passed);
+        const double rho_new = grid_sum(acc, passed);
 #ifdef NK_COOP_TIMING
         asm volatile("mov.u64 %0, %%globaltimer;" : "=l"(tt[4]));
         if ((blockIdx.x == 0 || blockIdx.x == 77) && tid == 0 && (k == 5 || k == 6))
@@ -883,16 +946,31 @@ cudaError_t launch_coop(nk_ctx *c, const double *f, double *x, int niter, double
     a.code = c->code; a.ctab = c->ctab; a.nbr = c->nbr; a.gx = c->gx; a.gx_rows = c->gx_rows; a.n_gx_rows = c->n_gx_rows;
     a.hist = hist; a.part = c->red.partials; a.scal = c->red.scal; a.bar = c->coop_bar;
     a.E = c->E; a.L = c->L; a.niter = niter;
-    cudaError_t e = cudaMemsetAsync(c->coop_bar, 0, sizeof(unsigned), st);
-    if (e != cudaSuccess) return e;
+    cudaError_t e;
     cudaLaunchConfig_t cfg = {};
+    if (c->L <= NK_CLUSTER_AUTO_MAX_L && c->cluster_ok) {
+        // a few thousand points: ONE cluster of COOP_CS CTAs, exchanges through distributed shared memory
+        cfg.gridDim = dim3(COOP_CS); cfg.blockDim = dim3(C::THREADS);
+        cfg.dynamicSmemBytes = C::SMEM; cfg.stream = st;
+        cudaLaunchAttribute ac[1];
+        ac[0].id = cudaLaunchAttributeClusterDimension;
+        ac[0].val.clusterDim.x = COOP_CS; ac[0].val.clusterDim.y = 1; ac[0].val.clusterDim.z = 1;
+        cfg.attrs = ac; cfg.numAttrs = 1;
+        e = cudaLaunchKernelEx(&cfg, cg_coop_kernel<N, true>, a);
+        if (e == cudaSuccess) { c->launches++; return cudaGetLastError(); }
+        (void)cudaGetLastError();
+        c->cluster_ok = 0;                                     // this device cannot place such a cluster: the grid variant from now on
+    }
+    e = cudaMemsetAsync(c->coop_bar, 0, sizeof(unsigned), st);
+    if (e != cudaSuccess) return e;
+    cfg = cudaLaunchConfig_t{};
     cfg.gridDim = dim3((unsigned)c->sm_count); cfg.blockDim = dim3(C::THREADS);
     cfg.dynamicSmemBytes = C::SMEM; cfg.stream = st;
     cudaLaunchAttribute at[1];
     at[0].id = cudaLaunchAttributeCooperative;                 // all CTAs co-resident, or the launch fails
     at[0].val.cooperative = 1;
     cfg.attrs = at; cfg.numAttrs = 1;
-    e = cudaLaunchKernelEx(&cfg, cg_coop_kernel<N>, a);
+    e = cudaLaunchKernelEx(&cfg, cg_coop_kernel<N, false>, a);
     c->launches++;
     return e != cudaSuccess ? e : cudaGetLastError();
 }
@@ -967,8 +1045,13 @@ cudaError_t prepare_tma()
     if (e != cudaSuccess) return e;
     e = cudaFuncSetAttribute(ax_tma_kernel<N, false>, cudaFuncAttributeMaxDynamicSharedMemorySize, TmaCfg<N>::SMEM);
     if (e != cudaSuccess) return e;
-    if constexpr (N <= 13)           // nk_coop_supported
-        e = cudaFuncSetAttribute(cg_coop_kernel<N>, cudaFuncAttributeMaxDynamicSharedMemorySize, TmaCfg<N>::SMEM);
+    if constexpr (N <= 13) {         // nk_coop_supported
+        e = cudaFuncSetAttribute(cg_coop_kernel<N, false>, cudaFuncAttributeMaxDynamicSharedMemorySize, TmaCfg<N>::SMEM);
+        if (e != cudaSuccess) return e;
+        e = cudaFuncSetAttribute(cg_coop_kernel<N, true>, cudaFuncAttributeMaxDynamicSharedMemorySize, TmaCfg<N>::SMEM);
+        if (e != cudaSuccess) return e;
+        e = cudaFuncSetAttribute(cg_coop_kernel<N, true>, cudaFuncAttributeNonPortableClusterSizeAllowed, 1);
+    }
     return e;
 }
 

@@ -24,6 +24,9 @@ enum { NK_EPI_STORE = 0,   // out[0] = total
 #define NK_GRAPH_AUTO_MAX_L (1 << 24)   // "graph" = 2: nk_cg replays a CUDA graph up to this many local points
 #define NK_COOP_AUTO_MAX_L (1 << 19)     // "coop" = 2: one cooperative launch per solve up to this many local points
                                         // (measured crossover against the graph replay: 0.7 - 0.9 M points, N = 3..11)
+#ifndef NK_CLUSTER_AUTO_MAX_L
+#define NK_CLUSTER_AUTO_MAX_L (1 << 15)  // within "coop": up to this many points the solve runs on ONE 16-CTA cluster
+#endif
 #define NK_FUSE_GS_AUTO_MIN_L (1 << 21)  // "fuse_gs" = 2: gs rides in the residual update above this many local points
 #define NK_GS_CHUNK 32768          // rows per gs chunk (128 blocks of 256 threads)
 #define NK_CTAB 128                // code & 0x7f indexes ctab[] = 1/multiplicity
@@ -90,6 +93,7 @@ struct nk_ctx {
     int *errflag;                // geometry error flag
     unsigned *coop_bar;          // grid-barrier counter of the cooperative solve (nk_ax_tma.cu cg_coop_kernel)
     int coop_ok;                 // the device supports cooperative launches
+    int cluster_ok;              // ... and has placed a 16-CTA cluster of the solve kernel so far (cleared on the first failure)
     nk_reduce_ws red;
     // sizes
     int64_t n_unique, n_shared_unique, n_masked_unique;

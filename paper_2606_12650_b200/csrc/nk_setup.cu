@@ -373,6 +373,7 @@ extern "C" int nk_setup(nk_ctx **ctx, int64_t E, int N, const double *coords, co
         int coop = 0;
         NK_CUDA(cudaDeviceGetAttribute(&coop, cudaDevAttrCooperativeLaunch, dev));
         c->coop_ok = coop;
+        c->cluster_ok = 1;
     }
     int rc;
     try {
