@@ -185,8 +185,10 @@ int nk_dist_cg(nk_ctx *ctx, const double *f, double *x, int niter, double *res_h
  *                  that sit in L2, where launch gaps and kernel tails are most of an iteration.  Orders
  *                  N <= 13; otherwise, and under "profile", the next rule applies.  Sums run in fixed but
  *                  different orders than launch by launch: the two agree to rounding, each is bitwise
- *                  reproducible.  0 = never; 2 (default) = 1 for meshes of up to 2^19 local points (1.1-1.3x the
- *                  graph replay there; slower from about 0.8 M points on).
+ *                  reproducible.  Up to 2^15 points the launch is one 16-CTA thread-block cluster (exchanges through
+ *                  distributed shared memory: 1.6-2x the graph replay), above that one CTA per SM with grid
+ *                  barriers (1.1-1.3x).  0 = never; 2 (default) = 1 for meshes of up to 2^19 local points
+ *                  (slower than the graph replay from about 0.8 M points on).
  *   "graph"        0 = nk_cg enqueues its launches one by one; 1 = records them into a CUDA graph
  *                  (cached per f, x, res_hist, niter; updated in place when the pointers change) and
  *                  replays it; 2 (default) = 1 for meshes of up to 2^24 local points, where launch gaps
