@@ -339,14 +339,16 @@ def test_fused_gs_against_separate_gs(name, fuse_p):
     gpu.close()
 
 
-def test_fused_gs_on_irregular_ids():
-    """Rows of 3, 5, 12 copies and scattered ids take the fused gather's CSR path; Dirichlet rows its zero path."""
+@pytest.mark.parametrize("brick", [(3, 2, 2, 4), (10, 8, 7, 4)])
+def test_fused_gs_on_irregular_ids(brick):
+    """Rows of 3, 5, 12 copies and scattered ids take the fused gather's CSR path; Dirichlet rows its zero path.
+    1500 points: the cooperative solve runs on one cluster; 70 000 points: on the grid."""
     from oracle.nko import Oracle
     from paper_2606_12650_b200 import Nekbone
     from workloads import brick_mesh
-    m = brick_mesh(3, 2, 2, 4, 0.05)
+    m = brick_mesh(*brick, 0.05)
     rng = np.random.Generator(np.random.PCG64(12))
-    glo = rng.integers(0, 400, m.L).astype(np.int64) * 1_000_003 + 17      # ~3.75 copies per id, scattered
+    glo = rng.integers(0, m.L // 4 + 25, m.L).astype(np.int64) * 1_000_003 + 17      # ~3.75 copies per id, scattered
     glo[:12] = 5                                                            # one row of >= 12 copies
     glo[m.L - 1] = 999_999_999_999                                          # the last point alone (odd L: 1500... even; harmless)
     mask = np.ones(m.L)
@@ -356,6 +358,11 @@ def test_fused_gs_on_irregular_ids():
     f = rng.uniform(-1, 1, inv.max() + 1)[inv]                              # consistent on every copy
     xo, ho = orc.cg(f, 15)
     res = {}
+    # the cooperative whole-solve launch (one cluster at this size) takes the same rows through coop_row_update
+    assert gpu.solve_path() == "cooperative"
+    xc, hc = gpu.cg(to_dev(f), 15)
+    assert np.all(np.abs(to_np(hc) - ho) <= TOL_CG * ho) and elem_err(to_np(xc), xo, m.n ** 3) <= TOL_CG
+    gpu.set_option("coop", 0)
     for fuse_p in (0, 1):
         for fuse_gs in (0, 1):
             gpu.set_option("fuse_p", fuse_p)
