@@ -67,6 +67,11 @@ void nk_free(nk_ctx *ctx);
  * sort of (global id, local index), the group walk, the packing); n < 1 restores the default.  Every array
  * nk_setup builds is independent of this number. */
 int nk_set_host_threads(int n);
+/* Which builder nk_setup uses for the gather-scatter plan from now on: 0 (default) = on the device (ids and mask are
+ * uploaded, then a stable radix sort of (global id, local index), scans and per-point kernels; the host only turns
+ * the list of distinct multiplicities into the 1/multiplicity table); 1 = on the host cores.  Both produce the same
+ * arrays bit for bit.  NK_ERR_ARG for any other value. */
+int nk_set_plan_builder(int which);
 
 /* w = A_L u : element-local Laplacian, no gs, no mask (S 8(a) a1).  u, w DEVICE, L; u != w. */
 int nk_ax_e(nk_ctx *ctx, const double *u, double *w, void *stream);
@@ -212,6 +217,16 @@ int nk_get_sizes(nk_ctx *ctx, int64_t *n_local, int64_t *n_unique, int64_t *n_sh
                  int64_t *n_masked_unique);
 /* gs plan sizes: CSR rows, listed local copies, rows that are summed (shared, unmasked). */
 int nk_get_gs_sizes(nk_ctx *ctx, int64_t *n_rows, int64_t *n_listed, int64_t *n_sum_rows);
+/* What nk_setup did: the plan builder that ran (0 device, 1 host: chosen by nk_set_plan_builder, or the fallback for
+ * meshes with more than 8192 nodes of more than 4096 copies each), wall seconds of the plan part (uploads of ids and
+ * mask included) and of the whole call.  Any pointer may be NULL. */
+int nk_get_setup_info(nk_ctx *ctx, int *plan_builder, double *plan_seconds, double *total_seconds);
+/* Where one array of the gather-scatter plan lives inside the caller's workspace (DEVICE pointer, bytes in use):
+ * which = 0 per-point code (multiplicity-table index | 0x80 Dirichlet), 1 CSR row offsets, 2 CSR local indices,
+ * 3 packed rows, 4 their chunk descriptors, 5 per-point gather code of the fused update, 6 its rows of three or more
+ * copies, 7 the list of those rows, 8 that list cut per block, 9 the 1/multiplicity table, 10 the multiplicity table.
+ * For tests and tools (the two plan builders are compared through it); NK_ERR_ARG for another `which`. */
+int nk_get_plan_array(nk_ctx *ctx, int which, const void **dev, size_t *bytes);
 int nk_get_mult(nk_ctx *ctx, double *mult, void *stream);   /* DEVICE out, L: multiplicity per point */
 int nk_get_geom(nk_ctx *ctx, double *G6, void *stream);     /* DEVICE out, planes rr|rs|rt|ss|st|tt, each L */
 /* HOST out: D[(N+1)^2] row-major D[i*(N+1)+m] = l_m'(xi_i); xi[N+1]; w[N+1].  Any may be NULL. */

@@ -26,6 +26,7 @@ SIGNATURES = {
     "nk_setup": (_i, [C.POINTER(_vp), _i64, _i, _vp, _vp, _vp, _vp, _sz, _vp]),
     "nk_free": (None, [_vp]),
     "nk_set_host_threads": (_i, [_i]),
+    "nk_set_plan_builder": (_i, [_i]),
     "nk_ax_e": (_i, [_vp, _vp, _vp, _vp]),
     "nk_gs": (_i, [_vp, _vp, _vp]),
     "nk_ax": (_i, [_vp, _vp, _vp, _vp]),
@@ -42,6 +43,8 @@ SIGNATURES = {
     "nk_set_option": (_i, [_vp, C.c_char_p, _i]),
     "nk_get_option": (_i, [_vp, C.c_char_p, C.POINTER(_i)]),
     "nk_get_sizes": (_i, [_vp, C.POINTER(_i64), C.POINTER(_i64), C.POINTER(_i64), C.POINTER(_i64)]),
+    "nk_get_setup_info": (_i, [_vp, C.POINTER(_i), C.POINTER(_d), C.POINTER(_d)]),
+    "nk_get_plan_array": (_i, [_vp, _i, C.POINTER(_vp), C.POINTER(_sz)]),
     "nk_get_gs_sizes": (_i, [_vp, C.POINTER(_i64), C.POINTER(_i64), C.POINTER(_i64)]),
     "nk_get_mult": (_i, [_vp, _vp, _vp]),
     "nk_get_geom": (_i, [_vp, _vp, _vp]),
@@ -121,6 +124,11 @@ def fp64_peak() -> dict:
 def set_host_threads(n: int) -> None:
     """Host threads of later set-ups (0 = all cores); the plan they build does not depend on it."""
     _check(load().nk_set_host_threads(int(n)))
+
+
+def set_plan_builder(which: str) -> None:
+    """Builder of the gather-scatter plan in later set-ups: "device" (default) or "host"; same arrays bit for bit."""
+    _check(load().nk_set_plan_builder({"device": 0, "host": 1}[which]))
 
 
 def _np_ptr(a: np.ndarray):
@@ -279,6 +287,24 @@ class Nekbone:
         v = [_i64() for _ in range(3)]
         _check(self._lib.nk_get_gs_sizes(self._ctx, *[C.byref(a) for a in v]))
         return dict(n_rows=v[0].value, n_listed=v[1].value, n_sum_rows=v[2].value)
+
+    def setup_info(self) -> dict:
+        b, tp, tt = _i(), _d(), _d()
+        _check(self._lib.nk_get_setup_info(self._ctx, C.byref(b), C.byref(tp), C.byref(tt)))
+        return dict(plan_builder=("device", "host")[b.value], plan_s=tp.value, total_s=tt.value)
+
+    PLAN_ARRAYS = ("code", "row_off", "row_idx", "pk", "gs_desc", "nbr", "gx", "gx_rows", "gx_blk", "ctab", "mtab")
+
+    def plan_arrays(self) -> dict:
+        """The arrays of the gather-scatter plan as byte views of the workspace (name -> uint8 tensor)."""
+        out = {}
+        for which, name in enumerate(self.PLAN_ARRAYS):
+            ptr, n = _vp(), _sz()
+            _check(self._lib.nk_get_plan_array(self._ctx, which, C.byref(ptr), C.byref(n)))
+            start = (ptr.value or 0) - self._ws.data_ptr()
+            assert 0 <= start and start + n.value <= self._ws.numel()
+            out[name] = self._ws[start:start + n.value]
+        return out
 
     def mult(self):
         m = self.empty()

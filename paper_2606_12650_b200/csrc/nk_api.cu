@@ -414,6 +414,40 @@ int nk_get_sizes(nk_ctx *c, int64_t *n_local, int64_t *n_unique, int64_t *n_shar
     return NK_OK;
 }
 
+int nk_get_setup_info(nk_ctx *c, int *plan_builder, double *plan_seconds, double *total_seconds)
+{
+    if (!c) return NK_ERR_ARG;
+    if (plan_builder) *plan_builder = c->plan_builder;
+    if (plan_seconds) *plan_seconds = c->setup_plan_s;
+    if (total_seconds) *total_seconds = c->setup_total_s;
+    return NK_OK;
+}
+
+int nk_get_plan_array(nk_ctx *c, int which, const void **dev, size_t *bytes)
+{
+    if (!c || !dev || !bytes) return NK_ERR_ARG;
+    const int nvb = nk_gsu_blocks(c->sm_count, c->L >> 1);
+    const void *p = nullptr;
+    size_t n = 0;
+    switch (which) {
+    case 0: p = c->code; n = (size_t)c->L; break;
+    case 1: p = c->row_off; n = ((size_t)c->n_rows + 1) * 4; break;
+    case 2: p = c->row_idx; n = (size_t)c->n_listed * 4; break;
+    case 3: p = c->pk; n = (size_t)c->n_pk * 4; break;
+    case 4: p = c->gs_desc; n = (size_t)(c->n_gs_chunks > 0 ? c->n_gs_chunks : 1) * 32; break;
+    case 5: p = c->nbr; n = (size_t)c->L * 4; break;
+    case 6: p = c->gx; n = (size_t)(c->gx_rows - c->gx) * 4; break;
+    case 7: p = c->gx_rows; n = (size_t)c->n_gx_rows * 4; break;
+    case 8: p = c->gx_blk; n = ((size_t)nvb + 1) * 4; break;
+    case 9: p = c->ctab; n = NK_CTAB * sizeof(double); break;
+    case 10: p = c->mtab; n = NK_CTAB * sizeof(double); break;
+    default: return NK_ERR_ARG;
+    }
+    *dev = p;
+    *bytes = n;
+    return NK_OK;
+}
+
 int nk_get_gs_sizes(nk_ctx *c, int64_t *n_rows, int64_t *n_listed, int64_t *n_sum_rows)
 {
     if (!c) return NK_ERR_ARG;

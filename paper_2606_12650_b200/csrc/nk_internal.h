@@ -86,6 +86,9 @@ struct nk_ctx {
     int32_t *gx_blk;               // nk_vec_blocks(L/2) + 1 ints: block b of the fused kernel takes nodes [gx_blk[b], gx_blk[b+1])
     int64_t n_gx_rows;
     int64_t n_gs_chunks;
+    int64_t n_pk;                // ints of pk in use
+    int plan_builder;            // who built the plan: 0 device (nk_plan.cu), 1 host (nk_setup.cu)
+    double setup_plan_s, setup_total_s;   // wall time of the plan part and of all of nk_setup
     double *ctab;                // NK_CTAB doubles: 1/multiplicity
     double *mtab;                // NK_CTAB doubles: multiplicity
     double *hist;                // NK_HIST_MAX doubles (nk_cg_host)
@@ -155,8 +158,35 @@ static inline int nk_vec_blocks(int sm_count, int64_t pairs)
     return (int)want;
 }
 
+// The fused gs + residual update (nk_vec.cu gs_update_kernel) has its own block geometry: NK_GSU_THREADS threads,
+// NK_GSU_MINB resident blocks per SM, NK_GSU_WAVES chunks per resident slot on large meshes.
+#ifndef NK_GSU_THREADS
+#define NK_GSU_THREADS 512
+#endif
+#ifndef NK_GSU_MINB
+#define NK_GSU_MINB 2
+#endif
+#ifndef NK_GSU_WAVES
+#define NK_GSU_WAVES 8
+#endif
+static inline int nk_gsu_blocks(int sm_count, int64_t pairs)
+{
+    const int64_t one = (pairs + NK_GSU_THREADS - 1) / NK_GSU_THREADS;
+    const int64_t floor2 = (int64_t)sm_count * 2, cap = (int64_t)sm_count * NK_GSU_MINB * NK_GSU_WAVES;
+    int64_t want = (pairs + NK_GSU_THREADS * 8 - 1) / (NK_GSU_THREADS * 8);
+    const int64_t lo = one < floor2 ? one : floor2;
+    if (want < lo) want = lo;
+    if (want > cap) want = cap;
+    if (want < 1) want = 1;
+    return (int)want;
+}
+
 // ---- kernels' host launchers (each returns a cudaError_t from the launch) -----------------------
 // nk_dist.cu
+// nk_plan.cu: the gather-scatter plan built on the device (nk_setup.cu falls back to its host builder on NK_PLAN_FALLBACK:
+// more than 8192 groups longer than 4096 copies).  ctab / mtab: NK_CTAB doubles each, host, filled here.
+#define NK_PLAN_FALLBACK (-1000)
+int nk_plan_device(nk_ctx *c, const int64_t *glo_num, const double *mask, double *ctab, double *mtab, cudaStream_t st);
 void nk_dist_release(nk_ctx *c);              // frees the distributed plan (nk_free)
 // nk_basis.cpp
 void nk_host_basis(int N, double *xi, double *w, double *D);

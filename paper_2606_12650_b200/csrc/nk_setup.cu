@@ -1,10 +1,13 @@
 // nk_setup.cu -- nk_setup (S 8(a) row a0, S 3 call stack (4)): validate, GLL basis, carve the
-// caller's workspace, build the gather-scatter plan on the host (sort (global id, local index)
-// pairs -> CSR of nodes that are shared or masked -> multiplicity codes), upload, run the geometry
-// kernel.  One-time cost; the paper discards set-up and warm-up from its timings too.
-// The host part runs on all cores (OpenMP: parallel radix sort, group walk cut at group boundaries, chunked
-// packing); every array it builds is independent of the thread count (tests/test_abi.py::test_plan_threads).
+// caller's workspace, build the gather-scatter plan (sort (global id, local index) pairs -> CSR of nodes that are
+// shared or masked -> multiplicity codes, gather codes, packed rows), run the geometry kernel.  One-time cost; the
+// paper discards set-up and warm-up from its timings too.
+// The plan is built on the DEVICE by default (nk_plan.cu).  This file keeps the host builder (nk_set_plan_builder(1),
+// and the fallback for degenerate inputs): all cores via OpenMP (parallel radix sort, group walk cut at group
+// boundaries, chunked packing); every array it builds is independent of the thread count and equal, bit for bit, to
+// the device builder's (tests/test_gpu_operators.py).
 #include <algorithm>
+#include <chrono>
 #include <cmath>
 #ifdef _OPENMP
 #include <omp.h>
@@ -93,7 +96,10 @@ void radix_sort_pairs(KeyBuf &key, ValBuf &val, uint64_t max_key)
 
 struct Row { uint32_t first, begin, len; };   // first local index, position in the sorted list, copies
 
-int setup_impl(nk_ctx *c, const double *coords, const int64_t *glo_num, const double *mask, cudaStream_t st)
+int g_plan_builder = 0;          // nk_set_plan_builder: 0 = device (nk_plan.cu), 1 = host (below)
+
+// The plan built on the host cores; the device builder (nk_plan.cu) produces the same arrays bit for bit.
+int plan_host(nk_ctx *c, const int64_t *glo_num, const double *mask, double *ctab, double *mtab, cudaStream_t st)
 {
     const int64_t L = c->L;
     const int T = host_threads();
@@ -155,7 +161,6 @@ int setup_impl(nk_ctx *c, const double *coords, const int64_t *glo_num, const do
             if (std::find(mult_values.begin(), mult_values.end(), v) == mult_values.end()) mult_values.push_back(v);
     if (mult_values.size() > NK_CTAB) return NK_ERR_MULT;
     std::sort(mult_values.begin(), mult_values.end());
-    double ctab[NK_CTAB], mtab[NK_CTAB];
     for (int t = 0; t < NK_CTAB; ++t) { ctab[t] = 0.0; mtab[t] = 0.0; }
     for (size_t t = 0; t < mult_values.size(); ++t) {
         mtab[t] = (double)mult_values[t];
@@ -278,11 +283,14 @@ int setup_impl(nk_ctx *c, const double *coords, const int64_t *glo_num, const do
             nbr[loc[row.begin + q]] = -p4 - 2;
         }
     }
-    gx.resize((gx.size() + 12 + 3) / 4 * 4, 0);              // vector loads of the last row stay in bounds; 16-byte multiple
+    {   // 4 (Q + 3) ints, Q = the quad the next row would start at: vector loads of the last row stay in bounds
+        const size_t Q = gx_rows.empty() ? 1 : (size_t)gx_rows.back() + (size_t)gx[4 * (size_t)gx_rows.back() - 1] / 4 + 1;
+        gx.resize(4 * (Q + 3), 0);
+    }
     c->n_gx_rows = (int64_t)gx_rows.size();
     c->gx_rows = c->gx + gx.size();
     // the list cut by the chunks of the fused kernel's blocks: a node goes to the block whose chunk holds its first copy
-    const int nvb = nk_vec_blocks(c->sm_count, L >> 1);
+    const int nvb = nk_gsu_blocks(c->sm_count, L >> 1);
     std::vector<int32_t> gx_blk((size_t)nvb + 1);
     {
         const int64_t pairs = L >> 1;
@@ -301,13 +309,12 @@ int setup_impl(nk_ctx *c, const double *coords, const int64_t *glo_num, const do
         for (uint32_t q = 0; q < row.len; ++q) nbr[loc[row.begin + q]] = -1;
     }
     c->n_gs_chunks = n_chunks;
+    c->n_pk = (int64_t)pk.size();
     c->gs_desc = c->pk + nk_align_up(pk.size(), 64);
     c->n_unique = n_unique; c->n_shared_unique = n_shared; c->n_masked_unique = n_masked;
     c->n_rows = n_rows; c->n_listed = n_listed; c->n_sum_rows = n_sum_rows; c->n_sum_listed = n_sum_listed;
 
-    // ---- upload plan, tables, coordinates; geometry kernel -------------------------------------
-    double *D_dev = c->ctab + 2 * NK_CTAB;
-    double *wq_dev = D_dev + 16 * 16;
+    // ---- upload the plan ------------------------------------------------------------------------------------
     NK_CUDA(cudaMemcpyAsync(c->code, code.data(), (size_t)L, cudaMemcpyHostToDevice, st));
     NK_CUDA(cudaMemcpyAsync(c->row_off, off.data(), off.size() * sizeof(int32_t), cudaMemcpyHostToDevice, st));
     if (n_listed > 0)
@@ -319,6 +326,26 @@ int setup_impl(nk_ctx *c, const double *coords, const int64_t *glo_num, const do
         NK_CUDA(cudaMemcpyAsync(c->gx_rows, gx_rows.data(), gx_rows.size() * sizeof(int32_t), cudaMemcpyHostToDevice, st));
     NK_CUDA(cudaMemcpyAsync(c->gx_blk, gx_blk.data(), gx_blk.size() * sizeof(int32_t), cudaMemcpyHostToDevice, st));
     NK_CUDA(cudaMemcpyAsync(c->gs_desc, desc.data(), desc.size() * sizeof(int32_t), cudaMemcpyHostToDevice, st));
+    NK_CUDA(cudaStreamSynchronize(st));                          // the host arrays go out of scope here
+    return NK_OK;
+}
+
+int setup_impl(nk_ctx *c, const double *coords, const int64_t *glo_num, const double *mask, cudaStream_t st)
+{
+    const int64_t L = c->L;
+    double ctab[NK_CTAB], mtab[NK_CTAB];
+    const auto t0 = std::chrono::steady_clock::now();
+    int rc = g_plan_builder == 0 ? nk_plan_device(c, glo_num, mask, ctab, mtab, st) : NK_PLAN_FALLBACK;
+    c->plan_builder = 0;
+    if (rc == NK_PLAN_FALLBACK) {
+        rc = plan_host(c, glo_num, mask, ctab, mtab, st);
+        c->plan_builder = 1;
+    }
+    if (rc != NK_OK) return rc;
+    c->setup_plan_s = std::chrono::duration<double>(std::chrono::steady_clock::now() - t0).count();
+    // ---- tables, coordinates; geometry kernel ------------------------------------------------------------------
+    double *D_dev = c->ctab + 2 * NK_CTAB;
+    double *wq_dev = D_dev + 16 * 16;
     NK_CUDA(cudaMemcpyAsync(c->ctab, ctab, sizeof(ctab), cudaMemcpyHostToDevice, st));
     NK_CUDA(cudaMemcpyAsync(c->mtab, mtab, sizeof(mtab), cudaMemcpyHostToDevice, st));
     NK_CUDA(cudaMemcpyAsync(D_dev, c->D, sizeof(double) * c->n * c->n, cudaMemcpyHostToDevice, st));
@@ -339,6 +366,7 @@ int setup_impl(nk_ctx *c, const double *coords, const int64_t *glo_num, const do
     NK_CUDA(cudaMemcpyAsync(&err, c->errflag, sizeof(int), cudaMemcpyDeviceToHost, st));
     NK_CUDA(cudaStreamSynchronize(st));
     if (err) return NK_ERR_GEOM;
+    c->setup_total_s = std::chrono::duration<double>(std::chrono::steady_clock::now() - t0).count();
     return NK_OK;
 }
 
@@ -347,6 +375,13 @@ int setup_impl(nk_ctx *c, const double *coords, const int64_t *glo_num, const do
 extern "C" int nk_set_host_threads(int n)
 {
     g_host_threads = n > 0 ? n : 0;
+    return NK_OK;
+}
+
+extern "C" int nk_set_plan_builder(int which)
+{
+    if (which != 0 && which != 1) return NK_ERR_ARG;
+    g_plan_builder = which;
     return NK_OK;
 }
 

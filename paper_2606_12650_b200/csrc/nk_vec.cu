@@ -188,10 +188,13 @@ __device__ __forceinline__ double gs_row_update(const double *w, double *r, cons
     return acc;
 }
 
-constexpr int GS_U = 2;                                   // pairs per thread and step of the large-mesh variant
+#ifndef NK_GSU_U
+#define NK_GSU_U 2
+#endif
+constexpr int GS_U = NK_GSU_U;                                   // pairs per thread and step of the large-mesh variant
 
 template <bool WITH_X>
-__global__ void __launch_bounds__(NK_VEC_THREADS, 2)
+__global__ void __launch_bounds__(NK_GSU_THREADS, NK_GSU_MINB)
 gs_update_kernel(double *__restrict__ x, double *r, const double *p, const double *w,
                  const uint8_t *__restrict__ code, const double *__restrict__ ctab, int64_t L, nk_reduce_ws ws,
                  double *hist_k, nk_gather gp)
@@ -540,8 +543,8 @@ cudaError_t launch_gs_update(nk_ctx *c, double *x, double *hist_k, cudaStream_t 
 {
     nk_gather gp;
     gp.nbr = c->nbr; gp.gx = c->gx; gp.rows = c->gx_rows; gp.blk = c->gx_blk;
-    const int nb = vec_blocks(c, c->L >> 1);                      // the grid nk_setup cut the row list for (gx_blk)
-    const cudaError_t e = nk_launch(gs_update_kernel<WITH_X>, nb, NK_VEC_THREADS, 0, st, c->pdl_now == 2, x, c->r,
+    const int nb = nk_gsu_blocks(c->sm_count, c->L >> 1);         // the grid nk_setup cut the row list for (gx_blk)
+    const cudaError_t e = nk_launch(gs_update_kernel<WITH_X>, nb, NK_GSU_THREADS, 0, st, c->pdl_now == 2, x, c->r,
                                     (const double *)c->p, (const double *)c->w, (const uint8_t *)c->code,
                                     (const double *)c->ctab, c->L, c->red, hist_k, gp);
     if (e != cudaSuccess) return e;

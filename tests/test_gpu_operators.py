@@ -187,7 +187,8 @@ def test_plan_does_not_depend_on_host_threads():
     boundaries, chunked packing); the plan -- hence gs, ax and a CG solve with the fused gs, bit for bit -- must be
     the one a single thread builds.  Irregular ids (rows of 3, 5, 12 copies) and a brick with several gs chunks."""
     from paper_2606_12650_b200 import Nekbone
-    from paper_2606_12650_b200.binding import set_host_threads
+    from paper_2606_12650_b200.binding import set_host_threads, set_plan_builder
+    set_plan_builder("host")                                  # the default builder runs on the device (test below)
     m1 = brick_mesh(3, 2, 2, 4, 0.05)
     rng = np.random.Generator(np.random.PCG64(13))
     glo = rng.integers(0, 400, m1.L).astype(np.int64) * 1_000_003 + 17
@@ -212,7 +213,76 @@ def test_plan_does_not_depend_on_host_threads():
                         to_np(x), to_np(h)))
             gpu.close()
         set_host_threads(0)
+        set_plan_builder("device")
         for o in out[1:]:
             assert o[0] == out[0][0] and o[1] == out[0][1]
             for a, b in zip(o[2:], out[0][2:]):
                 assert np.array_equal(a, b)
+
+
+def _irregular_case(rng):
+    """Ids drawn at random (rows of many lengths, some longer than 8), a run of 12 equal ids, Dirichlet nodes."""
+    m = brick_mesh(3, 2, 2, 4, 0.05)
+    glo = rng.integers(0, 400, m.L).astype(np.int64) * 1_000_003 + 17
+    glo[:12] = 5
+    mask = np.ones(m.L)
+    mask[np.isin(glo, glo[100:110])] = 0.0
+    return m.E, m.N, m.coords, glo, mask
+
+
+def test_device_plan_equals_host_plan():
+    """nk_setup builds the gather-scatter plan on the device by default (csrc/nk_plan.cu: radix sort, scans, per-point
+    kernels); every array of it -- codes, CSR, packed rows and descriptors, gather codes, gx rows and their per-block
+    cut, multiplicity tables -- and every size must equal, byte for byte, what the host builder produces.  Cases: a
+    single element (no shared node), irregular ids (rows of 3, 5, 12 copies, ids up to 4e8: four sort passes), all ids
+    equal (one group of L copies), a brick with several gs chunks and an odd point count, ids above 2^40."""
+    from paper_2606_12650_b200 import Nekbone
+    from paper_2606_12650_b200.binding import set_plan_builder
+    rng = np.random.Generator(np.random.PCG64(29))
+    m0 = brick_mesh(1, 1, 1, 2, 0.0)
+    m2 = brick_mesh(24, 20, 16, 3, 0.05)
+    m3 = brick_mesh(5, 3, 3, 6, 0.05)
+    m4 = brick_mesh(2, 2, 1, 2, 0.0)
+    cases = {
+        "single element": (m0.E, m0.N, m0.coords, m0.glo_num, m0.mask),
+        "irregular ids": _irregular_case(rng),
+        "all ids equal": (m4.E, m4.N, m4.coords, np.full(m4.L, 7, dtype=np.int64), np.ones(m4.L)),
+        "all ids zero, masked": (m4.E, m4.N, m4.coords, np.zeros(m4.L, dtype=np.int64), np.zeros(m4.L)),
+        "four gs chunks": (m2.E, m2.N, m2.coords, m2.glo_num, m2.mask),
+        "odd point count": (m3.E, m3.N, m3.coords, m3.glo_num, m3.mask),
+        "ids above 2^40": (m3.E, m3.N, m3.coords, m3.glo_num * 3 + (1 << 41), m3.mask),
+    }
+    try:
+        for name, (E, N, co, g, mk) in cases.items():
+            got = {}
+            for which in ("host", "device"):
+                set_plan_builder(which)
+                gpu = Nekbone(E, N, co, g, mk)
+                assert gpu.setup_info()["plan_builder"] == which
+                got[which] = (gpu.sizes(), gpu.gs_sizes(), {k: v.cpu().numpy().copy() for k, v in gpu.plan_arrays().items()})
+                gpu.close()
+            assert got["host"][0] == got["device"][0], name
+            assert got["host"][1] == got["device"][1], name
+            for k, a in got["host"][2].items():
+                b = got["device"][2][k]
+                assert a.shape == b.shape, (name, k, a.shape, b.shape)
+                assert np.array_equal(a, b), (name, k, int(np.flatnonzero(a != b)[0]))
+    finally:
+        set_plan_builder("device")
+
+
+def test_device_plan_rejects_what_the_host_plan_rejects():
+    from paper_2606_12650_b200 import Nekbone
+    from paper_2606_12650_b200.binding import NkError
+    m = brick_mesh(2, 2, 2, 3, 0.0)
+    bad_id = m.glo_num.copy()
+    bad_id[5] = -1
+    bad_mask = m.mask.copy()
+    bad_mask[7] = 0.5
+    clash = m.mask.copy()
+    shared = np.flatnonzero(np.bincount(m.glo_num)[m.glo_num] > 1)
+    clash[shared[0]] = 1.0 - clash[shared[0]]
+    for g, mk, code in ((bad_id, m.mask, -3), (m.glo_num, bad_mask, -4), (m.glo_num, clash, -4)):
+        with pytest.raises(NkError) as e:
+            Nekbone(m.E, m.N, m.coords, g, mk)
+        assert e.value.code == code
