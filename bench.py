@@ -310,6 +310,7 @@ def run_ours(args) -> dict | None:
     t0 = time.perf_counter()
     nk = Nekbone.from_mesh(mesh)
     setup_s = time.perf_counter() - t0
+    setup_info = nk.setup_info()                           # who built the gs plan, and the library's own clock
     for k, v in (("fuse_pap", args.fuse_pap), ("fuse_p", args.fuse_p), ("fuse_gs", args.fuse_gs), ("graph", args.graph),
                  ("pdl", args.pdl), ("coop", args.coop)):
         if v is not None:                                  # None: the library's default
@@ -415,7 +416,7 @@ def run_ours(args) -> dict | None:
            "options": {**opts, "solve_path": solve_path, "pdl_effective": nk.pdl_effective(),
                        "fuse_p_effective": int(fused_p), "fuse_gs_effective": int(fused_gs),
                        "profile_in_timed_region": False},
-           "setup_s": setup_s, "final_residual": res_final}
+           "setup_s": setup_s, "setup": setup_info, "final_residual": res_final}
 
     # ---- iteration-level and kernel-level bandwidth ---------------------------------------------------
     # real bytes per point of each kernel class as launched: ax_e u 8 + G 48 + w 8 (+ r 8 read and

@@ -197,27 +197,30 @@ def test_plan_does_not_depend_on_host_threads():
     mask[np.isin(glo, glo[100:110])] = 0.0
     m2 = brick_mesh(24, 20, 16, 3, 0.05)                      # 7680 elements, 116 K summed rows: four gs chunks
     cases = [(m1.E, m1.N, m1.coords, glo, mask), (m2.E, m2.N, m2.coords, m2.glo_num, m2.mask)]
-    for E, N, co, g, mk in cases:
-        L = E * (N + 1) ** 3
-        v = to_dev(rng.uniform(-1, 1, L))
-        _, inv = np.unique(g, return_inverse=True)
-        f = to_dev(rng.uniform(-1, 1, inv.max() + 1)[inv])
-        out = []
-        for threads in (1, 3, 0):
-            set_host_threads(threads)
-            gpu = Nekbone(E, N, co, g, mk)
-            gpu.set_option("coop", 0)
-            gpu.set_option("fuse_gs", 1)
-            x, h = gpu.cg(f, 10)
-            out.append((gpu.sizes(), gpu.gs_sizes(), to_np(gpu.gs(v.clone())), to_np(gpu.ax(v)), to_np(gpu.mult()),
-                        to_np(x), to_np(h)))
-            gpu.close()
+    try:
+        for E, N, co, g, mk in cases:
+            L = E * (N + 1) ** 3
+            v = to_dev(rng.uniform(-1, 1, L))
+            _, inv = np.unique(g, return_inverse=True)
+            f = to_dev(rng.uniform(-1, 1, inv.max() + 1)[inv])
+            out = []
+            for threads in (1, 3, 0):
+                set_host_threads(threads)
+                gpu = Nekbone(E, N, co, g, mk)
+                gpu.set_option("coop", 0)
+                gpu.set_option("fuse_gs", 1)
+                x, h = gpu.cg(f, 10)
+                assert gpu.setup_info()["plan_builder"] == "host"
+                out.append((gpu.sizes(), gpu.gs_sizes(), to_np(gpu.gs(v.clone())), to_np(gpu.ax(v)), to_np(gpu.mult()),
+                            to_np(x), to_np(h)) + tuple(a.cpu().numpy().copy() for a in gpu.plan_arrays().values()))
+                gpu.close()
+            for o in out[1:]:
+                assert o[0] == out[0][0] and o[1] == out[0][1]
+                for a, b in zip(o[2:], out[0][2:]):
+                    assert np.array_equal(a, b)
+    finally:
         set_host_threads(0)
         set_plan_builder("device")
-        for o in out[1:]:
-            assert o[0] == out[0][0] and o[1] == out[0][1]
-            for a, b in zip(o[2:], out[0][2:]):
-                assert np.array_equal(a, b)
 
 
 def _irregular_case(rng):
