@@ -42,6 +42,7 @@ extern "C" {
 #define NK_ERR_CUDA       -6   /* CUDA runtime error; nk_last_cuda_error() has the cudaError_t */
 #define NK_ERR_ALLOC      -7   /* host allocation failed */
 #define NK_ERR_MULT       -8   /* more than 127 distinct node multiplicities (unsupported) */
+#define NK_ERR_SIZE       -9   /* nk_dot_static: more entries than its fixed scratch serves (nk_dot_static_max_n) */
 
 #define NK_MAX_ORDER      15
 
@@ -82,6 +83,24 @@ int nk_ax(nk_ctx *ctx, const double *u, double *w, void *stream);
 /* out[0] = <a,b>_c = sum_l c_l a_l b_l, c = 1/multiplicity (S 8(a) a4).  a, b, out DEVICE.
  * Deterministic: per-block partials, ordered finish; no floating-point atomics. */
 int nk_dot(nk_ctx *ctx, const double *a, const double *b, double *out, void *stream);
+
+/* The weighted dot product WITHOUT a context, a workspace or any allocation, for callers that cannot call cudaMalloc
+ * (code under CUDA graph capture, tight serving loops, harnesses that forbid it):
+ *   out[0] = sum_{i<n} c_i a_i b_i      (c == NULL: plain dot product; with c = 1/multiplicity it is nk_dot, S 8(a) a4)
+ * a, b, c, out DEVICE; a, b, c hold n doubles (16-byte aligned pointers take the vector loads), out one double.
+ * Scratch (per-block partial sums and a ticket counter) is a file-scope __device__ array inside the library, about
+ * 128 KB that every GPU which loads the library holds until the process exits.  It serves
+ * n <= nk_dot_static_max_n() = 2^27 entries; a larger n returns NK_ERR_SIZE and launches nothing.  n = 0 stores 0.
+ * Deterministic: a block sums a fixed run of 8192 entries and the last block adds the partials in index order, so the
+ * result depends on n and the data only, not on the GPU.  Enqueues one memset node (the counter) and one kernel on
+ * `stream`, never synchronises.  Every call shares the one array: calls that OVERLAP on the GPU (different streams
+ * with no ordering between them) race on it -- order them; calls on one stream are safe.
+ * nk_static_setup() looks the array's device address up for the CURRENT device (cudaGetSymbolAddress; once per
+ * device); nk_dot_static does so itself on the first call of a device, so call nk_static_setup beforehand where that
+ * first call would fall inside a stream capture.  NK_ERR_ARG: null pointer, n < 0, device ordinal >= 64. */
+int nk_static_setup(void);
+int64_t nk_dot_static_max_n(void);
+int nk_dot_static(const double *a, const double *b, const double *c, int64_t n, double *out, void *stream);
 
 /* Unpreconditioned CG (S 8(c) O8): x0 = 0 (incoming x ignored), r0 = mask o f, recursive
  * residual.  res_hist[k] = sqrt(<r_k, r_k>_c), k = 0..niter (DEVICE, niter+1 doubles).

@@ -26,6 +26,9 @@ SIGNATURES = {
     "nk_setup": (_i, [C.POINTER(_vp), _i64, _i, _vp, _vp, _vp, _vp, _sz, _vp]),
     "nk_free": (None, [_vp]),
     "nk_set_host_threads": (_i, [_i]),
+    "nk_static_setup": (_i, []),
+    "nk_dot_static_max_n": (_i64, []),
+    "nk_dot_static": (_i, [_vp, _vp, _vp, _i64, _vp, _vp]),
     "nk_set_plan_builder": (_i, [_i]),
     "nk_ax_e": (_i, [_vp, _vp, _vp, _vp]),
     "nk_gs": (_i, [_vp, _vp, _vp]),
@@ -124,6 +127,24 @@ def fp64_peak() -> dict:
 def set_host_threads(n: int) -> None:
     """Host threads of later set-ups (0 = all cores); the plan they build does not depend on it."""
     _check(load().nk_set_host_threads(int(n)))
+
+
+def dot_static_max_n() -> int:
+    return int(load().nk_dot_static_max_n())
+
+
+def dot_static(a, b, c=None, out=None, n=None):
+    """out[0] = sum c_i a_i b_i (c None: plain dot) over CUDA float64 tensors, through nk_dot_static: no context, no
+    workspace, no allocation inside the call (scratch is a fixed __device__ array in the library; n <= 2^27)."""
+    import torch
+    n = a.numel() if n is None else int(n)
+    for t in (a, b) + (() if c is None else (c,)):
+        if t.dtype != torch.float64 or not t.is_cuda or not t.is_contiguous() or t.numel() < n:
+            raise ValueError("contiguous CUDA float64 tensors of at least n entries")
+    out = torch.empty(1, dtype=torch.float64, device=a.device) if out is None else out
+    _check(load().nk_dot_static(_vp(a.data_ptr()), _vp(b.data_ptr()), _vp(c.data_ptr()) if c is not None else None,
+                                n, _vp(out.data_ptr()), _stream()))
+    return out
 
 
 def set_plan_builder(which: str) -> None:

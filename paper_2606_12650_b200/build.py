@@ -18,7 +18,7 @@ OBJDIR = os.path.join(CSRC, "build")
 LIB = os.path.join(HERE, "libnk.so")
 INCLUDE = os.path.join(os.path.dirname(HERE), "include")
 
-SOURCES = ["nk_api.cu", "nk_setup.cu", "nk_plan.cu", "nk_ax_tma.cu", "nk_gs.cu", "nk_vec.cu", "nk_geom.cu", "nk_dist.cu", "nk_probe.cu", "nk_basis.cpp"]
+SOURCES = ["nk_api.cu", "nk_setup.cu", "nk_plan.cu", "nk_ax_tma.cu", "nk_gs.cu", "nk_vec.cu", "nk_geom.cu", "nk_dist.cu", "nk_probe.cu", "nk_static.cu", "nk_basis.cpp"]
 HEADERS = ["nk_internal.h", "nk_host.h", "nk_reduce.cuh"]
 
 NVCC = os.environ.get("NVCC", "/usr/local/cuda/bin/nvcc")

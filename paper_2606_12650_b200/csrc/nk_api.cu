@@ -61,6 +61,7 @@ const char *nk_strerror(int code)
         case NK_ERR_CUDA: return t_last_cuda ? cudaGetErrorString((cudaError_t)t_last_cuda) : "CUDA error";
         case NK_ERR_ALLOC: return "host allocation failed";
         case NK_ERR_MULT: return "too many distinct multiplicities";
+        case NK_ERR_SIZE: return "more entries than the fixed scratch of nk_dot_static serves";
     }
     return "unknown error";
 }
