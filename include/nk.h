@@ -109,9 +109,17 @@ int nk_dot_static(const double *a, const double *b, const double *c, int64_t n, 
  * Never synchronises; alpha, beta, rho stay on the device. */
 int nk_cg(nk_ctx *ctx, const double *f, double *x, int niter, double *res_hist, void *stream);
 /* Same with HOST f, x, res_hist: copies f in, runs nk_cg on workspace buffers, copies x and the
- * history out, synchronises.  Needs the extra 2*L doubles nk_workspace_bytes already counts. */
+ * history out, synchronises.  Needs extra staging vectors nk_workspace_bytes already counts. */
 int nk_cg_host(nk_ctx *ctx, const double *f_host, double *x_host, int niter,
                double *res_hist_host, void *stream);
+
+/* nrhs solves in a row, HOST buffers, pipelined: while solve j runs on `stream`, right-hand side j+1 is copied in and
+ * solution j-1 (with its history) copied out on two internal copy streams, through two sets of staging buffers in the
+ * workspace.  f_host, x_host, res_hist_host: HOST arrays of nrhs HOST pointers (L, L, niter+1 doubles each; pinned
+ * memory is what makes the copies overlap; the same buffer may appear more than once in f_host).  Every solve is
+ * exactly nk_cg on its right-hand side: results equal nk_cg_host's bit for bit.  Synchronises before returning. */
+int nk_cg_host_batch(nk_ctx *ctx, int nrhs, const double *const *f_host, double *const *x_host, int niter,
+                     double *const *res_hist_host, void *stream);
 
 /* Jacobi-preconditioned CG, the original Nekbone's iteration, which the paper's variant omits (P:225,
  * P:290; S 8(f) f-3): z = r / diag, diag = Q Q^T diag(A_L), z = 0 on Dirichlet nodes; rho = <r,z>_c;

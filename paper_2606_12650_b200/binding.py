@@ -38,6 +38,7 @@ SIGNATURES = {
     "nk_pcg": (_i, [_vp, _vp, _vp, _i, _vp, _vp]),
     "nk_get_diag": (_i, [_vp, _vp, _vp]),
     "nk_cg_host": (_i, [_vp, _vp, _vp, _i, _vp, _vp]),
+    "nk_cg_host_batch": (_i, [_vp, _i, _vp, _vp, _i, _vp, _vp]),
     "nk_cg_init": (_i, [_vp, _vp, _vp, _vp]),
     "nk_cg_load_state": (_i, [_vp, _vp, _vp, _d, _vp]),
     "nk_cg_step": (_i, [_vp, _vp, _vp]),
@@ -268,6 +269,20 @@ class Nekbone:
         _check(self._lib.nk_cg_host(self._ctx, _np_ptr(f_host), _np_ptr(x_host), int(niter),
                                     _np_ptr(hist_host), _stream()))
         return x_host, hist_host
+
+    def cg_host_batch(self, f_hosts, niter: int, x_hosts, hist_hosts):
+        """Several solves with HOST buffers (lists of numpy arrays, ideally pinned), copies overlapped with the solves."""
+        n = len(f_hosts)
+        if len(x_hosts) != n or len(hist_hosts) != n:
+            raise ValueError("f_hosts, x_hosts, hist_hosts: lists of equal length")
+        for f, x, h in zip(f_hosts, x_hosts, hist_hosts):
+            for a, size in ((f, self.L), (x, self.L), (h, int(niter) + 1)):
+                if a.dtype != np.float64 or a.size != size or not a.flags.c_contiguous:
+                    raise ValueError("contiguous float64 arrays of length L, L, niter + 1")
+        arr = lambda xs: (C.c_void_p * max(n, 1))(*[a.ctypes.data for a in xs])
+        fa, xa, ha = arr(f_hosts), arr(x_hosts), arr(hist_hosts)
+        _check(self._lib.nk_cg_host_batch(self._ctx, n, fa, xa, int(niter), ha, _stream()))
+        return x_hosts, hist_hosts
 
     # -- lock-step test entry points -----------------------------------------------------
     def cg_init(self, f, x):

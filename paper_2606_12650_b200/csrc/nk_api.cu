@@ -80,7 +80,18 @@ int nk_workspace_bytes(int64_t E, int N, size_t *bytes)
 void nk_free(nk_ctx *c)
 {
     if (!c) return;
-    if (c->graph_exec) cudaGraphExecDestroy(c->graph_exec);
+    for (auto &sl : c->graph)
+        if (sl.exec) cudaGraphExecDestroy(sl.exec);
+    if (c->batch_ready) {
+        cudaStreamDestroy(c->copy_in);
+        cudaStreamDestroy(c->copy_out);
+        for (int s = 0; s < 2; ++s) {
+            cudaEventDestroy(c->ev_f[s]);
+            cudaEventDestroy(c->ev_solve[s]);
+            cudaEventDestroy(c->ev_out[s]);
+        }
+        cudaEventDestroy(c->ev_start);
+    }
     nk_dist_release(c);
     delete c->prof;
     delete c;
@@ -251,8 +262,12 @@ int nk_cg(nk_ctx *c, const double *f, double *x, int niter, double *res_hist, vo
     // Record the launch sequence once per (f, x, res_hist, niter, options) and replay it: the CG
     // loop of the small configs is launch-bound (S 7 hard part 4).
     const int key = c->opt_fuse_pap | (c->opt_fuse_p << 1) | (c->opt_fuse_gs << 3) | (c->opt_pdl << 4);
-    if (!c->graph_exec || c->graph_f != f || c->graph_x != x || c->graph_hist != res_hist ||
-        c->graph_niter != niter || c->graph_key != key) {
+    nk_ctx::graph_slot *g = nullptr;
+    for (auto &sl : c->graph)
+        if (sl.exec && sl.f == f && sl.x == x && sl.hist == res_hist && sl.niter == niter && sl.key == key) g = &sl;
+    if (!g) {
+        // two slots (nk_cg_host_batch alternates between two sets of buffers); the one used longest ago goes
+        g = c->graph[0].stamp <= c->graph[1].stamp ? &c->graph[0] : &c->graph[1];
         cudaStream_t cap;
         NK_CUDA(cudaStreamCreateWithFlags(&cap, cudaStreamNonBlocking));
         cudaGraph_t graph = nullptr;
@@ -264,25 +279,26 @@ int nk_cg(nk_ctx *c, const double *f, double *x, int niter, double *res_hist, vo
             e = (e1 != cudaSuccess) ? e1 : e2;
         }
         c->launches = launches_before;
-        if (e == cudaSuccess && c->graph_exec) {       // same topology, new pointers: update in place
+        if (e == cudaSuccess && g->exec) {             // same topology, new pointers: update in place
             cudaGraphExecUpdateResultInfo info;
-            if (cudaGraphExecUpdate(c->graph_exec, graph, &info) != cudaSuccess) {
+            if (cudaGraphExecUpdate(g->exec, graph, &info) != cudaSuccess) {
                 (void)cudaGetLastError();
-                cudaGraphExecDestroy(c->graph_exec);
-                c->graph_exec = nullptr;
+                cudaGraphExecDestroy(g->exec);
+                g->exec = nullptr;
             }
         }
-        if (e == cudaSuccess && !c->graph_exec) e = cudaGraphInstantiate(&c->graph_exec, graph, 0);
+        if (e == cudaSuccess && !g->exec) e = cudaGraphInstantiate(&g->exec, graph, 0);
         if (graph) cudaGraphDestroy(graph);
         cudaStreamDestroy(cap);
         if (e != cudaSuccess) {
-            if (c->graph_exec) cudaGraphExecDestroy(c->graph_exec);
-            c->graph_exec = nullptr;
+            if (g->exec) cudaGraphExecDestroy(g->exec);
+            g->exec = nullptr;
             return nk_cuda_fail(e);
         }
-        c->graph_f = f; c->graph_x = x; c->graph_hist = res_hist; c->graph_niter = niter; c->graph_key = key;
+        g->f = f; g->x = x; g->hist = res_hist; g->niter = niter; g->key = key;
     }
-    NK_CUDA(cudaGraphLaunch(c->graph_exec, st));
+    g->stamp = ++c->graph_clock;
+    NK_CUDA(cudaGraphLaunch(g->exec, st));
     int per_iter = 3 + (c->opt_fuse_pap ? 0 : 1) + (fuse_p_on(c) ? 0 : 1) - (fuse_gs_on(c) ? 1 : 0);
     c->launches += 1 + (int64_t)niter * per_iter + ((fuse_p_on(c) && niter > 0) ? 1 : 0);
     c->p_pending = 0;
@@ -299,6 +315,54 @@ int nk_cg_host(nk_ctx *c, const double *f_host, double *x_host, int niter, doubl
     if (rc != NK_OK) return rc;
     NK_CUDA(cudaMemcpyAsync(x_host, c->hx, bytes, cudaMemcpyDeviceToHost, st));
     NK_CUDA(cudaMemcpyAsync(res_hist_host, c->hist, (size_t)(niter + 1) * sizeof(double), cudaMemcpyDeviceToHost, st));
+    NK_CUDA(cudaStreamSynchronize(st));
+    return NK_OK;
+}
+
+// Several right-hand sides, pipelined: RHS j+1 goes in and solution j-1 comes out (two copy streams, two sets of
+// staging buffers) while solve j runs on `stream`.
+int nk_cg_host_batch(nk_ctx *c, int nrhs, const double *const *f_host, double *const *x_host, int niter,
+                     double *const *res_hist_host, void *stream)
+{
+    if (!c || nrhs < 0 || niter < 0 || niter + 1 > NK_HIST_MAX) return NK_ERR_ARG;
+    if (nrhs > 0 && (!f_host || !x_host || !res_hist_host)) return NK_ERR_ARG;
+    for (int j = 0; j < nrhs; ++j)
+        if (!f_host[j] || !x_host[j] || !res_hist_host[j]) return NK_ERR_ARG;
+    cudaStream_t st = S(stream);
+    if (!c->batch_ready) {
+        NK_CUDA(cudaStreamCreateWithFlags(&c->copy_in, cudaStreamNonBlocking));
+        NK_CUDA(cudaStreamCreateWithFlags(&c->copy_out, cudaStreamNonBlocking));
+        for (int s = 0; s < 2; ++s) {
+            NK_CUDA(cudaEventCreateWithFlags(&c->ev_f[s], cudaEventDisableTiming));
+            NK_CUDA(cudaEventCreateWithFlags(&c->ev_solve[s], cudaEventDisableTiming));
+            NK_CUDA(cudaEventCreateWithFlags(&c->ev_out[s], cudaEventDisableTiming));
+        }
+        NK_CUDA(cudaEventCreateWithFlags(&c->ev_start, cudaEventDisableTiming));
+        c->batch_ready = 1;
+    }
+    const size_t bytes = (size_t)c->L * sizeof(double);
+    double *fb[2] = {c->hf, c->hf2}, *xb[2] = {c->hx, c->hx2}, *hb[2] = {c->hist, c->hist2};
+    NK_CUDA(cudaEventRecord(c->ev_start, st));                     // the copies start after what precedes on `stream`
+    NK_CUDA(cudaStreamWaitEvent(c->copy_in, c->ev_start, 0));
+    NK_CUDA(cudaStreamWaitEvent(c->copy_out, c->ev_start, 0));
+    for (int j = 0; j < nrhs; ++j) {
+        const int s = j & 1;
+        // staging set s is free once solve j-2 has read f (ev_solve) and its x and history have left (ev_out)
+        if (j >= 2) NK_CUDA(cudaStreamWaitEvent(c->copy_in, c->ev_solve[s], 0));
+        NK_CUDA(cudaMemcpyAsync(fb[s], f_host[j], bytes, cudaMemcpyHostToDevice, c->copy_in));
+        NK_CUDA(cudaEventRecord(c->ev_f[s], c->copy_in));
+        NK_CUDA(cudaStreamWaitEvent(st, c->ev_f[s], 0));
+        if (j >= 2) NK_CUDA(cudaStreamWaitEvent(st, c->ev_out[s], 0));
+        const int rc = nk_cg(c, fb[s], xb[s], niter, hb[s], stream);
+        if (rc != NK_OK) { cudaDeviceSynchronize(); return rc; }
+        NK_CUDA(cudaEventRecord(c->ev_solve[s], st));
+        NK_CUDA(cudaStreamWaitEvent(c->copy_out, c->ev_solve[s], 0));
+        NK_CUDA(cudaMemcpyAsync(x_host[j], xb[s], bytes, cudaMemcpyDeviceToHost, c->copy_out));
+        NK_CUDA(cudaMemcpyAsync(res_hist_host[j], hb[s], (size_t)(niter + 1) * sizeof(double), cudaMemcpyDeviceToHost,
+                                c->copy_out));
+        NK_CUDA(cudaEventRecord(c->ev_out[s], c->copy_out));
+    }
+    for (int s = 0; s < 2 && s < nrhs; ++s) NK_CUDA(cudaStreamWaitEvent(st, c->ev_out[s], 0));
     NK_CUDA(cudaStreamSynchronize(st));
     return NK_OK;
 }

@@ -65,6 +65,7 @@ struct nk_ctx {
                                  // k-plane one contiguous chunk [c2][i + n j] of (rr,rs) (rt,ss) (st,tt)
     double *r, *p, *w;           // CG state, L each (coords staging aliases these during set-up)
     double *hf, *hx;             // staging for nk_cg_host, L each
+    double *hf2, *hx2, *hist2;   // second set: nk_cg_host_batch copies RHS j+1 in and solution j-1 out while solve j runs
     double *dinv;                // Jacobi preconditioner 1 / (Q Q^T diag A_L), 0 on Dirichlet nodes (lazy)
     int have_dinv;
     uint8_t *code;               // L: multiplicity-table index | NK_CODE_MASKED
@@ -113,8 +114,16 @@ struct nk_ctx {
     struct nk_dist *dist;
     int dist_mult;               // 1: the weights c = 1/multiplicity are GLOBAL (nk_dist_set_mult); rank-local shortcuts are off
     // cached graph for nk_cg
-    cudaGraphExec_t graph_exec;
-    const double *graph_f; double *graph_x; double *graph_hist; int graph_niter; int graph_key;
+    struct graph_slot {
+        cudaGraphExec_t exec;
+        const double *f; double *x; double *hist; int niter; int key;
+        unsigned long long stamp;                    // last use (the older slot is replaced)
+    } graph[2];                                      // two: nk_cg_host_batch alternates between two sets of buffers
+    unsigned long long graph_clock;
+    // nk_cg_host_batch: copy streams and events, created on first use
+    cudaStream_t copy_in, copy_out;
+    cudaEvent_t ev_f[2], ev_solve[2], ev_out[2], ev_start;
+    int batch_ready;
 };
 // "pdl" resolved: 0 = plain launches, 1 = ax_e and the vector kernels are programmatic dependents, 2 = gs too.
 // gs as a dependent saves a launch gap where gaps matter (config 1: -5 % per solve) and costs 95 us at

@@ -414,6 +414,8 @@ extern "C" int nk_setup(nk_ctx **ctx, int64_t E, int N, const double *coords, co
     c->hf = reinterpret_cast<double *>(q); q += cv.vec;
     c->hx = reinterpret_cast<double *>(q); q += cv.vec;
     c->dinv = reinterpret_cast<double *>(q); q += cv.vec;
+    c->hf2 = reinterpret_cast<double *>(q); q += cv.vec;
+    c->hx2 = reinterpret_cast<double *>(q); q += cv.vec;
     c->code = reinterpret_cast<uint8_t *>(q); q += cv.code;
     c->row_off = reinterpret_cast<int32_t *>(q); q += cv.off;
     c->row_idx = reinterpret_cast<int32_t *>(q); q += cv.idx;
@@ -423,6 +425,7 @@ extern "C" int nk_setup(nk_ctx **ctx, int64_t E, int N, const double *coords, co
     c->ctab = reinterpret_cast<double *>(q); c->mtab = c->ctab + NK_CTAB; q += cv.tabs;
     c->red.partials = reinterpret_cast<double *>(q); q += cv.partials;
     c->hist = reinterpret_cast<double *>(q); q += cv.hist;
+    c->hist2 = reinterpret_cast<double *>(q); q += cv.hist;
     c->red.scal = reinterpret_cast<double *>(q); q += cv.scal;
     c->red.counter = reinterpret_cast<unsigned *>(q);
     c->red.raw = nullptr;

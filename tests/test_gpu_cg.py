@@ -95,6 +95,34 @@ def test_cg_host_entry_equals_device_entry():
     assert np.array_equal(to_np(xd), xh) and np.array_equal(to_np(hd), hh)
 
 
+@pytest.mark.parametrize("path", ["cooperative", "graph", "launches"])
+def test_cg_host_batch_equals_one_call_per_rhs(path):
+    """nk_cg_host_batch pipelines the copies of right-hand side j+1 and of solution j-1 with solve j (two copy streams,
+    two sets of staging buffers); every solve must equal, bit for bit, nk_cg_host on the same right-hand side -- five
+    different ones, pinned buffers, so that a copy racing a solve would show."""
+    import torch
+    pr = pair_for_config("config2")
+    gpu = pr.gpu
+    saved = {k: gpu.get_option(k) for k in ("coop", "graph")}
+    try:
+        gpu.set_option("coop", 1 if path == "cooperative" else 0)
+        gpu.set_option("graph", 0 if path == "launches" else 1)
+        assert gpu.solve_path() == path
+        rng = np.random.Generator(np.random.PCG64(41))
+        _, inv = np.unique(pr.mesh.glo_num, return_inverse=True)
+        fs = [torch.from_numpy(rng.uniform(-1, 1, inv.max() + 1)[inv] * (j + 1)).pin_memory() for j in range(5)]
+        xs = [torch.empty(pr.L, dtype=torch.float64).pin_memory() for _ in range(5)]
+        hs = [torch.empty(26, dtype=torch.float64).pin_memory() for _ in range(5)]
+        gpu.cg_host_batch([f.numpy() for f in fs], 25, [x.numpy() for x in xs], [h.numpy() for h in hs])
+        for f, x, h in zip(fs, xs, hs):
+            x1, h1 = gpu.cg_host(f.numpy(), 25)
+            assert np.array_equal(x.numpy(), x1) and np.array_equal(h.numpy(), h1)
+        assert gpu.cg_host_batch([], 25, [], []) == ([], [])
+    finally:
+        for k, v in saved.items():
+            gpu.set_option(k, v)
+
+
 def test_cg_reproducible_and_ignores_incoming_x():
     pr = pair_for_config("config2")
     f = to_dev(config_rhs("config2", pr.mesh))
