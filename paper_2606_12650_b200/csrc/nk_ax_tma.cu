@@ -216,6 +216,14 @@ __device__ __forceinline__ void bulk_g2s(uint32_t dst, const void *src, uint32_t
     asm volatile("cp.async.bulk.shared::cluster.global.mbarrier::complete_tx::bytes [%0], [%1], %2, [%3];"
                  ::"r"(dst), "l"(src), "r"(bytes), "r"(bar) : "memory");
 }
+// the 16-byte-aligned part of [p, p + bytes) into L2, nothing else: no destination, no barrier, no register
+__device__ __forceinline__ void bulk_prefetch_l2(const void *p, uint32_t bytes)
+{
+    const uintptr_t a = (reinterpret_cast<uintptr_t>(p) + 15u) & ~(uintptr_t)15u;
+    const uintptr_t e = (reinterpret_cast<uintptr_t>(p) + bytes) & ~(uintptr_t)15u;
+    if (e > a)
+        asm volatile("cp.async.bulk.prefetch.L2.global [%0], %1;" ::"l"(a), "r"((uint32_t)(e - a)) : "memory");
+}
 template <int COUNT>
 __device__ __forceinline__ void group_sync(int grp)     // named barrier 1 + grp: one sync group's warps
 {
@@ -357,9 +365,16 @@ struct AxSmem {                 // carve-up of the dynamic shared memory (the sa
 };
 
 // Producer lane: the geometric factors of elements [elo, ehi) into the ring, batch by batch.
+// pf0, pf1 (may be null): the vectors the compute warps read their pencils from.  When the producer starts on the
+// factors of a batch it also asks for that batch's part of these vectors to be brought into L2 (bulk prefetch: no
+// destination, no register), so that the compute warps' loads, issued a phase or two later, find them there instead
+// of paying the DRAM latency at the head of every batch.  (Stale data is harmless: L2 is the point of coherence.)
+#ifndef NK_TMA_UPF
+#define NK_TMA_UPF 1
+#endif
 template <int N>
 __device__ __forceinline__ void ax_produce(const AxSmem<N> &sm, const double2 *__restrict__ g, int64_t elo, int64_t ehi,
-                                           RingState &rs)
+                                           RingState &rs, const double *pf0 = nullptr, const double *pf1 = nullptr)
 {
     using C = TmaCfg<N>;
     constexpr int n = C::n, n2 = C::n2, P = C::P, EPB = C::EPB, R = C::R, KP = C::KP;
@@ -367,6 +382,10 @@ __device__ __forceinline__ void ax_produce(const AxSmem<N> &sm, const double2 *_
     for (int it = 0; it < nit; ++it) {
         const int64_t e0 = elo + (int64_t)it * EPB;
         const int ne = (int)((ehi - e0 < EPB) ? (ehi - e0) : EPB);
+        if (NK_TMA_UPF && it > 0) {
+            if (pf0) bulk_prefetch_l2(pf0 + e0 * P, (uint32_t)ne * P * 8);
+            if (pf1) bulk_prefetch_l2(pf1 + e0 * P, (uint32_t)ne * P * 8);
+        }
 #pragma unroll 1
         for (int ks = 0; ks < C::SPB; ++ks) {
             mbar_wait(sm.empty0 + 8 * rs.stage, rs.phase ^ 1u);
@@ -574,7 +593,7 @@ ax_tma_kernel(double *u_rw, const double *u_ro, const double *r_in,
     RingState rs{0, 0u};
     if (tid >= C::CT) {
         // ---- producer warp: one lane streams G into the ring (static data: no need to wait for the predecessor)
-        if (tid == C::CT) ax_produce<N>(sm, g, elo, ehi, rs);
+        if (tid == C::CT) ax_produce<N>(sm, g, elo, ehi, rs, FUSEP ? u_rw : u_ro, FUSEP ? r_in : nullptr);
     } else {
         nk_pdl_wait();                                  // u, r, beta come from the preceding kernels
         const double beta = FUSEP ? red.scal[NK_S_BETA] : 0.0;
