@@ -165,11 +165,13 @@ struct TmaCfg {
 #define NK_TMA_IB 2
 #endif
     static constexpr int IB = NK_TMA_IB;                      // table rows advanced together in lines_apply
-    // where the next batch's u pencil is requested: 1 = after P3, 2 = after P4 (measured per order)
+    // where the next batch's u pencil is requested: 1 = after P3, 2 = after P4, 0 = after P5.  1 everywhere: since the
+    // producer prefetches u into L2 (ax_produce) n = 12 is spill-free at 160 registers with it and gains 6 % over 2
+    // (16^3: 77.5 -> 72.5 us; before that prefetch 1 cost 4 % there).
 #ifdef NK_TMA_PF12
     static constexpr int PF = (n == 12) ? NK_TMA_PF12 : 1;
 #else
-    static constexpr int PF = (n == 12) ? 2 : 1;
+    static constexpr int PF = 1;
 #endif
 };
 
@@ -382,7 +384,7 @@ __device__ __forceinline__ void ax_produce(const AxSmem<N> &sm, const double2 *_
     for (int it = 0; it < nit; ++it) {
         const int64_t e0 = elo + (int64_t)it * EPB;
         const int ne = (int)((ehi - e0 < EPB) ? (ehi - e0) : EPB);
-        if (NK_TMA_UPF && it > 0) {
+        if (NK_TMA_UPF && it > 0) {                  // (the first batch too: no gain, measured)
             if (pf0) bulk_prefetch_l2(pf0 + e0 * P, (uint32_t)ne * P * 8);
             if (pf1) bulk_prefetch_l2(pf1 + e0 * P, (uint32_t)ne * P * 8);
         }
@@ -422,6 +424,7 @@ __device__ __forceinline__ double ax_compute(const AxSmem<N> &sm, double *u_rw, 
     using C = TmaCfg<N>;
     constexpr int n = C::n, n2 = C::n2, P = C::P, S1 = C::S1, S2 = C::S2, SE = C::SE, EPB = C::EPB;
     constexpr int R = C::R, KP = C::KP, NW = C::NW, GTH = C::GTH, SG = C::SG;
+    constexpr int PF = (CG && n == 12) ? 2 : C::PF;   // the cooperative solve at n = 12 spills with 1 (its vectors sit in L2 anyway)
     constexpr int DOFF = eo_off(n), TOFF = DOFF + eo_mat(n);     // even-odd tables of D and D^T in c_Dt
     const int tid = threadIdx.x;
     const int lane = tid & 31;
@@ -535,7 +538,7 @@ __device__ __forceinline__ double ax_compute(const AxSmem<N> &sm, double *u_rw, 
                 if (FUSEP) nr[k] = act ? ld_vec<CG>(r_in + gb + k * n2) : 0.0;
             }
         };
-        if (C::PF == 1) prefetch();
+        if (PF == 1) prefetch();
         // P4: D^T along the row (B in place), the column (C in place) and the pencil (wt -> rw), one pass
         double rw[n];
         {
@@ -553,7 +556,7 @@ __device__ __forceinline__ double ax_compute(const AxSmem<N> &sm, double *u_rw, 
             });
         }
         group_sync<GTH>(grp);
-        if (C::PF == 2) prefetch();
+        if (PF == 2) prefetch();
         // P5: sum the three directions, store
 #pragma unroll
         for (int k = 0; k < n; ++k) {
@@ -562,7 +565,7 @@ __device__ __forceinline__ double ax_compute(const AxSmem<N> &sm, double *u_rw, 
         }
         // (no barrier here even when C aliases A: P5 reads and the next P1 writes the same pencil
         //  positions, by the same thread)
-        if (C::PF == 0) prefetch();
+        if (PF == 0) prefetch();
     }
     return dsum;
 }
