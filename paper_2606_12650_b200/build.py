@@ -65,7 +65,7 @@ def build(force: bool = False, verbose: bool = False) -> str:
 
 def census() -> str:
     """SASS / ptxas census of every kernel in libnk.so as a markdown table: registers and spill bytes (ptxas -v, kept
-    beside the objects), and from `cuobjdump -sass` the counts of UBLKCP (bulk-copy / TMA engine), SYNCS (mbarrier),
+    beside the objects), and from `cuobjdump -sass` the counts of UBLKCP (bulk-copy / TMA engine), UBLKPF (bulk prefetch into L2), SYNCS (mbarrier),
     DFMA, DFMA with a uniform-register operand (D through the uniform datapath), LDL/STL (local memory), ACQBULK
     (griddepcontrol.wait), LDGSTS, and tensor-core MMA opcodes (none expected: fp64, HBM-bound)."""
     import re
@@ -94,19 +94,19 @@ def census() -> str:
             dem = re.sub(r"\(anonymous namespace\)::", "", dem)
             dem = re.sub(r"\(.*", "", dem)[:60]
             r = regs.get(name, ("?", "?", "?"))
-            rows.append((src, dem, r[0], f"{r[1]}/{r[2]}", counts["UBLKCP"], counts["SYNCS"], counts["DFMA"], counts["DFMA_UR"],
+            rows.append((src, dem, r[0], f"{r[1]}/{r[2]}", counts["UBLKCP"], counts["UBLKPF"], counts["SYNCS"], counts["DFMA"], counts["DFMA_UR"],
                          counts["LDL"] + counts["STL"], counts["ACQBULK"], counts["MMA"]))
         for line in sass.splitlines():
             m = re.search(r"Function : (\S+)", line)
             if m:
                 flush()
                 name = m.group(1)
-                counts = dict(UBLKCP=0, SYNCS=0, DFMA=0, DFMA_UR=0, LDL=0, STL=0, ACQBULK=0, MMA=0)
+                counts = dict(UBLKCP=0, UBLKPF=0, SYNCS=0, DFMA=0, DFMA_UR=0, LDL=0, STL=0, ACQBULK=0, MMA=0)
                 continue
             if counts is None or "/*" not in line:
                 continue
             ins = line.split("*/", 1)[-1]
-            for key in ("UBLKCP", "SYNCS", "ACQBULK"):
+            for key in ("UBLKCP", "UBLKPF", "SYNCS", "ACQBULK"):
                 if re.search(r"\b" + key, ins):
                     counts[key] += 1
             if re.search(r"\bDFMA\b", ins):
@@ -120,8 +120,8 @@ def census() -> str:
             if re.search(r"\b(UTC\w*MMA|HMMA|DMMA|IMMA)\b", ins):
                 counts["MMA"] += 1
         flush()
-    out = ["| file | kernel | registers | spill B (st/ld) | UBLKCP | SYNCS | DFMA | DFMA with UR operand | LDL+STL | ACQBULK | tensor MMA |",
-           "|---|---|---|---|---|---|---|---|---|---|---|"]
+    out = ["| file | kernel | registers | spill B (st/ld) | UBLKCP | UBLKPF | SYNCS | DFMA | DFMA with UR operand | LDL+STL | ACQBULK | tensor MMA |",
+           "|---|---|---|---|---|---|---|---|---|---|---|---|"]
     for r in rows:
         out.append("| " + " | ".join(str(x) for x in r) + " |")
     return "\n".join(out)
