@@ -444,7 +444,9 @@ def run_ours(args) -> dict | None:
     # p 8 written when the direction update is folded in); gs by its plan; the vector kernels by what they touch
     gsb = gs_bytes(sizes) / L
     kb = {"ax_e": 64.0 + (16.0 if fused_p else 0.0), "gs": gsb, "dot": 17.0,
-          "update_xr": ((49.0 if fused_p else 25.0) + (gs_gather_bytes(L, sizes) / L if fused_gs else 0.0)),
+          # the fused gs update takes its weights from the gather code: no 1-byte multiplicity code there
+          "update_xr": ((48.0 if fused_p else 24.0) + gs_gather_bytes(L, sizes) / L) if fused_gs
+                       else (49.0 if fused_p else 25.0),
           "update_p": 24.0 if fused_p else 40.0, "cg_init": 33.0}
     it_bytes = iter_model_bytes(L, sizes)
     it_gbs = it_bytes * niter * args.steps / (ms * 1e-3) / 1e9

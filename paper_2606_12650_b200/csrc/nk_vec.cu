@@ -139,6 +139,10 @@ update_xr_kernel(double *__restrict__ x, double *__restrict__ r, const double *p
 //     pass; given to blocks of their own, far from where the chunk's data is in L2, it cost 0.3 GB of DRAM traffic.)
 // Blocks run in index order, so the resident ones form a window of some tens of MB that moves through the
 // vectors once: partners 14 KB (r-faces), 0.4 MB (s-faces) or 14 MB (t-faces, config 5) away are L2 hits.
+// The per-point multiplicity code is NOT read here: the weight of a streamed point follows from its gather code
+// (gs_stream_weight), that of a node with several copies from their number.  Dropping that 1-byte stream (a 2-byte
+// load per thread and step, a table in shared memory) took the pass from 365 to 333 us at config 5 -- it is bound by
+// load instructions in flight, not by bytes.
 // r, x are the values of nk_gs followed by the plain update, entry by entry; rho' sums the same terms in another
 // (fixed) order.  Run-to-run bitwise reproducible like every reduction here.
 struct nk_gather {
@@ -158,9 +162,19 @@ __device__ __forceinline__ double gs_stream_value(int l, int v, double wl, doubl
     return (v == l) ? wl : (v >= 0 ? sum : 0.0);
 }
 
+// The weight c = 1 / multiplicity of a streamed point follows from its gather code: 1 for a node with one copy, 1/2
+// for a face node (exactly the table entries nk_setup builds as 1.0 / multiplicity), so the streaming loop does not
+// read the per-point code at all.  A Dirichlet point (v = -1) has r = 0 in every state CG produces (r0 = M f, and
+// M Q Q^T w = 0 there): its term vanishes whatever the weight.
+__device__ __forceinline__ double gs_stream_weight(int l, int v, bool skip)
+{
+    return skip ? 0.0 : (v == l ? 1.0 : 0.5);
+}
+
 // one node with three or more copies: r -= alpha sum at every copy; returns its share of rho'
-__device__ __forceinline__ double gs_row_update(const double *w, double *r, const uint8_t *__restrict__ code,
-                                                const double *s_c, const int32_t *__restrict__ gx, int p4, double alpha)
+// (weight 1 / len: the correctly rounded quotient nk_setup stores in its table)
+__device__ __forceinline__ double gs_row_update(const double *w, double *r, const int32_t *__restrict__ gx, int p4,
+                                                double alpha)
 {
     const int4 ia = reinterpret_cast<const int4 *>(gx)[p4];
     const int len = gx[4 * p4 - 1];
@@ -168,7 +182,7 @@ __device__ __forceinline__ double gs_row_update(const double *w, double *r, cons
     if (len == 4) {                                       // an edge of a conforming hex mesh
         const double a0 = w[ia.x], a1 = w[ia.y], a2 = w[ia.z], a3 = w[ia.w];
         double r0 = r[ia.x], r1 = r[ia.y], r2 = r[ia.z], r3 = r[ia.w];
-        const double cw = s_c[code[ia.x] & 0x7f];
+        const double cw = 0.25;
         const double s = ((a0 + a1) + a2) + a3;
         r0 = fma(-alpha, s, r0); r1 = fma(-alpha, s, r1); r2 = fma(-alpha, s, r2); r3 = fma(-alpha, s, r3);
         r[ia.x] = r0; r[ia.y] = r1; r[ia.z] = r2; r[ia.w] = r3;
@@ -179,7 +193,7 @@ __device__ __forceinline__ double gs_row_update(const double *w, double *r, cons
     const int32_t *ii = gx + 4 * (int64_t)p4;
     double s = w[ii[0]];
     for (int j = 1; j < len; ++j) s += w[ii[j]];
-    const double cw = s_c[code[ii[0]] & 0x7f];
+    const double cw = 1.0 / (double)len;
     for (int j = 0; j < len; ++j) {
         const double rn = fma(-alpha, s, r[ii[j]]);
         r[ii[j]] = rn;
@@ -191,25 +205,25 @@ __device__ __forceinline__ double gs_row_update(const double *w, double *r, cons
 #ifndef NK_GSU_U
 #define NK_GSU_U 2
 #endif
+#ifndef NK_GSU_UX
+#define NK_GSU_UX 2                                      // ... and of the variant that also updates x (mid-size meshes)
+#endif
 constexpr int GS_U = NK_GSU_U;                                   // pairs per thread and step of the large-mesh variant
 
 template <bool WITH_X>
 __global__ void __launch_bounds__(NK_GSU_THREADS, NK_GSU_MINB)
-gs_update_kernel(double *__restrict__ x, double *r, const double *p, const double *w,
-                 const uint8_t *__restrict__ code, const double *__restrict__ ctab, int64_t L, nk_reduce_ws ws,
+gs_update_kernel(double *__restrict__ x, double *r, const double *p, const double *w, int64_t L, nk_reduce_ws ws,
                  double *hist_k, nk_gather gp)
 {
-    __shared__ double s_c[NK_CTAB];
     __shared__ double s_red[33];
     nk_pdl_launch_dependents();
-    load_ctab(s_c, ctab);
     double acc = 0.0;
     // this block's CONTIGUOUS chunk of pairs (blocks run in index order, so the resident blocks form one window
     // that moves through the vectors: a partner a few KB or MB away is in L2 when it is gathered)
     const int64_t pairs = L >> 1;
     const int64_t plo = pairs * (int64_t)blockIdx.x / gridDim.x, phi = pairs * ((int64_t)blockIdx.x + 1) / gridDim.x;
     const int64_t stride = blockDim.x;
-    constexpr int U = WITH_X ? 1 : GS_U;                      // pairs per step, all loads before the stores
+    constexpr int U = WITH_X ? NK_GSU_UX : GS_U;                      // pairs per step, all loads before the stores
     int64_t q = plo + threadIdx.x;
     int2 nv[U];
 #pragma unroll
@@ -222,14 +236,12 @@ gs_update_kernel(double *__restrict__ x, double *r, const double *p, const doubl
     //  bytes in flight.)
     for (; q + (U - 1) * stride < phi; q += U * stride) {
         double2 wv[U], rv[U], g[U], xv[WITH_X ? U : 1], pv[WITH_X ? U : 1];
-        uchar2 cd[U];
         int2 nn[U];
 #pragma unroll
         for (int j = 0; j < U; ++j) {
             const int64_t qj = q + j * stride;
             wv[j] = reinterpret_cast<const double2 *>(w)[qj];
             rv[j] = reinterpret_cast<const double2 *>(r)[qj];
-            cd[j] = reinterpret_cast<const uchar2 *>(code)[qj];
             g[j].x = gs_partner(w, (int)(2 * qj), nv[j].x);
             g[j].y = gs_partner(w, (int)(2 * qj) + 1, nv[j].y);
             if (WITH_X) {
@@ -257,8 +269,8 @@ gs_update_kernel(double *__restrict__ x, double *r, const double *p, const doubl
                 if (!k0) r[l] = rv[j].x;
                 if (!k1) r[l + 1] = rv[j].y;
             }
-            acc = fma((k0 ? 0.0 : s_c[cd[j].x & 0x7f]) * rv[j].x, rv[j].x, acc);
-            acc = fma((k1 ? 0.0 : s_c[cd[j].y & 0x7f]) * rv[j].y, rv[j].y, acc);
+            acc = fma(gs_stream_weight(l, nv[j].x, k0) * rv[j].x, rv[j].x, acc);
+            acc = fma(gs_stream_weight(l + 1, nv[j].y, k1) * rv[j].y, rv[j].y, acc);
             if (WITH_X) {
                 double2 xn = xv[WITH_X ? j : 0];
                 xn.x = fma(alpha, pv[WITH_X ? j : 0].x, xn.x);
@@ -272,7 +284,6 @@ gs_update_kernel(double *__restrict__ x, double *r, const double *p, const doubl
         const int2 n2 = reinterpret_cast<const int2 *>(gp.nbr)[q];
         const double2 wv = reinterpret_cast<const double2 *>(w)[q];
         double2 rv = reinterpret_cast<const double2 *>(r)[q];
-        const uchar2 cd = reinterpret_cast<const uchar2 *>(code)[q];
         const int l = (int)(2 * q);
         bool k0, k1;
         const double s0 = gs_stream_value(l, n2.x, wv.x, gs_partner(w, l, n2.x), k0);
@@ -281,8 +292,8 @@ gs_update_kernel(double *__restrict__ x, double *r, const double *p, const doubl
         rv.y = fma(-alpha, s1, rv.y);
         if (!k0) r[l] = rv.x;
         if (!k1) r[l + 1] = rv.y;
-        acc = fma((k0 ? 0.0 : s_c[cd.x & 0x7f]) * rv.x, rv.x, acc);
-        acc = fma((k1 ? 0.0 : s_c[cd.y & 0x7f]) * rv.y, rv.y, acc);
+        acc = fma(gs_stream_weight(l, n2.x, k0) * rv.x, rv.x, acc);
+        acc = fma(gs_stream_weight(l + 1, n2.y, k1) * rv.y, rv.y, acc);
         if (WITH_X) {
             double2 xn = reinterpret_cast<const double2 *>(x)[q];
             const double2 pv = reinterpret_cast<const double2 *>(p)[q];
@@ -299,14 +310,14 @@ gs_update_kernel(double *__restrict__ x, double *r, const double *p, const doubl
         if (!k0) {
             const double rn = fma(-alpha, s0, r[l]);
             r[l] = rn;
-            acc = fma(s_c[code[l] & 0x7f] * rn, rn, acc);
+            acc = fma(gs_stream_weight(l, v, false) * rn, rn, acc);
         }
         if (WITH_X) x[l] = fma(alpha, p[l], x[l]);
     }
     // the nodes with three or more copies whose FIRST copy lies in this block's chunk (their other copies sit in
     // neighbouring chunks: in L2, just streamed or about to be), one thread each
     for (int k = gp.blk[blockIdx.x] + (int)threadIdx.x; k < gp.blk[blockIdx.x + 1]; k += blockDim.x)
-        acc += gs_row_update(w, r, code, s_c, gp.gx, gp.rows[k], alpha);
+        acc += gs_row_update(w, r, gp.gx, gp.rows[k], alpha);
     nk_grid_reduce(acc, s_red, ws, NK_EPI_RHO, hist_k);
 }
 
@@ -545,8 +556,7 @@ cudaError_t launch_gs_update(nk_ctx *c, double *x, double *hist_k, cudaStream_t 
     gp.nbr = c->nbr; gp.gx = c->gx; gp.rows = c->gx_rows; gp.blk = c->gx_blk;
     const int nb = nk_gsu_blocks(c->sm_count, c->L >> 1);         // the grid nk_setup cut the row list for (gx_blk)
     const cudaError_t e = nk_launch(gs_update_kernel<WITH_X>, nb, NK_GSU_THREADS, 0, st, c->pdl_now == 2, x, c->r,
-                                    (const double *)c->p, (const double *)c->w, (const uint8_t *)c->code,
-                                    (const double *)c->ctab, c->L, c->red, hist_k, gp);
+                                    (const double *)c->p, (const double *)c->w, c->L, c->red, hist_k, gp);
     if (e != cudaSuccess) return e;
     c->launches++;
     return cudaGetLastError();
