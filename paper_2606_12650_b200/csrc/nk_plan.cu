@@ -417,7 +417,7 @@ __global__ void gx_blk_kernel(const int32_t *gx, const int32_t *gx_rows, int n_g
     const int b = blockIdx.x * blockDim.x + threadIdx.x;
     if (b > nvb) return;
     const int64_t pairs = L >> 1;
-    const int64_t first_point = b == nvb ? L + 1 : 2 * (pairs * (int64_t)b / nvb);
+    const int64_t first_point = b == nvb ? L + 1 : 4 * ((L >> 2) * (int64_t)b / nvb);
     int lo = 0, hi = n_gx_rows;                               // smallest k with first(k) >= first_point
     while (lo < hi) {
         const int mid = (lo + hi) >> 1;

@@ -296,7 +296,7 @@ int plan_host(nk_ctx *c, const int64_t *glo_num, const double *mask, double *cta
         const int64_t pairs = L >> 1;
         size_t k = 0;
         for (int b = 0; b <= nvb; ++b) {
-            const int64_t first_point = b == nvb ? L + 1 : 2 * (pairs * (int64_t)b / nvb);
+            const int64_t first_point = b == nvb ? L + 1 : 4 * ((L >> 2) * (int64_t)b / nvb);
             while (k < gx_rows.size() && (int64_t)gx[4 * (size_t)gx_rows[k]] < first_point) ++k;
             gx_blk[(size_t)b] = (int32_t)k;
         }

@@ -202,13 +202,56 @@ __device__ __forceinline__ double gs_row_update(const double *w, double *r, cons
     return acc;
 }
 
+// 256-bit global accesses (sm_100: LDG.E.256 / STG.E.256): four doubles per instruction, 32-byte aligned
+struct double4v { double a, b, c, d; };
+__device__ __forceinline__ double4v ld256(const double *p)
+{
+    double4v v;
+    asm volatile("ld.global.v4.f64 {%0,%1,%2,%3}, [%4];" : "=d"(v.a), "=d"(v.b), "=d"(v.c), "=d"(v.d) : "l"(p) : "memory");
+    return v;
+}
+__device__ __forceinline__ void st256(double *p, const double4v &v)
+{
+    asm volatile("st.global.v4.f64 [%0], {%1,%2,%3,%4};" ::"l"(p), "d"(v.a), "d"(v.b), "d"(v.c), "d"(v.d) : "memory");
+}
+__device__ __forceinline__ bool aligned32(const void *a, const void *b, const void *c)
+{
+    return ((reinterpret_cast<uintptr_t>(a) | reinterpret_cast<uintptr_t>(b) | reinterpret_cast<uintptr_t>(c)) & 31u) == 0;
+}
+#ifndef NK_V256
+#define NK_V256 1
+#endif
+
 #ifndef NK_GSU_U
-#define NK_GSU_U 2
+#define NK_GSU_U 1
 #endif
 #ifndef NK_GSU_UX
-#define NK_GSU_UX 2                                      // ... and of the variant that also updates x (mid-size meshes)
+#define NK_GSU_UX 1                                      // ... and of the variant that also updates x (mid-size meshes)
 #endif
-constexpr int GS_U = NK_GSU_U;                                   // pairs per thread and step of the large-mesh variant
+constexpr int GS_U = NK_GSU_U;                           // QUADS (four consecutive points) per thread and step
+
+__device__ __forceinline__ double4v ld4(const double *p, bool a32)
+{
+    if (a32) return ld256(p);
+    const double2 lo = reinterpret_cast<const double2 *>(p)[0], hi = reinterpret_cast<const double2 *>(p)[1];
+    double4v v;
+    v.a = lo.x; v.b = lo.y; v.c = hi.x; v.d = hi.y;
+    return v;
+}
+__device__ __forceinline__ void st4(double *p, const double4v &v, bool a32)
+{
+    if (a32) { st256(p, v); return; }
+    reinterpret_cast<double2 *>(p)[0] = make_double2(v.a, v.b);
+    reinterpret_cast<double2 *>(p)[1] = make_double2(v.c, v.d);
+}
+
+// one streamed point: r -= alpha (M Q Q^T w)_l, its share of rho'; `skip`: the point belongs to gs_row_update
+__device__ __forceinline__ void gs_point(int l, int v, double wl, double g, double alpha, double &rl, bool &skip, double &acc)
+{
+    const double s = gs_stream_value(l, v, wl, g, skip);
+    rl = fma(-alpha, s, rl);
+    acc = fma(gs_stream_weight(l, v, skip) * rl, rl, acc);
+}
 
 template <bool WITH_X>
 __global__ void __launch_bounds__(NK_GSU_THREADS, NK_GSU_MINB)
@@ -218,100 +261,88 @@ gs_update_kernel(double *__restrict__ x, double *r, const double *p, const doubl
     __shared__ double s_red[33];
     nk_pdl_launch_dependents();
     double acc = 0.0;
-    // this block's CONTIGUOUS chunk of pairs (blocks run in index order, so the resident blocks form one window
-    // that moves through the vectors: a partner a few KB or MB away is in L2 when it is gathered)
-    const int64_t pairs = L >> 1;
-    const int64_t plo = pairs * (int64_t)blockIdx.x / gridDim.x, phi = pairs * ((int64_t)blockIdx.x + 1) / gridDim.x;
+    // this block's CONTIGUOUS chunk of quads (blocks run in index order, so the resident blocks form one window
+    // that moves through the vectors: a partner a few KB or MB away is in L2 when it is gathered).  Four points per
+    // thread and step through 256-bit loads and stores: the pass is bound by the load instructions in flight, not by
+    // bytes (r, p, w live in the workspace, 256-byte aligned; the caller's x may only be 16-byte aligned).
+    const int64_t quads = L >> 2;
+    const int64_t qlo = quads * (int64_t)blockIdx.x / gridDim.x, qhi = quads * ((int64_t)blockIdx.x + 1) / gridDim.x;
     const int64_t stride = blockDim.x;
-    constexpr int U = WITH_X ? NK_GSU_UX : GS_U;                      // pairs per step, all loads before the stores
-    int64_t q = plo + threadIdx.x;
-    int2 nv[U];
+    constexpr int U = WITH_X ? NK_GSU_UX : GS_U;              // quads per step, all loads before the stores
+    const bool x32 = WITH_X && (reinterpret_cast<uintptr_t>(x) & 31u) == 0;
+    int64_t q = qlo + threadIdx.x;
+    int4 nv[U];
 #pragma unroll
     for (int j = 0; j < U; ++j)                               // gather codes of the first step: static, before the wait
-        nv[j] = (q + j * stride < phi) ? reinterpret_cast<const int2 *>(gp.nbr)[q + j * stride] : make_int2(0, 0);
+        nv[j] = (q + j * stride < qhi) ? reinterpret_cast<const int4 *>(gp.nbr)[q + j * stride] : make_int4(0, 0, 0, 0);
     nk_pdl_wait();
     const double alpha = ws.scal[NK_S_ALPHA];
     // (Staging the streamed operands through shared memory with cp.async, four pairs per thread in flight instead of
-    //  two, was measured SLOWER: 394 vs 369 us at config 5 -- the pass is bound by the gathers' sector requests, not by
-    //  bytes in flight.)
-    for (; q + (U - 1) * stride < phi; q += U * stride) {
-        double2 wv[U], rv[U], g[U], xv[WITH_X ? U : 1], pv[WITH_X ? U : 1];
-        int2 nn[U];
+    //  two, was measured SLOWER: 394 vs 369 us at config 5.)
+    for (; q < qhi; q += U * stride) {
+        double4v wv[U], rv[U], g[U], xv[WITH_X ? U : 1], pv[WITH_X ? U : 1];
+        int4 nn[U];
+        bool on[U];
 #pragma unroll
         for (int j = 0; j < U; ++j) {
             const int64_t qj = q + j * stride;
-            wv[j] = reinterpret_cast<const double2 *>(w)[qj];
-            rv[j] = reinterpret_cast<const double2 *>(r)[qj];
-            g[j].x = gs_partner(w, (int)(2 * qj), nv[j].x);
-            g[j].y = gs_partner(w, (int)(2 * qj) + 1, nv[j].y);
-            if (WITH_X) {
-                xv[WITH_X ? j : 0] = reinterpret_cast<const double2 *>(x)[qj];
-                pv[WITH_X ? j : 0] = reinterpret_cast<const double2 *>(p)[qj];
+            on[j] = qj < qhi;
+            if (on[j]) {
+                const int l = (int)(4 * qj);
+                wv[j] = ld256(w + 4 * qj);
+                rv[j] = ld256(r + 4 * qj);
+                g[j].a = gs_partner(w, l, nv[j].x);
+                g[j].b = gs_partner(w, l + 1, nv[j].y);
+                g[j].c = gs_partner(w, l + 2, nv[j].z);
+                g[j].d = gs_partner(w, l + 3, nv[j].w);
+                if (WITH_X) {
+                    xv[WITH_X ? j : 0] = ld4(x + 4 * qj, x32);
+                    pv[WITH_X ? j : 0] = ld256(p + 4 * qj);
+                }
             }
         }
 #pragma unroll
         for (int j = 0; j < U; ++j) {                         // next step's gather codes
             const int64_t qn = q + (U + j) * stride;
-            nn[j] = (qn < phi) ? reinterpret_cast<const int2 *>(gp.nbr)[qn] : make_int2(0, 0);
+            nn[j] = (qn < qhi) ? reinterpret_cast<const int4 *>(gp.nbr)[qn] : make_int4(0, 0, 0, 0);
         }
 #pragma unroll
         for (int j = 0; j < U; ++j) {
-            const int64_t qj = q + j * stride;
-            const int l = (int)(2 * qj);
-            bool k0, k1;
-            const double s0 = gs_stream_value(l, nv[j].x, wv[j].x, g[j].x, k0);
-            const double s1 = gs_stream_value(l + 1, nv[j].y, wv[j].y, g[j].y, k1);
-            rv[j].x = fma(-alpha, s0, rv[j].x);
-            rv[j].y = fma(-alpha, s1, rv[j].y);
-            if (!(k0 || k1)) {
-                reinterpret_cast<double2 *>(r)[qj] = rv[j];
-            } else {                                          // gs_row_update owns the other entry of the pair
-                if (!k0) r[l] = rv[j].x;
-                if (!k1) r[l + 1] = rv[j].y;
-            }
-            acc = fma(gs_stream_weight(l, nv[j].x, k0) * rv[j].x, rv[j].x, acc);
-            acc = fma(gs_stream_weight(l + 1, nv[j].y, k1) * rv[j].y, rv[j].y, acc);
-            if (WITH_X) {
-                double2 xn = xv[WITH_X ? j : 0];
-                xn.x = fma(alpha, pv[WITH_X ? j : 0].x, xn.x);
-                xn.y = fma(alpha, pv[WITH_X ? j : 0].y, xn.y);
-                reinterpret_cast<double2 *>(x)[qj] = xn;
+            if (on[j]) {
+                const int64_t qj = q + j * stride;
+                const int l = (int)(4 * qj);
+                bool k0, k1, k2, k3;
+                gs_point(l, nv[j].x, wv[j].a, g[j].a, alpha, rv[j].a, k0, acc);
+                gs_point(l + 1, nv[j].y, wv[j].b, g[j].b, alpha, rv[j].b, k1, acc);
+                gs_point(l + 2, nv[j].z, wv[j].c, g[j].c, alpha, rv[j].c, k2, acc);
+                gs_point(l + 3, nv[j].w, wv[j].d, g[j].d, alpha, rv[j].d, k3, acc);
+                if (!(k0 || k1 || k2 || k3)) {
+                    st256(r + 4 * qj, rv[j]);
+                } else {                                      // gs_row_update owns the skipped entries
+                    if (!k0) r[l] = rv[j].a;
+                    if (!k1) r[l + 1] = rv[j].b;
+                    if (!k2) r[l + 2] = rv[j].c;
+                    if (!k3) r[l + 3] = rv[j].d;
+                }
+                if (WITH_X) {
+                    double4v xn = xv[WITH_X ? j : 0];
+                    const double4v pj = pv[WITH_X ? j : 0];
+                    xn.a = fma(alpha, pj.a, xn.a); xn.b = fma(alpha, pj.b, xn.b);
+                    xn.c = fma(alpha, pj.c, xn.c); xn.d = fma(alpha, pj.d, xn.d);
+                    st4(x + 4 * qj, xn, x32);
+                }
             }
             nv[j] = nn[j];
         }
     }
-    for (; q < phi; q += stride) {
-        const int2 n2 = reinterpret_cast<const int2 *>(gp.nbr)[q];
-        const double2 wv = reinterpret_cast<const double2 *>(w)[q];
-        double2 rv = reinterpret_cast<const double2 *>(r)[q];
-        const int l = (int)(2 * q);
-        bool k0, k1;
-        const double s0 = gs_stream_value(l, n2.x, wv.x, gs_partner(w, l, n2.x), k0);
-        const double s1 = gs_stream_value(l + 1, n2.y, wv.y, gs_partner(w, l + 1, n2.y), k1);
-        rv.x = fma(-alpha, s0, rv.x);
-        rv.y = fma(-alpha, s1, rv.y);
-        if (!k0) r[l] = rv.x;
-        if (!k1) r[l + 1] = rv.y;
-        acc = fma(gs_stream_weight(l, n2.x, k0) * rv.x, rv.x, acc);
-        acc = fma(gs_stream_weight(l + 1, n2.y, k1) * rv.y, rv.y, acc);
-        if (WITH_X) {
-            double2 xn = reinterpret_cast<const double2 *>(x)[q];
-            const double2 pv = reinterpret_cast<const double2 *>(p)[q];
-            xn.x = fma(alpha, pv.x, xn.x);
-            xn.y = fma(alpha, pv.y, xn.y);
-            reinterpret_cast<double2 *>(x)[q] = xn;
-        }
-    }
-    if ((L & 1) && blockIdx.x == gridDim.x - 1 && threadIdx.x == 0) {
-        const int l = (int)(L - 1);
+    if (blockIdx.x == gridDim.x - 1 && (int64_t)threadIdx.x < (L & 3)) {    // up to three points past the last quad
+        const int l = (int)((quads << 2) + threadIdx.x);
         const int v = gp.nbr[l];
         bool k0;
-        const double s0 = gs_stream_value(l, v, w[l], gs_partner(w, l, v), k0);
-        if (!k0) {
-            const double rn = fma(-alpha, s0, r[l]);
-            r[l] = rn;
-            acc = fma(gs_stream_weight(l, v, false) * rn, rn, acc);
-        }
+        double rl = r[l];
+        double a0 = 0.0;
+        gs_point(l, v, w[l], gs_partner(w, l, v), alpha, rl, k0, a0);
+        if (!k0) { r[l] = rl; acc += a0; }
         if (WITH_X) x[l] = fma(alpha, p[l], x[l]);
     }
     // the nodes with three or more copies whose FIRST copy lies in this block's chunk (their other copies sit in
@@ -407,9 +438,24 @@ update_px_kernel(double *__restrict__ x, double *__restrict__ p, const double *r
     nk_pdl_launch_dependents();
     nk_pdl_wait();
     const double alpha = scal[NK_S_ALPHA], beta = scal[NK_S_BETA];
-    const int64_t pairs = L >> 1;
     const int64_t stride = (int64_t)gridDim.x * blockDim.x;
-    for (int64_t q = (int64_t)blockIdx.x * blockDim.x + threadIdx.x; q < pairs; q += stride) {
+    int64_t done = 0;                                       // points handled four at a time
+    if (NK_V256 && aligned32(x, p, r)) {
+        const int64_t quads = L >> 2;
+        for (int64_t q = (int64_t)blockIdx.x * blockDim.x + threadIdx.x; q < quads; q += stride) {
+            const double4v rv = ld256(r + 4 * q);
+            double4v pv = ld256(p + 4 * q), xv = ld256(x + 4 * q);
+            xv.a = fma(alpha, pv.a, xv.a); xv.b = fma(alpha, pv.b, xv.b);
+            xv.c = fma(alpha, pv.c, xv.c); xv.d = fma(alpha, pv.d, xv.d);
+            pv.a = fma(beta, pv.a, rv.a); pv.b = fma(beta, pv.b, rv.b);
+            pv.c = fma(beta, pv.c, rv.c); pv.d = fma(beta, pv.d, rv.d);
+            st256(x + 4 * q, xv);
+            st256(p + 4 * q, pv);
+        }
+        done = quads << 2;
+    }
+    const int64_t pairs = L >> 1;
+    for (int64_t q = (done >> 1) + (int64_t)blockIdx.x * blockDim.x + threadIdx.x; q < pairs; q += stride) {
         const double2 rv = reinterpret_cast<const double2 *>(r)[q];
         double2 pv = reinterpret_cast<double2 *>(p)[q];
         double2 xv = reinterpret_cast<double2 *>(x)[q];
