@@ -209,8 +209,8 @@ int nk_dist_cg(nk_ctx *ctx, const double *f, double *x, int niter, double *res_h
  *                  adds the same terms in another fixed order, so iterates agree to rounding, not bitwise).
  *                  gs's write-back, its re-read and one launch per iteration are gone.  Needs "fuse_pap" = 1
  *                  (the separate weighted dot reads the summed w); 0 = nk_gs as its own kernel; 2 (default)
- *                  = 1 for meshes of more than 2^21 local points (below, everything sits in L2 and the
- *                  separate kernel is faster), else 0.
+ *                  = 1 for meshes of 2^20 local points or more (below, everything sits in L2 and the
+ *                  separate kernel is as fast or faster), else 0.
  *   "coop"         1 = nk_cg runs the whole solve as ONE cooperative launch: a persistent CTA per SM does all
  *                  iterations (ax_e with pap and the p update folded in | grid barrier | x, r update with gs
  *                  and the mask folded in, rho' | grid barrier), scalars never leave the chip.  For meshes

@@ -110,12 +110,14 @@ inline bool fuse_p_on(const nk_ctx *c)
     return c->opt_fuse_p == 1 || (c->opt_fuse_p == 2 && c->L <= NK_GRAPH_AUTO_MAX_L);
 }
 
-// "fuse_gs" = 2 (default): gs rides in the residual update where its traffic matters (measured: config 5 135.5 ->
-// 132.1 ms per solve, config 3 11.3 -> 10.9; on L2-resident meshes the separate kernel is faster: config 2 1.55 vs
-// 1.78 ms).  The separate weighted dot needs the summed w, so without "fuse_pap" gs stays a kernel of its own.
+// "fuse_gs" = 2 (default): gs rides in the residual update from 2^20 local points on (measured per iteration, graph
+// replay, fused against separate: N=7 1.05 M points 30.4 vs 33.1 us, 2.1 M 51.7 vs 55.1; N=11 1.77 M 49.1 vs 51.6;
+// N=9 2.05 M 54.9 vs 57.1, config 5 1.25 vs 1.28 ms; below, on meshes that sit in L2, the separate kernel is as fast
+// or faster: N=9 1.02 M 32.4 vs 31.8, N=7 0.52 M 21.9 vs 21.2).  The separate weighted dot needs the summed w, so
+// without "fuse_pap" gs stays a kernel of its own.
 inline bool fuse_gs_on(const nk_ctx *c)
 {
-    return c->opt_fuse_pap && (c->opt_fuse_gs == 1 || (c->opt_fuse_gs == 2 && c->L > NK_FUSE_GS_AUTO_MIN_L));
+    return c->opt_fuse_pap && (c->opt_fuse_gs == 1 || (c->opt_fuse_gs == 2 && c->L >= NK_FUSE_GS_AUTO_MIN_L));
 }
 
 // One CG iteration, enqueued (S 3 call stack (3)).  hist_k: where sqrt(rho') goes (DEVICE).
@@ -261,7 +263,8 @@ int nk_cg(nk_ctx *c, const double *f, double *x, int niter, double *res_hist, vo
     }
     // Record the launch sequence once per (f, x, res_hist, niter, options) and replay it: the CG
     // loop of the small configs is launch-bound (S 7 hard part 4).
-    const int key = c->opt_fuse_pap | (c->opt_fuse_p << 1) | (c->opt_fuse_gs << 3) | (c->opt_pdl << 4);
+    // one bit field per option (1, 2, 2, 2 bits): two option sets never share a key
+    const int key = c->opt_fuse_pap | (c->opt_fuse_p << 1) | (c->opt_fuse_gs << 3) | (c->opt_pdl << 5);
     nk_ctx::graph_slot *g = nullptr;
     for (auto &sl : c->graph)
         if (sl.exec && sl.f == f && sl.x == x && sl.hist == res_hist && sl.niter == niter && sl.key == key) g = &sl;

@@ -27,7 +27,7 @@ enum { NK_EPI_STORE = 0,   // out[0] = total
 #ifndef NK_CLUSTER_AUTO_MAX_L
 #define NK_CLUSTER_AUTO_MAX_L (1 << 15)  // within "coop": up to this many points the solve runs on ONE 16-CTA cluster
 #endif
-#define NK_FUSE_GS_AUTO_MIN_L (1 << 21)  // "fuse_gs" = 2: gs rides in the residual update above this many local points
+#define NK_FUSE_GS_AUTO_MIN_L (1 << 20)  // "fuse_gs" = 2: gs rides in the residual update from this many local points on
 #define NK_GS_CHUNK 32768          // rows per gs chunk (128 blocks of 256 threads)
 #define NK_CTAB 128                // code & 0x7f indexes ctab[] = 1/multiplicity
 

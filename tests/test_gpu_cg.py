@@ -6,7 +6,7 @@ import pytest
 
 from parity import elem_err, maxnorm_rel
 from gpu_common import pair_for_brick, pair_for_config, to_dev, to_np, TOL_OP, TOL_CG
-from workloads import CONFIGS, config_rhs, rhs_unique
+from workloads import CONFIGS, brick_mesh, config_rhs, rhs_unique
 
 pytestmark = pytest.mark.gpu
 
@@ -121,6 +121,37 @@ def test_cg_host_batch_equals_one_call_per_rhs(path):
     finally:
         for k, v in saved.items():
             gpu.set_option(k, v)
+
+
+def test_cached_graphs_are_keyed_by_every_option():
+    """nk_cg keeps two recorded graphs (nk_cg_host_batch alternates between two sets of buffers).  Each option has a
+    bit field of its own in the cache key: with fuse_gs = 2 and pdl = 3 sharing a bit, the graph recorded for
+    fuse_gs = 0 was replayed for fuse_gs = 2.  1 M points, so fuse_gs = 2 means fused; fused and separate gs differ in
+    the rounding of rho', which tells the replayed graphs apart."""
+    mesh = brick_mesh(16, 16, 8, 7, 0.05)
+    from paper_2606_12650_b200 import Nekbone
+    gpu = Nekbone.from_mesh(mesh)
+    try:
+        rng = np.random.Generator(np.random.PCG64(5))
+        _, inv = np.unique(mesh.glo_num, return_inverse=True)
+        f = to_dev(rng.uniform(-1, 1, inv.max() + 1)[inv])
+        gpu.set_option("coop", 0)
+        gpu.set_option("graph", 1)
+        x, h = gpu.empty(), gpu.empty()[:32]
+        hist = {}
+        for fuse_gs in (0, 1, 2, 0, 2, 1):                    # same buffers every time: only the key tells them apart
+            gpu.set_option("fuse_gs", fuse_gs)
+            assert gpu.solve_path() == "graph"
+            gpu.cg(f, 30, x=x, res_hist=h)
+            hn = to_np(h)[:31].copy()
+            if fuse_gs in hist:
+                assert np.array_equal(hist[fuse_gs], hn), fuse_gs
+            hist[fuse_gs] = hn
+        assert np.array_equal(hist[2], hist[1])               # 2 = fused at this size
+        assert not np.array_equal(hist[0], hist[1])           # ... and the two are distinguishable here
+        assert np.all(np.abs(hist[0] - hist[1]) <= 1e-10 * hist[0])
+    finally:
+        gpu.close()
 
 
 def test_cg_reproducible_and_ignores_incoming_x():
