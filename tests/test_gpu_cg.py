@@ -398,10 +398,11 @@ def test_fused_gs_against_separate_gs(name, fuse_p):
     gpu.close()
 
 
-@pytest.mark.parametrize("brick", [(3, 2, 2, 4), (10, 8, 7, 4)])
+@pytest.mark.parametrize("brick", [(3, 2, 2, 4), (10, 8, 7, 4), (3, 3, 3, 2), (6, 1, 1, 2), (5, 3, 3, 6)])
 def test_fused_gs_on_irregular_ids(brick):
     """Rows of 3, 5, 12 copies and scattered ids take the fused gather's CSR path; Dirichlet rows its zero path.
-    1500 points: the cooperative solve runs on one cluster; 70 000 points: on the grid."""
+    1500 points: the cooperative solve runs on one cluster; 70 000 points: on the grid.  The last three meshes have
+    729, 162 and 15435 points: one, two and three points past the last quad of the fused update's 256-bit loop."""
     from oracle.nko import Oracle
     from paper_2606_12650_b200 import Nekbone
     from workloads import brick_mesh
