@@ -121,7 +121,12 @@ inline bool fuse_gs_on(const nk_ctx *c)
 }
 
 // One CG iteration, enqueued (S 3 call stack (3)).  hist_k: where sqrt(rho') goes (DEVICE).
-cudaError_t enqueue_iteration(nk_ctx *c, double *x, double *hist_k, cudaStream_t st)
+// "defer_x" (default on; only where the direction update is a kernel of its own, i.e. without "fuse_p"): two iterations
+// share one pass over x (nk_vec.cu update_p2_kernel / update_pxx_kernel).  pair = 0: a plain iteration; 1: the first
+// of a pair (p2 = r + beta p, x untouched); 2: the second (runs on p2; x takes both steps, p = r + beta' p2).
+inline bool defer_x_on(const nk_ctx *c) { return c->opt_defer_x && !fuse_p_on(c); }
+
+cudaError_t enqueue_iteration(nk_ctx *c, double *x, double *hist_k, cudaStream_t st, int pair = 0)
 {
     cudaError_t e;
     const int fuse_pap = c->opt_fuse_pap;
@@ -129,13 +134,13 @@ cudaError_t enqueue_iteration(nk_ctx *c, double *x, double *hist_k, cudaStream_t
         NK_LAUNCH(NK_K_AX, nk_launch_ax_tma(c, c->p, nullptr, c->r, c->w, fuse_pap, st));
         c->p_pending = 0;
     } else {
-        NK_LAUNCH(NK_K_AX, nk_launch_ax_tma(c, nullptr, c->p, nullptr, c->w, fuse_pap, st));
+        NK_LAUNCH(NK_K_AX, nk_launch_ax_tma(c, nullptr, pair == 2 ? c->p2 : c->p, nullptr, c->w, fuse_pap, st));
     }
     // "fuse_gs": gs and the mask ride in the residual update, which gathers the copies of shared nodes from the
     // unsummed w (nk_vec.cu); the separate weighted dot needs the summed w, so it keeps gs in place
     const int fuse_gs = fuse_gs_on(c);
     if (!fuse_gs) NK_LAUNCH(NK_K_GS, nk_launch_gs(c, c->w, 1, st));
-    if (!fuse_pap) NK_LAUNCH(NK_K_DOT, nk_launch_dot(c, c->w, c->p, nullptr, NK_EPI_PAP, st));
+    if (!fuse_pap) NK_LAUNCH(NK_K_DOT, nk_launch_dot(c, c->w, pair == 2 ? c->p2 : c->p, nullptr, NK_EPI_PAP, st));
     c->w_unsummed = fuse_gs;
     if (fuse_p_on(c)) {
         NK_LAUNCH(NK_K_UPDATE_XR, nk_launch_update_xr(c, x, hist_k, fuse_gs, st));
@@ -143,7 +148,9 @@ cudaError_t enqueue_iteration(nk_ctx *c, double *x, double *hist_k, cudaStream_t
     } else {
         // r first, then x and p together: p is read once per iteration instead of twice (65 vs 73 B/pt)
         NK_LAUNCH(NK_K_UPDATE_XR, nk_launch_update_r(c, hist_k, fuse_gs, st));
-        NK_LAUNCH(NK_K_UPDATE_P, nk_launch_update_px(c, x, st));
+        if (pair == 1) NK_LAUNCH(NK_K_UPDATE_P, nk_launch_update_p2(c, st));
+        else if (pair == 2) NK_LAUNCH(NK_K_UPDATE_P, nk_launch_update_pxx(c, x, st));
+        else NK_LAUNCH(NK_K_UPDATE_P, nk_launch_update_px(c, x, st));
     }
     return cudaSuccess;
 }
@@ -158,8 +165,12 @@ cudaError_t enqueue_cg(nk_ctx *c, const double *f, double *x, int niter, double 
     // wrote, so the launches may overlap tail and prologue; the event pairs of "profile" would serialise them
     struct pdl_scope { nk_ctx *c; ~pdl_scope() { c->pdl_now = 0; } } scope{c};
     c->pdl_now = c->opt_profile ? 0 : nk_pdl_mode(c);
-    for (int k = 1; k <= niter; ++k)
-        if ((e = enqueue_iteration(c, x, res_hist + k, st)) != cudaSuccess) return e;
+    const bool defer = defer_x_on(c);
+    for (int k = 1; k <= niter; ++k) {
+        // pairs (k, k+1) from the front; an odd last iteration is a plain one, so x, r, p are complete at the end
+        const int pair = !defer ? 0 : (k % 2 == 1 ? (k < niter ? 1 : 0) : 2);
+        if ((e = enqueue_iteration(c, x, res_hist + k, st, pair)) != cudaSuccess) return e;
+    }
     if (c->p_pending) {          // leave the context with p up to date
         NK_LAUNCH(NK_K_UPDATE_P, nk_launch_update_p(c, st));
         c->p_pending = 0;
@@ -263,8 +274,8 @@ int nk_cg(nk_ctx *c, const double *f, double *x, int niter, double *res_hist, vo
     }
     // Record the launch sequence once per (f, x, res_hist, niter, options) and replay it: the CG
     // loop of the small configs is launch-bound (S 7 hard part 4).
-    // one bit field per option (1, 2, 2, 2 bits): two option sets never share a key
-    const int key = c->opt_fuse_pap | (c->opt_fuse_p << 1) | (c->opt_fuse_gs << 3) | (c->opt_pdl << 5);
+    // one bit field per option (1, 2, 2, 2, 1 bits): two option sets never share a key
+    const int key = c->opt_fuse_pap | (c->opt_fuse_p << 1) | (c->opt_fuse_gs << 3) | (c->opt_pdl << 5) | (c->opt_defer_x << 7);
     nk_ctx::graph_slot *g = nullptr;
     for (auto &sl : c->graph)
         if (sl.exec && sl.f == f && sl.x == x && sl.hist == res_hist && sl.niter == niter && sl.key == key) g = &sl;
@@ -447,6 +458,7 @@ static int *option_slot(nk_ctx *c, const char *name, int *lo, int *hi)
     if (!std::strcmp(name, "fuse_gs")) { *lo = 0; *hi = 2; return &c->opt_fuse_gs; }
     if (!std::strcmp(name, "graph")) { *lo = 0; *hi = 2; return &c->opt_graph; }
     if (!std::strcmp(name, "coop")) { *lo = 0; *hi = 2; return &c->opt_coop; }
+    if (!std::strcmp(name, "defer_x")) { *lo = 0; *hi = 1; return &c->opt_defer_x; }
     if (!std::strcmp(name, "pdl")) { *lo = 0; *hi = 3; return &c->opt_pdl; }
     if (!std::strcmp(name, "profile")) { *lo = 0; *hi = 1; return &c->opt_profile; }
     return nullptr;

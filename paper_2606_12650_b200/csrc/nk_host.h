@@ -30,7 +30,7 @@ inline nk_carve nk_carve_sizes(int64_t L)
 {
     nk_carve c;
     c.g = nk_align_up(3 * (size_t)L * sizeof(double2), 256);      // all six factors
-    c.vec = nk_align_up((size_t)L * sizeof(double), 256);         // x8 (r, p, w, hf, hx, dinv, hf2, hx2)
+    c.vec = nk_align_up((size_t)L * sizeof(double), 256);         // x9 (r, p, w, hf, hx, dinv, hf2, hx2, p2)
     c.code = nk_align_up((size_t)L, 256);
     c.off = nk_align_up(((size_t)L + 1) * sizeof(int32_t), 256);
     c.idx = nk_align_up((size_t)L * sizeof(int32_t), 256);
@@ -45,7 +45,7 @@ inline nk_carve nk_carve_sizes(int64_t L)
     c.hist = nk_align_up(NK_HIST_MAX * sizeof(double), 256);
     c.scal = 256;
     c.small = 256;                                                // counter, errflag, res_dummy
-    c.total = c.g + 8 * c.vec + c.code + c.off + c.idx + c.nbr + c.gx + c.pk + c.tabs + c.partials + 2 * c.hist + c.scal + c.small;
+    c.total = c.g + 9 * c.vec + c.code + c.off + c.idx + c.nbr + c.gx + c.pk + c.tabs + c.partials + 2 * c.hist + c.scal + c.small;
     return c;
 }
 

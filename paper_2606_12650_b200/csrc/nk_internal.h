@@ -9,6 +9,7 @@
 
 // Scalar block on the device (doubles).  Written only by reduction epilogues.
 enum { NK_S_RHO = 0, NK_S_PAP = 1, NK_S_ALPHA = 2, NK_S_RHO_NEW = 3, NK_S_BETA = 4, NK_S_RHO_OLD = 5,
+       NK_S_ALPHA_PREV = 6,     // alpha of the first iteration of a pair whose x update is deferred ("defer_x")
        NK_S_COUNT = 8 };
 
 // What the last block of a reduction does with the ordered total (S 8(a) a7).
@@ -65,6 +66,7 @@ struct nk_ctx {
                                  // k-plane one contiguous chunk [c2][i + n j] of (rr,rs) (rt,ss) (st,tt)
     double *r, *p, *w;           // CG state, L each (coords staging aliases these during set-up)
     double *hf, *hx;             // staging for nk_cg_host, L each
+    double *p2;                  // second direction vector: the deferred x update needs p_k and p_k+1 at once ("defer_x")
     double *hf2, *hx2, *hist2;   // second set: nk_cg_host_batch copies RHS j+1 in and solution j-1 out while solve j runs
     double *dinv;                // Jacobi preconditioner 1 / (Q Q^T diag A_L), 0 on Dirichlet nodes (lazy)
     int have_dinv;
@@ -103,7 +105,7 @@ struct nk_ctx {
     int64_t n_unique, n_shared_unique, n_masked_unique;
     int64_t n_rows, n_listed, n_sum_rows, n_sum_listed;
     // options / state
-    int opt_fuse_pap, opt_fuse_p, opt_fuse_gs, opt_coop, opt_graph, opt_profile, opt_pdl;
+    int opt_fuse_pap, opt_fuse_p, opt_fuse_gs, opt_coop, opt_graph, opt_profile, opt_pdl, opt_defer_x;
     int pdl_now;                 // nk_pdl_mode while nk_cg enqueues its loop (every kernel there waits), else 0
     int p_pending;               // 1: p = r + beta p has not been applied yet (fuse_p)
     int w_unsummed;              // 1: ctx w holds the unsummed ax_e output of the last iteration (fuse_gs)
@@ -228,6 +230,8 @@ cudaError_t nk_launch_update_xr(nk_ctx *c, double *x, double *hist_k, int gs, cu
 cudaError_t nk_launch_update_p(nk_ctx *c, cudaStream_t st);
 cudaError_t nk_launch_update_r(nk_ctx *c, double *hist_k, int gs, cudaStream_t st);     // r -= alpha w, rho'
 cudaError_t nk_launch_update_px(nk_ctx *c, double *x, cudaStream_t st);         // x += alpha p; p = r + beta p
+cudaError_t nk_launch_update_p2(nk_ctx *c, cudaStream_t st);                    // p2 = r + beta p; alpha kept for the next one
+cudaError_t nk_launch_update_pxx(nk_ctx *c, double *x, cudaStream_t st);        // x += alpha' p + alpha p2; p = r + beta p2
 cudaError_t nk_launch_get_mult(nk_ctx *c, double *mult, cudaStream_t st);
 // preconditioned CG
 cudaError_t nk_launch_diag(nk_ctx *c, double *diag, cudaStream_t st);          // nk_geom.cu: diag(A_L), local

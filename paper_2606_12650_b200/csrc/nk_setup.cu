@@ -404,7 +404,7 @@ extern "C" int nk_setup(nk_ctx **ctx, int64_t E, int N, const double *coords, co
     c->E = E; c->N = N; c->n = N + 1; c->P = (int64_t)c->n * c->n * c->n; c->L = L;
     c->device = dev; c->sm_count = sms;
     c->ws = workspace; c->ws_bytes = workspace_bytes;
-    c->opt_fuse_pap = 1; c->opt_fuse_p = 2; c->opt_fuse_gs = 2; c->opt_coop = 2; c->opt_graph = 2; c->opt_pdl = 3; c->pdl_now = 0;
+    c->opt_fuse_pap = 1; c->opt_fuse_p = 2; c->opt_fuse_gs = 2; c->opt_coop = 2; c->opt_graph = 2; c->opt_pdl = 3; c->opt_defer_x = 1; c->pdl_now = 0;
     nk_host_basis(N, c->xi, c->wq, c->D);
     char *q = static_cast<char *>(workspace);
     c->g = reinterpret_cast<double2 *>(q); q += cv.g;
@@ -416,6 +416,7 @@ extern "C" int nk_setup(nk_ctx **ctx, int64_t E, int N, const double *coords, co
     c->dinv = reinterpret_cast<double *>(q); q += cv.vec;
     c->hf2 = reinterpret_cast<double *>(q); q += cv.vec;
     c->hx2 = reinterpret_cast<double *>(q); q += cv.vec;
+    c->p2 = reinterpret_cast<double *>(q); q += cv.vec;
     c->code = reinterpret_cast<uint8_t *>(q); q += cv.code;
     c->row_off = reinterpret_cast<int32_t *>(q); q += cv.off;
     c->row_idx = reinterpret_cast<int32_t *>(q); q += cv.idx;

@@ -430,6 +430,60 @@ update_r_kernel(double *__restrict__ r, const double *w, const uint8_t *__restri
     nk_grid_reduce(acc, s_red, ws, NK_EPI_RHO, hist_k);
 }
 
+// ---- the x update deferred by one iteration ("defer_x"; large meshes, where the direction update is a kernel of its
+// own).  x_k+1 = x_k + alpha_k p_k is not needed before the solve ends, so two iterations share one pass over x:
+//   first of a pair   p2 = r + beta p                        (24 B/pt; alpha kept in NK_S_ALPHA_PREV)
+//   second            x = fma(alpha', p2, fma(alpha, p, x)); p = r + beta' p2                  (48 B/pt)
+// 72 B/pt per pair instead of 2 x 40, and x, entry by entry, is bit for bit what two separate updates give (the same
+// two fused multiply-adds in the same order).  Costs one more vector in the workspace.
+__global__ void __launch_bounds__(NK_VEC_THREADS)
+update_p2_kernel(double *__restrict__ p2, const double *p, const double *r, double *scal, int64_t L)
+{
+    nk_pdl_launch_dependents();
+    nk_pdl_wait();
+    const double beta = scal[NK_S_BETA];
+    if (blockIdx.x == 0 && threadIdx.x == 0) scal[NK_S_ALPHA_PREV] = scal[NK_S_ALPHA];   // the next ax_e overwrites alpha
+    const int64_t stride = (int64_t)gridDim.x * blockDim.x;
+    const int64_t quads = L >> 2;                            // p, p2, r live in the workspace: 256-byte aligned
+    for (int64_t q = (int64_t)blockIdx.x * blockDim.x + threadIdx.x; q < quads; q += stride) {
+        const double4v rv = ld256(r + 4 * q), pv = ld256(p + 4 * q);
+        double4v o;
+        o.a = fma(beta, pv.a, rv.a); o.b = fma(beta, pv.b, rv.b);
+        o.c = fma(beta, pv.c, rv.c); o.d = fma(beta, pv.d, rv.d);
+        st256(p2 + 4 * q, o);
+    }
+    if (blockIdx.x == 0 && (int64_t)threadIdx.x < (L & 3)) {
+        const int64_t l = (quads << 2) + threadIdx.x;
+        p2[l] = fma(beta, p[l], r[l]);
+    }
+}
+
+__global__ void __launch_bounds__(NK_VEC_THREADS)
+update_pxx_kernel(double *__restrict__ x, double *p, const double *p2, const double *r, const double *scal, int64_t L)
+{
+    nk_pdl_launch_dependents();
+    nk_pdl_wait();
+    const double alpha0 = scal[NK_S_ALPHA_PREV], alpha1 = scal[NK_S_ALPHA], beta = scal[NK_S_BETA];
+    const int64_t stride = (int64_t)gridDim.x * blockDim.x;
+    const int64_t quads = L >> 2;
+    const bool x32 = (reinterpret_cast<uintptr_t>(x) & 31u) == 0;      // the caller's x may only be 16-byte aligned
+    for (int64_t q = (int64_t)blockIdx.x * blockDim.x + threadIdx.x; q < quads; q += stride) {
+        const double4v rv = ld256(r + 4 * q), pa = ld256(p + 4 * q), pb = ld256(p2 + 4 * q);
+        double4v xv = ld4(x + 4 * q, x32), o;
+        xv.a = fma(alpha1, pb.a, fma(alpha0, pa.a, xv.a)); xv.b = fma(alpha1, pb.b, fma(alpha0, pa.b, xv.b));
+        xv.c = fma(alpha1, pb.c, fma(alpha0, pa.c, xv.c)); xv.d = fma(alpha1, pb.d, fma(alpha0, pa.d, xv.d));
+        o.a = fma(beta, pb.a, rv.a); o.b = fma(beta, pb.b, rv.b);
+        o.c = fma(beta, pb.c, rv.c); o.d = fma(beta, pb.d, rv.d);
+        st4(x + 4 * q, xv, x32);
+        st256(p + 4 * q, o);
+    }
+    if (blockIdx.x == 0 && (int64_t)threadIdx.x < (L & 3)) {
+        const int64_t l = (quads << 2) + threadIdx.x;
+        x[l] = fma(alpha1, p2[l], fma(alpha0, p[l], x[l]));
+        p[l] = fma(beta, p2[l], r[l]);
+    }
+}
+
 // x += alpha p (the OLD p); p = r + beta p
 __global__ void __launch_bounds__(NK_VEC_THREADS)
 update_px_kernel(double *__restrict__ x, double *__restrict__ p, const double *r,
@@ -672,6 +726,26 @@ cudaError_t nk_launch_update_r(nk_ctx *c, double *hist_k, int gs, cudaStream_t s
     const int nb = vec_blocks(c, c->L >> 1);
     const cudaError_t e = nk_launch(update_r_kernel, nb, NK_VEC_THREADS, 0, st, c->pdl_now, c->r, c->w, c->code, c->ctab,
                                     c->L, c->red, hist_k);
+    if (e != cudaSuccess) return e;
+    c->launches++;
+    return cudaGetLastError();
+}
+
+cudaError_t nk_launch_update_p2(nk_ctx *c, cudaStream_t st)
+{
+    const int nb = vec_blocks(c, c->L >> 1);
+    const cudaError_t e = nk_launch(update_p2_kernel, nb, NK_VEC_THREADS, 0, st, c->pdl_now, c->p2, (const double *)c->p,
+                                    (const double *)c->r, c->red.scal, c->L);
+    if (e != cudaSuccess) return e;
+    c->launches++;
+    return cudaGetLastError();
+}
+
+cudaError_t nk_launch_update_pxx(nk_ctx *c, double *x, cudaStream_t st)
+{
+    const int nb = vec_blocks(c, c->L >> 1);
+    const cudaError_t e = nk_launch(update_pxx_kernel, nb, NK_VEC_THREADS, 0, st, c->pdl_now, x, c->p, (const double *)c->p2,
+                                    (const double *)c->r, (const double *)c->red.scal, c->L);
     if (e != cudaSuccess) return e;
     c->launches++;
     return cudaGetLastError();

@@ -123,6 +123,39 @@ def test_cg_host_batch_equals_one_call_per_rhs(path):
             gpu.set_option(k, v)
 
 
+@pytest.mark.parametrize("niter", [1, 2, 7, 12])
+@pytest.mark.parametrize("fuse_gs", [0, 1])
+def test_deferred_x_update_is_bitwise_the_plain_one(niter, fuse_gs):
+    """"defer_x": two iterations share one pass over x (x = fma(alpha', p', fma(alpha, p, x)), the direction kept in two
+    vectors).  Same operations in the same order: x, the history and the state the context is left in (r, p, w) are
+    bit for bit those of the plain update -- odd and even iteration counts, launch by launch and graphed, with the
+    caller's x only 16-byte aligned (the 256-bit accesses fall back to 128-bit ones on x)."""
+    import torch
+    pr = pair_for_brick(7, 6, 5, 6, 0.05)                    # 72030 points: two past the last quad
+    gpu = pr.gpu
+    saved = {k: gpu.get_option(k) for k in ("coop", "fuse_p", "fuse_gs", "graph", "defer_x")}
+    try:
+        gpu.set_option("coop", 0)
+        gpu.set_option("fuse_p", 0)
+        gpu.set_option("fuse_gs", fuse_gs)
+        f = to_dev(rhs_unique(pr.mesh, 77))
+        xbuf = torch.empty(pr.L + 2, dtype=torch.float64, device="cuda")
+        out = {}
+        for defer in (0, 1):
+            for graph in (0, 1):
+                gpu.set_option("defer_x", defer)
+                gpu.set_option("graph", graph)
+                x = xbuf[2:] if defer else gpu.empty()        # 16-byte aligned only
+                x, h = gpu.cg(f, niter, x=x)
+                out[defer, graph] = (to_np(x),) + tuple(to_np(t) for t in gpu.cg_get_state()) + (to_np(h),)
+        for key in ((0, 1), (1, 0), (1, 1)):
+            for a, b in zip(out[0, 0], out[key]):
+                assert np.array_equal(a, b), key
+    finally:
+        for k, v in saved.items():
+            gpu.set_option(k, v)
+
+
 def test_cached_graphs_are_keyed_by_every_option():
     """nk_cg keeps two recorded graphs (nk_cg_host_batch alternates between two sets of buffers).  Each option has a
     bit field of its own in the cache key: with fuse_gs = 2 and pdl = 3 sharing a bit, the graph recorded for
