@@ -427,6 +427,7 @@ def run_ours(args) -> dict | None:
     fused_gs = bool(opts["fuse_pap"]) and (opts["fuse_gs"] == 1 or (opts["fuse_gs"] == 2 and L >= (1 << 20)))
     # "defer_x": two iterations share one pass over x (24 + 48 B/pt per pair instead of 2 x 40; an odd last one is plain)
     px_bytes = (72.0 * (niter // 2) + 40.0 * (niter % 2)) / max(niter, 1) if opts["defer_x"] else 40.0
+    xr_fused_p = (80.0 * (niter // 2) + 48.0 * (niter % 2)) / max(niter, 1) if opts["defer_x"] else 48.0
     out = {"metric": METRIC, "value": value, "unit": UNIT, "n_gpus": world, "steps": args.steps,
            "warmup": args.warmup, "ms_per_step": ms / args.steps, "higher_is_better": True,
            "scaling": "weak", "vs_baseline": None, "dtype": "f64", "data": "synthetic",
@@ -447,7 +448,8 @@ def run_ours(args) -> dict | None:
     gsb = gs_bytes(sizes) / L
     kb = {"ax_e": 64.0 + (16.0 if fused_p else 0.0), "gs": gsb, "dot": 17.0,
           # the fused gs update takes its weights from the gather code: no 1-byte multiplicity code there
-          "update_xr": ((48.0 if fused_p else 24.0) + gs_gather_bytes(L, sizes) / L) if fused_gs
+          # ... and with "fuse_p" + "defer_x" a pair costs 24 + 56 B/pt instead of 2 x 48 (x read and written once)
+          "update_xr": ((xr_fused_p if fused_p else 24.0) + gs_gather_bytes(L, sizes) / L) if fused_gs
                        else (49.0 if fused_p else 25.0),
           "update_p": 24.0 if fused_p else px_bytes, "cg_init": 33.0}
     it_bytes = iter_model_bytes(L, sizes)

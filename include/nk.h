@@ -211,12 +211,14 @@ int nk_dist_cg(nk_ctx *ctx, const double *f, double *x, int niter, double *res_h
  *                  (the separate weighted dot reads the summed w); 0 = nk_gs as its own kernel; 2 (default)
  *                  = 1 for meshes of 2^20 local points or more (below, everything sits in L2 and the
  *                  separate kernel is as fast or faster), else 0.
- *   "defer_x"      1 (default) = where the direction update is a kernel of its own (without "fuse_p": meshes of
- *                  more than 2^24 local points by default) two iterations share one pass over x: the first of a pair
- *                  only forms p' = r + beta p in a second direction vector, the second applies
- *                  x = fma(alpha', p', fma(alpha, p, x)) -- bit for bit what two separate updates give -- and
- *                  p = r + beta' p'.  72 B per point and pair instead of 80.  x is complete when nk_cg returns (an odd
- *                  last iteration is a plain one); 0 = x updated in every iteration.
+ *   "defer_x"      1 (default) = two iterations share one pass over x, which nothing reads before the solve ends:
+ *                  the first of a pair leaves x alone and keeps alpha, the second applies
+ *                  x = fma(alpha', p', fma(alpha, p, x)) -- bit for bit what two separate updates give.  The direction
+ *                  of the first iteration has to survive the second, so it lives in two vectors: without "fuse_p"
+ *                  (large meshes) the first forms p' = r + beta p in the second vector (72 B per point and pair
+ *                  instead of 80); with "fuse_p" and "fuse_gs" (mid-size meshes) the second ax_e writes its direction
+ *                  out of place and the fused gs update takes both directions (80 instead of 96).  x, r, p are
+ *                  complete when nk_cg returns (an odd last iteration is a plain one); 0 = x updated every iteration.
  *   "coop"         1 = nk_cg runs the whole solve as ONE cooperative launch: a persistent CTA per SM does all
  *                  iterations (ax_e with pap and the p update folded in | grid barrier | x, r update with gs
  *                  and the mask folded in, rho' | grid barrier), scalars never leave the chip.  For meshes

@@ -121,29 +121,42 @@ inline bool fuse_gs_on(const nk_ctx *c)
 }
 
 // One CG iteration, enqueued (S 3 call stack (3)).  hist_k: where sqrt(rho') goes (DEVICE).
-// "defer_x" (default on; only where the direction update is a kernel of its own, i.e. without "fuse_p"): two iterations
-// share one pass over x (nk_vec.cu update_p2_kernel / update_pxx_kernel).  pair = 0: a plain iteration; 1: the first
-// of a pair (p2 = r + beta p, x untouched); 2: the second (runs on p2; x takes both steps, p = r + beta' p2).
-inline bool defer_x_on(const nk_ctx *c) { return c->opt_defer_x && !fuse_p_on(c); }
+// "defer_x" (default on): two iterations share one pass over x.  pair = 0: a plain iteration; 1: the first of a pair
+// (x untouched, alpha kept); 2: the second (x takes both steps).  The direction of the first iteration must survive
+// the second, so the direction lives in two vectors (p, p2):
+//   without "fuse_p" (large meshes): first  p2 = r + beta p; second runs on p2, then x and p = r + beta' p2
+//                                    (nk_vec.cu update_p2_kernel / update_pxx_kernel);
+//   with "fuse_p" and "fuse_gs":     the second ax_e forms its direction OUT OF PLACE (reads c->pc, writes the other
+//                                    vector) and the fused gs update applies x = fma(alpha', p', fma(alpha, p, x));
+//                                    c->pc follows the current direction, the pending update at the end lands in p.
+// x, r, p and the history are bit for bit those of plain iterations.
+inline bool defer_x_on(const nk_ctx *c) { return c->opt_defer_x && (!fuse_p_on(c) || fuse_gs_on(c)); }
 
 cudaError_t enqueue_iteration(nk_ctx *c, double *x, double *hist_k, cudaStream_t st, int pair = 0)
 {
     cudaError_t e;
     const int fuse_pap = c->opt_fuse_pap;
+    const bool fuse_p = fuse_p_on(c);
+    double *const pa = c->pc;                                         // the direction before this iteration's update
+    double *const pb = (fuse_p && pair == 2) ? (pa == c->p ? c->p2 : c->p) : pa;     // where this iteration's direction goes
+    const double *const dir = fuse_p ? pb : (pair == 2 ? c->p2 : c->p);              // what ax_e is applied to
     if (c->p_pending) {          // p = r + beta p folded into this ax_e's load
-        NK_LAUNCH(NK_K_AX, nk_launch_ax_tma(c, c->p, nullptr, c->r, c->w, fuse_pap, st));
+        NK_LAUNCH(NK_K_AX, nk_launch_ax_tma(c, pb, pb == pa ? nullptr : pa, c->r, c->w, fuse_pap, st));
         c->p_pending = 0;
     } else {
-        NK_LAUNCH(NK_K_AX, nk_launch_ax_tma(c, nullptr, pair == 2 ? c->p2 : c->p, nullptr, c->w, fuse_pap, st));
+        NK_LAUNCH(NK_K_AX, nk_launch_ax_tma(c, nullptr, dir, nullptr, c->w, fuse_pap, st));
     }
     // "fuse_gs": gs and the mask ride in the residual update, which gathers the copies of shared nodes from the
     // unsummed w (nk_vec.cu); the separate weighted dot needs the summed w, so it keeps gs in place
     const int fuse_gs = fuse_gs_on(c);
     if (!fuse_gs) NK_LAUNCH(NK_K_GS, nk_launch_gs(c, c->w, 1, st));
-    if (!fuse_pap) NK_LAUNCH(NK_K_DOT, nk_launch_dot(c, c->w, pair == 2 ? c->p2 : c->p, nullptr, NK_EPI_PAP, st));
+    if (!fuse_pap) NK_LAUNCH(NK_K_DOT, nk_launch_dot(c, c->w, dir, nullptr, NK_EPI_PAP, st));
     c->w_unsummed = fuse_gs;
-    if (fuse_p_on(c)) {
-        NK_LAUNCH(NK_K_UPDATE_XR, nk_launch_update_xr(c, x, hist_k, fuse_gs, st));
+    if (fuse_p) {
+        if (pair == 1) NK_LAUNCH(NK_K_UPDATE_XR, nk_launch_update_r_first(c, hist_k, st));
+        else if (pair == 2) NK_LAUNCH(NK_K_UPDATE_XR, nk_launch_update_xxr(c, x, pa, pb, hist_k, st));
+        else NK_LAUNCH(NK_K_UPDATE_XR, nk_launch_update_xr(c, x, hist_k, fuse_gs, st));
+        c->pc = pb;
         c->p_pending = 1;
     } else {
         // r first, then x and p together: p is read once per iteration instead of twice (65 vs 73 B/pt)
@@ -159,6 +172,8 @@ cudaError_t enqueue_cg(nk_ctx *c, const double *f, double *x, int niter, double 
 {
     cudaError_t e;
     c->p_pending = 0;
+    c->pc = c->p;
+    struct pc_scope { nk_ctx *c; ~pc_scope() { c->pc = c->p; } } pcs{c};
     if ((e = prof_mark(c, -1, st)) != cudaSuccess) return e;
     NK_LAUNCH(NK_K_INIT, nk_launch_cg_init(c, f, x, res_hist, st));
     // "pdl": every kernel of the loop waits (griddepcontrol.wait) before it reads what its predecessor
@@ -171,7 +186,7 @@ cudaError_t enqueue_cg(nk_ctx *c, const double *f, double *x, int niter, double 
         const int pair = !defer ? 0 : (k % 2 == 1 ? (k < niter ? 1 : 0) : 2);
         if ((e = enqueue_iteration(c, x, res_hist + k, st, pair)) != cudaSuccess) return e;
     }
-    if (c->p_pending) {          // leave the context with p up to date
+    if (c->p_pending) {          // leave the context with p up to date, in c->p wherever the direction was last
         NK_LAUNCH(NK_K_UPDATE_P, nk_launch_update_p(c, st));
         c->p_pending = 0;
     }

@@ -412,7 +412,8 @@ __device__ __forceinline__ double ld_vec(const double *p) { return CG ? __ldcg(p
 // Compute warps: w = A_L u on elements [elo, ehi); returns the thread's share of sum_l u_l (A_L u)_l.
 // (u_rw, u_ro, r_in are what a predecessor wrote: no `const __restrict__` pair, or their loads could be hoisted
 //  above the caller's griddepcontrol.wait as invariant -- see nk_vec.cu.)
-// FUSEP: u = r_in + beta u is applied while loading and written back.  CG: see ld_vec.
+// FUSEP: u = r_in + beta u is applied while loading and written to u_rw; the old u is read from u_ro if that is given
+// (out of place: the "defer_x" pairs keep the previous direction), else from u_rw.  CG: see ld_vec.
 // No arithmetic below sits under a thread-dependent branch: D reaches the DFMAs through the uniform datapath
 // (LDCU -> UR operand), which ptxas only uses in warp-uniform code.  Threads without an element (ragged last
 // warp, tail batch) compute on stale shared memory and only their stores are predicated off.
@@ -442,6 +443,7 @@ __device__ __forceinline__ double ax_compute(const AxSmem<N> &sm, double *u_rw, 
     const double2 *gslot = sm.ring + slot * KP * 3 * n2 + t2;
     const int nit = (int)((ehi - elo + EPB - 1) / EPB);
     double dsum = 0.0;
+    const double *uin = FUSEP ? (u_ro ? u_ro : u_rw) : u_ro;
 
     double nu[n], nr[FUSEP ? n : 1];               // next batch's pencil, in flight
     {
@@ -450,7 +452,7 @@ __device__ __forceinline__ double ax_compute(const AxSmem<N> &sm, double *u_rw, 
         const int64_t gb = act ? e * P + t2 : 0;
 #pragma unroll
         for (int k = 0; k < n; ++k) {
-            nu[k] = act ? ld_vec<CG>((FUSEP ? u_rw : u_ro) + gb + k * n2) : 0.0;
+            nu[k] = act ? ld_vec<CG>(uin + gb + k * n2) : 0.0;
             if (FUSEP) nr[k] = act ? ld_vec<CG>(r_in + gb + k * n2) : 0.0;
         }
     }
@@ -534,7 +536,7 @@ __device__ __forceinline__ double ax_compute(const AxSmem<N> &sm, double *u_rw, 
             const int64_t gb = act ? e1 * P + t2 : 0;
 #pragma unroll
             for (int k = 0; k < n; ++k) {
-                nu[k] = act ? ld_vec<CG>((FUSEP ? u_rw : u_ro) + gb + k * n2) : 0.0;
+                nu[k] = act ? ld_vec<CG>(uin + gb + k * n2) : 0.0;
                 if (FUSEP) nr[k] = act ? ld_vec<CG>(r_in + gb + k * n2) : 0.0;
             }
         };
@@ -596,7 +598,7 @@ ax_tma_kernel(double *u_rw, const double *u_ro, const double *r_in,
     RingState rs{0, 0u};
     if (tid >= C::CT) {
         // ---- producer warp: one lane streams G into the ring (static data: no need to wait for the predecessor)
-        if (tid == C::CT) ax_produce<N>(sm, g, elo, ehi, rs, FUSEP ? u_rw : u_ro, FUSEP ? r_in : nullptr);
+        if (tid == C::CT) ax_produce<N>(sm, g, elo, ehi, rs, FUSEP ? (u_ro ? u_ro : u_rw) : u_ro, FUSEP ? r_in : nullptr);
     } else {
         nk_pdl_wait();                                  // u, r, beta come from the preceding kernels
         const double beta = FUSEP ? red.scal[NK_S_BETA] : 0.0;
@@ -1007,7 +1009,7 @@ cudaError_t launch_tma(nk_ctx *c, double *u_rw, const double *u_ro, const double
     const unsigned grid = (unsigned)(nb < (int64_t)c->sm_count ? nb : (int64_t)c->sm_count);   // one CTA per SM
     cudaError_t e;
     if (r_in != nullptr)
-        e = nk_launch(ax_tma_kernel<N, true>, grid, C::THREADS, C::SMEM, st, c->pdl_now, u_rw, (const double *)nullptr, r_in, w,
+        e = nk_launch(ax_tma_kernel<N, true>, grid, C::THREADS, C::SMEM, st, c->pdl_now, u_rw, u_ro, r_in, w,
                       (const double2 *)c->g, e_begin, e_count, dot, c->red);
     else
         e = nk_launch(ax_tma_kernel<N, false>, grid, C::THREADS, C::SMEM, st, c->pdl_now, (double *)nullptr, u_ro,

@@ -66,6 +66,7 @@ struct nk_ctx {
                                  // k-plane one contiguous chunk [c2][i + n j] of (rr,rs) (rt,ss) (st,tt)
     double *r, *p, *w;           // CG state, L each (coords staging aliases these during set-up)
     double *hf, *hx;             // staging for nk_cg_host, L each
+    double *pc;                  // where the current direction lives: p, except inside a "defer_x" pair on the "fuse_p" path
     double *p2;                  // second direction vector: the deferred x update needs p_k and p_k+1 at once ("defer_x")
     double *hf2, *hx2, *hist2;   // second set: nk_cg_host_batch copies RHS j+1 in and solution j-1 out while solve j runs
     double *dinv;                // Jacobi preconditioner 1 / (Q Q^T diag A_L), 0 on Dirichlet nodes (lazy)
@@ -230,6 +231,8 @@ cudaError_t nk_launch_update_xr(nk_ctx *c, double *x, double *hist_k, int gs, cu
 cudaError_t nk_launch_update_p(nk_ctx *c, cudaStream_t st);
 cudaError_t nk_launch_update_r(nk_ctx *c, double *hist_k, int gs, cudaStream_t st);     // r -= alpha w, rho'
 cudaError_t nk_launch_update_px(nk_ctx *c, double *x, cudaStream_t st);         // x += alpha p; p = r + beta p
+cudaError_t nk_launch_update_r_first(nk_ctx *c, double *hist_k, cudaStream_t st);          // fused gs update, alpha kept
+cudaError_t nk_launch_update_xxr(nk_ctx *c, double *x, const double *pa, const double *pb, double *hist_k, cudaStream_t st);
 cudaError_t nk_launch_update_p2(nk_ctx *c, cudaStream_t st);                    // p2 = r + beta p; alpha kept for the next one
 cudaError_t nk_launch_update_pxx(nk_ctx *c, double *x, cudaStream_t st);        // x += alpha' p + alpha p2; p = r + beta p2
 cudaError_t nk_launch_get_mult(nk_ctx *c, double *mult, cudaStream_t st);

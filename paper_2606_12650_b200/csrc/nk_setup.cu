@@ -410,6 +410,7 @@ extern "C" int nk_setup(nk_ctx **ctx, int64_t E, int N, const double *coords, co
     c->g = reinterpret_cast<double2 *>(q); q += cv.g;
     c->r = reinterpret_cast<double *>(q); q += cv.vec;
     c->p = reinterpret_cast<double *>(q); q += cv.vec;
+    c->pc = c->p;
     c->w = reinterpret_cast<double *>(q); q += cv.vec;
     c->hf = reinterpret_cast<double *>(q); q += cv.vec;
     c->hx = reinterpret_cast<double *>(q); q += cv.vec;

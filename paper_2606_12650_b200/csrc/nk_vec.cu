@@ -253,11 +253,15 @@ __device__ __forceinline__ void gs_point(int l, int v, double wl, double g, doub
     acc = fma(gs_stream_weight(l, v, skip) * rl, rl, acc);
 }
 
-template <bool WITH_X>
+// XM: what happens to x in the same pass.  0: nothing; 1: x += alpha p; 2: the deferred update of two iterations,
+// x = fma(alpha, pb, fma(alpha_prev, p, x)) (nk_api.cu "defer_x" on the "fuse_p" path: p, pb = the directions of the
+// first and second iteration of the pair).  stash != 0 (first of a pair): alpha is kept in NK_S_ALPHA_PREV.
+template <int XM>
 __global__ void __launch_bounds__(NK_GSU_THREADS, NK_GSU_MINB)
-gs_update_kernel(double *__restrict__ x, double *r, const double *p, const double *w, int64_t L, nk_reduce_ws ws,
-                 double *hist_k, nk_gather gp)
+gs_update_kernel(double *__restrict__ x, double *r, const double *p, const double *pb, const double *w, int64_t L,
+                 nk_reduce_ws ws, double *hist_k, nk_gather gp, int stash)
 {
+    constexpr bool WITH_X = XM != 0;
     __shared__ double s_red[33];
     nk_pdl_launch_dependents();
     double acc = 0.0;
@@ -277,10 +281,12 @@ gs_update_kernel(double *__restrict__ x, double *r, const double *p, const doubl
         nv[j] = (q + j * stride < qhi) ? reinterpret_cast<const int4 *>(gp.nbr)[q + j * stride] : make_int4(0, 0, 0, 0);
     nk_pdl_wait();
     const double alpha = ws.scal[NK_S_ALPHA];
+    const double alpha_prev = XM == 2 ? ws.scal[NK_S_ALPHA_PREV] : 0.0;
+    if (stash && blockIdx.x == 0 && threadIdx.x == 0) ws.scal[NK_S_ALPHA_PREV] = alpha;   // the next ax_e overwrites alpha
     // (Staging the streamed operands through shared memory with cp.async, four pairs per thread in flight instead of
     //  two, was measured SLOWER: 394 vs 369 us at config 5.)
     for (; q < qhi; q += U * stride) {
-        double4v wv[U], rv[U], g[U], xv[WITH_X ? U : 1], pv[WITH_X ? U : 1];
+        double4v wv[U], rv[U], g[U], xv[WITH_X ? U : 1], pv[WITH_X ? U : 1], qv[XM == 2 ? U : 1];
         int4 nn[U];
         bool on[U];
 #pragma unroll
@@ -298,6 +304,7 @@ gs_update_kernel(double *__restrict__ x, double *r, const double *p, const doubl
                 if (WITH_X) {
                     xv[WITH_X ? j : 0] = ld4(x + 4 * qj, x32);
                     pv[WITH_X ? j : 0] = ld256(p + 4 * qj);
+                    if (XM == 2) qv[XM == 2 ? j : 0] = ld256(pb + 4 * qj);
                 }
             }
         }
@@ -327,8 +334,14 @@ gs_update_kernel(double *__restrict__ x, double *r, const double *p, const doubl
                 if (WITH_X) {
                     double4v xn = xv[WITH_X ? j : 0];
                     const double4v pj = pv[WITH_X ? j : 0];
-                    xn.a = fma(alpha, pj.a, xn.a); xn.b = fma(alpha, pj.b, xn.b);
-                    xn.c = fma(alpha, pj.c, xn.c); xn.d = fma(alpha, pj.d, xn.d);
+                    if (XM == 2) {
+                        const double4v qj2 = qv[XM == 2 ? j : 0];
+                        xn.a = fma(alpha, qj2.a, fma(alpha_prev, pj.a, xn.a)); xn.b = fma(alpha, qj2.b, fma(alpha_prev, pj.b, xn.b));
+                        xn.c = fma(alpha, qj2.c, fma(alpha_prev, pj.c, xn.c)); xn.d = fma(alpha, qj2.d, fma(alpha_prev, pj.d, xn.d));
+                    } else {
+                        xn.a = fma(alpha, pj.a, xn.a); xn.b = fma(alpha, pj.b, xn.b);
+                        xn.c = fma(alpha, pj.c, xn.c); xn.d = fma(alpha, pj.d, xn.d);
+                    }
                     st4(x + 4 * qj, xn, x32);
                 }
             }
@@ -343,7 +356,8 @@ gs_update_kernel(double *__restrict__ x, double *r, const double *p, const doubl
         double a0 = 0.0;
         gs_point(l, v, w[l], gs_partner(w, l, v), alpha, rl, k0, a0);
         if (!k0) { r[l] = rl; acc += a0; }
-        if (WITH_X) x[l] = fma(alpha, p[l], x[l]);
+        if (XM == 1) x[l] = fma(alpha, p[l], x[l]);
+        if (XM == 2) x[l] = fma(alpha, pb[l], fma(alpha_prev, p[l], x[l]));
     }
     // the nodes with three or more copies whose FIRST copy lies in this block's chunk (their other copies sit in
     // neighbouring chunks: in L2, just streamed or about to be), one thread each
@@ -354,7 +368,7 @@ gs_update_kernel(double *__restrict__ x, double *r, const double *p, const doubl
 
 // p = r + beta p                                       (S 8(a) a6)
 __global__ void __launch_bounds__(NK_VEC_THREADS)
-update_p_kernel(double *__restrict__ p, const double *r, const double *scal, int64_t L)
+update_p_kernel(double *p, const double *pin, const double *r, const double *scal, int64_t L)   // pin == p: in place
 {
     nk_pdl_launch_dependents();
     nk_pdl_wait();
@@ -363,14 +377,14 @@ update_p_kernel(double *__restrict__ p, const double *r, const double *scal, int
     const int64_t stride = (int64_t)gridDim.x * blockDim.x;
     for (int64_t q = (int64_t)blockIdx.x * blockDim.x + threadIdx.x; q < pairs; q += stride) {
         const double2 rv = reinterpret_cast<const double2 *>(r)[q];
-        double2 pv = reinterpret_cast<double2 *>(p)[q];
+        double2 pv = reinterpret_cast<const double2 *>(pin)[q];
         pv.x = fma(beta, pv.x, rv.x);
         pv.y = fma(beta, pv.y, rv.y);
         reinterpret_cast<double2 *>(p)[q] = pv;
     }
     if ((L & 1) && blockIdx.x == 0 && threadIdx.x == 0) {
         const int64_t l = L - 1;
-        p[l] = fma(beta, p[l], r[l]);
+        p[l] = fma(beta, pin[l], r[l]);
     }
 }
 
@@ -649,14 +663,14 @@ cudaError_t nk_launch_cg_init(nk_ctx *c, const double *f, double *x, double *his
 namespace {
 // gs != 0: the fused kernel (gs_update_kernel).  It is a programmatic dependent only where gs itself would be
 // (nk_pdl_mode: its gathers want the L1 that ax_e's shared-memory carve-out takes away on large meshes).
-template <bool WITH_X>
-cudaError_t launch_gs_update(nk_ctx *c, double *x, double *hist_k, cudaStream_t st)
+template <int XM>
+cudaError_t launch_gs_update(nk_ctx *c, double *x, const double *pa, const double *pb, double *hist_k, int stash, cudaStream_t st)
 {
     nk_gather gp;
     gp.nbr = c->nbr; gp.gx = c->gx; gp.rows = c->gx_rows; gp.blk = c->gx_blk;
     const int nb = nk_gsu_blocks(c->sm_count, c->L >> 1);         // the grid nk_setup cut the row list for (gx_blk)
-    const cudaError_t e = nk_launch(gs_update_kernel<WITH_X>, nb, NK_GSU_THREADS, 0, st, c->pdl_now == 2, x, c->r,
-                                    (const double *)c->p, (const double *)c->w, c->L, c->red, hist_k, gp);
+    const cudaError_t e = nk_launch(gs_update_kernel<XM>, nb, NK_GSU_THREADS, 0, st, c->pdl_now == 2, x, c->r, pa, pb,
+                                    (const double *)c->w, c->L, c->red, hist_k, gp, stash);
     if (e != cudaSuccess) return e;
     c->launches++;
     return cudaGetLastError();
@@ -665,9 +679,9 @@ cudaError_t launch_gs_update(nk_ctx *c, double *x, double *hist_k, cudaStream_t 
 
 cudaError_t nk_launch_update_xr(nk_ctx *c, double *x, double *hist_k, int gs, cudaStream_t st)
 {
-    if (gs) return launch_gs_update<true>(c, x, hist_k, st);
+    if (gs) return launch_gs_update<1>(c, x, c->pc, nullptr, hist_k, 0, st);
     const int nb = vec_blocks(c, c->L >> 1);
-    const cudaError_t e = nk_launch(update_xr_kernel, nb, NK_VEC_THREADS, 0, st, c->pdl_now, x, c->r, c->p, c->w, c->code,
+    const cudaError_t e = nk_launch(update_xr_kernel, nb, NK_VEC_THREADS, 0, st, c->pdl_now, x, c->r, c->pc, c->w, c->code,
                                     c->ctab, c->L, c->red, hist_k);
     if (e != cudaSuccess) return e;
     c->launches++;
@@ -677,7 +691,8 @@ cudaError_t nk_launch_update_xr(nk_ctx *c, double *x, double *hist_k, int gs, cu
 cudaError_t nk_launch_update_p(nk_ctx *c, cudaStream_t st)
 {
     const int nb = vec_blocks(c, c->L >> 1);
-    const cudaError_t e = nk_launch(update_p_kernel, nb, NK_VEC_THREADS, 0, st, c->pdl_now, c->p, c->r, c->red.scal, c->L);
+    const cudaError_t e = nk_launch(update_p_kernel, nb, NK_VEC_THREADS, 0, st, c->pdl_now, c->p, (const double *)c->pc, (const double *)c->r,
+                                    (const double *)c->red.scal, c->L);   // c->pc != c->p: the pending update lands in c->p
     if (e != cudaSuccess) return e;
     c->launches++;
     return cudaGetLastError();
@@ -722,7 +737,7 @@ cudaError_t nk_launch_update_pz(nk_ctx *c, double *x, cudaStream_t st)
 
 cudaError_t nk_launch_update_r(nk_ctx *c, double *hist_k, int gs, cudaStream_t st)
 {
-    if (gs) return launch_gs_update<false>(c, nullptr, hist_k, st);
+    if (gs) return launch_gs_update<0>(c, nullptr, nullptr, nullptr, hist_k, 0, st);
     const int nb = vec_blocks(c, c->L >> 1);
     const cudaError_t e = nk_launch(update_r_kernel, nb, NK_VEC_THREADS, 0, st, c->pdl_now, c->r, c->w, c->code, c->ctab,
                                     c->L, c->red, hist_k);
@@ -758,4 +773,15 @@ cudaError_t nk_launch_update_px(nk_ctx *c, double *x, cudaStream_t st)
     if (e != cudaSuccess) return e;
     c->launches++;
     return cudaGetLastError();
+}
+
+// "defer_x" on the "fuse_p" path: the fused gs update of the first iteration of a pair (no x, alpha kept) and of the
+// second (x takes both steps: pa, pb = the directions of the first and second iteration)
+cudaError_t nk_launch_update_r_first(nk_ctx *c, double *hist_k, cudaStream_t st)
+{
+    return launch_gs_update<0>(c, nullptr, nullptr, nullptr, hist_k, 1, st);
+}
+cudaError_t nk_launch_update_xxr(nk_ctx *c, double *x, const double *pa, const double *pb, double *hist_k, cudaStream_t st)
+{
+    return launch_gs_update<2>(c, x, pa, pb, hist_k, 0, st);
 }

@@ -123,20 +123,22 @@ def test_cg_host_batch_equals_one_call_per_rhs(path):
             gpu.set_option(k, v)
 
 
-@pytest.mark.parametrize("niter", [1, 2, 7, 12])
-@pytest.mark.parametrize("fuse_gs", [0, 1])
-def test_deferred_x_update_is_bitwise_the_plain_one(niter, fuse_gs):
+@pytest.mark.parametrize("niter", [1, 2, 3, 7, 12])
+@pytest.mark.parametrize("fuse_p,fuse_gs", [(0, 0), (0, 1), (1, 1)])
+def test_deferred_x_update_is_bitwise_the_plain_one(niter, fuse_p, fuse_gs):
     """"defer_x": two iterations share one pass over x (x = fma(alpha', p', fma(alpha, p, x)), the direction kept in two
     vectors).  Same operations in the same order: x, the history and the state the context is left in (r, p, w) are
     bit for bit those of the plain update -- odd and even iteration counts, launch by launch and graphed, with the
-    caller's x only 16-byte aligned (the 256-bit accesses fall back to 128-bit ones on x)."""
+    caller's x only 16-byte aligned (the 256-bit accesses fall back to 128-bit ones on x).  With "fuse_p" the second
+    ax_e of a pair forms its direction out of place and the fused gs update applies both steps to x; the direction
+    ends in either of the two vectors depending on the count, the context always shows it in p."""
     import torch
     pr = pair_for_brick(7, 6, 5, 6, 0.05)                    # 72030 points: two past the last quad
     gpu = pr.gpu
     saved = {k: gpu.get_option(k) for k in ("coop", "fuse_p", "fuse_gs", "graph", "defer_x")}
     try:
         gpu.set_option("coop", 0)
-        gpu.set_option("fuse_p", 0)
+        gpu.set_option("fuse_p", fuse_p)
         gpu.set_option("fuse_gs", fuse_gs)
         f = to_dev(rhs_unique(pr.mesh, 77))
         xbuf = torch.empty(pr.L + 2, dtype=torch.float64, device="cuda")
