@@ -423,7 +423,7 @@ def run_ours(args) -> dict | None:
     value = whole_job_value(flops_step, args.steps, world, ms)
     e2e = whole_job_value(flops_step, args.steps, world, ms_e2e)
     opts = {k: nk.get_option(k) for k in ("fuse_pap", "fuse_p", "fuse_gs", "graph", "pdl", "coop", "defer_x")}
-    fused_p = opts["fuse_p"] == 1 or (opts["fuse_p"] == 2 and L <= (1 << 24))
+    fused_p = opts["fuse_p"] != 0
     fused_gs = bool(opts["fuse_pap"]) and (opts["fuse_gs"] == 1 or (opts["fuse_gs"] == 2 and L >= (1 << 20)))
     # "defer_x": two iterations share one pass over x (24 + 48 B/pt per pair instead of 2 x 40; an odd last one is plain)
     px_bytes = (72.0 * (niter // 2) + 40.0 * (niter % 2)) / max(niter, 1) if opts["defer_x"] else 40.0

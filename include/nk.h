@@ -201,7 +201,8 @@ int nk_dist_cg(nk_ctx *ctx, const double *f, double *x, int niter, double *res_h
  *   "fuse_pap"     1 (default) = pap accumulated inside ax_e through the dot-fusion identity
  *                  <M QQ^T A_L p, p>_c = sum_l (A_L p)_l p_l; 0 = separate weighted dot after gs
  *   "fuse_p"       1 = p = r + beta p folded into the load of the next ax_e; 0 = own kernel;
- *                  2 (default) = 1 for meshes of up to 2^24 local points (one launch fewer), else 0
+ *                  2 (default) = the library's choice: 1 at every size (with "defer_x" it moves fewer bytes than the
+ *                  separate update and saves a launch)
  *   "fuse_gs"      1 = inside nk_cg the gather-scatter and the mask are folded into the residual
  *                  update: w = M Q Q^T A_L p is only ever read by r -= alpha w, so that kernel streams the
  *                  UNSUMMED ax_e output and sums the copies of every shared node on the fly (in ascending
@@ -214,10 +215,10 @@ int nk_dist_cg(nk_ctx *ctx, const double *f, double *x, int niter, double *res_h
  *   "defer_x"      1 (default) = two iterations share one pass over x, which nothing reads before the solve ends:
  *                  the first of a pair leaves x alone and keeps alpha, the second applies
  *                  x = fma(alpha', p', fma(alpha, p, x)) -- bit for bit what two separate updates give.  The direction
- *                  of the first iteration has to survive the second, so it lives in two vectors: without "fuse_p"
- *                  (large meshes) the first forms p' = r + beta p in the second vector (72 B per point and pair
- *                  instead of 80); with "fuse_p" and "fuse_gs" (mid-size meshes) the second ax_e writes its direction
- *                  out of place and the fused gs update takes both directions (80 instead of 96).  x, r, p are
+ *                  of the first iteration has to survive the second, so it lives in two vectors: with "fuse_p" and
+ *                  "fuse_gs" (the default from 2^20 points on) the second ax_e writes its direction out of place and
+ *                  the fused gs update takes both directions (80 B per point and pair instead of 96); without
+ *                  "fuse_p" the first forms p' = r + beta p in the second vector (72 instead of 80).  x, r, p are
  *                  complete when nk_cg returns (an odd last iteration is a plain one); 0 = x updated every iteration.
  *   "coop"         1 = nk_cg runs the whole solve as ONE cooperative launch: a persistent CTA per SM does all
  *                  iterations (ax_e with pap and the p update folded in | grid barrier | x, r update with gs

@@ -103,11 +103,14 @@ namespace {
 
 inline cudaStream_t S(void *stream) { return static_cast<cudaStream_t>(stream); }
 
-// "fuse_p" = 2 (default): fold p = r + beta p into ax_e's load where the launch saved matters more than
-// the registers it costs (measured: -6..-9 % per solve on configs 1-2, -2.5 % on config 3, +0 at config 5)
+// "fuse_p" = 2 (default): fold p = r + beta p into ax_e's load.  On at every size since the x update is deferred
+// ("defer_x": the fused path then moves 127 B per point and iteration against 131 for the separate direction update,
+// with one launch fewer); measured per iteration, fused against separate: 4.1 M points 97.8 vs 100.5 us, 8.2 M 183 vs
+// 198, 16.8 M 359 vs 378, 28.3 M 583 vs 607, config 5 (56.6 M) 1.177 vs 1.204 ms.  (Before the deferral it paid off
+// only up to 2^24 points: -6..-9 % on configs 1-2, -2.5 % on config 3, +-0 at config 5.)
 inline bool fuse_p_on(const nk_ctx *c)
 {
-    return c->opt_fuse_p == 1 || (c->opt_fuse_p == 2 && c->L <= NK_GRAPH_AUTO_MAX_L);
+    return c->opt_fuse_p != 0;
 }
 
 // "fuse_gs" = 2 (default): gs rides in the residual update from 2^20 local points on (measured per iteration, graph
