@@ -475,7 +475,7 @@ def run_ours(args) -> dict | None:
         if traffic is None:
             try:
                 with open(os.path.join(ROOT, "profiles", "traffic.json.txt")) as fh:
-                    rec = json.load(fh)[args.workload]
+                    rec = json.load(fh)[args.workload if fused_p else args.workload + "_ax_e_alone"]
                 traffic = float(rec["dram_bytes_per_launch"])
                 traffic_source = ("constant from the committed ncu --set full capture " + rec.get("source", "under profiles/")
                                   + " (dram__bytes_read.sum + dram__bytes_write.sum per launch); NOT measured in this run")
