@@ -271,7 +271,7 @@ int nk_get_D(nk_ctx *ctx, double *D_host, double *xi_host, double *w_host);
  * stream while the "profile" option is 1 (S 8(d): per-kernel time inside the timed region).
  * HOST out: ms[6], count[6], classes NK_K_*: 0 ax_e (with whatever is fused into it), 1 gs(+mask),
  * 2 dot, 3 the residual update with rtr (update_r; update x,r on the fuse_p path), 4 the direction
- * update (update_px: x and p; update p on the fuse_p path), 5 cg init.  Synchronises `stream`; resets
+ * update (x and p, or the pending direction update at the end of a solve on the fuse_p path), 5 cg init.  Synchronises `stream`; resets
  * the record. */
 #define NK_K_CLASSES 6
 int nk_get_kernel_times(nk_ctx *ctx, double *ms_host, int64_t *count_host, void *stream);
