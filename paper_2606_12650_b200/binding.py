@@ -236,7 +236,9 @@ class Nekbone:
         return out
 
     def cg(self, f, niter: int, x=None, res_hist=None):
-        """Device-resident CG: returns (x, res_hist) CUDA tensors; does not synchronise."""
+        """Device-resident CG: returns (x, res_hist) CUDA tensors; does not synchronise.
+        On meshes where nk_cg replays a recorded CUDA graph (it keeps the last two, keyed by f, x, res_hist, niter and
+        the options) pass the same x and res_hist tensors on every call: fresh ones mean a new capture each time."""
         import torch
         x = self.empty() if x is None else x
         if res_hist is None:
