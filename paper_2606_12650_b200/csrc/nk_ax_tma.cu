@@ -165,13 +165,13 @@ struct TmaCfg {
 #define NK_TMA_IB 2
 #endif
     static constexpr int IB = NK_TMA_IB;                      // table rows advanced together in lines_apply
-    // where the next batch's u pencil is requested: 1 = after P3, 2 = after P4, 0 = after P5.  1 everywhere: since the
+    // where the next batch's u pencil is requested: 1 = after P3, 2 = after P4, 0 = after P5.  1 nearly everywhere: since the
     // producer prefetches u into L2 (ax_produce) n = 12 is spill-free at 160 registers with it and gains 6 % over 2
     // (16^3: 77.5 -> 72.5 us; before that prefetch 1 cost 4 % there).
-#ifdef NK_TMA_PF12
-    static constexpr int PF = (n == 12) ? NK_TMA_PF12 : 1;
+#if defined(NK_TMA_PF_N) && defined(NK_TMA_PF_VAL)
+    static constexpr int PF = (n == NK_TMA_PF_N) ? NK_TMA_PF_VAL : (n == 15 ? 2 : 1);   // A/B knob: one order, another position
 #else
-    static constexpr int PF = 1;
+    static constexpr int PF = (n == 15) ? 2 : 1;     // n = 15 spills 104 B with 1, 72 B with 2: 186 -> 176 us at 16^3
 #endif
 };
 
