@@ -874,14 +874,12 @@ cg_coop_kernel(nk_coop_args a)
         acc = 0.0;
         for (int64_t q0 = plo + tid; q0 < phi; q0 += 4 * CT) {          // four pairs per thread in flight
             double2 pv[4], wv[4], xv[4], rv[4], gv[4];
-            uchar2 cd[4];
             int2 nv[4];
 #pragma unroll
             for (int j = 0; j < 4; ++j) {
                 const int64_t q = q0 + j * CT;
                 const bool on = q < phi;
                 nv[j] = on ? reinterpret_cast<const int2 *>(a.nbr)[q] : make_int2(0, 0);
-                cd[j] = on ? reinterpret_cast<const uchar2 *>(a.code)[q] : make_uchar2(0, 0);
                 pv[j] = on ? __ldcg(reinterpret_cast<const double2 *>(p2) + q) : make_double2(0.0, 0.0);
                 wv[j] = on ? __ldcg(reinterpret_cast<const double2 *>(a.w) + q) : make_double2(0.0, 0.0);
                 xv[j] = on ? reinterpret_cast<const double2 *>(x2)[q] : make_double2(0.0, 0.0);
@@ -912,8 +910,9 @@ cg_coop_kernel(nk_coop_args a)
                         if (!k0) r2[l] = rv[j].x;
                         if (!k1) r2[l + 1] = rv[j].y;
                     }
-                    acc = fma((k0 ? 0.0 : s_c[cd[j].x & 0x7f]) * rv[j].x, rv[j].x, acc);
-                    acc = fma((k1 ? 0.0 : s_c[cd[j].y & 0x7f]) * rv[j].y, rv[j].y, acc);
+                    // weight 1 / multiplicity from the gather code: own copy 1, face partner 1/2 (nk_vec.cu gs_stream_weight)
+                    acc = fma((k0 ? 0.0 : (nv[j].x == l ? 1.0 : 0.5)) * rv[j].x, rv[j].x, acc);
+                    acc = fma((k1 ? 0.0 : (nv[j].y == l + 1 ? 1.0 : 0.5)) * rv[j].y, rv[j].y, acc);
                 }
             }
         }
@@ -927,7 +926,7 @@ cg_coop_kernel(nk_coop_args a)
             if (!k0) {
                 const double rn = fma(-alpha, s0, r2[l]);
                 r2[l] = rn;
-                acc = fma(s_c[a.code[l] & 0x7f] * rn, rn, acc);
+                acc = fma((vt == l ? 1.0 : 0.5) * rn, rn, acc);
             }
         }
 #ifdef NK_COOP_TIMING
