@@ -579,7 +579,7 @@ ax_tma_kernel(double *u_rw, const double *u_ro, const double *r_in,
 {
     using C = TmaCfg<N>;
     extern __shared__ __align__(128) unsigned char smem_raw[];
-    __shared__ double s_red[33];
+    __shared__ double s_red[34];
     const AxSmem<N> sm(smem_raw);
     const int tid = threadIdx.x;
     if (tid == 0) sm.init_barriers();
@@ -661,7 +661,14 @@ __device__ __forceinline__ void coop_grid_barrier(unsigned *bar, unsigned &passe
     ++passed;
 }
 
-// Sum of v over all compute threads of all CTAs, the same bits in every thread of every CTA.
+// Sum of v over all compute threads of all CTAs, the same bits in every thread of every CTA.  `s_red`: 34 doubles.
+// Two CTA barriers per exchange: warp 0 alone talks to the other CTAs -- lane 0 stores the CTA's partial, arrives
+// with a release reduction (which orders that store and, through the CTA barrier before it, everything the CTA wrote
+// in the phase), polls the counter with acquire loads; then the warp adds all partials in index order.  The result
+// slot alternates with the parity of the exchange, so no third barrier is needed before s_red is reused.
+#ifndef NK_COOP_SUM_V2
+#define NK_COOP_SUM_V2 1
+#endif
 template <int CT>
 __device__ __forceinline__ double coop_grid_sum(double v, double *s_red, double *part, unsigned *bar, unsigned &passed)
 {
@@ -671,6 +678,30 @@ __device__ __forceinline__ double coop_grid_sum(double v, double *s_red, double 
     if (lane == 0) s_red[wid] = v;
     coop_cta_sync<CT>();
     double *mine = part + (size_t)(passed & 1u) * gridDim.x;
+#if NK_COOP_SUM_V2
+    const int slot = 32 + (int)(passed & 1u);
+    if (wid == 0) {
+        double t = (lane < NWARP) ? s_red[lane] : 0.0;
+        t = nk_warp_sum(t);
+        if (lane == 0) {
+            __stcg(mine + blockIdx.x, t);
+            const unsigned target = gridDim.x * (passed + 1u);
+            asm volatile("red.release.gpu.global.add.u32 [%0], 1;" ::"l"(bar) : "memory");
+            unsigned seen;
+            do {
+                asm volatile("ld.acquire.gpu.global.u32 %0, [%1];" : "=r"(seen) : "l"(bar) : "memory");
+            } while (seen < target);
+        }
+        __syncwarp();
+        double sum = 0.0;
+        for (unsigned i = lane; i < gridDim.x; i += 32) sum += __ldcg(mine + i);
+        sum = nk_warp_sum(sum);
+        if (lane == 0) s_red[slot] = sum;
+    }
+    coop_cta_sync<CT>();
+    ++passed;
+    return s_red[slot];
+#else
     if (wid == 0) {
         double t = (lane < NWARP) ? s_red[lane] : 0.0;
         t = nk_warp_sum(t);
@@ -687,6 +718,7 @@ __device__ __forceinline__ double coop_grid_sum(double v, double *s_red, double 
     const double total = s_red[32];
     coop_cta_sync<CT>();                           // s_red is free again
     return total;
+#endif
 }
 
 // The same for ONE THREAD-BLOCK CLUSTER of CS CTAs (meshes of a few thousand points: a handful of CTAs has all the
@@ -751,12 +783,12 @@ __device__ __forceinline__ double coop_gs_value(int l, int v, double wl, double 
 // One node with three or more copies (edges, corners): gather w (past the L1) and r at all copies, sum in ascending
 // local index, r -= alpha sum at every copy; returns the node's share of rho'.  One thread per node, so that the
 // dependent loads of many nodes overlap (inlined per point they serialised behind each other: 10 us per phase).
+// (len, ia: the row's length and first four indices -- static, so a thread keeps those of its first row in registers
+//  for the whole solve and the phase pays one memory round trip for the row instead of three.)
 __device__ __forceinline__ double coop_row_update(const double *w, double *r, const int32_t *__restrict__ gx, int p4,
-                                                  double alpha, const double (&cw_of_len)[9])
+                                                  int len, int4 ia, double alpha, const double (&cw_of_len)[9])
 {
     const int32_t *ii = gx + 4 * (int64_t)p4;
-    const int len = ii[-1];
-    const int4 ia = *reinterpret_cast<const int4 *>(ii);
     double acc = 0.0;
     if (len == 4) {
         const double a0 = __ldcg(w + ia.x), a1 = __ldcg(w + ia.y), a2 = __ldcg(w + ia.z), a3 = __ldcg(w + ia.w);
@@ -796,7 +828,7 @@ cg_coop_kernel(nk_coop_args a)
     __shared__ __align__(8) unsigned long long s_cbar;
     const uint32_t cbar = smem_u32(&s_cbar);
     extern __shared__ __align__(128) unsigned char smem_raw[];
-    __shared__ double s_red[33];
+    __shared__ double s_red[34];
     __shared__ double s_c[NK_CTAB];
     const AxSmem<N> sm(smem_raw);
     const int tid = threadIdx.x;
@@ -830,6 +862,9 @@ cg_coop_kernel(nk_coop_args a)
     double cw_of_len[9];
 #pragma unroll
     for (int j = 0; j < 9; ++j) cw_of_len[j] = j ? 1.0 / (double)j : 0.0;      // = ctab of that multiplicity, bit for bit
+    // the thread's first such node: where its row sits (static: kept in a register for the whole solve; its length and
+    // first four copies are requested at the head of every phase B, ahead of the streaming loop)
+    const int row0_p4 = (rlo + tid < rhi) ? a.gx_rows[rlo + tid] : -1;
     unsigned passed = 0;
     double *x2 = a.x, *r2 = a.r, *p2 = a.p;
     // ---- r = mask o f, x = 0, p = r, rho = <r,r>_c -------------------------------------------------------------
@@ -872,6 +907,8 @@ cg_coop_kernel(nk_coop_args a)
         alpha = (rho == 0.0 || pap == 0.0) ? 0.0 : rho / pap;
         // ---- phase B: x += alpha p; r -= alpha M Q Q^T w; rho' ----------------------------------------------------
         acc = 0.0;
+        const int row0_len = row0_p4 >= 0 ? a.gx[4 * (int64_t)row0_p4 - 1] : 0;
+        const int4 row0_ia = row0_p4 >= 0 ? *reinterpret_cast<const int4 *>(a.gx + 4 * (int64_t)row0_p4) : make_int4(0, 0, 0, 0);
         for (int64_t q0 = plo + tid; q0 < phi; q0 += 4 * CT) {          // four pairs per thread in flight
             double2 pv[4], wv[4], xv[4], rv[4], gv[4];
             int2 nv[4];
@@ -916,7 +953,12 @@ cg_coop_kernel(nk_coop_args a)
                 }
             }
         }
-        for (int64_t kr = rlo + tid; kr < rhi; kr += CT) acc += coop_row_update(a.w, r2, a.gx, a.gx_rows[kr], alpha, cw_of_len);
+        if (row0_p4 >= 0) acc += coop_row_update(a.w, r2, a.gx, row0_p4, row0_len, row0_ia, alpha, cw_of_len);
+        for (int64_t kr = rlo + tid + CT; kr < rhi; kr += CT) {
+            const int p4 = a.gx_rows[kr];
+            acc += coop_row_update(a.w, r2, a.gx, p4, a.gx[4 * (int64_t)p4 - 1], *reinterpret_cast<const int4 *>(a.gx + 4 * (int64_t)p4),
+                                   alpha, cw_of_len);
+        }
         if (odd_tail) {
             const int l = (int)(a.L - 1);
             const int vt = a.nbr[l];
