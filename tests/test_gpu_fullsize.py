@@ -167,3 +167,24 @@ def test_jacobi_diag_and_pcg_early_iterations(full):
         xg, hg = gpu.pcg(to_dev(f), 60)
         assert np.all(np.abs(to_np(hg) - ho) <= TOL_CG * ho), float(np.abs(to_np(hg) / ho - 1).max())
         assert elem_err(to_np(xg), xo, P) <= TOL_CG
+
+
+def test_device_plan_equals_host_plan_at_full_size(full):
+    """The gather-scatter plan built on the device (radix sort over hundreds of blocks and thousands of tiles, scans,
+    1728 gs chunks at config 5) against the host builder's, byte for byte, at the sizes the bench runs."""
+    from paper_2606_12650_b200 import Nekbone
+    from paper_2606_12650_b200.binding import set_plan_builder
+    mesh = full.mesh
+    assert full.gpu.setup_info()["plan_builder"] == "device"
+    dev = {k: v.cpu().numpy().copy() for k, v in full.gpu.plan_arrays().items()}
+    try:
+        set_plan_builder("host")
+        host = Nekbone.from_mesh(mesh)
+        assert host.setup_info()["plan_builder"] == "host"
+        assert host.sizes() == full.gpu.sizes() and host.gs_sizes() == full.gpu.gs_sizes()
+        for k, v in host.plan_arrays().items():
+            a = v.cpu().numpy()
+            assert a.shape == dev[k].shape and np.array_equal(a, dev[k]), k
+        host.close()
+    finally:
+        set_plan_builder("device")
