@@ -188,3 +188,18 @@ def test_device_plan_equals_host_plan_at_full_size(full):
         host.close()
     finally:
         set_plan_builder("device")
+
+
+def test_default_iteration_is_two_kernels(full):
+    """At these sizes the default CG iteration is two launches -- ax_e with the direction update folded into its load
+    and pap fused, and the fused gs + mask + residual update (which every second time also applies the x update of
+    two iterations) -- plus cg_init at the start and the one pending direction update at the end."""
+    gpu = full.gpu
+    niter = CONFIGS[full.name]["niter"]
+    for k, v in (("fuse_pap", 1), ("fuse_p", 2), ("fuse_gs", 2), ("defer_x", 1)):
+        assert gpu.get_option(k) == v, k
+    f = to_dev(config_rhs(full.name, full.mesh))
+    n0 = gpu.launch_count()
+    gpu.cg(f, niter)
+    assert gpu.launch_count() - n0 == 1 + 2 * niter + 1
+    assert gpu.solve_path() == ("graph" if full.mesh.L <= (1 << 24) else "launches")
